@@ -1,0 +1,327 @@
+"""Pins for the oracle's whole step (Fig. 1 A-F; readings R1-R16).  -m "not gpu".
+
+Closed forms (Gaussian selection integral, Wright-Fisher drift, Beverton-Holt fixed point),
+invariants (scan, parent arrays, compaction order, patch bookkeeping, capture accounting) and
+determinism.  A dropped term, wrong sign/index or transposed operand fails one of them."""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import stats
+
+from helpers import cfg, species
+from paper_1603_09255_b200 import workloads
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def popcount_rows(rows):
+    return np.unpackbits(rows.view(np.uint8), axis=1).sum(axis=1).astype(np.int64)
+
+
+def zi_numpy(sp, rows):
+    if sp["kind"] == "bit":
+        return 2 * popcount_rows(rows) - 2 * sp["n_loci"]
+    return rows.astype(np.int64).sum(axis=1)
+
+
+def run(oracle_mod, c, n_steps=1, n0=None):
+    o = oracle_mod.Oracle(c)
+    for s in range(len(c["species"])):
+        o.write_state(s, workloads.initial_rows(c, s, n=None if n0 is None else n0[s]),
+                      workloads.initial_patch_start(c, s), 0)
+    o.step(n_steps)
+    return o
+
+
+def test_scan_and_parent_arrays(oracle_mod):
+    c = workloads.config(3, scale=0.02)
+    o = run(oracle_mod, c)
+    d = o.debug(0)
+    n, m = d["n_t"], d["m_t"]
+    f = d["f"].astype(np.int64)
+    assert n == c["n0"][0] and m == f.sum()
+    assert d["off"][0] == 0 and np.array_equal(d["off"], np.concatenate([[0], np.cumsum(f)[:-1]]))
+    # every offspring has exactly one mother, mothers non-decreasing, f_i offspring each
+    assert np.all(np.diff(d["mother"].astype(np.int64)) >= 0)
+    assert np.array_equal(np.bincount(d["mother"], minlength=n), f)
+    # fathers uniform over adults (chi-square over 50 bins), selfing allowed
+    assert d["father"].max() < n
+    cnt, _ = np.histogram(d["father"], bins=50, range=(0, n))
+    assert ((cnt - m / 50) ** 2 / (m / 50)).sum() < stats.chi2.ppf(1 - 1e-5, 49)
+    # mean offspring count equals the Poisson mean lam = 2/(1+N/K) = 1 (north_star)
+    assert abs(f.mean() - 1.0) < 4.5 / math.sqrt(n)
+    assert abs(f.var() - 1.0) < 0.05
+    # u01 has 24 bits, in [0,1)
+    assert d["u01"].min() >= 0 and d["u01"].max() < 1
+    assert np.all(d["u01"] * 2 ** 24 == np.floor(d["u01"] * 2 ** 24))
+
+
+def test_phenotype_is_exact_integer_sum(oracle_mod):
+    for which, scale in [(1, 1.0), (3, 0.005)]:
+        c = workloads.config(which, scale=scale)
+        o = run(oracle_mod, c)
+        d = o.debug(0)
+        sp = c["species"][0]
+        zi = zi_numpy(sp, d["offspring"])
+        assert np.array_equal(zi, d["zi"])
+        assert np.array_equal(d["z"], (zi * sp["pheno_scale"]).astype(np.float32))
+        assert np.array_equal(d["z"].astype(np.float64), zi * sp["pheno_scale"])  # exact in fp32
+        rows, _, zis = o.read_state(0)
+        assert np.array_equal(zi_numpy(sp, rows), zis)
+
+
+def test_offspring_rows_are_parent_gametes(oracle_mod):
+    # offspring hap0 comes from the mother, hap1 from the father (mu = 0: Mendelian)
+    c = workloads.config(3, scale=0.002)
+    c["species"][0]["mu"] = 0.0
+    rows0 = workloads.initial_rows(c, 0)
+    o = run(oracle_mod, c)
+    d = o.debug(0)
+    W = 32
+    mo, fa, off = rows0[d["mother"]], rows0[d["father"]], d["offspring"]
+    assert not (((off[:, :W] ^ mo[:, :W]) & (off[:, :W] ^ mo[:, W:])).any())
+    assert not (((off[:, W:] ^ fa[:, :W]) & (off[:, W:] ^ fa[:, W:])).any())
+    # and really recombinant: most maternal gametes differ from both maternal haplotypes
+    assert ((off[:, :W] != mo[:, :W]).any(axis=1) & (off[:, :W] != mo[:, W:]).any(axis=1)).mean() > 0.9
+
+
+def test_survival_rule_and_compaction_order(oracle_mod):
+    c = workloads.config(2, scale=0.05)
+    o = run(oracle_mod, c, n_steps=3)  # step index 2 -> theta = 0.02
+    d = o.debug(0)
+    assert abs(d["theta_t"] - np.float32(0.02)) < 1e-9
+    s64 = np.exp(-((d["z"].astype(np.float64) - d["theta_t"]) ** 2) / 2.0)
+    assert np.max(np.abs(d["s"] - s64) / s64) < 1e-6  # fitness within 1e-6 relative (north_star)
+    assert np.array_equal(d["alive"], (d["u01"] < d["s"]).astype(np.uint8))
+    rows, _, zi = o.read_state(0)
+    keep = d["alive"].astype(bool)
+    assert np.array_equal(rows, d["offspring"][keep])  # stable: survivors in offspring order
+    assert np.array_equal(zi, d["zi"][keep])
+    le = o.log(0)[-1]
+    assert le["n_next"] == keep.sum() == o.n(0) and le["m_t"] == d["m_t"]
+    assert le["sum_zi"] == int(zi.astype(np.int64).sum()) and le["sum_zi2"] == int((zi.astype(np.int64) ** 2).sum())
+    assert le["near_ties"] == int((np.abs(d["u01"] - d["s"]) < np.float32(1e-6)).sum())
+
+
+def _closed_forms():
+    out = {}
+    for l in open(os.path.join(HERE, "golden", "closed_forms.txt")):
+        if l.strip() and l[0] != "#":
+            name, V, om, th, w = l.split()
+            out[name] = (float(V), float(om), float(th), float(w))
+    return out
+
+
+@pytest.mark.parametrize("which,scale", [(1, 40.0), (2, 0.4), (3, 0.04), (5, 0.04)])
+def test_first_step_survivor_fraction_closed_form(oracle_mod, which, scale):
+    V, om, th, wref = _closed_forms()["C%d" % which]
+    c = workloads.config(which, scale=scale, grid=(8, 8) if which == 5 else None)
+    sp = c["species"][0]
+    if which == 5:  # theta = 0 everywhere, no dispersal: the C5 row of the table
+        sp["gaussian"]["theta_patch"] = np.zeros(64, np.float32)
+    sp["mu"] = 0.0
+    o = run(oracle_mod, c)
+    d = o.debug(0)
+    m = d["m_t"]
+    # the closed form itself (retyped here from the textbook Gaussian integral)
+    assert abs(om / math.sqrt(V + om * om) * math.exp(-th * th / (2 * (V + om * om))) - wref) < 2e-5
+    z = d["z"].astype(np.float64)
+    assert abs(z.var() / V - 1) < 0.05  # offspring variance = parental variance under random mating
+    frac = d["alive"].mean()
+    assert abs(frac - wref) < 4.5 * math.sqrt(wref * (1 - wref) / m) + 0.002
+    # post-selection mean and variance: (zbar*om^2+theta*V)/(V+om^2), V*om^2/(V+om^2)
+    zs = z[d["alive"].astype(bool)]
+    assert abs(zs.var() / (V * om * om / (V + om * om)) - 1) < 0.05
+    assert abs(zs.mean() - z.mean() * om * om / (V + om * om)) < 5 * math.sqrt(V / m)
+
+
+def test_directional_selection_shifts_mean(oracle_mod):
+    # theta != 0: survivors' mean moves towards theta by V/(V+omega^2) of the distance
+    c = workloads.config(2, scale=0.3)
+    c["species"][0]["gaussian"].update(theta0=0.8, dtheta=0.0)
+    o = run(oracle_mod, c)
+    d = o.debug(0)
+    z = d["z"].astype(np.float64)
+    zs = z[d["alive"].astype(bool)]
+    V = z.var()
+    assert abs((zs.mean() - z.mean()) - (0.8 - z.mean()) * V / (V + 1.0)) < 5 * math.sqrt(V / len(zs))
+    w = 1 / math.sqrt(V + 1) * math.exp(-(0.8 - z.mean()) ** 2 / (2 * (V + 1)))
+    assert abs(d["alive"].mean() - w) < 0.006
+
+
+def test_neutral_drift_heterozygosity_and_wf_variance(oracle_mod):
+    # omega = inf (c = 0), mu = 0: E[H_{t+1}] = H_t (1 - 1/(2 N_{t+1})); Var(dp) = p(1-p)/(2 N_{t+1})
+    c = workloads.config(3, scale=0.001)
+    sp = c["species"][0]
+    sp["mu"] = 0.0
+    sp["gaussian"]["omega"] = 0.0
+    o = oracle_mod.Oracle(c)
+    rows = workloads.initial_rows(c, 0)
+    o.write_state(0, rows, None, 0)
+
+    def freqs(r):
+        b = np.unpackbits(r.view(np.uint8), axis=1, bitorder="little")  # [n, 2048]
+        return (b[:, :1024] + b[:, 1024:]).sum(axis=0) / (2.0 * len(r))
+
+    p = freqs(rows)
+    H0 = (2 * p * (1 - p)).mean()
+    expect = 1.0
+    wf_ratio = []
+    for t in range(200):
+        o.step(1)
+        r, _, _ = o.read_state(0)
+        assert o.log(0)[-1]["n_next"] == o.log(0)[-1]["m_t"]  # everyone survives
+        p2 = freqs(r)
+        if t < 20:
+            wf_ratio.append(((p2 - p) ** 2).mean() / ((p * (1 - p)).mean() / (2 * len(r))))
+        p = p2
+        expect *= 1 - 1 / (2.0 * len(r))
+    H = (2 * p * (1 - p)).mean()
+    assert abs(expect - 0.9048) < 0.01  # N ~ 1000, 200 steps
+    # 1024 loci on 4 chromosomes: sd of the ratio ~ sqrt(Var(H)/n_eff); generous 5 %
+    assert abs(H / H0 / expect - 1) < 0.05
+    assert abs(np.mean(wf_ratio) - 1) < 0.08
+
+
+def test_regulation_fixed_point(oracle_mod):
+    # neutral: E[N_{t+1}|N_t] = 2N/(1+N/K); with selection N* = K(2w-1)
+    c = workloads.config(1, scale=20.0)  # K = 20000
+    c["species"][0]["gaussian"]["omega"] = 0.0
+    o = run(oracle_mod, c, n_steps=1, n0=[5000])
+    lam = 2 / (1 + 5000 / 20000.0)
+    assert abs(o.n(0) - 5000 * lam) < 4.5 * math.sqrt(5000 * lam)
+    c = workloads.config(3, scale=0.02)
+    o = run(oracle_mod, c, n_steps=25)
+    ns = np.array([e["n_next"] for e in o.log(0)[10:]], dtype=np.float64)
+    K = c["species"][0]["K"]
+    assert abs(ns.mean() / K - 0.8856) < 0.02  # K(2*0.942809-1)
+
+
+def test_two_steps_equal_one_plus_one_and_checkpoint(oracle_mod):
+    for which, scale, grid in [(1, 1.0, None), (3, 0.003, None), (5, 0.02, (4, 4))]:
+        c = workloads.config(which, scale=scale, grid=grid)
+        a = run(oracle_mod, c, n_steps=3)
+        b = run(oracle_mod, c, n_steps=1)
+        rows, ps, _ = b.read_state(0)
+        b2 = oracle_mod.Oracle(c)  # checkpoint = rows + patch_start + step (counter-based RNG)
+        b2.write_state(0, rows, ps if c["grid"] != (1, 1) else None, 1)
+        b2.step(2)
+        ra, pa, za = a.read_state(0)
+        rb, pb, zb = b2.read_state(0)
+        assert np.array_equal(ra, rb) and np.array_equal(pa, pb) and np.array_equal(za, zb)
+        assert a.step_counter == b2.step_counter == 3
+
+
+def test_overflow_and_extinction_flags(oracle_mod):
+    c = workloads.config(1, scale=1.0)
+    c["species"][0]["capacity"] = 1000
+    c["species"][0]["K"] = 1e9  # lam = 2 -> M ~ 2000 > capacity
+    o = run(oracle_mod, c)
+    d = o.debug(0)
+    assert d["m_t"] == 1000 and o.flags & 1 and o.log(0)[-1]["flags"] & 1
+    full = int(d["f"].sum())
+    assert full > 1000 and d["mother"][-1] == np.searchsorted(np.cumsum(d["f"]), 999, side="right")
+    # fecundity mean 0 -> extinct next step, then steps are no-ops
+    c = workloads.config(1, scale=1.0)
+    c["species"][0]["fec_a"] = 0.0
+    o = run(oracle_mod, c, n_steps=3)
+    assert o.n(0) == 0 and o.flags & 2
+    assert [e["n_t"] for e in o.log(0)] == [1000, 0, 0]
+
+
+def test_patches_bookkeeping(oracle_mod):
+    c = workloads.config(5, scale=0.05, grid=(6, 5))
+    P = 30
+    o = run(oracle_mod, c)
+    d = o.debug(0)
+    ps0 = workloads.initial_patch_start(c, 0)
+    natal = np.searchsorted(ps0, d["mother"], side="right") - 1
+    fa_patch = np.searchsorted(ps0, d["father"], side="right") - 1
+    assert np.array_equal(natal, fa_patch)  # mating within the natal patch
+    moved = d["dest"] != natal
+    assert abs(moved.mean() - 0.05) < 4.5 * math.sqrt(0.05 * 0.95 / d["m_t"])
+    # destination is one of the 4 torus neighbours, each direction equally likely
+    x, y = natal % 6, natal // 6
+    nb = np.stack([((y - 1) % 5) * 6 + x, y * 6 + (x + 1) % 6, ((y + 1) % 5) * 6 + x, y * 6 + (x - 1) % 6], axis=1)
+    which = (nb[moved] == d["dest"][moved][:, None])
+    assert np.all(which.sum(axis=1) == 1)
+    cnt = which.sum(axis=0)
+    assert ((cnt - cnt.mean()) ** 2 / cnt.mean()).sum() < stats.chi2.ppf(1 - 1e-5, 3)
+    # selection uses theta of the destination patch
+    th = c["species"][0]["gaussian"]["theta_patch"][d["dest"]]
+    s64 = np.exp(-((d["z"].astype(np.float64) - th) ** 2) / 2.0)
+    assert np.max(np.abs(d["s"] - s64) / s64) < 1e-6
+    # next generation ordered by (dest, j); patch_start = histogram scan
+    rows, ps, _ = o.read_state(0)
+    keep = np.flatnonzero(d["alive"])
+    order = keep[np.argsort(d["dest"][keep], kind="stable")]
+    assert np.array_equal(rows, d["offspring"][order])
+    assert np.array_equal(ps, np.concatenate([[0], np.cumsum(np.bincount(d["dest"][keep], minlength=P))]))
+    # per-patch Beverton-Holt tables: lam_p = 2/(1+n_p/K_p)
+    assert len(d["table_len"]) == P
+    # m = 0: nobody changes patch, an emptied patch stays empty
+    c0 = workloads.config(5, scale=0.05, grid=(6, 5))
+    c0["species"][0]["migration"] = 0.0
+    o0 = oracle_mod.Oracle(c0)
+    rows0 = workloads.initial_rows(c0, 0)
+    ps0 = workloads.initial_patch_start(c0, 0).copy()
+    n7 = ps0[8] - ps0[7]
+    rows0 = np.delete(rows0, np.arange(ps0[7], ps0[8]), axis=0)
+    ps0[8:] -= n7  # patch 7 empty
+    o0.write_state(0, rows0, ps0, 0)
+    for _ in range(3):
+        o0.step(1)
+        dd = o0.debug(0)
+        _, ps, _ = o0.read_state(0)
+        assert ps[8] == ps[7]
+        natal = np.searchsorted(ps0, dd["mother"], side="right") - 1
+        assert np.array_equal(dd["dest"], natal)
+        ps0 = ps
+
+
+def test_two_species_capture_accounting(oracle_mod):
+    c = workloads.config(4, scale=0.01)
+    o = run(oracle_mod, c)
+    prey, pred = o.debug(0), o.debug(1)
+    le_prey = o.log(0)[-1]
+    n_c = c["n0"][1]
+    # A = a*N_C is scale-free (= 0.1); captured iff u01 >= s_pred
+    assert abs(prey["attack_n"] - 0.1) < 1e-6
+    g = np.exp(-0.5 * (prey["z"].astype(np.float64) - prey["zbar_pred"]) ** 2)
+    s_pred = np.exp(-prey["attack_n"] * g)
+    cap_ref = prey["u01"] >= s_pred
+    near = np.abs(prey["u01"] - s_pred) < 2e-6
+    assert np.array_equal(prey["captured"].astype(bool)[~near], cap_ref[~near])
+    assert le_prey["captures"] == prey["captured"].sum() == pred["cap"].sum()
+    assert pred["cap"].shape[0] == n_c
+    # s = s_pred * s_stab ; alive iff u01 < s ; captured individuals are dead
+    s_stab = np.exp(-(prey["z"].astype(np.float64) ** 2) / 8.0)
+    assert np.max(np.abs(prey["s"] - s_pred * s_stab) / (s_pred * s_stab)) < 2e-6
+    assert not (prey["captured"].astype(bool) & prey["alive"].astype(bool)).any()
+    # expected capture fraction = 1 - E[exp(-A g)] (numerical integral over the offspring z)
+    assert abs(prey["captured"].mean() - (1 - s_pred.mean())) < 4.5 * math.sqrt(0.1 / prey["m_t"])
+    # prey fecundity: logistic mean max(0, 1 + rho(1 - N/K)) = 1 + 1/3
+    assert abs(prey["f"].mean() - (1 + 1 / 3.0)) < 4.5 * math.sqrt(1.34 / prey["n_t"])
+    # predator fecundity table k has mean eps*k*(1 - N_C/K_C) = 1.2 k ; zero captures -> no offspring
+    assert pred["table_len"][0] == 0
+    f, cap = pred["f"].astype(np.float64), pred["cap"]
+    assert f[cap == 0].sum() == 0
+    for k in (1, 2):
+        sel = cap == k
+        if sel.sum() > 50:
+            assert abs(f[sel].mean() - 1.2 * k) < 5 * math.sqrt(1.2 * k / sel.sum())
+    assert pred["alive"].all()  # predator offspring all survive
+    # A = 0 -> no captures -> predator extinct in one step
+    c2 = workloads.config(4, scale=0.005)
+    c2["species"][0]["predation"]["attack"] = 0.0
+    o2 = run(oracle_mod, c2, n_steps=2)
+    assert o2.log(0)[0]["captures"] == 0 and o2.n(1) == 0 and (o2.flags & 2)
+
+
+def test_c4_reading_persists_at_small_scale(oracle_mod):
+    # R14 default (prey under stabilising selection): both species persist over 60 steps at 1/200 scale
+    c = workloads.config(4, scale=0.005)
+    o = run(oracle_mod, c, n_steps=60)
+    assert o.n(0) > 0.5 * c["n0"][0] and o.n(1) > 0.2 * c["n0"][1]
