@@ -1,0 +1,181 @@
+/*
+ * spegg.h -- C ABI of libspegg: the B200-native per-time-step update of an individual-based,
+ * forward-time, multi-locus diploid population (the hot path of sPEGG, arXiv 1603.09255).
+ *
+ * One call of spegg_step() performs, for every species and entirely on the GPU, the loop of the
+ * paper's Fig. 1:
+ *   A  parents identified, number of neonates determined   (Poisson fecundity + exclusive scan)
+ *   B  parents assigned to neonates, genes transmitted      (recombination + mutation)
+ *   C  genotype -> phenotype map                             (additive, eq. S2-14)
+ *   D  selection updates phenotypes incl. mortality risk    (Gaussian / predation survival)
+ *   E  survivors identified, dead removed                    (stable stream compaction)
+ *   F  environment updated from the survivors' phenotypes   (exact integer reductions, counts)
+ * plus migration between patches.  What the paper leaves open (RNG, samplers,
+ * density regulation, ...) is fixed by the readings R1-R16 in DESIGN.md.
+ *
+ * Conventions
+ *   - Plain C, no exceptions.  Every call returns an int: 0 = SPEGG_OK, <0 = error code
+ *     (spegg_strerror gives text).  A failed call leaves the simulation unchanged.
+ *   - OWNERSHIP: the caller owns all device memory (one workspace block, e.g. a torch uint8
+ *     tensor) and the CUDA stream.  The handle owns a small host struct, the captured CUDA graph
+ *     and host copies of the parameter arrays.  spegg_destroy never frees caller memory.
+ *   - Pointers named d_* are DEVICE pointers; `genomes` in write/read_state is host or device
+ *     as said by the *_is_device argument; everything else is a HOST pointer.
+ *   - Population rows ("one contiguous row per individual"):
+ *       SPEGG_BIT : 2*W uint32, W = n_loci/32: [hap0 words | hap1 words]; locus l is bit l%32
+ *                   (LSB first) of word l/32; hap0 is the haplotype received from the mother.
+ *       SPEGG_Q10 : 2*L int16: [hap0 | hap1], allelic value = k * 2^-10.
+ *   - spegg_step is asynchronous on the caller's stream and never touches the host afterwards;
+ *     population counts stay on the device (no host sync per generation).
+ */
+#ifndef SPEGG_H
+#define SPEGG_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPEGG_ABI_VERSION 1u
+
+enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
+       SPEGG_ESTATE = -5 };
+
+enum { SPEGG_BIT = 0, SPEGG_Q10 = 1 };                 /* genome_kind                        */
+enum { SPEGG_INTERVAL = 0, SPEGG_POISSON = 1 };        /* linkage_mode (R7 / R8)             */
+enum { SPEGG_FEC_BEVERTON_HOLT = 0,                    /* lam = R0/(1+n/K)            (R13)  */
+       SPEGG_FEC_LOGISTIC = 1,                         /* lam = max(0, 1+rho(1-n/K))  (R14)  */
+       SPEGG_FEC_CAPTURES = 2 };                       /* lam = eps*cap_i*max(0,1-N/K) (R14) */
+enum { SPEGG_FLAG_OVERFLOW = 1u,  /* M_t exceeded capacity; offspring j >= capacity dropped */
+       SPEGG_FLAG_EXTINCT = 2u }; /* a species reached N = 0; its further steps are no-ops   */
+
+#define SPEGG_TMAX 128       /* max stored thresholds of a Poisson table (R5)                */
+#define SPEGG_CAP_TABLES 32  /* capture-indexed fecundity tables (R14)                       */
+
+/* Genetic architecture and ecology of one species (Fig. S4 :495). */
+typedef struct spegg_species_params {
+    uint32_t n_loci;            /* L; SPEGG_BIT needs L % 32 == 0                            */
+    uint32_t genome_kind;
+    uint32_t n_chrom;
+    const uint32_t *chrom_len;  /* [n_chrom], sum = L; SPEGG_BIT: each a multiple of 32      */
+    uint32_t linkage_mode;
+    const double *r;            /* INTERVAL: [L-1] recombination fraction of each adjacent
+                                   interval, in [0, 0.5] (0.5 across chromosome boundaries)  */
+    const double *xover_mean;   /* POISSON: [n_chrom] mean crossover count per chromosome    */
+    double mu;                  /* per-locus mutation probability             */
+    double mut_sd;              /* Q10: sd of the Gaussian mutational step, allelic units    */
+    float pheno_scale;          /* z = (float)zi * pheno_scale; BIT: zi = 2*ones-2L (each
+                                   allele +-1), Q10: zi = sum of the 2L allelic integers     */
+    uint32_t fecundity_model;
+    double fec_a;               /* BH: R0; LOGISTIC: rho; CAPTURES: conversion efficiency    */
+    double K;                   /* carrying capacity                                         */
+    const double *K_patch;      /* [n_patches] per-patch K, or NULL (then K for every patch) */
+    uint32_t sel_gaussian;      /* 1: s *= exp(-(z-theta)^2/(2 omega^2))                     */
+    double theta0, dtheta;      /* theta_t = theta0 + t*dtheta                               */
+    double omega;               /* <= 0: infinite width (everyone passes this term)          */
+    const float *theta_patch;   /* [n_patches] optimum of the DESTINATION patch, or NULL     */
+    uint32_t sel_predation;     /* 1: s *= exp(-a*N_C*exp(-(z-zbar_C)^2/2)), captures counted */
+    double attack;              /* a                                                         */
+    uint32_t predator_species;  /* index of the species whose N_C, zbar_C enter the term     */
+    double migration;           /* m: probability that a newborn disperses to one of the 4
+                                   torus neighbours of its natal patch (R15)                 */
+    uint64_t capacity;          /* rows per population buffer (>= any N_t, M_t), < 2^31      */
+} spegg_species_params;
+
+typedef struct spegg_params {
+    uint32_t struct_size;       /* sizeof(spegg_params)                                      */
+    uint32_t abi_version;       /* SPEGG_ABI_VERSION                                         */
+    uint64_t seed;              /* Philox key (R3)                                           */
+    uint32_t n_species;         /* 1..8; species are updated in index order                 */
+    uint32_t grid_w, grid_h;    /* torus of patches; 1x1 = unstructured                      */
+    uint32_t debug;             /* 1: every intermediate of the step is materialised and can
+                                   be read with spegg_read_debug (slower, same results)      */
+    uint32_t log_capacity;      /* per-step log ring entries (0 -> 4096)                     */
+    uint32_t flags;             /* reserved, 0                                               */
+    const spegg_species_params *species;
+} spegg_params;
+
+typedef struct spegg_log_entry {
+    uint64_t n_t, m_t, n_next;  /* adults at start, offspring produced, survivors            */
+    int64_t sum_zi, sum_zi2;    /* over survivors, integer phenotype units (exact)           */
+    uint64_t captures;          /* predation captures this step                              */
+    uint64_t near_ties;         /* decisions with |u01 - s| < 1e-6 (reported, north_star)    */
+    uint32_t flags, step;
+} spegg_log_entry;
+
+/* Device pointers into the workspace; valid until the next spegg_step. debug = 1 only.      */
+typedef struct spegg_debug_view {
+    uint64_t n_t, m_t;
+    const uint8_t *d_f;         /* [n_t] fecundity                                           */
+    const uint32_t *d_off;      /* [n_t] exclusive scan of f                                 */
+    const uint32_t *d_mother, *d_father, *d_dest; /* [m_t]                                   */
+    const float *d_u01, *d_s;   /* [m_t] survival uniform, survival probability              */
+    const int32_t *d_zi;        /* [m_t] integer phenotype                                   */
+    const uint8_t *d_alive, *d_captured; /* [m_t]                                            */
+    const void *d_offspring;    /* [m_t] rows                                                */
+    const uint32_t *d_tables;   /* [n_tables][SPEGG_TMAX] fecundity thresholds               */
+    const uint32_t *d_table_len;/* [n_tables]                                                */
+    uint32_t n_tables;
+    float theta_t, zbar_pred, attack_n;
+    const uint32_t *d_cap;      /* [n_t] capture counts (SPEGG_FEC_CAPTURES species)          */
+} spegg_debug_view;
+
+typedef struct spegg_sim spegg_sim;
+
+/* Validates `p` and returns the device bytes spegg_create needs (two population buffers of
+ * `capacity` rows per species + index / scan / table / log arrays).  SPEGG_EINVAL on bad params. */
+int spegg_workspace_bytes(const spegg_params *p, uint64_t *bytes);
+
+/* Builds the constant threshold tables (Bernoulli, Poisson, discrete normal), uploads them and
+ * captures the step graph on `cuda_stream` (a cudaStream_t, may be 0).  d_workspace must be
+ * 256-byte aligned device memory of at least spegg_workspace_bytes().  Populations start empty. */
+int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void *cuda_stream,
+                 spegg_sim **out);
+
+/* Loads a whole population of `species` (n rows, n <= capacity) and sets the global step counter.
+ * patch_start: HOST [n_patches+1] CSR of the rows, sorted by patch (NULL iff 1x1 grid).
+ * Serves as initialisation and as "resume": with the counter-based RNG the state
+ * (rows, patch_start, step, seed) is a complete checkpoint.  Synchronises the stream. */
+int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *genomes,
+                      int genomes_is_device, const uint32_t *patch_start, uint32_t step);
+
+/* Enqueues n_steps steps on the stream and returns; no host synchronisation.  Never fails for
+ * model reasons: overflow / extinction set sticky device flags (spegg_status). */
+int spegg_step(spegg_sim *s, uint32_t n_steps);
+
+/* Synchronises, then copies the current adults of `species` out.  Any output may be NULL.
+ * n, step: HOST scalars.  genomes_out: host or device buffer of cap_bytes; SPEGG_ERANGE if too
+ * small (*n is still set).  patch_start_out: HOST [n_patches+1].  zi_out: HOST [n] integer
+ * phenotypes (z = zi * pheno_scale). */
+int spegg_read_state(spegg_sim *s, uint32_t species, uint64_t *n, uint32_t *step,
+                     void *genomes_out, int genomes_is_device, uint64_t cap_bytes,
+                     uint32_t *patch_start_out, int32_t *zi_out);
+
+/* Synchronises and copies log entries [first_step_index, first_step_index + n) of the ring;
+ * index 0 is the first step taken since the last spegg_write_state of that species' simulation.
+ * *n_avail (nullable) receives the number of entries available. */
+int spegg_read_log(spegg_sim *s, uint32_t species, uint32_t first, uint32_t n,
+                   spegg_log_entry *out, uint32_t *n_avail);
+
+/* Synchronises; fills device pointers to the intermediates of the last step (debug = 1 only,
+ * else SPEGG_ESTATE). */
+int spegg_read_debug(spegg_sim *s, uint32_t species, spegg_debug_view *out);
+
+/* Synchronises; returns the sticky flags (SPEGG_FLAG_*). */
+int spegg_status(spegg_sim *s, uint32_t *flags);
+
+/* Number of kernel launches one spegg_step(1) replays (graph kernel nodes). */
+int spegg_launches_per_step(const spegg_sim *s, uint32_t *n);
+
+/* CUDA-event timing of the dominant kernel: when enabled, spegg_step brackets the main
+ * (gamete) kernel of species 0 with events on the stream; read back with the mean duration in
+ * milliseconds over the launches since enabling.  For bench.py's roofline figure. */
+int spegg_kernel_timing(spegg_sim *s, int enable, float *mean_ms, uint32_t *n_launches);
+
+void spegg_destroy(spegg_sim *s);
+const char *spegg_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,609 @@
+// spegg_api.cu -- the C ABI of libspegg (include/spegg.h) and the step orchestration.
+//
+// Host side only marshals: it validates parameters, builds the constant threshold tables, lays
+// the caller's workspace out, captures ONE CUDA graph of the step's kernel sequence and replays
+// it.  Every step of the path runs in the kernels of spegg_kernels.cuh / spegg_fused.cuh;
+// there is no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/spegg.h"
+#include "spegg_fused.cuh"
+#include "spegg_kernels.cuh"
+
+using namespace spegg;
+
+static_assert(sizeof(LogEntry) == sizeof(spegg_log_entry), "log entry layout");
+static_assert(TMAX == SPEGG_TMAX && CAP_TABLES == SPEGG_CAP_TABLES, "table constants");
+
+namespace {
+
+// ------------------------------------------------------------- host-side constant tables
+// (the library's own builders; same specified arithmetic as the device code, R4-R9)
+double h_exp_neg64(double lam) {
+    if (!(lam >= 0.0)) lam = 0.0;
+    if (lam > 700.0) return 0.0;
+    const double x = -lam;
+    const double t = x * 0x1.71547652b82fep+0;
+    const double kf = std::floor(t + 0.5);
+    const double r = (x - kf * 0x1.62e42fee00000p-1) - kf * 0x1.a39ef35793c76p-33;
+    const double c[15] = {
+        0x1.0000000000000p+0,  0x1.0000000000000p+0,  0x1.0000000000000p-1,
+        0x1.5555555555555p-3,  0x1.5555555555555p-5,  0x1.1111111111111p-7,
+        0x1.6c16c16c16c17p-10, 0x1.a01a01a01a01ap-13, 0x1.a01a01a01a01ap-16,
+        0x1.71de3a556c734p-19, 0x1.27e4fb7789f5cp-22, 0x1.ae64567f544e4p-26,
+        0x1.1eed8eff8d898p-29, 0x1.6124613a86d09p-33, 0x1.93974a8c07c9dp-37};
+    double p = c[14];
+    for (int i = 13; i >= 0; --i) { p = p * r; p = p + c[i]; }
+    const long long bits = (long long)(1023 + (int)kf) << 52;
+    double scale;
+    std::memcpy(&scale, &bits, 8);
+    return p * scale;
+}
+
+int h_poisson_table(double lam, uint32_t *T, int maxlen) {
+    double p = h_exp_neg64(lam), F = p;
+    int k = 0;
+    for (;;) {
+        const double tk = std::floor(F * 4294967296.0);
+        if (tk >= 4294967295.0) break;
+        if (k == maxlen) break;
+        T[k++] = (uint32_t)tk;
+        p = (p * lam) / (double)k;
+        F = F + p;
+    }
+    return k;
+}
+
+unsigned long long h_bernoulli_T(double p) {
+    if (!(p > 0.0)) return 0ull;
+    if (p >= 1.0) return 4294967296ull;
+    return (unsigned long long)std::floor(p * 4294967296.0);
+}
+
+int h_normal_table(double sq, std::vector<uint32_t> &T) {
+    int R = (int)std::ceil(8.0 * sq);
+    if (R < 1) R = 1;
+    T.resize(2 * (size_t)R);
+    for (int k = -R; k < R; ++k) {
+        const double a = (double)k + 0.5;
+        const double x = a / sq;
+        const double y = -x * 0.70710678118654752440;
+        const double ph = 0.5 * std::erfc(y);
+        double tk = std::floor(ph * 4294967296.0);
+        if (tk > 4294967295.0) tk = 4294967295.0;
+        T[(size_t)(k + R)] = (uint32_t)tk;
+    }
+    return R;
+}
+
+// ------------------------------------------------------------------------------ layout
+struct Carver {
+    uint64_t off = 0;
+    uint64_t take(uint64_t bytes) {
+        const uint64_t a = (off + 255) & ~255ull;
+        off = a + bytes;
+        return a;
+    }
+};
+
+struct SpeciesLayout {
+    uint64_t pop[2], patch_start[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
+        cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
+    uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, K_patch, theta_patch;
+    uint32_t norm_len, n_tables, row_bytes;
+};
+
+struct HostSpecies {
+    spegg_species_params p;
+    std::vector<uint32_t> chrom_len, chrom_start, T_recomb, T_xover, xover_len, T_mut, T_norm;
+    std::vector<double> K_patch;
+    std::vector<float> theta_patch;
+    int R_norm = 0;
+    SpeciesLayout lay;
+    SpK k;
+};
+
+int validate(const spegg_params *p) {
+    if (!p || p->struct_size != sizeof(spegg_params) || p->abi_version != SPEGG_ABI_VERSION) return SPEGG_EINVAL;
+    if (!p->species || p->n_species == 0 || p->n_species > (uint32_t)MAX_SPECIES) return SPEGG_EINVAL;
+    const uint32_t gw = p->grid_w ? p->grid_w : 1, gh = p->grid_h ? p->grid_h : 1;
+    const uint64_t P = (uint64_t)gw * gh;
+    if (P > (1u << 20)) return SPEGG_EINVAL;
+    for (uint32_t s = 0; s < p->n_species; ++s) {
+        const spegg_species_params &q = p->species[s];
+        if (q.n_loci == 0 || q.n_loci > (1u << 20) || q.n_chrom == 0 || !q.chrom_len) return SPEGG_EINVAL;
+        if (q.genome_kind > 1 || q.linkage_mode > 1 || q.fecundity_model > 2) return SPEGG_EINVAL;
+        uint64_t acc = 0;
+        for (uint32_t c = 0; c < q.n_chrom; ++c) {
+            if (q.chrom_len[c] == 0) return SPEGG_EINVAL;
+            if (q.genome_kind == SPEGG_BIT && q.chrom_len[c] % 32) return SPEGG_EINVAL;
+            acc += q.chrom_len[c];
+        }
+        if (acc != q.n_loci) return SPEGG_EINVAL;
+        if (q.genome_kind == SPEGG_BIT && q.n_loci % 32) return SPEGG_EINVAL;
+        if (q.genome_kind == SPEGG_Q10 && q.n_loci % 4) return SPEGG_EINVAL;  // rows are 16-byte multiples
+        // kernels exist for bit+Poisson-crossover and q10+per-interval genomes
+        if (q.genome_kind == SPEGG_BIT && q.linkage_mode != SPEGG_POISSON) return SPEGG_EINVAL;
+        if (q.genome_kind == SPEGG_Q10 && q.linkage_mode != SPEGG_INTERVAL) return SPEGG_EINVAL;
+        if (q.genome_kind == SPEGG_BIT && q.n_loci % 64) return SPEGG_EINVAL;
+        if (q.linkage_mode == SPEGG_INTERVAL) {
+            if (q.n_loci > 1 && !q.r) return SPEGG_EINVAL;
+            for (uint32_t l = 0; l + 1 < q.n_loci; ++l)
+                if (!(q.r[l] >= 0.0 && q.r[l] < 1.0)) return SPEGG_EINVAL;
+        } else {
+            if (!q.xover_mean) return SPEGG_EINVAL;
+            for (uint32_t c = 0; c < q.n_chrom; ++c)
+                if (!(q.xover_mean[c] >= 0.0 && q.xover_mean[c] <= 32.0)) return SPEGG_EINVAL;
+        }
+        if (!(q.mu >= 0.0 && q.mu <= 1.0) || !(q.migration >= 0.0 && q.migration <= 1.0)) return SPEGG_EINVAL;
+        if (q.genome_kind == SPEGG_Q10 && !(q.mut_sd > 0.0 && q.mut_sd * 1024.0 * 8.0 < 32000.0)) return SPEGG_EINVAL;
+        if (!(q.K > 0.0) || !(q.fec_a >= 0.0)) return SPEGG_EINVAL;
+        if (q.capacity == 0 || q.capacity >= (1ull << 31)) return SPEGG_EINVAL;
+        if (q.fecundity_model == SPEGG_FEC_CAPTURES && P != 1) return SPEGG_EINVAL;
+        if (q.sel_predation) {
+            if (q.predator_species >= p->n_species || q.predator_species <= s) return SPEGG_EINVAL;
+            if (p->species[q.predator_species].fecundity_model != SPEGG_FEC_CAPTURES) return SPEGG_EINVAL;
+            if (!(q.attack >= 0.0)) return SPEGG_EINVAL;
+        }
+    }
+    return SPEGG_OK;
+}
+
+uint32_t row_bytes_of(const spegg_species_params &q) {
+    return q.genome_kind == SPEGG_BIT ? 2 * (q.n_loci / 32) * 4 : 2 * q.n_loci * 2;
+}
+
+// Lays out the whole workspace; returns total bytes.  Header: DevGlobal + DevSpecies[MAX].
+uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
+    Carver c;
+    c.take(4096);  // header
+    const uint32_t gw = p->grid_w ? p->grid_w : 1, gh = p->grid_h ? p->grid_h : 1;
+    const uint64_t P = (uint64_t)gw * gh;
+    const uint32_t logcap = p->log_capacity ? p->log_capacity : 4096;
+    out.resize(p->n_species);
+    for (uint32_t s = 0; s < p->n_species; ++s) {
+        const spegg_species_params &q = p->species[s];
+        SpeciesLayout &l = out[s];
+        const uint64_t cap = q.capacity;
+        l.row_bytes = row_bytes_of(q);
+        l.n_tables = q.fecundity_model == SPEGG_FEC_CAPTURES ? CAP_TABLES : (uint32_t)P;
+        const uint64_t n_status = (cap + SCAN_TILE - 1) / SCAN_TILE + 1;
+        l.pop[0] = c.take(cap * l.row_bytes);
+        l.pop[1] = c.take(cap * l.row_bytes);
+        l.patch_start[0] = c.take((P + 1) * 4);
+        l.patch_start[1] = c.take((P + 1) * 4);
+        l.f = c.take(cap);
+        l.off = c.take(cap * 4);
+        l.mother = c.take(cap * 4);
+        l.father = c.take(cap * 4);
+        l.dest = c.take(cap * 4);
+        l.pos = c.take(cap * 4);
+        l.u01 = c.take(cap * 4);
+        l.s = c.take(cap * 4);
+        l.zi = c.take(cap * 4);
+        l.alive = c.take(cap);
+        l.captured = c.take(cap);
+        l.cap = c.take(cap * 4);
+        l.offbuf = c.take(cap * l.row_bytes);
+        l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
+        l.table_len = c.take((uint64_t)l.n_tables * 4);
+        l.status_fec = c.take(n_status * 8);
+        l.status_cmp = c.take(n_status * 8);
+        l.patch_cnt = c.take(P * 5 * 4);
+        l.patch_base = c.take(P * 5 * 4);
+        l.log = c.take((uint64_t)logcap * sizeof(LogEntry));
+        l.T_recomb = c.take((uint64_t)q.n_loci * 4);
+        l.T_xover = c.take((uint64_t)q.n_chrom * XMAX * 4);
+        l.xover_len = c.take((uint64_t)q.n_chrom * 4);
+        l.chrom_start = c.take((uint64_t)q.n_chrom * 4);
+        l.chrom_len = c.take((uint64_t)q.n_chrom * 4);
+        l.T_mut = c.take(TMAX * 4);
+        l.norm_len = q.genome_kind == SPEGG_Q10 ? 2 * (uint32_t)std::max(1.0, std::ceil(8.0 * q.mut_sd * 1024.0)) : 0;
+        l.T_norm = c.take((uint64_t)l.norm_len * 4 + 16);
+        l.K_patch = c.take(P * 8);
+        l.theta_patch = c.take(P * 4);
+    }
+    return (c.off + 255) & ~255ull;
+}
+
+#define CU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { s_last_cuda = e_; return SPEGG_ECUDA; } } while (0)
+thread_local cudaError_t s_last_cuda = cudaSuccess;
+
+}  // namespace
+
+struct spegg_sim {
+    spegg_params p;
+    std::vector<HostSpecies> sp;
+    uint8_t *ws = nullptr;
+    uint64_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    DevGlobal *d_glob = nullptr;
+    DevSpecies *d_st = nullptr;
+    uint32_t P = 1, n_sms = 148, launches = 0;
+    uint32_t log_capacity = 4096;
+    bool debug = false;
+    // kernel timing (direct launches bracketed by events)
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;
+    uint32_t ev_used = 0;
+    double timing_ms = 0.0;
+    uint32_t timing_n = 0;
+};
+
+namespace {
+
+template <typename T> T *at(spegg_sim *s, uint64_t off) { return reinterpret_cast<T *>(s->ws + off); }
+
+int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
+    if (bytes == 0) return SPEGG_OK;
+    CU(cudaMemcpyAsync(s->ws + off, src, bytes, cudaMemcpyHostToDevice, s->stream));
+    return SPEGG_OK;
+}
+
+// true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
+bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
+    return !s->debug && s->P == 1 && fused_bit_supported(h.k);
+}
+
+// Enqueue the kernels of one step on the stream (captured into the graph, or launched directly
+// when kernel timing is on).  Returns the number of kernel launches through *n_launch.
+int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
+    uint32_t nl = 0;
+    const uint32_t G = s->n_sms;
+    for (auto &h : s->sp)
+        if (h.p.fecundity_model == SPEGG_FEC_CAPTURES)
+            CU(cudaMemsetAsync(h.k.cap, 0, (size_t)h.p.capacity * 4, s->stream));
+    k_step_begin<<<1, 32, 0, s->stream>>>(s->d_st, s->p.n_species); ++nl;
+    for (size_t si = 0; si < s->sp.size(); ++si) {
+        HostSpecies &h = s->sp[si];
+        const SpK &k = h.k;
+        const bool time_this = timed && si == 0 && s->ev_used + 2 <= s->ev.size();
+        k_begin<<<std::max(1u, std::min(G, (k.n_tables + 255) / 256 + 8)), 256, 0, s->stream>>>(k); ++nl;
+        k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
+        if (fused_ok(s, h)) {
+            if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
+            launch_fused_bit(k, G, s->stream); ++nl;
+            if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
+        } else {
+            k_scalar<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+            if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
+            if (k.kind == 0) k_gamete_bit<<<G * 8, 256, 0, s->stream>>>(k);
+            else k_gamete_q10<<<G * 8, 256, 0, s->stream>>>(k);
+            ++nl;
+            if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
+            k_mutate<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+            k_phenotype<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+            k_survival<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+            if (s->P == 1) {
+                k_cmp_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
+            } else {
+                k_patch_count<<<std::min(s->P, G * 8), 256, 0, s->stream>>>(k); ++nl;
+                k_patch_base<<<1, 1024, 0, s->stream>>>(k); ++nl;
+                k_patch_pos<<<std::min(s->P, G * 8), 256, 0, s->stream>>>(k); ++nl;
+            }
+            k_cmp_scatter<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+        }
+        k_end<<<1, 32, 0, s->stream>>>(k); ++nl;
+    }
+    k_step_end<<<1, 1, 0, s->stream>>>(s->d_glob); ++nl;
+    CU(cudaGetLastError());
+    if (n_launch) *n_launch = nl;
+    return SPEGG_OK;
+}
+
+void drain_timing(spegg_sim *s) {
+    for (uint32_t i = 0; i + 1 < s->ev_used; i += 2) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, s->ev[i], s->ev[i + 1]) == cudaSuccess) { s->timing_ms += ms; s->timing_n += 1; }
+    }
+    s->ev_used = 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *spegg_strerror(int code) {
+    switch (code) {
+    case SPEGG_OK: return "ok";
+    case SPEGG_EINVAL: return "invalid parameter";
+    case SPEGG_ENOMEM: return "workspace too small";
+    case SPEGG_ECUDA: return cudaGetErrorString(s_last_cuda);
+    case SPEGG_ERANGE: return "output buffer too small";
+    case SPEGG_ESTATE: return "call not valid in this state";
+    default: return "unknown error";
+    }
+}
+
+int spegg_workspace_bytes(const spegg_params *p, uint64_t *bytes) {
+    const int rc = validate(p);
+    if (rc != SPEGG_OK) return rc;
+    if (!bytes) return SPEGG_EINVAL;
+    std::vector<SpeciesLayout> l;
+    *bytes = layout(p, l);
+    return SPEGG_OK;
+}
+
+int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void *cuda_stream, spegg_sim **out) {
+    int rc = validate(p);
+    if (rc != SPEGG_OK) return rc;
+    if (!d_workspace || !out || ((uintptr_t)d_workspace & 255u)) return SPEGG_EINVAL;
+    std::vector<SpeciesLayout> lays;
+    const uint64_t need = layout(p, lays);
+    if (bytes < need) return SPEGG_ENOMEM;
+    spegg_sim *s = new (std::nothrow) spegg_sim();
+    if (!s) return SPEGG_ENOMEM;
+    s->p = *p;
+    s->p.species = nullptr;
+    s->ws = (uint8_t *)d_workspace;
+    s->ws_bytes = bytes;
+    s->debug = p->debug != 0;
+    s->log_capacity = p->log_capacity ? p->log_capacity : 4096;
+    const uint32_t gw = p->grid_w ? p->grid_w : 1, gh = p->grid_h ? p->grid_h : 1;
+    s->P = gw * gh;
+    auto fail = [&](int code) { spegg_destroy(s); return code; };
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        s_last_cuda = cudaGetLastError();
+        return fail(SPEGG_ECUDA);
+    }
+    s->n_sms = (uint32_t)prop.multiProcessorCount;
+    if (cuda_stream) s->stream = (cudaStream_t)cuda_stream;
+    else {  // the legacy default stream cannot be captured: use a private one
+        if (cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(SPEGG_ECUDA);
+        s->own_stream = true;
+    }
+    s->d_glob = at<DevGlobal>(s, 0);
+    s->d_st = at<DevSpecies>(s, 256);
+    if (cudaMemsetAsync(s->ws, 0, 4096, s->stream) != cudaSuccess) return fail(SPEGG_ECUDA);
+
+    s->sp.resize(p->n_species);
+    for (uint32_t si = 0; si < p->n_species; ++si) {
+        HostSpecies &h = s->sp[si];
+        const spegg_species_params &q = p->species[si];
+        h.p = q;
+        h.lay = lays[si];
+        const uint32_t L = q.n_loci;
+        uint32_t acc = 0;
+        for (uint32_t c = 0; c < q.n_chrom; ++c) { h.chrom_start.push_back(acc); h.chrom_len.push_back(q.chrom_len[c]); acc += q.chrom_len[c]; }
+        h.T_recomb.assign(L, 0);
+        if (q.linkage_mode == SPEGG_INTERVAL) {
+            h.T_recomb[0] = 2147483648u;  // start phase ~ Bernoulli(1/2) (R7)
+            for (uint32_t l = 1; l < L; ++l) h.T_recomb[l] = (uint32_t)h_bernoulli_T(q.r[l - 1]);
+        }
+        h.T_xover.assign((size_t)q.n_chrom * XMAX, 0);
+        h.xover_len.assign(q.n_chrom, 0);
+        if (q.linkage_mode == SPEGG_POISSON)
+            for (uint32_t c = 0; c < q.n_chrom; ++c)
+                h.xover_len[c] = (uint32_t)h_poisson_table(q.xover_mean[c], &h.T_xover[(size_t)c * XMAX], 62);
+        h.T_mut.assign(TMAX, 0);
+        const uint32_t mut_len = (uint32_t)h_poisson_table((double)L * q.mu, h.T_mut.data(), TMAX);
+        if (q.genome_kind == SPEGG_Q10) h.R_norm = h_normal_table(q.mut_sd * 1024.0, h.T_norm);
+        if (q.K_patch) h.K_patch.assign(q.K_patch, q.K_patch + s->P);
+        if (q.theta_patch) h.theta_patch.assign(q.theta_patch, q.theta_patch + s->P);
+        h.p.chrom_len = nullptr; h.p.r = nullptr; h.p.xover_mean = nullptr; h.p.K_patch = nullptr; h.p.theta_patch = nullptr;
+
+        const SpeciesLayout &l = h.lay;
+        if ((rc = upload(s, l.T_recomb, h.T_recomb.data(), h.T_recomb.size() * 4)) ||
+            (rc = upload(s, l.T_xover, h.T_xover.data(), h.T_xover.size() * 4)) ||
+            (rc = upload(s, l.xover_len, h.xover_len.data(), h.xover_len.size() * 4)) ||
+            (rc = upload(s, l.chrom_start, h.chrom_start.data(), h.chrom_start.size() * 4)) ||
+            (rc = upload(s, l.chrom_len, h.chrom_len.data(), h.chrom_len.size() * 4)) ||
+            (rc = upload(s, l.T_mut, h.T_mut.data(), TMAX * 4)) ||
+            (rc = upload(s, l.T_norm, h.T_norm.data(), h.T_norm.size() * 4)) ||
+            (rc = upload(s, l.K_patch, h.K_patch.data(), h.K_patch.size() * 8)) ||
+            (rc = upload(s, l.theta_patch, h.theta_patch.data(), h.theta_patch.size() * 4)))
+            return fail(rc);
+        if (cudaMemsetAsync(s->ws + l.patch_start[0], 0, (s->P + 1) * 4, s->stream) != cudaSuccess ||
+            cudaMemsetAsync(s->ws + l.patch_start[1], 0, (s->P + 1) * 4, s->stream) != cudaSuccess ||
+            cudaMemsetAsync(s->ws + l.cap, 0, (size_t)q.capacity * 4, s->stream) != cudaSuccess)
+            return fail(SPEGG_ECUDA);
+
+        SpK &k = h.k;
+        std::memset(&k, 0, sizeof k);
+        k.species = si; k.n_species = p->n_species;
+        k.L = L; k.W = L / 32; k.kind = q.genome_kind; k.n_chrom = q.n_chrom; k.linkage = q.linkage_mode;
+        k.row_bytes = l.row_bytes; k.row_u4 = l.row_bytes / 16;
+        k.P = s->P; k.grid_w = gw; k.grid_h = gh;
+        k.capacity = (uint32_t)q.capacity;
+        k.fec_model = q.fecundity_model; k.fec_a = q.fec_a; k.K = q.K;
+        k.K_patch = q.K_patch ? at<double>(s, l.K_patch) : nullptr;
+        k.sel_gaussian = q.sel_gaussian; k.sel_predation = q.sel_predation; k.predator = q.predator_species;
+        k.theta0 = q.theta0; k.dtheta = q.dtheta; k.attack = q.attack;
+        // R11: c = fp32(1/(2 omega^2)) from fp64; omega <= 0 -> c = 0
+        k.sel_c = q.omega > 0.0 ? (float)(1.0 / (2.0 * (q.omega * q.omega))) : 0.0f;
+        k.pheno_scale = q.pheno_scale;
+        k.pred_scale = q.sel_predation ? p->species[q.predator_species].pheno_scale : 0.0f;
+        k.theta_patch = q.theta_patch ? at<float>(s, l.theta_patch) : nullptr;
+        k.T_mig = h_bernoulli_T(q.migration);
+        k.n_tables = l.n_tables;
+        k.key.k0 = (uint32_t)p->seed; k.key.k1 = (uint32_t)(p->seed >> 32);
+        k.T_recomb = at<uint32_t>(s, l.T_recomb);
+        k.T_xover = at<uint32_t>(s, l.T_xover); k.xover_len = at<uint32_t>(s, l.xover_len);
+        k.chrom_start = at<uint32_t>(s, l.chrom_start); k.chrom_len = at<uint32_t>(s, l.chrom_len);
+        k.T_mut = at<uint32_t>(s, l.T_mut); k.mut_len = mut_len;
+        k.T_norm = at<uint32_t>(s, l.T_norm); k.R_norm = h.R_norm;
+        k.pop[0] = at<uint8_t>(s, l.pop[0]); k.pop[1] = at<uint8_t>(s, l.pop[1]);
+        k.patch_start[0] = at<uint32_t>(s, l.patch_start[0]); k.patch_start[1] = at<uint32_t>(s, l.patch_start[1]);
+        k.f = at<uint8_t>(s, l.f); k.off = at<uint32_t>(s, l.off);
+        k.mother = at<uint32_t>(s, l.mother); k.father = at<uint32_t>(s, l.father);
+        k.dest = at<uint32_t>(s, l.dest); k.pos = at<uint32_t>(s, l.pos);
+        k.u01 = at<float>(s, l.u01); k.s = at<float>(s, l.s);
+        k.offbuf = at<uint8_t>(s, l.offbuf); k.zi = at<int32_t>(s, l.zi);
+        k.alive = at<uint8_t>(s, l.alive); k.captured = at<uint8_t>(s, l.captured);
+        k.cap = at<uint32_t>(s, l.cap);
+        k.tables = at<uint32_t>(s, l.tables); k.table_len = at<uint32_t>(s, l.table_len);
+        k.status_fec = at<unsigned long long>(s, l.status_fec); k.status_cmp = at<unsigned long long>(s, l.status_cmp);
+        k.patch_cnt = at<uint32_t>(s, l.patch_cnt); k.patch_base = at<uint32_t>(s, l.patch_base);
+        k.st = s->d_st + si; k.st_all = s->d_st; k.glob = s->d_glob;
+        k.log = at<LogEntry>(s, l.log); k.log_capacity = s->log_capacity;
+        k.debug = p->debug;
+    }
+    for (uint32_t si = 0; si < p->n_species; ++si)
+        if (s->sp[si].p.sel_predation) s->sp[si].k.cap_pred = s->sp[s->sp[si].p.predator_species].k.cap;
+
+    // capture the step graph once; spegg_step replays it
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }
+    if (cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }
+    rc = enqueue_step(s, &s->launches, false);
+    cudaError_t ce = cudaStreamEndCapture(s->stream, &s->graph);
+    if (rc != SPEGG_OK) return fail(rc);
+    if (ce != cudaSuccess) { s_last_cuda = ce; return fail(SPEGG_ECUDA); }
+    if ((ce = cudaGraphInstantiate(&s->exec, s->graph, 0)) != cudaSuccess) { s_last_cuda = ce; return fail(SPEGG_ECUDA); }
+    *out = s;
+    return SPEGG_OK;
+}
+
+void spegg_destroy(spegg_sim *s) {
+    if (!s) return;
+    if (s->stream) cudaStreamSynchronize(s->stream);
+    for (auto e : s->ev) cudaEventDestroy(e);
+    if (s->exec) cudaGraphExecDestroy(s->exec);
+    if (s->graph) cudaGraphDestroy(s->graph);
+    if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
+    delete s;
+}
+
+int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *genomes, int genomes_is_device,
+                      const uint32_t *patch_start, uint32_t step) {
+    if (!s || species >= s->sp.size() || (n && !genomes)) return SPEGG_EINVAL;
+    HostSpecies &h = s->sp[species];
+    if (n > h.p.capacity) return SPEGG_ERANGE;
+    std::vector<uint32_t> ps(s->P + 1, 0);
+    if (s->P > 1) {
+        if (!patch_start || patch_start[0] != 0 || patch_start[s->P] != n) return SPEGG_EINVAL;
+        for (uint32_t p = 0; p < s->P; ++p) if (patch_start[p] > patch_start[p + 1]) return SPEGG_EINVAL;
+        ps.assign(patch_start, patch_start + s->P + 1);
+    } else ps[1] = (uint32_t)n;
+    CU(cudaStreamSynchronize(s->stream));
+    DevSpecies st;
+    CU(cudaMemcpy(&st, s->d_st + species, sizeof st, cudaMemcpyDeviceToHost));
+    const uint32_t cur = st.cur;
+    CU(cudaMemcpyAsync(h.k.pop[cur], genomes, (size_t)n * h.k.row_bytes,
+                       genomes_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream));
+    CU(cudaMemcpyAsync(h.k.patch_start[cur], ps.data(), ps.size() * 4, cudaMemcpyHostToDevice, s->stream));
+    std::memset(&st, 0, sizeof st);
+    st.cur = cur;
+    st.n = (uint32_t)n;
+    CU(cudaMemcpyAsync(s->d_st + species, &st, sizeof st, cudaMemcpyHostToDevice, s->stream));
+    DevGlobal g;
+    CU(cudaMemcpy(&g, s->d_glob, sizeof g, cudaMemcpyDeviceToHost));
+    g.step = step;
+    CU(cudaMemcpyAsync(s->d_glob, &g, sizeof g, cudaMemcpyHostToDevice, s->stream));
+    if (n) k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(s->stream));
+    return SPEGG_OK;
+}
+
+int spegg_step(spegg_sim *s, uint32_t n_steps) {
+    if (!s) return SPEGG_EINVAL;
+    for (uint32_t i = 0; i < n_steps; ++i) {
+        if (s->timing) {
+            if (s->ev_used + 2 > s->ev.size()) { CU(cudaStreamSynchronize(s->stream)); drain_timing(s); }
+            const int rc = enqueue_step(s, nullptr, true);
+            if (rc != SPEGG_OK) return rc;
+        } else {
+            CU(cudaGraphLaunch(s->exec, s->stream));
+        }
+    }
+    return SPEGG_OK;
+}
+
+int spegg_read_state(spegg_sim *s, uint32_t species, uint64_t *n, uint32_t *step, void *genomes_out,
+                     int genomes_is_device, uint64_t cap_bytes, uint32_t *patch_start_out, int32_t *zi_out) {
+    if (!s || species >= s->sp.size()) return SPEGG_EINVAL;
+    HostSpecies &h = s->sp[species];
+    CU(cudaStreamSynchronize(s->stream));
+    DevSpecies st;
+    DevGlobal g;
+    CU(cudaMemcpy(&st, s->d_st + species, sizeof st, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(&g, s->d_glob, sizeof g, cudaMemcpyDeviceToHost));
+    if (n) *n = st.n;
+    if (step) *step = g.step;
+    if (genomes_out) {
+        if (cap_bytes < (uint64_t)st.n * h.k.row_bytes) return SPEGG_ERANGE;
+        CU(cudaMemcpy(genomes_out, h.k.pop[st.cur], (size_t)st.n * h.k.row_bytes,
+                      genomes_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+    }
+    if (patch_start_out) CU(cudaMemcpy(patch_start_out, h.k.patch_start[st.cur], (s->P + 1) * 4, cudaMemcpyDeviceToHost));
+    if (zi_out && st.n) {
+        k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, st.n, 0);
+        CU(cudaGetLastError());
+        CU(cudaStreamSynchronize(s->stream));
+        CU(cudaMemcpy(zi_out, h.k.zi, (size_t)st.n * 4, cudaMemcpyDeviceToHost));
+    }
+    return SPEGG_OK;
+}
+
+int spegg_read_log(spegg_sim *s, uint32_t species, uint32_t first, uint32_t n, spegg_log_entry *out, uint32_t *n_avail) {
+    if (!s || species >= s->sp.size()) return SPEGG_EINVAL;
+    HostSpecies &h = s->sp[species];
+    CU(cudaStreamSynchronize(s->stream));
+    DevSpecies st;
+    CU(cudaMemcpy(&st, s->d_st + species, sizeof st, cudaMemcpyDeviceToHost));
+    if (n_avail) *n_avail = st.log_pos;
+    if (n == 0) return SPEGG_OK;
+    if (!out || (uint64_t)first + n > st.log_pos) return SPEGG_ERANGE;
+    if (st.log_pos - first > s->log_capacity) return SPEGG_ERANGE;  // overwritten by the ring
+    for (uint32_t i = 0; i < n; ++i)
+        CU(cudaMemcpy(out + i, h.k.log + ((first + i) % s->log_capacity), sizeof(LogEntry), cudaMemcpyDeviceToHost));
+    return SPEGG_OK;
+}
+
+int spegg_read_debug(spegg_sim *s, uint32_t species, spegg_debug_view *o) {
+    if (!s || species >= s->sp.size() || !o) return SPEGG_EINVAL;
+    if (!s->debug) return SPEGG_ESTATE;
+    HostSpecies &h = s->sp[species];
+    CU(cudaStreamSynchronize(s->stream));
+    DevSpecies st;
+    CU(cudaMemcpy(&st, s->d_st + species, sizeof st, cudaMemcpyDeviceToHost));
+    const SpK &k = h.k;
+    o->n_t = st.n0; o->m_t = st.m;
+    o->d_f = k.f; o->d_off = k.off; o->d_mother = k.mother; o->d_father = k.father; o->d_dest = k.dest;
+    o->d_u01 = k.u01; o->d_s = k.s; o->d_zi = k.zi; o->d_alive = k.alive; o->d_captured = k.captured;
+    o->d_offspring = k.offbuf; o->d_tables = k.tables; o->d_table_len = k.table_len; o->n_tables = k.n_tables;
+    o->theta_t = st.theta_t; o->zbar_pred = st.zbar_pred; o->attack_n = st.attack_n;
+    o->d_cap = k.cap;
+    return SPEGG_OK;
+}
+
+int spegg_status(spegg_sim *s, uint32_t *flags) {
+    if (!s || !flags) return SPEGG_EINVAL;
+    CU(cudaStreamSynchronize(s->stream));
+    DevGlobal g;
+    CU(cudaMemcpy(&g, s->d_glob, sizeof g, cudaMemcpyDeviceToHost));
+    *flags = g.flags;
+    return SPEGG_OK;
+}
+
+int spegg_launches_per_step(const spegg_sim *s, uint32_t *n) {
+    if (!s || !n) return SPEGG_EINVAL;
+    *n = s->launches;
+    return SPEGG_OK;
+}
+
+int spegg_kernel_timing(spegg_sim *s, int enable, float *mean_ms, uint32_t *n_launches) {
+    if (!s) return SPEGG_EINVAL;
+    CU(cudaStreamSynchronize(s->stream));
+    drain_timing(s);
+    if (mean_ms) *mean_ms = s->timing_n ? (float)(s->timing_ms / s->timing_n) : 0.0f;
+    if (n_launches) *n_launches = s->timing_n;
+    if (enable && s->ev.empty()) {
+        s->ev.resize(512);
+        for (auto &e : s->ev) CU(cudaEventCreate(&e));
+    }
+    if (enable && !s->timing) { s->timing_ms = 0.0; s->timing_n = 0; }
+    s->timing = enable != 0;
+    return SPEGG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,96 @@
+// spegg_internal.h -- structs shared by the host orchestration and the kernels of libspegg.
+#pragma once
+#include <cstdint>
+
+#include "spegg_device.cuh"
+
+namespace spegg {
+
+constexpr int TMAX = 128;        // thresholds per Poisson table (R5)
+constexpr int XMAX = 64;         // row stride of the crossover-count tables (len <= 62, R8)
+constexpr int CAP_TABLES = 32;   // R14
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = 4;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+constexpr int MAX_SPECIES = 8;
+
+// Device-resident per-species state: counts never leave the GPU between steps.
+struct DevSpecies {
+    uint32_t cur;          // which population buffer holds the adults
+    uint32_t n;            // adults
+    uint32_t n0;           // adults at the start of the current step (snapshot)
+    uint32_t m;            // offspring of the current step (after capacity truncation)
+    uint32_t n_next;       // survivors of the current step
+    uint32_t flags_step;   // flags raised during the current step
+    uint32_t ticket_fec, ticket_cmp, ticket_fused, done_fused;
+    uint32_t log_pos;      // entries written to the log ring
+    uint32_t pad0;
+    long long sum_zi;      // over the current adults (survivors of the last step)
+    long long sum_zi0;     // snapshot at the start of the step
+    long long acc_zi, acc_zi2;  // accumulators of the current step's survivors
+    unsigned long long captures, near_ties;
+    float theta_t, zbar_pred, attack_n;
+    uint32_t n_pred0;      // predator count snapshot used by this step
+};
+
+struct DevGlobal {
+    uint32_t step;
+    uint32_t flags;        // sticky
+};
+
+struct LogEntry {          // == spegg_log_entry
+    unsigned long long n_t, m_t, n_next;
+    long long sum_zi, sum_zi2;
+    unsigned long long captures, near_ties;
+    uint32_t flags, step;
+};
+
+// Per-species constants and device pointers, passed to kernels by value.
+struct SpK {
+    uint32_t species, n_species;
+    uint32_t L, W, kind, n_chrom, linkage;
+    uint32_t row_bytes, row_u4;          // bytes / uint4 per row
+    uint32_t P, grid_w, grid_h;
+    uint32_t capacity;
+    uint32_t fec_model;
+    double fec_a, K;
+    const double *K_patch;
+    uint32_t sel_gaussian, sel_predation, predator;
+    double theta0, dtheta, attack;
+    float sel_c, pheno_scale, pred_scale;
+    const float *theta_patch;
+    unsigned long long T_mig;
+    uint32_t n_tables;
+    Key key;
+    // constant tables
+    const uint32_t *T_recomb;   // [L] INTERVAL switch thresholds (T_0 = 2^31)
+    const uint32_t *T_xover;    // [n_chrom][XMAX]
+    const uint32_t *xover_len;  // [n_chrom]
+    const uint32_t *chrom_start, *chrom_len;
+    const uint32_t *T_mut;
+    uint32_t mut_len;
+    const uint32_t *T_norm;
+    int R_norm;
+    // state
+    uint8_t *pop[2];
+    uint32_t *patch_start[2];   // [P+1] each
+    uint8_t *f;
+    uint32_t *off, *mother, *father, *dest, *pos;
+    float *u01, *s;
+    uint8_t *offbuf;
+    int32_t *zi;
+    uint8_t *alive, *captured;
+    uint32_t *cap;              // capture counts of THIS species' adults (CAPTURES model)
+    uint32_t *cap_pred;         // capture counts of the predator species (predation term)
+    uint32_t *tables, *table_len;
+    unsigned long long *status_fec, *status_cmp;
+    uint32_t *patch_cnt, *patch_base;  // [P][5]
+    DevSpecies *st;             // this species
+    DevSpecies *st_all;         // all species
+    DevGlobal *glob;
+    LogEntry *log;
+    uint32_t log_capacity;
+    uint32_t debug;
+};
+
+}  // namespace spegg

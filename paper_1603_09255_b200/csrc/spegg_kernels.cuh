@@ -1,0 +1,647 @@
+// spegg_kernels.cuh -- the step pipeline of libspegg as separate kernels (sm_100a).
+//
+// One time step of one species (Fig. 1 A-F) is the sequence
+//   k_begin        a0  derived parameters: fecundity tables from device-resident counts, theta_t
+//   k_fec_scan     a1-a3  Poisson fecundity, single-pass decoupled look-back scan, mother fill
+//   k_scalar       a3  father (uniform mate), dispersal, survival uniform
+//   k_gamete_*     a4  recombination (bit: Poisson crossovers; q10: per-interval draws)
+//   k_mutate       a4  sparse mutation
+//   k_phenotype    a5  additive map, exact integers
+//   k_survival     a6  fp32 survival probability, decision, captures
+//   k_cmp_* / k_patch_*  a7-a8  stable compaction into the other buffer + reductions
+//   k_end          a9  counts stay on the device; log entry; buffer flip
+// This file is the general ("materialised") pipeline that serves every configuration and the
+// debug view; spegg_fused.cuh holds the fused single-pass kernels of the hot configurations.
+// All grids are fixed at graph-capture time and loop against device-side counts.
+#pragma once
+#include "spegg_internal.h"
+
+namespace spegg {
+
+// ------------------------------------------------------------------------------- helpers
+__device__ __forceinline__ uint32_t patch_of(const uint32_t *__restrict__ ps, uint32_t P, uint32_t i) {
+    uint32_t lo = 0, hi = P;  // largest lo with ps[lo] <= i
+    while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (ps[mid] <= i) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+__device__ __forceinline__ uint32_t neighbour(uint32_t p, uint32_t dir, uint32_t gw, uint32_t gh) {
+    uint32_t px = p % gw, py = p / gw;
+    switch (dir) {
+    case 0: py = (py + gh - 1) % gh; break;
+    case 1: px = (px + 1) % gw; break;
+    case 2: py = (py + 1) % gh; break;
+    default: px = (px + gw - 1) % gw; break;
+    }
+    return py * gw + px;
+}
+
+// R13/R14: fecundity mean, fp64 with the stated op order
+__device__ __forceinline__ double fecundity_mean(const SpK &sp, double n, double K, uint32_t cap_index) {
+    if (sp.fec_model == 0) {  // Beverton-Holt
+        const double q = __ddiv_rn(n, K);
+        const double d = __dadd_rn(1.0, q);
+        return __ddiv_rn(sp.fec_a, d);
+    } else if (sp.fec_model == 1) {  // logistic
+        const double q = __ddiv_rn(n, K);
+        const double a = __dsub_rn(1.0, q);
+        const double b = __dmul_rn(sp.fec_a, a);
+        const double l = __dadd_rn(1.0, b);
+        return l < 0.0 ? 0.0 : l;
+    }
+    const double q = __ddiv_rn(n, K);
+    double a = __dsub_rn(1.0, q);
+    if (a < 0.0) a = 0.0;
+    const double b = __dmul_rn(sp.fec_a, (double)cap_index);
+    return __dmul_rn(b, a);
+}
+
+// R11/R14 survival probability in fp32, in the stated order.  Returns s; sets captured.
+__device__ __forceinline__ float survival_prob(const SpK &sp, float z, float theta, float u01, bool &captured) {
+    float s = 1.0f;
+    captured = false;
+    if (sp.sel_predation) {
+        const float d = __fsub_rn(z, sp.st->zbar_pred);
+        const float g = expf_spec(-__fmul_rn(0.5f, __fmul_rn(d, d)));
+        const float spd = expf_spec(-__fmul_rn(sp.st->attack_n, g));
+        captured = !(u01 < spd);
+        s = spd;
+    }
+    if (sp.sel_gaussian) {
+        const float d = __fsub_rn(z, theta);
+        const float sq = __fmul_rn(d, d);
+        const float ss = expf_spec(-__fmul_rn(sq, sp.sel_c));
+        s = sp.sel_predation ? __fmul_rn(s, ss) : ss;
+    }
+    return s;
+}
+
+// ------------------------------------------------------------------------ step bookkeeping
+__global__ void k_step_begin(DevSpecies *st, uint32_t n_species) {
+    const uint32_t s = threadIdx.x;
+    if (s < n_species) {
+        DevSpecies &d = st[s];
+        d.n0 = d.n;
+        d.sum_zi0 = d.sum_zi;
+        d.m = 0; d.n_next = 0; d.flags_step = 0;
+        d.ticket_fec = 0; d.ticket_cmp = 0; d.ticket_fused = 0; d.done_fused = 0;
+        d.acc_zi = 0; d.acc_zi2 = 0; d.captures = 0; d.near_ties = 0;
+    }
+}
+
+__global__ void k_step_end(DevGlobal *g) { g->step += 1; }
+
+// a0: derived parameters (Fig. 1 F -> A)
+__global__ void __launch_bounds__(256) k_begin(const __grid_constant__ SpK sp) {
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
+    const uint32_t n_status = (sp.capacity + SCAN_TILE - 1) / SCAN_TILE + 1;
+    for (uint32_t i = g; i < n_status; i += stride) { sp.status_fec[i] = 0ull; sp.status_cmp[i] = 0ull; }
+    if (sp.P > 1)
+        for (uint32_t i = g; i < sp.P * 5; i += stride) sp.patch_cnt[i] = 0u;
+    const DevSpecies &st = *sp.st;
+    const uint32_t N = st.n0;
+    const uint32_t *ps = sp.patch_start[st.cur];
+    for (uint32_t tab = g; tab < sp.n_tables; tab += stride) {
+        double lam;
+        if (sp.fec_model == 2) lam = fecundity_mean(sp, (double)N, sp.K, tab);
+        else if (sp.P == 1) lam = fecundity_mean(sp, (double)N, sp.K_patch ? sp.K_patch[0] : sp.K, 0);
+        else lam = fecundity_mean(sp, (double)(ps[tab + 1] - ps[tab]), sp.K_patch ? sp.K_patch[tab] : sp.K, 0);
+        sp.table_len[tab] = (uint32_t)build_poisson_table(lam, sp.tables + (size_t)tab * TMAX, TMAX);
+    }
+    if (g == 0) {
+        DevSpecies &w = *sp.st;
+        // R6: theta_t = fp32(theta0 + t*dtheta), fp64, never accumulated
+        w.theta_t = __double2float_rn(__dadd_rn(sp.theta0, __dmul_rn((double)sp.glob->step, sp.dtheta)));
+        if (sp.sel_predation) {
+            const DevSpecies &pr = sp.st_all[sp.predator];
+            const uint32_t NC = pr.n0;
+            w.n_pred0 = NC;
+            // R14: zbar_C = fp32((sum zi / N_C) * scale_C) ; A = fp32(a * N_C)
+            w.zbar_pred = NC ? __double2float_rn(__dmul_rn(__ddiv_rn((double)pr.sum_zi0, (double)NC), (double)sp.pred_scale)) : 0.0f;
+            w.attack_n = __double2float_rn(__dmul_rn(sp.attack, (double)NC));
+        }
+        if (N == 0) w.flags_step |= 2u;
+    }
+}
+
+// a1-a3: fecundity (one FEC block per adult), exclusive scan by decoupled look-back, mother fill
+__global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant__ SpK sp) {
+    __shared__ uint32_t s_tab[TMAX];
+    __shared__ uint32_t s_warp[SCAN_THREADS / 32];
+    __shared__ uint32_t s_tile;
+    __shared__ unsigned long long s_excl;
+    DevSpecies &st = *sp.st;
+    const uint32_t N = st.n0, step = sp.glob->step;
+    const uint32_t n_tiles = (N + SCAN_TILE - 1) / SCAN_TILE;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const bool one_table = sp.n_tables == 1;
+    uint32_t len0 = 0;
+    if (one_table) {
+        len0 = sp.table_len[0];
+        for (uint32_t i = tid; i < len0; i += SCAN_THREADS) s_tab[i] = sp.tables[i];
+    }
+    const uint32_t *ps = sp.patch_start[st.cur];
+    for (;;) {
+        if (tid == 0) s_tile = atomicAdd(&st.ticket_fec, 1u);
+        __syncthreads();
+        const uint32_t tile = s_tile;
+        if (tile >= n_tiles) break;
+        const uint32_t base = tile * SCAN_TILE + tid * SCAN_ITEMS;
+        uint32_t f[SCAN_ITEMS], sum = 0;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const uint32_t i = base + k;
+            f[k] = 0;
+            if (i < N) {
+                uint32_t x[4];
+                draw(sp.key, sp.species, ST_FEC, i, 0, step, x);
+                if (one_table) {
+                    f[k] = poisson_count(s_tab, len0, x[0]);
+                } else {
+                    const uint32_t tab = (sp.fec_model == 2) ? min(sp.cap[i], (uint32_t)(CAP_TABLES - 1)) : patch_of(ps, sp.P, i);
+                    f[k] = poisson_count(sp.tables + (size_t)tab * TMAX, sp.table_len[tab], x[0]);
+                }
+            }
+            sum += f[k];
+        }
+        const uint32_t incl = warp_incl_scan(sum);
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
+            const uint32_t wi = warp_incl_scan(w);
+            const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
+            const unsigned long long excl = lookback(sp.status_fec, tile, (unsigned long long)total);
+            if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;  // exclusive warp prefix
+            if (lane == 0) {
+                s_excl = excl;
+                if (tile == n_tiles - 1) {  // the last tile knows M
+                    const unsigned long long Mtot = excl + total;
+                    if (Mtot > (unsigned long long)sp.capacity) { st.m = sp.capacity; st.flags_step |= 1u; }
+                    else st.m = (uint32_t)Mtot;
+                }
+            }
+        }
+        __syncthreads();
+        unsigned long long o = s_excl + s_warp[warp] + (incl - sum);
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const uint32_t i = base + k;
+            if (i < N) {
+                sp.off[i] = (uint32_t)min(o, (unsigned long long)0xFFFFFFFFull);
+                sp.f[i] = (uint8_t)f[k];
+                for (uint32_t c = 0; c < f[k]; ++c) {
+                    const unsigned long long j = o + c;
+                    if (j < (unsigned long long)sp.capacity) sp.mother[j] = i;
+                }
+                o += f[k];
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// a3: scalar draws of each offspring: father (R2), dispersal (R15), survival uniform (R4)
+__global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) {
+    const DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
+    const uint32_t *ps = sp.patch_start[st.cur];
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
+        const uint32_t mo = sp.mother[j];
+        uint32_t x[4];
+        draw(sp.key, sp.species, ST_SCALAR, j, 0, step, x);
+        uint32_t pm = 0, base = 0, np = N;
+        if (sp.P > 1) { pm = patch_of(ps, sp.P, mo); base = ps[pm]; np = ps[pm + 1] - base; }
+        sp.father[j] = base + uniform_index(x[0], np);
+        uint32_t dest = pm;
+        if (sp.P > 1 && (unsigned long long)x[1] < sp.T_mig) dest = neighbour(pm, x[2] >> 30, sp.grid_w, sp.grid_h);
+        sp.dest[j] = dest;
+        sp.u01[j] = u01_of(x[3]);
+    }
+}
+
+// a4 (bit genomes, Poisson crossovers, R8): one thread per (offspring, gamete, chromosome)
+__global__ void __launch_bounds__(256) k_gamete_bit(const __grid_constant__ SpK sp) {
+    const DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, step = sp.glob->step;
+    const uint32_t per = 2 * sp.n_chrom;
+    const unsigned long long total = (unsigned long long)M * per;
+    const uint32_t *pop = (const uint32_t *)sp.pop[st.cur];
+    uint32_t *out = (uint32_t *)sp.offbuf;
+    const uint32_t rw = 2 * sp.W;
+    for (unsigned long long idx = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t j = (uint32_t)(idx / per), rem = (uint32_t)(idx % per);
+        const uint32_t g = rem / sp.n_chrom, c = rem % sp.n_chrom;
+        const uint32_t parent = g == 0 ? sp.mother[j] : sp.father[j];
+        const uint32_t cs = sp.chrom_start[c] >> 5, cw = sp.chrom_len[c] >> 5, clen = sp.chrom_len[c];
+        const uint32_t *h0 = pop + (size_t)parent * rw + cs, *h1 = h0 + sp.W;
+        uint32_t *o = out + (size_t)j * rw + g * sp.W + cs;
+        const uint32_t stream = g == 0 ? ST_RECOMB_M : ST_RECOMB_P;
+        uint32_t x[4], y[4];
+        draw(sp.key, sp.species, stream, j, c * 16, step, x);
+        const uint32_t nc = poisson_count(sp.T_xover + c * XMAX, sp.xover_len[c], x[0]);
+        const uint32_t phi = (x[1] >> 31) ? 0xFFFFFFFFu : 0u;
+        for (uint32_t w = 0; w < cw; ++w) {
+            uint32_t m = phi;
+            int yb = -1;
+            for (uint32_t k = 0; k < nc; ++k) {
+                uint32_t u;
+                if (k == 0) u = x[2];
+                else if (k == 1) u = x[3];
+                else {
+                    const int blk = (int)(c * 16 + 1 + (k - 2) / 4);
+                    if (blk != yb) { draw(sp.key, sp.species, stream, j, (uint32_t)blk, step, y); yb = blk; }
+                    u = y[(k - 2) & 3];
+                }
+                // crossover in interval b (between local loci b and b+1) flips every locus > b
+                const int t = (int)uniform_index(u, clen - 1) + 1 - (int)(32 * w);
+                m ^= (t <= 0) ? 0xFFFFFFFFu : (t >= 32 ? 0u : (0xFFFFFFFFu << t));
+            }
+            o[w] = (h0[w] & ~m) | (h1[w] & m);
+        }
+    }
+}
+
+// a4 (q10 genomes, per-interval draws, R7): one lane per Philox block = 4 loci; the phase is a
+// prefix parity over the gamete, done with a ballot inside lane groups of GS = min(nb, 32).
+__global__ void __launch_bounds__(256) k_gamete_q10(const __grid_constant__ SpK sp) {
+    const DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, step = sp.glob->step, L = sp.L;
+    const uint32_t nb = (L + 3) / 4;
+    uint32_t GS = 32;  // lane-group size: a power of two that holds a whole gamete, else 32
+    if (nb < 32 && (nb & (nb - 1)) == 0) GS = nb;
+    const uint32_t gpw = 32 / GS;          // gametes per warp pass
+    const uint32_t chunks = (nb + GS - 1) / GS;
+    const uint32_t lane = threadIdx.x & 31u, sub = lane / GS, sl = lane % GS;
+    const uint32_t gmask = (GS == 32) ? 0xFFFFFFFFu : (((1u << GS) - 1u) << (sub * GS));
+    const uint32_t lt = gmask & ((1u << lane) - 1u);
+    const unsigned long long n_gam = 2ull * M;
+    const unsigned long long warp0 = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned long long n_warps = ((unsigned long long)gridDim.x * blockDim.x) >> 5;
+    const int16_t *pop = (const int16_t *)sp.pop[st.cur];
+    int16_t *out = (int16_t *)sp.offbuf;
+    for (unsigned long long gb = warp0 * gpw; gb < n_gam; gb += n_warps * gpw) {
+        const unsigned long long gi = gb + sub;
+        const bool live = gi < n_gam;
+        const uint32_t j = (uint32_t)(gi >> 1), g = (uint32_t)(gi & 1);
+        uint32_t parent = 0;
+        if (live) parent = g == 0 ? sp.mother[j] : sp.father[j];
+        const int16_t *h0 = pop + (size_t)parent * 2 * L, *h1 = h0 + L;
+        int16_t *o = out + (size_t)j * 2 * L + (size_t)g * L;
+        uint32_t carry = 0;
+        for (uint32_t ch = 0; ch < chunks; ++ch) {
+            const uint32_t blk = ch * GS + sl;
+            const bool act = live && blk < nb;
+            uint32_t p[4] = {0, 0, 0, 0};
+            if (act) {
+                uint32_t x[4];
+                draw(sp.key, sp.species, g == 0 ? ST_RECOMB_M : ST_RECOMB_P, j, blk, step, x);
+                uint32_t run = 0;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t l = 4 * blk + k;
+                    if (l < L) run ^= (x[k] < sp.T_recomb[l]) ? 1u : 0u;
+                    p[k] = run;
+                }
+            }
+            const uint32_t bal = __ballot_sync(0xffffffffu, p[3] != 0);
+            const uint32_t excl = (__popc(bal & lt) & 1u) ^ carry;
+            carry ^= __popc(bal & gmask) & 1u;
+            if (act) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t l = 4 * blk + k;
+                    if (l < L) o[l] = (excl ^ p[k]) ? h1[l] : h0[l];
+                }
+            }
+        }
+    }
+}
+
+// a4: sparse mutation (R9), one thread per (offspring, gamete), applied after recombination
+__global__ void __launch_bounds__(256) k_mutate(const __grid_constant__ SpK sp) {
+    const DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, step = sp.glob->step, L = sp.L;
+    const unsigned long long total = 2ull * M;
+    for (unsigned long long gi = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; gi < total;
+         gi += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t j = (uint32_t)(gi >> 1), g = (uint32_t)(gi & 1);
+        const uint32_t stream = g == 0 ? ST_MUT_M : ST_MUT_P;
+        uint32_t x[4];
+        draw(sp.key, sp.species, stream, j, 0, step, x);
+        const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
+        for (uint32_t k = 0; k < nm; ++k) {
+            if (k > 0) draw(sp.key, sp.species, stream, j, k, step, x);
+            const uint32_t pos = uniform_index(x[1], L);
+            if (sp.kind == 0) {
+                uint32_t *row = (uint32_t *)sp.offbuf + (size_t)j * 2 * sp.W + (size_t)g * sp.W;
+                row[pos >> 5] ^= 1u << (pos & 31u);
+            } else {
+                int16_t *row = (int16_t *)sp.offbuf + (size_t)j * 2 * L + (size_t)g * L;
+                int v = (int)row[pos] + normal_delta(sp.T_norm, sp.R_norm, x[2]);
+                v = max(-32767, min(32767, v));
+                row[pos] = (int16_t)v;
+            }
+        }
+    }
+}
+
+// integer phenotype of one row, computed by a whole warp (R10)
+__device__ __forceinline__ int32_t warp_row_zi(const SpK &sp, const uint8_t *row) {
+    const uint32_t lane = threadIdx.x & 31u;
+    int32_t acc = 0;
+    const uint32_t *w = (const uint32_t *)row;
+    const uint32_t nw = sp.row_bytes >> 2;
+    if (sp.kind == 0) {
+        for (uint32_t i = lane; i < nw; i += 32) acc += __popc(w[i]);
+    } else {
+        for (uint32_t i = lane; i < nw; i += 32) {
+            const uint32_t v = w[i];
+            acc += (int32_t)(int16_t)(v & 0xFFFFu) + (int32_t)(int16_t)(v >> 16);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    return sp.kind == 0 ? 2 * acc - 2 * (int32_t)sp.L : acc;
+}
+
+// a5: additive genotype -> phenotype map, one warp per offspring
+__global__ void __launch_bounds__(256) k_phenotype(const __grid_constant__ SpK sp) {
+    const uint32_t M = sp.st->m;
+    const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t j = warp0; j < M; j += nw) {
+        const int32_t zi = warp_row_zi(sp, sp.offbuf + (size_t)j * sp.row_bytes);
+        if ((threadIdx.x & 31u) == 0) sp.zi[j] = zi;
+    }
+}
+
+// phenotypes of the current adults (write_state / read_state): zi[] and their sum
+__global__ void __launch_bounds__(256) k_adult_zi(const __grid_constant__ SpK sp, uint32_t n, int accumulate) {
+    const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    long long acc = 0;
+    for (uint32_t i = warp0; i < n; i += nw) {
+        const int32_t zi = warp_row_zi(sp, sp.pop[sp.st->cur] + (size_t)i * sp.row_bytes);
+        if ((threadIdx.x & 31u) == 0) { sp.zi[i] = zi; acc += zi; }
+    }
+    if (accumulate && (threadIdx.x & 31u) == 0 && acc != 0)
+        atomicAdd((unsigned long long *)&sp.st->sum_zi, (unsigned long long)acc);
+}
+
+// a6: selection / survival (Fig. 1D), fp32; captures credited to a uniformly drawn predator
+__global__ void __launch_bounds__(256) k_survival(const __grid_constant__ SpK sp) {
+    DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, step = sp.glob->step;
+    unsigned int ties = 0, caps = 0;
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
+        const float z = __fmul_rn((float)sp.zi[j], sp.pheno_scale);
+        const float u = sp.u01[j];
+        const float theta = sp.theta_patch ? sp.theta_patch[sp.dest[j]] : st.theta_t;
+        bool captured;
+        const float s = survival_prob(sp, z, theta, u, captured);
+        sp.s[j] = s;
+        sp.alive[j] = (u < s) ? 1 : 0;
+        sp.captured[j] = captured ? 1 : 0;
+        if (fabsf(__fsub_rn(u, s)) < 1e-6f) ++ties;
+        if (captured) {
+            ++caps;
+            if (st.n_pred0) {
+                uint32_t y[4];
+                draw(sp.key, sp.species, ST_SCALAR, j, 1, step, y);
+                atomicAdd(&sp.cap_pred[uniform_index(y[0], st.n_pred0)], 1u);
+            }
+        }
+    }
+    if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
+    if (caps) atomicAdd(&st.captures, (unsigned long long)caps);
+}
+
+// a7 (unstructured): stable compaction positions by decoupled look-back + survivor reductions
+__global__ void __launch_bounds__(SCAN_THREADS) k_cmp_scan(const __grid_constant__ SpK sp) {
+    __shared__ uint32_t s_warp[SCAN_THREADS / 32];
+    __shared__ uint32_t s_tile;
+    __shared__ unsigned long long s_excl;
+    DevSpecies &st = *sp.st;
+    const uint32_t M = st.m;
+    const uint32_t n_tiles = (M + SCAN_TILE - 1) / SCAN_TILE;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    long long a1 = 0, a2 = 0;
+    for (;;) {
+        if (tid == 0) s_tile = atomicAdd(&st.ticket_cmp, 1u);
+        __syncthreads();
+        const uint32_t tile = s_tile;
+        if (tile >= n_tiles) break;
+        const uint32_t base = tile * SCAN_TILE + tid * SCAN_ITEMS;
+        uint32_t a[SCAN_ITEMS], sum = 0;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const uint32_t j = base + k;
+            a[k] = (j < M) ? sp.alive[j] : 0u;
+            sum += a[k];
+            if (a[k]) { const long long z = sp.zi[j]; a1 += z; a2 += z * z; }
+        }
+        const uint32_t incl = warp_incl_scan(sum);
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
+            const uint32_t wi = warp_incl_scan(w);
+            const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
+            const unsigned long long excl = lookback(sp.status_cmp, tile, (unsigned long long)total);
+            if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;
+            if (lane == 0) {
+                s_excl = excl;
+                if (tile == n_tiles - 1) st.n_next = (uint32_t)(excl + total);
+            }
+        }
+        __syncthreads();
+        uint32_t o = (uint32_t)s_excl + s_warp[warp] + (incl - sum);
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const uint32_t j = base + k;
+            if (j < M) { sp.pos[j] = a[k] ? o : 0xFFFFFFFFu; o += a[k]; }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o); }
+    if (lane == 0 && (a1 != 0 || a2 != 0)) {
+        atomicAdd((unsigned long long *)&st.acc_zi, (unsigned long long)a1);
+        atomicAdd((unsigned long long *)&st.acc_zi2, (unsigned long long)a2);
+    }
+}
+
+// a7: move the surviving rows to their positions in the other buffer, one warp per row
+__global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK sp) {
+    const DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, lane = threadIdx.x & 31u;
+    const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    uint8_t *dst = sp.pop[st.cur ^ 1u];
+    for (uint32_t j = warp0; j < M; j += nw) {
+        const uint32_t p = sp.pos[j];
+        if (p == 0xFFFFFFFFu) continue;
+        const uint4 *src = (const uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes);
+        uint4 *d = (uint4 *)(dst + (size_t)p * sp.row_bytes);
+        for (uint32_t i = lane; i < sp.row_u4; i += 32) d[i] = src[i];
+    }
+}
+
+// ---- a7 (patches, R15): the next generation is ordered by (destination patch, j).  Offspring of
+// natal patch p are a contiguous j-range and land in p or one of its 4 torus neighbours, so the
+// stable order is: for destination d, the sources {d, neighbours(d)} in increasing patch index,
+// each in j order.  slot = index of the destination in p's de-duplicated list [p, nb0..nb3].
+__device__ __forceinline__ uint32_t dest_slot(uint32_t p, uint32_t dest, uint32_t gw, uint32_t gh) {
+    if (dest == p) return 0;
+#pragma unroll
+    for (uint32_t k = 0; k < 4; ++k)
+        if (neighbour(p, k, gw, gh) == dest) return k + 1;
+    return 0;
+}
+
+__device__ __forceinline__ void patch_offspring_range(const SpK &sp, const uint32_t *ps, uint32_t p, uint32_t N,
+                                                      uint32_t M, uint32_t &j0, uint32_t &j1) {
+    const uint32_t a0 = ps[p], a1 = ps[p + 1];
+    j0 = (a0 < N) ? min(sp.off[a0], M) : M;
+    j1 = (a1 < N) ? min(sp.off[a1], M) : M;
+}
+
+// counts of survivors per (natal patch, slot); one CTA per natal patch
+__global__ void __launch_bounds__(256) k_patch_count(const __grid_constant__ SpK sp) {
+    __shared__ uint32_t s_cnt[5];
+    const DevSpecies &st = *sp.st;
+    const uint32_t *ps = sp.patch_start[st.cur];
+    for (uint32_t p = blockIdx.x; p < sp.P; p += gridDim.x) {
+        if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
+        __syncthreads();
+        uint32_t j0, j1;
+        patch_offspring_range(sp, ps, p, st.n0, st.m, j0, j1);
+        for (uint32_t j = j0 + threadIdx.x; j < j1; j += blockDim.x)
+            if (sp.alive[j]) atomicAdd(&s_cnt[dest_slot(p, sp.dest[j], sp.grid_w, sp.grid_h)], 1u);
+        __syncthreads();
+        if (threadIdx.x < 5) sp.patch_cnt[p * 5 + threadIdx.x] = s_cnt[threadIdx.x];
+        __syncthreads();
+    }
+}
+
+// next patch_start and the base position of every (natal patch, slot) group; single CTA
+__global__ void __launch_bounds__(1024) k_patch_base(const __grid_constant__ SpK sp) {
+    __shared__ uint32_t s_part[1024];
+    DevSpecies &st = *sp.st;
+    uint32_t *psn = sp.patch_start[st.cur ^ 1u];
+    const uint32_t P = sp.P, gw = sp.grid_w, gh = sp.grid_h, tid = threadIdx.x;
+    const uint32_t per = (P + 1023) / 1024;
+    const uint32_t d0 = min(tid * per, P), d1 = min(d0 + per, P);
+    // sources of destination d: (p', slot) pairs, unique per p', sorted by p'
+    auto sources = [&](uint32_t d, uint32_t (&sp_)[5], uint32_t (&ss_)[5]) -> int {
+        int n = 0;
+        sp_[n] = d; ss_[n] = 0; ++n;
+        for (uint32_t k = 0; k < 4; ++k) {
+            const uint32_t pp = neighbour(d, (k + 2) & 3u, gw, gh);  // opposite direction
+            if (pp == d) continue;  // d is its own neighbour: counted in slot 0
+            if (neighbour(pp, k, gw, gh) != d) continue;
+            const uint32_t slot = dest_slot(pp, d, gw, gh);
+            bool dup = false;
+            for (int i = 0; i < n; ++i) dup |= (sp_[i] == pp);
+            if (!dup) { sp_[n] = pp; ss_[n] = slot; ++n; }
+        }
+        for (int i = 1; i < n; ++i)
+            for (int k2 = i; k2 > 0 && sp_[k2] < sp_[k2 - 1]; --k2) {
+                uint32_t t = sp_[k2]; sp_[k2] = sp_[k2 - 1]; sp_[k2 - 1] = t;
+                t = ss_[k2]; ss_[k2] = ss_[k2 - 1]; ss_[k2 - 1] = t;
+            }
+        return n;
+    };
+    uint32_t mine = 0;
+    for (uint32_t d = d0; d < d1; ++d) {
+        uint32_t a[5], b[5];
+        const int n = sources(d, a, b);
+        for (int i = 0; i < n; ++i) mine += sp.patch_cnt[a[i] * 5 + b[i]];
+    }
+    s_part[tid] = mine;
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t run = 0;
+        for (int i = 0; i < 1024; ++i) { const uint32_t t = s_part[i]; s_part[i] = run; run += t; }
+        st.n_next = run;
+        psn[P] = run;
+    }
+    __syncthreads();
+    uint32_t run = s_part[tid];
+    for (uint32_t d = d0; d < d1; ++d) {
+        psn[d] = run;
+        uint32_t a[5], b[5];
+        const int n = sources(d, a, b);
+        for (int i = 0; i < n; ++i) {
+            sp.patch_base[a[i] * 5 + b[i]] = run;
+            run += sp.patch_cnt[a[i] * 5 + b[i]];
+        }
+    }
+}
+
+// positions of the survivors of each natal patch (j order within each slot) + reductions
+__global__ void __launch_bounds__(256) k_patch_pos(const __grid_constant__ SpK sp) {
+    __shared__ uint32_t s_w[8][5];
+    __shared__ uint32_t s_run[5];
+    DevSpecies &st = *sp.st;
+    const uint32_t *ps = sp.patch_start[st.cur];
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    long long a1 = 0, a2 = 0;
+    for (uint32_t p = blockIdx.x; p < sp.P; p += gridDim.x) {
+        if (tid < 5) s_run[tid] = sp.patch_base[p * 5 + tid];
+        uint32_t j0, j1;
+        patch_offspring_range(sp, ps, p, st.n0, st.m, j0, j1);
+        __syncthreads();
+        for (uint32_t c0 = j0; c0 < j1; c0 += 256) {
+            const uint32_t j = c0 + tid;
+            const bool al = j < j1 && sp.alive[j];
+            const uint32_t slot = al ? dest_slot(p, sp.dest[j], sp.grid_w, sp.grid_h) : 7u;
+            uint32_t rank = 0;
+#pragma unroll
+            for (uint32_t k = 0; k < 5; ++k) {
+                const uint32_t bal = __ballot_sync(0xffffffffu, slot == k);
+                if (slot == k) rank = __popc(bal & ((1u << lane) - 1u));
+                if (lane == 0) s_w[warp][k] = __popc(bal);
+            }
+            __syncthreads();
+            if (al) {
+                uint32_t o = s_run[slot] + rank;
+                for (uint32_t w = 0; w < warp; ++w) o += s_w[w][slot];
+                sp.pos[j] = o;
+                const long long z = sp.zi[j]; a1 += z; a2 += z * z;
+            } else if (j < j1) sp.pos[j] = 0xFFFFFFFFu;
+            __syncthreads();
+            if (tid < 5) { uint32_t t = 0; for (int w = 0; w < 8; ++w) t += s_w[w][tid]; s_run[tid] += t; }
+            __syncthreads();
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o); }
+    if (lane == 0 && (a1 != 0 || a2 != 0)) {
+        atomicAdd((unsigned long long *)&st.acc_zi, (unsigned long long)a1);
+        atomicAdd((unsigned long long *)&st.acc_zi2, (unsigned long long)a2);
+    }
+}
+
+// a9: counts stay on the device; log entry; buffer flip
+__global__ void k_end(const __grid_constant__ SpK sp) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    DevSpecies &st = *sp.st;
+    const uint32_t nn = st.n_next;
+    LogEntry &e = sp.log[st.log_pos % sp.log_capacity];
+    e.n_t = st.n0; e.m_t = st.m; e.n_next = nn;
+    e.sum_zi = st.acc_zi; e.sum_zi2 = st.acc_zi2;
+    e.captures = st.captures; e.near_ties = st.near_ties;
+    e.flags = st.flags_step; e.step = sp.glob->step;
+    st.log_pos += 1;
+    if (st.flags_step) atomicOr(&sp.glob->flags, st.flags_step);
+    st.n = nn;
+    st.sum_zi = st.acc_zi;
+    st.cur ^= 1u;
+    if (sp.P == 1) { uint32_t *psn = sp.patch_start[st.cur]; psn[0] = 0; psn[1] = nn; }
+}
+
+}  // namespace spegg

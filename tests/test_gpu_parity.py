@@ -1,0 +1,130 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C ABI, against the oracle
+element by element on the same seeded inputs.  Bar: bit-exact for genomes, indices, counts and
+decisions; survival probabilities are produced by the same specified fp32 sequence on both sides
+(so they are bit-equal, which implies north_star's 1e-6 relative bound); decisions with
+|u01 - s| < 1e-6 are counted and reported in the log (`near_ties`)."""
+import numpy as np
+import pytest
+
+import parity
+from paper_1603_09255_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_1603_09255_b200 import binding as b
+    b.load()
+    return b
+
+
+@pytest.mark.parametrize("which,scale,grid,steps", [
+    (1, 1.0, None, 6),        # C1 at full size
+    (2, 0.05, None, 3),       # C2: 5,000 individuals, 4 chromosomes
+    (3, 0.02, None, 3),       # C3: 20,000 individuals: several tiles and a ragged tail
+    (4, 0.004, None, 3),      # C4: two species
+    (5, 0.03, (6, 5), 3),     # C5: 30 patches on a 6x5 torus
+])
+def test_per_step_parity_debug(oracle_mod, binding, which, scale, grid, steps):
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    parity.per_step_parity(oracle_mod, binding, cfg, steps, debug=True)
+
+
+@pytest.mark.parametrize("which,scale,grid,steps", [
+    (1, 1.0, None, 4), (3, 0.013, None, 3), (5, 0.03, (4, 4), 2), (4, 0.004, None, 2), (2, 0.03, None, 2)])
+def test_per_step_parity_fast_path(oracle_mod, binding, which, scale, grid, steps):
+    # debug off: the production (fused where available) kernels; state and log must still match
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    parity.per_step_parity(oracle_mod, binding, cfg, steps, debug=False)
+
+
+@pytest.mark.parametrize("which,scale,grid,steps", [(1, 1.0, None, 100), (3, 0.01, None, 40), (5, 0.02, (5, 4), 25),
+                                                    (4, 0.003, None, 25), (2, 0.02, None, 30)])
+def test_free_running_trajectory(oracle_mod, binding, which, scale, grid, steps):
+    # no re-seeding: because every decision is taken in identical arithmetic the whole trajectory
+    # (N_t, M_t, sums of phenotypes, genomes) must stay bit-identical
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    orc.step(steps)
+    sim.step(steps)
+    for s in range(len(cfg["species"])):
+        parity.assert_logs_equal(sim.read_log(s), orc.log(s), tag="species %d" % s)
+    parity.assert_state_equal(sim, orc, cfg)
+    assert sim.step_counter == orc.step_counter == steps
+    sim.close()
+
+
+def test_step_n_equals_n_steps_and_checkpoint(binding):
+    cfg = workloads.config(3, scale=0.01)
+    a = binding.Sim(cfg)
+    b = binding.Sim(cfg)
+    parity.load_initial(a, cfg)
+    parity.load_initial(b, cfg)
+    a.step(4)
+    b.step(1); b.step(1)
+    rows, ps, _ = b.read_state(0)
+    c = binding.Sim(cfg)                     # resume from a checkpoint in a fresh handle
+    c.write_state(0, rows, None, 2)
+    c.step(2)
+    ra, _, za = a.read_state(0)
+    rc, _, zc = c.read_state(0)
+    assert np.array_equal(ra, rc) and np.array_equal(za, zc)
+    # write_state(read_state()) is the identity
+    c.write_state(0, rc, None, 4)
+    assert np.array_equal(c.read_state(0)[0], rc)
+    for s in (a, b, c):
+        s.close()
+
+
+def test_overflow_and_extinction(oracle_mod, binding):
+    cfg = workloads.config(1)
+    cfg["species"][0]["capacity"] = 1024
+    cfg["species"][0]["K"] = 1e9
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=True)
+    sim = binding.Sim(cfg)
+    parity.load_initial(sim, cfg)
+    sim.step(1)
+    assert sim.status() & 1
+    sim.close()
+    cfg = workloads.config(1)
+    cfg["species"][0]["fec_a"] = 0.0
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    orc.step(3); sim.step(3)
+    parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+    assert sim.n(0) == 0 and sim.status() == orc.flags and sim.status() & 2
+    sim.close()
+
+
+def test_empty_population_and_device_rows(binding):
+    import torch
+    cfg = workloads.config(3, scale=0.004)
+    sim = binding.Sim(cfg)
+    sim.step(2)                               # nothing loaded: N = 0, steps are no-ops
+    assert sim.n(0) == 0
+    rows = workloads.initial_rows(cfg, 0)
+    dev = torch.from_numpy(rows.view(np.int32)).cuda()
+    sim.write_state(0, dev, None, 0)          # rows given as a DEVICE pointer
+    other = binding.Sim(cfg)
+    other.write_state(0, rows, None, 0)
+    sim.step(2); other.step(2)
+    assert np.array_equal(sim.read_state(0)[0], other.read_state(0)[0])
+    sim.close(); other.close()
+
+
+def test_bad_parameters_are_rejected(binding):
+    cfg = workloads.config(3, scale=0.001)
+    cfg["species"][0]["chrom_len"] = [100, 924]   # bit chromosomes must be word-aligned
+    cfg["species"][0]["xover_mean"] = [1.0, 1.0]
+    with pytest.raises(binding.SpeggError):
+        binding.workspace_bytes(cfg)
+    cfg = workloads.config(1)
+    cfg["species"][0]["mu"] = 1.5
+    with pytest.raises(binding.SpeggError):
+        binding.workspace_bytes(cfg)
