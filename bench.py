@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py -- individual-generations/s of the sPEGG per-time-step update on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+One "step" is one pass of the whole hot path (Fig. 1 A-F: fecundity + scan + parents, gametes,
+phenotype, survival, compaction, reductions) over the whole population.  Workload at N=1:
+BASELINE.json's metric configuration, config 3 (N0 = K = 1,000,000 diploids, L = 1,024 bit-packed
+loci), synthetic seeded input.  Prints ONE JSON line (see the contract in the task statement):
+`value` is device-timed with inputs resident in HBM, `e2e` goes through the C ABI with host
+buffers, `roofline` is the dominant kernel against the measured HBM copy bandwidth, `cpu_baseline`
+is the oracle timed on the host cores on a bounded sample.
+
+N > 1 (torchrun): a single panmictic population does not shard (every father row may live on any
+GPU), so ranks run independent replicas with different seeds -- "replicas only", weak scaling, no
+data-path collective; NCCL is used for the barrier and the max-over-ranks time only.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "individual-generations/sec"
+UNIT = "individual-generations/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples SM clocks and throttle reasons with nvidia-smi while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+                for nm, v in zip(names, r[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def workload(which, seed_offset=0):
+    from paper_1603_09255_b200 import workloads
+    cfg = workloads.config(which)
+    cfg["seed"] = cfg["seed"] + 1000 * seed_offset
+    return cfg
+
+
+def describe(cfg):
+    sp = cfg["species"][0]
+    return "%s: N0=K=%d diploids, L=%d %s loci, %d chromosomes, %s" % (
+        cfg["name"], cfg["n0"][0], sp["n_loci"], "bit-packed" if sp["kind"] == "bit" else "2^-10-quantised",
+        len(sp["chrom_len"]), "patches %dx%d" % cfg["grid"] if cfg["grid"] != (1, 1) else "one panmictic population")
+
+
+def row_bytes(sp):
+    return 2 * (sp["n_loci"] // 32) * 4 if sp["kind"] == "bit" else 4 * sp["n_loci"]
+
+
+def alg_bytes(cfg, log, kernel_only):
+    """Algorithmic bytes: G*(N_t + M_t + N_{t+1}) + 8*M_t for the gamete kernel
+    (+ 4*N_t for the scan when the whole step is counted), summed over the given log entries."""
+    G = row_bytes(cfg["species"][0])
+    tot = 0
+    for e in log:
+        tot += G * (e["n_t"] + e["m_t"] + e["n_next"]) + 8 * e["m_t"]
+        if not kernel_only:
+            tot += 4 * e["n_t"]
+    return tot
+
+
+def oracle_run(cfg, n_steps, warm=0):
+    """Times the oracle as it stands on the host cores (one thread)."""
+    import oracle
+    from paper_1603_09255_b200 import workloads
+    o = oracle.Oracle(cfg)
+    for s in range(len(cfg["species"])):
+        o.write_state(s, workloads.initial_rows(cfg, s), workloads.initial_patch_start(cfg, s), 0)
+    if warm:
+        o.step(warm)
+    k0 = len(o.log(0))
+    t0 = time.perf_counter()
+    o.step(n_steps)
+    dt = time.perf_counter() - t0
+    units = sum(sum(e["n_t"] for e in o.log(s)[k0:]) for s in range(len(cfg["species"])))
+    return units, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle is this tier's reference arm (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1603_09255_b200 import workloads
+    full = workload(args.config)
+    # bounded sample: shrink the population so that K+W oracle steps end within ~2 minutes
+    per_step_s = 120.0 / max(1, args.steps + args.warmup)
+    scale = min(1.0, max(0.001, per_step_s * 7.0e4 / full["n0"][0]))
+    cfg = workloads.config(args.config, scale=scale)
+    units, dt = oracle_run(cfg, args.steps, warm=args.warmup)
+    val = units / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": describe(full), "sample": "population scaled by %.4g (N0=%d) per step" % (scale, cfg["n0"][0])},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": "%d steps of the workload at N0=%d (scale %.4g)" % (args.steps, cfg["n0"][0], scale)},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    from paper_1603_09255_b200 import binding, workloads
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    binding.load()  # fails loudly if the CUDA extension is missing
+
+    cfg = workload(args.config, seed_offset=rank)
+    n_sp = len(cfg["species"])
+    sim = binding.Sim(cfg, debug=False, log_capacity=max(4096, args.steps * 3 + args.warmup + 64), device=str(dev))
+    rows0 = [workloads.initial_rows(cfg, s) for s in range(n_sp)]
+    ps0 = [workloads.initial_patch_start(cfg, s) for s in range(n_sp)]
+    for s in range(n_sp):
+        sim.write_state(s, rows0[s], ps0[s], 0)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-timed run: inputs resident in HBM, K graph replays, no host sync inside
+    sim.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    k0 = len(sim.read_log(0))
+    barrier()
+    with torch.cuda.stream(sim.stream):
+        ev0.record(sim.stream)
+        sim.step(args.steps)
+        ev1.record(sim.stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    logs = [sim.read_log(s)[k0:k0 + args.steps] for s in range(n_sp)]
+    units = sum(sum(e["n_t"] for e in lg) for lg in logs)
+    offspring = sum(sum(e["m_t"] for e in lg) for lg in logs)
+    flags = sim.status()
+
+    # ---- dominant kernel timed alone with CUDA events on its own stream (direct launches)
+    kt_steps = min(args.steps, 100)
+    sim.kernel_timing(True)
+    kl0 = len(sim.read_log(0))
+    sim.step(kt_steps)
+    k_ms, k_n = sim.kernel_timing(False)
+    klog = sim.read_log(0)[kl0:kl0 + kt_steps]
+    k_bytes = alg_bytes(cfg, klog, kernel_only=True) / max(1, len(klog))
+
+    # ---- end to end through the C ABI with HOST buffers: upload, K x (step + read of the step's
+    # result), download -- all inside the timed region
+    e2e_steps = min(args.steps, 50)
+    pinned = [torch.from_numpy(r.view(np.int32).reshape(-1) if r.dtype == np.uint32 else r.view(np.int16).reshape(-1)).pin_memory() for r in rows0]
+    host_rows = [p.numpy().view(rows0[s].dtype).reshape(rows0[s].shape) for s, p in enumerate(pinned)]
+    outs = [torch.empty(int(cfg["species"][s]["capacity"]) * sim.row_shape[s], dtype=torch.int32 if rows0[s].dtype == np.uint32 else torch.int16).pin_memory() for s in range(n_sp)]
+    out_np = [o.numpy().view(rows0[s].dtype).reshape(-1, sim.row_shape[s]) for s, o in enumerate(outs)]
+    barrier()
+    t0 = time.perf_counter()
+    for s in range(n_sp):
+        sim.write_state(s, host_rows[s], ps0[s], 0)
+    h2d = sum(r.nbytes for r in host_rows)
+    e_units, d2h = 0, 0
+    for _ in range(e2e_steps):
+        sim.step(1)
+        for s in range(n_sp):
+            e = sim.read_log(s)[-1]      # device -> host read of the step's result (64-byte entry)
+            e_units += e["n_t"]
+            d2h += 64
+    for s in range(n_sp):
+        r, _, _ = sim.read_state(s, want_zi=False, out=out_np[s])
+        d2h += r.nbytes
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+
+    # ---- reduce over ranks: max time, summed units
+    if dist is not None:
+        t = torch.tensor([ms, e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        u = torch.tensor([units, e_units, offspring], device=dev, dtype=torch.float64)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        ms, e2e_s = float(t[0]), float(t[1])
+        units, e_units, offspring = float(u[0]), float(u[1]), float(u[2])
+    launches = sim.launches_per_step() * args.steps
+
+    if rank == 0:
+        peak, peak_src = load_peaks()
+        achieved = k_bytes / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
+        step_bytes = alg_bytes(cfg, logs[0], kernel_only=False) / max(1, len(logs[0]))
+        # oracle on a bounded sample of the same workload: ~10-30 s of CPU work
+        cb_cfg = workload(args.config)
+        cb_steps = 1 if cb_cfg["n0"][0] >= 500_000 else max(1, int(1.0e6 / cb_cfg["n0"][0]))
+        cb_units, cb_dt = oracle_run(cb_cfg, cb_steps)
+        line = {
+            "metric": METRIC, "value": units / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+            "config": {"workload": describe(cfg), "parallelism": "replicas only x%d" % world,
+                       "l2": "inputs larger than L2 (two %d MB population buffers vs 126 MB L2)" % (
+                           cfg["species"][0]["capacity"] * row_bytes(cfg["species"][0]) // 2 ** 20),
+                       "mean_N_t": units / args.steps / world, "mean_M_t": offspring / args.steps / world,
+                       "flags": flags, "offspring_per_s": offspring / (ms * 1e-3),
+                       "step_alg_bytes": step_bytes,
+                       "step_frac_of_peak": step_bytes / (ms / args.steps * 1e-3) / 1e9 / peak},
+            "clocks": clocks,
+            "e2e": {"value": e_units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d / e2e_steps,
+                    "d2h_bytes_per_step": d2h / e2e_steps, "steps": e2e_steps,
+                    "what": "spegg_write_state(host) + K x (spegg_step(1) + spegg_read_log) + spegg_read_state(host)"},
+            "gpu_launches": launches,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": TRAFFIC_BYTES.get(cfg["name"]),
+                         "kernel": "fused gamete+phenotype+survival+compaction" if k_n else "none",
+                         "kernel_ms": k_ms, "kernel_launches_timed": k_n, "alg_bytes_per_launch": k_bytes,
+                         "peak_source": peak_src},
+            "cpu_baseline": {"value": cb_units / cb_dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": "%d step(s) of the full workload (N0=%d), %.1f s" % (cb_steps, cb_cfg["n0"][0], cb_dt)},
+        }
+        print(json.dumps(line))
+    sim.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+# `ncu --set full` capture summarised under profiles/ (None until a capture exists).
+TRAFFIC_BYTES = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -11,8 +11,8 @@
 #include <vector>
 
 #include "../../include/spegg.h"
-#include "spegg_fused.cuh"
 #include "spegg_kernels.cuh"
+#include "spegg_fused.cuh"
 
 using namespace spegg;
 
@@ -91,7 +91,7 @@ struct Carver {
 };
 
 struct SpeciesLayout {
-    uint64_t pop[2], patch_start[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
+    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask, f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
     uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, K_patch, theta_patch;
     uint32_t norm_len, n_tables, row_bytes;
@@ -172,8 +172,12 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.row_bytes = row_bytes_of(q);
         l.n_tables = q.fecundity_model == SPEGG_FEC_CAPTURES ? CAP_TABLES : (uint32_t)P;
         const uint64_t n_status = (cap + SCAN_TILE - 1) / SCAN_TILE + 1;
-        l.pop[0] = c.take(cap * l.row_bytes);
-        l.pop[1] = c.take(cap * l.row_bytes);
+        const uint64_t cap32 = (cap + 31) / 32 * 32;  // fused path: one 32-row slab per offspring chunk
+        l.pop[0] = c.take(cap32 * l.row_bytes);
+        l.pop[1] = c.take(cap32 * l.row_bytes);
+        l.rowptr[0] = c.take(cap32 * 4);
+        l.rowptr[1] = c.take(cap32 * 4);
+        l.chunk_mask = c.take((cap / 32 + 2) * 4);
         l.patch_start[0] = c.take((P + 1) * 4);
         l.patch_start[1] = c.take((P + 1) * 4);
         l.f = c.take(cap);
@@ -192,7 +196,7 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
         l.table_len = c.take((uint64_t)l.n_tables * 4);
         l.status_fec = c.take(n_status * 8);
-        l.status_cmp = c.take(n_status * 8);
+        l.status_cmp = c.take((cap / 32 + 2) * 8);  // fused tiles are 32 offspring
         l.patch_cnt = c.take(P * 5 * 4);
         l.patch_base = c.take(P * 5 * 4);
         l.log = c.take((uint64_t)logcap * sizeof(LogEntry));
@@ -268,9 +272,11 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
         k_begin<<<std::max(1u, std::min(G, (k.n_tables + 255) / 256 + 8)), 256, 0, s->stream>>>(k); ++nl;
         k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
         if (fused_ok(s, h)) {
+            launch_offspring_draws(k, G, s->stream); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             launch_fused_bit(k, G, s->stream); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
+            launch_index(k, G, s->stream); ++nl;
         } else {
             k_scalar<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
@@ -433,6 +439,8 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.T_norm = at<uint32_t>(s, l.T_norm); k.R_norm = h.R_norm;
         k.pop[0] = at<uint8_t>(s, l.pop[0]); k.pop[1] = at<uint8_t>(s, l.pop[1]);
         k.patch_start[0] = at<uint32_t>(s, l.patch_start[0]); k.patch_start[1] = at<uint32_t>(s, l.patch_start[1]);
+        k.rowptr[0] = at<uint32_t>(s, l.rowptr[0]); k.rowptr[1] = at<uint32_t>(s, l.rowptr[1]);
+        k.chunk_mask = at<uint32_t>(s, l.chunk_mask);
         k.f = at<uint8_t>(s, l.f); k.off = at<uint32_t>(s, l.off);
         k.mother = at<uint32_t>(s, l.mother); k.father = at<uint32_t>(s, l.father);
         k.dest = at<uint32_t>(s, l.dest); k.pos = at<uint32_t>(s, l.pos);
@@ -446,6 +454,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.st = s->d_st + si; k.st_all = s->d_st; k.glob = s->d_glob;
         k.log = at<LogEntry>(s, l.log); k.log_capacity = s->log_capacity;
         k.debug = p->debug;
+        k.phys_parents = fused_ok(s, h) ? 1u : 0u;
     }
     for (uint32_t si = 0; si < p->n_species; ++si)
         if (s->sp[si].p.sel_predation) s->sp[si].k.cap_pred = s->sp[s->sp[si].p.predator_species].k.cap;
@@ -498,7 +507,10 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
     CU(cudaMemcpy(&g, s->d_glob, sizeof g, cudaMemcpyDeviceToHost));
     g.step = step;
     CU(cudaMemcpyAsync(s->d_glob, &g, sizeof g, cudaMemcpyHostToDevice, s->stream));
-    if (n) k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1);
+    if (n) {
+        k_iota<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k.rowptr[cur], (uint32_t)n);
+        k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1);
+    }
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(s->stream));
     return SPEGG_OK;
@@ -531,8 +543,13 @@ int spegg_read_state(spegg_sim *s, uint32_t species, uint64_t *n, uint32_t *step
     if (step) *step = g.step;
     if (genomes_out) {
         if (cap_bytes < (uint64_t)st.n * h.k.row_bytes) return SPEGG_ERANGE;
-        CU(cudaMemcpy(genomes_out, h.k.pop[st.cur], (size_t)st.n * h.k.row_bytes,
-                      genomes_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+        if (st.n) {  // rows in logical order: gather through rowptr into the staging buffer
+            k_gather_rows<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, st.n, h.k.offbuf);
+            CU(cudaGetLastError());
+            CU(cudaStreamSynchronize(s->stream));
+            CU(cudaMemcpy(genomes_out, h.k.offbuf, (size_t)st.n * h.k.row_bytes,
+                          genomes_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
+        }
     }
     if (patch_start_out) CU(cudaMemcpy(patch_start_out, h.k.patch_start[st.cur], (s->P + 1) * 4, cudaMemcpyDeviceToHost));
     if (zi_out && st.n) {

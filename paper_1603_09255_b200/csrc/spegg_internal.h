@@ -74,6 +74,9 @@ struct SpK {
     // state
     uint8_t *pop[2];
     uint32_t *patch_start[2];   // [P+1] each
+    uint32_t *rowptr[2];        // logical adult index -> physical row of pop[]
+    uint32_t *chunk_mask;       // fused path: survivor bitmask of each 32-offspring chunk
+    uint32_t phys_parents;      // 1: mother[] / father[] hold physical rows (fused path)
     uint8_t *f;
     uint32_t *off, *mother, *father, *dest, *pos;
     float *u01, *s;

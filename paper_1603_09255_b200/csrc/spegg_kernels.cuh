@@ -98,7 +98,9 @@ __global__ void k_step_end(DevGlobal *g) { g->step += 1; }
 __global__ void __launch_bounds__(256) k_begin(const __grid_constant__ SpK sp) {
     const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
     const uint32_t n_status = (sp.capacity + SCAN_TILE - 1) / SCAN_TILE + 1;
-    for (uint32_t i = g; i < n_status; i += stride) { sp.status_fec[i] = 0ull; sp.status_cmp[i] = 0ull; }
+    const uint32_t n_status_cmp = sp.capacity / 32 + 2;
+    for (uint32_t i = g; i < n_status; i += stride) sp.status_fec[i] = 0ull;
+    for (uint32_t i = g; i < n_status_cmp; i += stride) sp.status_cmp[i] = 0ull;
     if (sp.P > 1)
         for (uint32_t i = g; i < sp.P * 5; i += stride) sp.patch_cnt[i] = 0u;
     const DevSpecies &st = *sp.st;
@@ -144,6 +146,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
         for (uint32_t i = tid; i < len0; i += SCAN_THREADS) s_tab[i] = sp.tables[i];
     }
     const uint32_t *ps = sp.patch_start[st.cur];
+    const uint32_t *rowptr = sp.rowptr[st.cur];
     for (;;) {
         if (tid == 0) s_tile = atomicAdd(&st.ticket_fec, 1u);
         __syncthreads();
@@ -193,9 +196,10 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
             if (i < N) {
                 sp.off[i] = (uint32_t)min(o, (unsigned long long)0xFFFFFFFFull);
                 sp.f[i] = (uint8_t)f[k];
+                const uint32_t mval = (sp.phys_parents && f[k]) ? rowptr[i] : i;
                 for (uint32_t c = 0; c < f[k]; ++c) {
                     const unsigned long long j = o + c;
-                    if (j < (unsigned long long)sp.capacity) sp.mother[j] = i;
+                    if (j < (unsigned long long)sp.capacity) sp.mother[j] = mval;
                 }
                 o += f[k];
             }
@@ -230,13 +234,14 @@ __global__ void __launch_bounds__(256) k_gamete_bit(const __grid_constant__ SpK 
     const uint32_t per = 2 * sp.n_chrom;
     const unsigned long long total = (unsigned long long)M * per;
     const uint32_t *pop = (const uint32_t *)sp.pop[st.cur];
+    const uint32_t *rowptr = sp.rowptr[st.cur];
     uint32_t *out = (uint32_t *)sp.offbuf;
     const uint32_t rw = 2 * sp.W;
     for (unsigned long long idx = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
          idx += (unsigned long long)gridDim.x * blockDim.x) {
         const uint32_t j = (uint32_t)(idx / per), rem = (uint32_t)(idx % per);
         const uint32_t g = rem / sp.n_chrom, c = rem % sp.n_chrom;
-        const uint32_t parent = g == 0 ? sp.mother[j] : sp.father[j];
+        const uint32_t parent = rowptr[g == 0 ? sp.mother[j] : sp.father[j]];
         const uint32_t cs = sp.chrom_start[c] >> 5, cw = sp.chrom_len[c] >> 5, clen = sp.chrom_len[c];
         const uint32_t *h0 = pop + (size_t)parent * rw + cs, *h1 = h0 + sp.W;
         uint32_t *o = out + (size_t)j * rw + g * sp.W + cs;
@@ -283,13 +288,14 @@ __global__ void __launch_bounds__(256) k_gamete_q10(const __grid_constant__ SpK 
     const unsigned long long warp0 = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const unsigned long long n_warps = ((unsigned long long)gridDim.x * blockDim.x) >> 5;
     const int16_t *pop = (const int16_t *)sp.pop[st.cur];
+    const uint32_t *rowptr = sp.rowptr[st.cur];
     int16_t *out = (int16_t *)sp.offbuf;
     for (unsigned long long gb = warp0 * gpw; gb < n_gam; gb += n_warps * gpw) {
         const unsigned long long gi = gb + sub;
         const bool live = gi < n_gam;
         const uint32_t j = (uint32_t)(gi >> 1), g = (uint32_t)(gi & 1);
         uint32_t parent = 0;
-        if (live) parent = g == 0 ? sp.mother[j] : sp.father[j];
+        if (live) parent = rowptr[g == 0 ? sp.mother[j] : sp.father[j]];
         const int16_t *h0 = pop + (size_t)parent * 2 * L, *h1 = h0 + L;
         int16_t *o = out + (size_t)j * 2 * L + (size_t)g * L;
         uint32_t carry = 0;
@@ -384,11 +390,28 @@ __global__ void __launch_bounds__(256) k_adult_zi(const __grid_constant__ SpK sp
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     long long acc = 0;
     for (uint32_t i = warp0; i < n; i += nw) {
-        const int32_t zi = warp_row_zi(sp, sp.pop[sp.st->cur] + (size_t)i * sp.row_bytes);
+        const int32_t zi = warp_row_zi(sp, sp.pop[sp.st->cur] + (size_t)sp.rowptr[sp.st->cur][i] * sp.row_bytes);
         if ((threadIdx.x & 31u) == 0) { sp.zi[i] = zi; acc += zi; }
     }
     if (accumulate && (threadIdx.x & 31u) == 0 && acc != 0)
         atomicAdd((unsigned long long *)&sp.st->sum_zi, (unsigned long long)acc);
+}
+
+// rowptr = identity for a freshly written, dense population
+__global__ void __launch_bounds__(256) k_iota(uint32_t *p, uint32_t n) {
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = i;
+}
+
+// rows of the current adults in logical order (read_state): out[i] = pop[rowptr[i]], one warp per row
+__global__ void __launch_bounds__(256) k_gather_rows(const __grid_constant__ SpK sp, uint32_t n, uint8_t *out) {
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t cur = sp.st->cur;
+    for (uint32_t i = warp0; i < n; i += nw) {
+        const uint4 *src = (const uint4 *)(sp.pop[cur] + (size_t)sp.rowptr[cur][i] * sp.row_bytes);
+        uint4 *d = (uint4 *)(out + (size_t)i * sp.row_bytes);
+        for (uint32_t q = lane; q < sp.row_u4; q += 32) d[q] = src[q];
+    }
 }
 
 // a6: selection / survival (Fig. 1D), fp32; captures credited to a uniformly drawn predator
@@ -480,9 +503,11 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
     const uint32_t M = st.m, lane = threadIdx.x & 31u;
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     uint8_t *dst = sp.pop[st.cur ^ 1u];
+    uint32_t *rp = sp.rowptr[st.cur ^ 1u];
     for (uint32_t j = warp0; j < M; j += nw) {
         const uint32_t p = sp.pos[j];
         if (p == 0xFFFFFFFFu) continue;
+        if (lane == 0) rp[p] = p;  // materialised path: rows are dense, rowptr is the identity
         const uint4 *src = (const uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes);
         uint4 *d = (uint4 *)(dst + (size_t)p * sp.row_bytes);
         for (uint32_t i = lane; i < sp.row_u4; i += 32) d[i] = src[i];
