@@ -160,7 +160,7 @@ uint32_t row_bytes_of(const spegg_species_params &q) {
 // Lays out the whole workspace; returns total bytes.  Header: DevGlobal + DevSpecies[MAX].
 uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
     Carver c;
-    c.take(4096);  // header
+    c.take(4096 + MAX_SPECIES * sizeof(SpK));  // header: DevGlobal, DevSpecies[], SpK[]
     const uint32_t gw = p->grid_w ? p->grid_w : 1, gh = p->grid_h ? p->grid_h : 1;
     const uint64_t P = (uint64_t)gw * gh;
     const uint32_t logcap = p->log_capacity ? p->log_capacity : 4096;
@@ -171,7 +171,6 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         const uint64_t cap = q.capacity;
         l.row_bytes = row_bytes_of(q);
         l.n_tables = q.fecundity_model == SPEGG_FEC_CAPTURES ? CAP_TABLES : (uint32_t)P;
-        const uint64_t n_status = (cap + SCAN_TILE - 1) / SCAN_TILE + 1;
         const uint64_t cap32 = (cap + 31) / 32 * 32;  // fused path: one 32-row slab per offspring chunk
         l.pop[0] = c.take(cap32 * l.row_bytes);
         l.pop[1] = c.take(cap32 * l.row_bytes);
@@ -195,7 +194,7 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.offbuf = c.take(cap * l.row_bytes);
         l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
         l.table_len = c.take((uint64_t)l.n_tables * 4);
-        l.status_fec = c.take(n_status * 8);
+        l.status_fec = c.take((cap / SCAN_THREADS + 2) * 8);
         l.status_cmp = c.take((cap / 32 + 2) * 8);  // fused tiles are 32 offspring
         l.patch_cnt = c.take(P * 5 * 4);
         l.patch_base = c.take(P * 5 * 4);
@@ -230,6 +229,7 @@ struct spegg_sim {
     cudaGraphExec_t exec = nullptr;
     DevGlobal *d_glob = nullptr;
     DevSpecies *d_st = nullptr;
+    SpK *d_spk = nullptr;
     uint32_t P = 1, n_sms = 148, launches = 0;
     uint32_t log_capacity = 4096;
     bool debug = false;
@@ -256,23 +256,27 @@ bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
     return !s->debug && s->P == 1 && fused_bit_supported(h.k);
 }
 
+void launch_prepare(spegg_sim *s) {
+    uint32_t blocks = 8;
+    for (auto &h : s->sp) {
+        blocks = std::max(blocks, (h.k.n_tables + 255) / 256);
+        if (h.p.fecundity_model == SPEGG_FEC_CAPTURES) blocks = std::max(blocks, s->n_sms);
+    }
+    k_prepare_all<<<dim3(std::min(blocks, 4 * s->n_sms), s->p.n_species), 256, 0, s->stream>>>(s->d_spk);
+}
+
 // Enqueue the kernels of one step on the stream (captured into the graph, or launched directly
 // when kernel timing is on).  Returns the number of kernel launches through *n_launch.
 int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
     uint32_t nl = 0;
     const uint32_t G = s->n_sms;
-    for (auto &h : s->sp)
-        if (h.p.fecundity_model == SPEGG_FEC_CAPTURES)
-            CU(cudaMemsetAsync(h.k.cap, 0, (size_t)h.p.capacity * 4, s->stream));
-    k_step_begin<<<1, 32, 0, s->stream>>>(s->d_st, s->p.n_species); ++nl;
+    if (s->debug) { launch_prepare(s); ++nl; }
     for (size_t si = 0; si < s->sp.size(); ++si) {
         HostSpecies &h = s->sp[si];
         const SpK &k = h.k;
         const bool time_this = timed && si == 0 && s->ev_used + 2 <= s->ev.size();
-        k_begin<<<std::max(1u, std::min(G, (k.n_tables + 255) / 256 + 8)), 256, 0, s->stream>>>(k); ++nl;
         k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
         if (fused_ok(s, h)) {
-            launch_offspring_draws(k, G, s->stream); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             launch_fused_bit(k, G, s->stream); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
@@ -296,9 +300,9 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             }
             k_cmp_scatter<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
         }
-        k_end<<<1, 32, 0, s->stream>>>(k); ++nl;
     }
-    k_step_end<<<1, 1, 0, s->stream>>>(s->d_glob); ++nl;
+    k_finish_all<<<1, 32, 0, s->stream>>>(s->d_spk, s->p.n_species); ++nl;
+    if (!s->debug) { launch_prepare(s); ++nl; }  // debug: prepared at the start, so the view stays valid
     CU(cudaGetLastError());
     if (n_launch) *n_launch = nl;
     return SPEGG_OK;
@@ -369,7 +373,8 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     }
     s->d_glob = at<DevGlobal>(s, 0);
     s->d_st = at<DevSpecies>(s, 256);
-    if (cudaMemsetAsync(s->ws, 0, 4096, s->stream) != cudaSuccess) return fail(SPEGG_ECUDA);
+    s->d_spk = at<SpK>(s, 4096);
+    if (cudaMemsetAsync(s->ws, 0, 4096 + MAX_SPECIES * sizeof(SpK), s->stream) != cudaSuccess) return fail(SPEGG_ECUDA);
 
     s->sp.resize(p->n_species);
     for (uint32_t si = 0; si < p->n_species; ++si) {
@@ -459,6 +464,9 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     for (uint32_t si = 0; si < p->n_species; ++si)
         if (s->sp[si].p.sel_predation) s->sp[si].k.cap_pred = s->sp[s->sp[si].p.predator_species].k.cap;
 
+    for (uint32_t si = 0; si < p->n_species; ++si)
+        if (cudaMemcpyAsync(s->d_spk + si, &s->sp[si].k, sizeof(SpK), cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return fail(SPEGG_ECUDA);
+    launch_prepare(s);
     // capture the step graph once; spegg_step replays it
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }
     if (cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }
@@ -511,6 +519,7 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
         k_iota<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k.rowptr[cur], (uint32_t)n);
         k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1);
     }
+    launch_prepare(s);
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(s->stream));
     return SPEGG_OK;

@@ -3,12 +3,11 @@
 // Bit-packed genomes with NC chromosomes of WPC 32-bit words each (config 3: 4 x 8 words = 1,024
 // loci, 256-byte rows).  After k_fec_scan (fecundity, scan, mother[]) the step is two kernels:
 //
-//   k_offspring_draws  one thread per offspring: the SCALAR block (father, survival uniform, R2/R4)
-//                      and the two MUT blocks' counts (R9) -> father[], u01[], mutflag[]
-//   k_fused_bit        a4-a8 in one pass: gather both parents' rows, build the crossover masks from
-//                      the RECOMB blocks (R8), select, mutate, popcount -> phenotype -> survival ->
-//                      stable compaction straight into the other population buffer.  Offspring rows
-//                      never touch memory unless they survive.
+//   k_fused_bit   a3-a8 in one pass: father draw, gather of both parents' rows, crossover masks
+//                 from the RECOMB blocks (R8), select, mutate, popcount -> phenotype -> survival,
+//                 survivors stored once into the other population buffer.  Offspring rows never
+//                 touch memory unless they survive.
+//   k_index       stable order of the next generation from 4-byte chunk masks (rowptr).
 //
 // Thread mapping of k_fused_bit: 8 consecutive lanes own one offspring, lane q = (gamete g = q/4,
 // chromosome c = q%4): it loads the 8 words of chromosome c of both haplotypes of parent g with
@@ -37,49 +36,41 @@ __device__ __forceinline__ uint4 ldg_u4(const uint4 *p) {
     return v;
 }
 
-// one thread per offspring: SCALAR block and the mutation counts of both gametes
-__global__ void __launch_bounds__(256) k_offspring_draws(const __grid_constant__ SpK sp) {
-    const DevSpecies &st = *sp.st;
-    const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
-    const uint32_t *rowptr = sp.rowptr[st.cur];
-    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
-        uint32_t x[4];
-        draw(sp.key, sp.species, ST_SCALAR, j, 0, step, x);
-        sp.father[j] = rowptr[uniform_index(x[0], N)];
-        sp.u01[j] = u01_of(x[3]);
-        uint32_t a[4], b[4];
-        draw(sp.key, sp.species, ST_MUT_M, j, 0, step, a);
-        draw(sp.key, sp.species, ST_MUT_P, j, 0, step, b);
-        const uint32_t t0 = sp.mut_len ? sp.T_mut[0] : 0xFFFFFFFFu;
-        const bool any = sp.mut_len && (a[0] >= t0 || b[0] >= t0);
-        sp.alive[j] = any ? 1 : 0;  // alive[] doubles as the mutation flag in the fused path
-    }
-}
-
 // Warp-autonomous fused kernel.  A warp takes a chunk of FUSED_CHUNK = 32 consecutive offspring
-// from an atomic ticket and processes it in 8 passes of 4 offspring (8 lanes each).  Chunk c owns
-// the 32-row slab [32c, 32c+32) of the other population buffer: its survivors are stored packed at
-// the start of the slab, in j order, straight from registers with 128-bit stores, and the chunk's
-// survivor bitmask goes to chunk_mask[c].  Nothing in this kernel waits on another warp: the
-// stable order of the next generation is established afterwards by k_index, which scans the
-// 4-byte chunk masks and writes rowptr (logical adult index -> physical row).  The heavy rows are
-// written exactly once; only 4-byte indices are compacted.
+// from an atomic ticket.
+//   prologue (dense, every lane busy, independent Philox chains interleave):
+//     - lane = offspring: mother row, SCALAR block (father -> rowptr -> row, survival uniform),
+//       the two MUT blocks' counts
+//     - lane = (gamete g, chromosome c) of offspring it*4+sub, it = 0..7: the 8 RECOMB blocks this
+//       lane will need, decoded to a packed word (count, start phase, first two positions)
+//     - the few chromosomes with more than two crossovers (8 % at mean 1) are queued and their
+//       extra blocks / mask contributions computed one per lane, so no divergent Philox later
+//   8 passes of 4 offspring (8 lanes each): four 128-bit loads of the lane's 8-word chromosome
+//   from both haplotypes of its parent, mask words from the packed draw (+ queued extras), select,
+//   rare mutation, popcount -> phenotype -> fp32 survival, and the surviving rows are stored,
+//   packed and in j order, at the start of the chunk's own 32-row slab of the other buffer.
+// Nothing waits on another warp: the stable order of the next generation is established
+// afterwards by k_index, which scans the 4-byte chunk masks and writes rowptr (logical adult index
+// -> physical row).  The 256-byte rows are written exactly once; only indices are compacted.
 constexpr int FUSED_CHUNK = 32;
 constexpr int FUSED_WARPS = 8;
 
 template <int NC, int WPC>
 __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_constant__ SpK sp) {
     static_assert(NC == 4 && WPC == 8, "lane group of 8 = 2 gametes x 4 chromosomes of 8 words");
+    __shared__ uint4 s_xmask[FUSED_WARPS][32][2];   // mask contribution of queued extra crossovers
+    __shared__ uint32_t s_P[FUSED_WARPS][8][32];    // packed recombination draws of the chunk
+    __shared__ uint32_t s_q[FUSED_WARPS][32];       // queue of chromosomes with > 2 crossovers
     DevSpecies &st = *sp.st;
-    const uint32_t M = st.m, step = sp.glob->step;
+    const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
     const uint32_t n_chunks = (M + FUSED_CHUNK - 1) / FUSED_CHUNK;
-    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t sub = lane >> 3, q = lane & 7u, g = q >> 2, c = q & 3u;
     constexpr uint32_t ROW4 = 2 * NC * WPC / 4;   // uint4 per row (16)
     constexpr uint32_t L = NC * WPC * 32;
     const uint4 *pop = (const uint4 *)sp.pop[st.cur];
     uint4 *nxt = (uint4 *)sp.pop[st.cur ^ 1u];
-    const uint32_t *parent_idx = g ? sp.father : sp.mother;   // physical rows (phys_parents)
+    const uint32_t *rowptr = sp.rowptr[st.cur];
     const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
     // this chromosome's crossover-count thresholds in registers (count <= 6 without a loop)
     const uint32_t xl = sp.xover_len[c];
@@ -89,6 +80,8 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
     for (int i = 0; i < 6; ++i) T[i] = (uint32_t)i < xl ? XT[i] : 0xFFFFFFFFu;
     const bool short_table = xl <= 6;
     const uint32_t clen1 = sp.chrom_len[c] - 1;
+    const uint32_t Tm0 = sp.mut_len ? sp.T_mut[0] : 0xFFFFFFFFu;
+    const bool has_mut = sp.mut_len != 0;
     const float theta = st.theta_t;
     long long acc1 = 0, acc2 = 0;
     uint32_t ties = 0;
@@ -98,56 +91,118 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
         if (lane == 0) chunk = atomicAdd(&st.ticket_fused, 1u);
         chunk = __shfl_sync(0xffffffffu, chunk, 0);
         if (chunk >= n_chunks) break;
-        uint32_t cnt = 0, cmask = 0;  // survivors stored so far / survivor bitmask (warp-uniform)
-#pragma unroll 1
-        for (uint32_t it = 0; it < FUSED_CHUNK / 4; ++it) {
-            const uint32_t j = chunk * FUSED_CHUNK + it * 4 + sub;
-            const bool valid = j < M;
-            uint32_t h0[8], h1[8];
-            uint32_t mflag = 0;
-            float u01 = 2.0f;
-            if (valid) {
-                const uint32_t parent = parent_idx[j];
-                const uint4 *row = pop + (size_t)parent * ROW4 + c * 2;
-                const uint4 a = ldg_u4(row), b = ldg_u4(row + 1), d = ldg_u4(row + ROW4 / 2), e = ldg_u4(row + ROW4 / 2 + 1);
-                h0[0] = a.x; h0[1] = a.y; h0[2] = a.z; h0[3] = a.w; h0[4] = b.x; h0[5] = b.y; h0[6] = b.z; h0[7] = b.w;
-                h1[0] = d.x; h1[1] = d.y; h1[2] = d.z; h1[3] = d.w; h1[4] = e.x; h1[5] = e.y; h1[6] = e.z; h1[7] = e.w;
-                mflag = sp.alive[j];
-                u01 = sp.u01[j];
-            } else {
-#pragma unroll
-                for (int w = 0; w < 8; ++w) { h0[w] = 0; h1[w] = 0; }
+        const uint32_t j0 = chunk * FUSED_CHUNK;
+        // ---- prologue (a): lane = offspring j0 + lane
+        uint32_t mo = 0, fa = 0, mf = 0;
+        float ul = 2.0f;
+        {
+            const uint32_t jl = j0 + lane;
+            uint32_t x[4], a[4], b[4];
+            draw(sp.key, sp.species, ST_SCALAR, jl, 0, step, x);
+            draw(sp.key, sp.species, ST_MUT_M, jl, 0, step, a);
+            draw(sp.key, sp.species, ST_MUT_P, jl, 0, step, b);
+            if (jl < M) {
+                mo = sp.mother[jl];                        // physical row (phys_parents)
+                fa = rowptr[uniform_index(x[0], N)];       // R2: uniform mate, selfing allowed
+                ul = u01_of(x[3]);
+                if (has_mut) mf = (a[0] >= Tm0 ? 1u : 0u) | (b[0] >= Tm0 ? 2u : 0u);
             }
-            // ---- R8: crossover mask of chromosome c of gamete g
+        }
+        // ---- prologue (b): the 8 RECOMB blocks of this lane's (gamete, chromosome) role
+        uint32_t qn = 0;
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+            const uint32_t j = j0 + it * 4 + sub;
             uint32_t x[4];
             draw(sp.key, sp.species, stream, j, c * 16, step, x);
             uint32_t nc = 0;
 #pragma unroll
             for (int i = 0; i < 6; ++i) nc += (x[0] >= T[i]) ? 1u : 0u;
             if (!short_table && nc == 6) nc = poisson_count(XT, xl, x[0]);
-            uint32_t m[8];
-            const uint32_t phi = (x[1] >> 31) ? 0xFFFFFFFFu : 0u;
-            {
-                const int s0 = nc > 0 ? (int)__umulhi(x[2], clen1) + 1 : 4096;
-                const int s1 = nc > 1 ? (int)__umulhi(x[3], clen1) + 1 : 4096;
-#pragma unroll
-                for (int w = 0; w < 8; ++w)
-                    m[w] = phi ^ shl_clamp(0xFFFFFFFFu, (uint32_t)max(s0 - 32 * w, 0)) ^
-                           shl_clamp(0xFFFFFFFFu, (uint32_t)max(s1 - 32 * w, 0));
+            uint32_t P = nc | ((x[1] >> 31) << 6) | ((__umulhi(x[2], clen1) + 1) << 8) | ((__umulhi(x[3], clen1) + 1) << 16);
+            // queue the chromosomes that need crossovers beyond the first two
+            const bool need = nc > 2;
+            const uint32_t bal = __ballot_sync(0xffffffffu, need);
+            uint32_t id = 63;
+            if (need) {
+                const uint32_t e = qn + __popc(bal & ((1u << lane) - 1u));
+                if (e < 32) { id = e; s_q[warp][e] = (nc << 8) | ((uint32_t)it << 5) | lane; }
             }
-            if (__any_sync(0xffffffffu, nc > 2)) {
-                // later crossovers come from blocks c*16+1.. (4 per block); lanes that need them
-                // run in lock-step on k, so the word index is uniform and statically unrolled
-                const uint32_t extra = nc > 2 ? nc - 2 : 0;
-                for (uint32_t b = 0; b * 4 < extra; ++b) {
-                    uint32_t y[4];
-                    draw(sp.key, sp.species, stream, j, c * 16 + 1 + b, step, y);
+            qn += __popc(bal);
+            s_P[warp][it][lane] = P | (id << 24);
+        }
+        __syncwarp();
+        // ---- prologue (c): one lane per queued chromosome computes its extra crossovers
+        if (lane < min(qn, 32u)) {
+            const uint32_t e = s_q[warp][lane];
+            const uint32_t e_nc = e >> 8, e_it = (e >> 5) & 7u, e_ln = e & 31u;
+            const uint32_t e_c = e_ln & 3u, e_g = (e_ln >> 2) & 1u;
+            const uint32_t e_j = j0 + e_it * 4 + (e_ln >> 3);
+            const uint32_t e_clen1 = sp.chrom_len[e_c] - 1;
+            uint32_t xm[8];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        if (b * 4 + i < extra) {
-                            const int s = (int)__umulhi(y[i], clen1) + 1;
+            for (int w = 0; w < 8; ++w) xm[w] = 0;
+            const uint32_t extra = e_nc - 2;
+            for (uint32_t b = 0; b * 4 < extra; ++b) {
+                uint32_t y[4];
+                draw(sp.key, sp.species, e_g ? ST_RECOMB_P : ST_RECOMB_M, e_j, e_c * 16 + 1 + b, step, y);
 #pragma unroll
-                            for (int w = 0; w < 8; ++w) m[w] ^= shl_clamp(0xFFFFFFFFu, (uint32_t)max(s - 32 * w, 0));
+                for (int i = 0; i < 4; ++i) {
+                    if (b * 4 + i < extra) {
+                        const int s = (int)__umulhi(y[i], e_clen1) + 1;
+#pragma unroll
+                        for (int w = 0; w < 8; ++w) xm[w] ^= shl_clamp(0xFFFFFFFFu, (uint32_t)max(s - 32 * w, 0));
+                    }
+                }
+            }
+            s_xmask[warp][lane][0] = make_uint4(xm[0], xm[1], xm[2], xm[3]);
+            s_xmask[warp][lane][1] = make_uint4(xm[4], xm[5], xm[6], xm[7]);
+        }
+        __syncwarp();
+
+        uint32_t cnt = 0, cmask = 0;  // survivors stored so far / survivor bitmask (warp-uniform)
+#pragma unroll 1
+        for (uint32_t it = 0; it < FUSED_CHUNK / 4; ++it) {
+            const uint32_t src = it * 4 + sub;
+            const uint32_t j = j0 + src;
+            const bool valid = j < M;
+            const uint32_t pm = __shfl_sync(0xffffffffu, mo, src), pf = __shfl_sync(0xffffffffu, fa, src);
+            const float u01 = __shfl_sync(0xffffffffu, ul, src);
+            const uint32_t mflag = (__shfl_sync(0xffffffffu, mf, src) >> g) & 1u;
+            const uint32_t parent = g ? pf : pm;
+            const uint4 *row = pop + (size_t)parent * ROW4 + c * 2;
+            const uint4 a = ldg_u4(row), b = ldg_u4(row + 1), d = ldg_u4(row + ROW4 / 2), e = ldg_u4(row + ROW4 / 2 + 1);
+            const uint32_t h0[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+            const uint32_t h1[8] = {d.x, d.y, d.z, d.w, e.x, e.y, e.z, e.w};
+            // ---- R8: crossover mask of chromosome c of gamete g from the packed draw
+            const uint32_t P = s_P[warp][it][lane];
+            const uint32_t nc = P & 63u;
+            const uint32_t phi = ((P >> 6) & 1u) ? 0xFFFFFFFFu : 0u;
+            const int s0 = nc > 0 ? (int)((P >> 8) & 0xFFu) : 4096;
+            const int s1 = nc > 1 ? (int)((P >> 16) & 0xFFu) : 4096;
+            uint32_t m[8];
+#pragma unroll
+            for (int w = 0; w < 8; ++w)
+                m[w] = phi ^ shl_clamp(0xFFFFFFFFu, (uint32_t)max(s0 - 32 * w, 0)) ^
+                       shl_clamp(0xFFFFFFFFu, (uint32_t)max(s1 - 32 * w, 0));
+            if (nc > 2) {
+                const uint32_t id = (P >> 24) & 63u;
+                if (id < 32) {
+                    const uint4 xa = s_xmask[warp][id][0], xb = s_xmask[warp][id][1];
+                    m[0] ^= xa.x; m[1] ^= xa.y; m[2] ^= xa.z; m[3] ^= xa.w;
+                    m[4] ^= xb.x; m[5] ^= xb.y; m[6] ^= xb.z; m[7] ^= xb.w;
+                } else {  // queue overflow (> 32 such chromosomes in one chunk): compute in place
+                    const uint32_t extra = nc - 2;
+                    for (uint32_t bb = 0; bb * 4 < extra; ++bb) {
+                        uint32_t y[4];
+                        draw(sp.key, sp.species, stream, j, c * 16 + 1 + bb, step, y);
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            if (bb * 4 + i < extra) {
+                                const int s = (int)__umulhi(y[i], clen1) + 1;
+#pragma unroll
+                                for (int w = 0; w < 8; ++w) m[w] ^= shl_clamp(0xFFFFFFFFu, (uint32_t)max(s - 32 * w, 0));
+                            }
                         }
                     }
                 }
@@ -156,9 +211,10 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             uint32_t gw[8];
 #pragma unroll
             for (int w = 0; w < 8; ++w) gw[w] = (h0[w] & ~m[w]) | (h1[w] & m[w]);
-            // ---- R9: mutation (rare; flagged per offspring by k_offspring_draws)
+            // ---- R9: mutation (rare; flagged per gamete in the prologue)
             if (mflag) {
                 const uint32_t ms = g ? ST_MUT_P : ST_MUT_M;
+                uint32_t x[4];
                 draw(sp.key, sp.species, ms, j, 0, step, x);
                 const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
                 for (uint32_t k = 0; k < nm; ++k) {
@@ -192,7 +248,7 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             // ---- a7: store the surviving row at its rank within the chunk's slab
             const uint32_t bal = __ballot_sync(0xffffffffu, alive && q == 0);
             if (alive) {
-                const uint32_t slot = chunk * FUSED_CHUNK + cnt + __popc(bal & ((1u << (lane & 24u)) - 1u));
+                const uint32_t slot = j0 + cnt + __popc(bal & ((1u << (lane & 24u)) - 1u));
                 uint4 *o = nxt + (size_t)slot * ROW4 + g * (ROW4 / 2) + c * 2;
                 o[0] = make_uint4(gw[0], gw[1], gw[2], gw[3]);
                 o[1] = make_uint4(gw[4], gw[5], gw[6], gw[7]);
@@ -201,6 +257,7 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             cmask |= ((bal & 1u) | ((bal >> 7) & 2u) | ((bal >> 14) & 4u) | ((bal >> 21) & 8u)) << (it * 4);
         }
         if (lane == 0) sp.chunk_mask[chunk] = cmask;
+        __syncwarp();
     }
     // ---- a8: survivor reductions (exact integers)
 #pragma unroll
@@ -219,32 +276,26 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
 }
 
 // a7: stable order of the next generation.  One thread per chunk: exclusive scan of the chunks'
-// survivor counts (decoupled look-back over tiles of 1,024 chunks), then rowptr_next[base + r] =
-// 32*chunk + r.  Moves 4 bytes per survivor instead of the 256-byte rows.
+// survivor counts (decoupled look-back over tiles of 256 chunks), then one warp per chunk writes
+// rowptr_next[base + r] = 32*chunk + r (coalesced).  Moves 4 bytes per survivor instead of rows.
 __global__ void __launch_bounds__(SCAN_THREADS) k_index(const __grid_constant__ SpK sp) {
     __shared__ uint32_t s_warp[SCAN_THREADS / 32];
+    __shared__ uint32_t s_base[SCAN_THREADS], s_cnt[SCAN_THREADS];
     __shared__ uint32_t s_tile;
     __shared__ unsigned long long s_excl;
     DevSpecies &st = *sp.st;
     const uint32_t n_chunks = (st.m + FUSED_CHUNK - 1) / FUSED_CHUNK;
-    const uint32_t n_tiles = (n_chunks + SCAN_TILE - 1) / SCAN_TILE;
+    const uint32_t n_tiles = (n_chunks + SCAN_THREADS - 1) / SCAN_THREADS;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     uint32_t *rp = sp.rowptr[st.cur ^ 1u];
-    if (n_chunks == 0 && blockIdx.x == 0 && tid == 0) st.n_next = 0;
     for (;;) {
         if (tid == 0) s_tile = atomicAdd(&st.ticket_cmp, 1u);
         __syncthreads();
         const uint32_t tile = s_tile;
         if (tile >= n_tiles) break;
-        const uint32_t base = tile * SCAN_TILE + tid * SCAN_ITEMS;
-        uint32_t cnt[SCAN_ITEMS], sum = 0;
-#pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
-            const uint32_t ch = base + k;
-            cnt[k] = ch < n_chunks ? __popc(sp.chunk_mask[ch]) : 0u;
-            sum += cnt[k];
-        }
-        const uint32_t incl = warp_incl_scan(sum);
+        const uint32_t ch = tile * SCAN_THREADS + tid;
+        const uint32_t cnt = ch < n_chunks ? __popc(sp.chunk_mask[ch]) : 0u;
+        const uint32_t incl = warp_incl_scan(cnt);
         if (lane == 31) s_warp[warp] = incl;
         __syncthreads();
         if (warp == 0) {
@@ -259,12 +310,12 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_index(const __grid_constant__ 
             }
         }
         __syncthreads();
-        uint32_t o = (uint32_t)s_excl + s_warp[warp] + (incl - sum);
-#pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
-            const uint32_t ch = base + k;
-            for (uint32_t r = 0; r < cnt[k]; ++r) rp[o + r] = ch * FUSED_CHUNK + r;
-            o += cnt[k];
+        s_base[tid] = (uint32_t)s_excl + s_warp[warp] + (incl - cnt);
+        s_cnt[tid] = cnt;
+        __syncthreads();
+        for (uint32_t k = 0; k < 32; ++k) {
+            const uint32_t t = warp * 32 + k;
+            if (lane < s_cnt[t]) rp[s_base[t] + lane] = (tile * SCAN_THREADS + t) * FUSED_CHUNK + lane;
         }
         __syncthreads();
     }
@@ -275,16 +326,12 @@ __host__ inline bool fused_bit_supported(const SpK &k) {
            k.fec_model != 2 && k.theta_patch == nullptr;
 }
 
-inline void launch_offspring_draws(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
-    k_offspring_draws<<<n_sms * 8, 256, 0, stream>>>(k);
-}
-
 inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
     k_fused_bit<4, 8><<<n_sms * 3, FUSED_WARPS * 32, 0, stream>>>(k);
 }
 
 inline void launch_index(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
-    k_index<<<n_sms, SCAN_THREADS, 0, stream>>>(k);
+    k_index<<<n_sms * 2, SCAN_THREADS, 0, stream>>>(k);
 }
 
 }  // namespace spegg

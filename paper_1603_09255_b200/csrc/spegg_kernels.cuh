@@ -1,7 +1,7 @@
 // spegg_kernels.cuh -- the step pipeline of libspegg as separate kernels (sm_100a).
 //
 // One time step of one species (Fig. 1 A-F) is the sequence
-//   k_begin        a0  derived parameters: fecundity tables from device-resident counts, theta_t
+//   k_prepare_all  a0  derived parameters: fecundity tables from device-resident counts, theta_t
 //   k_fec_scan     a1-a3  Poisson fecundity, single-pass decoupled look-back scan, mother fill
 //   k_scalar       a3  father (uniform mate), dispersal, survival uniform
 //   k_gamete_*     a4  recombination (bit: Poisson crossovers; q10: per-interval draws)
@@ -9,7 +9,7 @@
 //   k_phenotype    a5  additive map, exact integers
 //   k_survival     a6  fp32 survival probability, decision, captures
 //   k_cmp_* / k_patch_*  a7-a8  stable compaction into the other buffer + reductions
-//   k_end          a9  counts stay on the device; log entry; buffer flip
+//   k_finish_all   a9  counts stay on the device; log entry; buffer flip
 // This file is the general ("materialised") pipeline that serves every configuration and the
 // debug view; spegg_fused.cuh holds the fused single-pass kernels of the hot configurations.
 // All grids are fixed at graph-capture time and loop against device-side counts.
@@ -80,31 +80,44 @@ __device__ __forceinline__ float survival_prob(const SpK &sp, float z, float the
 }
 
 // ------------------------------------------------------------------------ step bookkeeping
-__global__ void k_step_begin(DevSpecies *st, uint32_t n_species) {
-    const uint32_t s = threadIdx.x;
-    if (s < n_species) {
-        DevSpecies &d = st[s];
-        d.n0 = d.n;
-        d.sum_zi0 = d.sum_zi;
-        d.m = 0; d.n_next = 0; d.flags_step = 0;
-        d.ticket_fec = 0; d.ticket_cmp = 0; d.ticket_fused = 0; d.done_fused = 0;
-        d.acc_zi = 0; d.acc_zi2 = 0; d.captures = 0; d.near_ties = 0;
+// a9: end of step for every species (one thread each): counts stay on the device, log entry,
+// buffer flip; then the step counter advances.  Single block, so nothing races on glob->step.
+__global__ void k_finish_all(const SpK *__restrict__ spk, uint32_t n_species) {
+    if (threadIdx.x < n_species) {
+        const SpK &sp = spk[threadIdx.x];
+        DevSpecies &st = *sp.st;
+        const uint32_t nn = st.n_next;
+        if (st.n0 == 0) st.flags_step |= 2u;
+        LogEntry &e = sp.log[st.log_pos % sp.log_capacity];
+        e.n_t = st.n0; e.m_t = st.m; e.n_next = nn;
+        e.sum_zi = st.acc_zi; e.sum_zi2 = st.acc_zi2;
+        e.captures = st.captures; e.near_ties = st.near_ties;
+        e.flags = st.flags_step; e.step = sp.glob->step;
+        st.log_pos += 1;
+        if (st.flags_step) atomicOr(&sp.glob->flags, st.flags_step);
+        st.n = nn;
+        st.sum_zi = st.acc_zi;
+        st.cur ^= 1u;
+        if (sp.P == 1) { uint32_t *psn = sp.patch_start[st.cur]; psn[0] = 0; psn[1] = nn; }
     }
+    __syncthreads();
+    if (threadIdx.x == 0) spk[0].glob->step += 1;
 }
 
-__global__ void k_step_end(DevGlobal *g) { g->step += 1; }
-
-// a0: derived parameters (Fig. 1 F -> A)
-__global__ void __launch_bounds__(256) k_begin(const __grid_constant__ SpK sp) {
+// a0: everything the next step needs before its first kernel (Fig. 1 F -> A): start-of-step
+// snapshots, fecundity tables from the device-resident counts, theta_t, predation scalars, cleared
+// look-back statuses / tickets / capture counts.  grid = (blocks, n_species).
+__global__ void __launch_bounds__(256) k_prepare_all(const SpK *__restrict__ spk) {
+    const SpK &sp = spk[blockIdx.y];
     const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
-    const uint32_t n_status = (sp.capacity + SCAN_TILE - 1) / SCAN_TILE + 1;
-    const uint32_t n_status_cmp = sp.capacity / 32 + 2;
-    for (uint32_t i = g; i < n_status; i += stride) sp.status_fec[i] = 0ull;
-    for (uint32_t i = g; i < n_status_cmp; i += stride) sp.status_cmp[i] = 0ull;
-    if (sp.P > 1)
-        for (uint32_t i = g; i < sp.P * 5; i += stride) sp.patch_cnt[i] = 0u;
-    const DevSpecies &st = *sp.st;
-    const uint32_t N = st.n0;
+    const uint32_t n_status_fec = sp.capacity / SCAN_THREADS + 2, n_status_cmp = sp.capacity / 32 / SCAN_THREADS + 2;
+    const uint32_t n_status_gen = sp.capacity / SCAN_TILE + 2;
+    for (uint32_t i = g; i < n_status_fec; i += stride) sp.status_fec[i] = 0ull;
+    for (uint32_t i = g; i < max(n_status_cmp, n_status_gen); i += stride) sp.status_cmp[i] = 0ull;
+    if (sp.fec_model == 2)
+        for (uint32_t i = g; i < sp.capacity; i += stride) sp.cap[i] = 0u;
+    DevSpecies &st = *sp.st;
+    const uint32_t N = st.n;
     const uint32_t *ps = sp.patch_start[st.cur];
     for (uint32_t tab = g; tab < sp.n_tables; tab += stride) {
         double lam;
@@ -114,30 +127,49 @@ __global__ void __launch_bounds__(256) k_begin(const __grid_constant__ SpK sp) {
         sp.table_len[tab] = (uint32_t)build_poisson_table(lam, sp.tables + (size_t)tab * TMAX, TMAX);
     }
     if (g == 0) {
-        DevSpecies &w = *sp.st;
+        st.n0 = N;
+        st.sum_zi0 = st.sum_zi;
+        st.m = 0; st.n_next = 0; st.flags_step = 0;
+        st.ticket_fec = 0; st.ticket_cmp = 0; st.ticket_fused = 0; st.done_fused = 0;
+        st.acc_zi = 0; st.acc_zi2 = 0; st.captures = 0; st.near_ties = 0;
         // R6: theta_t = fp32(theta0 + t*dtheta), fp64, never accumulated
-        w.theta_t = __double2float_rn(__dadd_rn(sp.theta0, __dmul_rn((double)sp.glob->step, sp.dtheta)));
+        st.theta_t = __double2float_rn(__dadd_rn(sp.theta0, __dmul_rn((double)sp.glob->step, sp.dtheta)));
         if (sp.sel_predation) {
             const DevSpecies &pr = sp.st_all[sp.predator];
-            const uint32_t NC = pr.n0;
-            w.n_pred0 = NC;
+            const uint32_t NC = pr.n;
+            st.n_pred0 = NC;
             // R14: zbar_C = fp32((sum zi / N_C) * scale_C) ; A = fp32(a * N_C)
-            w.zbar_pred = NC ? __double2float_rn(__dmul_rn(__ddiv_rn((double)pr.sum_zi0, (double)NC), (double)sp.pred_scale)) : 0.0f;
-            w.attack_n = __double2float_rn(__dmul_rn(sp.attack, (double)NC));
+            st.zbar_pred = NC ? __double2float_rn(__dmul_rn(__ddiv_rn((double)pr.sum_zi, (double)NC), (double)sp.pred_scale)) : 0.0f;
+            st.attack_n = __double2float_rn(__dmul_rn(sp.attack, (double)NC));
         }
-        if (N == 0) w.flags_step |= 2u;
     }
 }
 
-// a1-a3: fecundity (one FEC block per adult), exclusive scan by decoupled look-back, mother fill
+// a1-a3: fecundity (one FEC block per adult), exclusive scan by decoupled look-back, mother fill.
+// Each CTA takes a contiguous RANGE of adults (about N / gridDim.x, at most FEC_RANGE_MAX): pass 1
+// draws the fecundities into shared memory and reduces them, ONE look-back per range gives the
+// range's offspring base, pass 2 scans inside the range and writes off[], f[] and mother[].  With
+// a few hundred ranges the look-back chain is a handful of hops instead of one per 1,024 adults.
+constexpr int FEC_RANGE_MAX = 8192;
+
+__device__ __forceinline__ uint32_t fec_range_size(uint32_t N, uint32_t n_ctas) {
+    uint32_t R = (N + n_ctas - 1) / n_ctas;
+    R = (R + SCAN_THREADS - 1) / SCAN_THREADS * SCAN_THREADS;
+    return min(max(R, (uint32_t)SCAN_THREADS), (uint32_t)FEC_RANGE_MAX);
+}
+
 __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant__ SpK sp) {
     __shared__ uint32_t s_tab[TMAX];
+    __shared__ uint8_t s_f[FEC_RANGE_MAX];
+    __shared__ uint32_t s_off[FEC_RANGE_MAX];
     __shared__ uint32_t s_warp[SCAN_THREADS / 32];
     __shared__ uint32_t s_tile;
     __shared__ unsigned long long s_excl;
     DevSpecies &st = *sp.st;
     const uint32_t N = st.n0, step = sp.glob->step;
-    const uint32_t n_tiles = (N + SCAN_TILE - 1) / SCAN_TILE;
+    const uint32_t R = fec_range_size(N, gridDim.x);
+    const uint32_t n_ranges = (N + R - 1) / R;
+    const uint32_t per = R / SCAN_THREADS;  // adults per thread in pass 2 (<= 32)
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const bool one_table = sp.n_tables == 1;
     uint32_t len0 = 0;
@@ -150,26 +182,29 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
     for (;;) {
         if (tid == 0) s_tile = atomicAdd(&st.ticket_fec, 1u);
         __syncthreads();
-        const uint32_t tile = s_tile;
-        if (tile >= n_tiles) break;
-        const uint32_t base = tile * SCAN_TILE + tid * SCAN_ITEMS;
-        uint32_t f[SCAN_ITEMS], sum = 0;
-#pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
-            const uint32_t i = base + k;
-            f[k] = 0;
+        const uint32_t range = s_tile;
+        if (range >= n_ranges) break;
+        const uint32_t r0 = range * R;
+        // ---- pass 1: fecundity draws (coalesced in i), staged as bytes
+        for (uint32_t k = tid; k < R; k += SCAN_THREADS) {
+            const uint32_t i = r0 + k;
+            uint32_t f = 0;
             if (i < N) {
                 uint32_t x[4];
                 draw(sp.key, sp.species, ST_FEC, i, 0, step, x);
                 if (one_table) {
-                    f[k] = poisson_count(s_tab, len0, x[0]);
+                    f = poisson_count(s_tab, len0, x[0]);
                 } else {
                     const uint32_t tab = (sp.fec_model == 2) ? min(sp.cap[i], (uint32_t)(CAP_TABLES - 1)) : patch_of(ps, sp.P, i);
-                    f[k] = poisson_count(sp.tables + (size_t)tab * TMAX, sp.table_len[tab], x[0]);
+                    f = poisson_count(sp.tables + (size_t)tab * TMAX, sp.table_len[tab], x[0]);
                 }
             }
-            sum += f[k];
+            s_f[k] = (uint8_t)f;
         }
+        __syncthreads();
+        // ---- block scan over the range: per-thread slices [tid*per, tid*per+per) in shared memory
+        uint32_t sum = 0;
+        for (uint32_t k = 0; k < per; ++k) { s_off[tid * per + k] = sum; sum += s_f[tid * per + k]; }
         const uint32_t incl = warp_incl_scan(sum);
         if (lane == 31) s_warp[warp] = incl;
         __syncthreads();
@@ -177,11 +212,11 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
             uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
             const uint32_t wi = warp_incl_scan(w);
             const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
-            const unsigned long long excl = lookback(sp.status_fec, tile, (unsigned long long)total);
+            const unsigned long long excl = lookback(sp.status_fec, range, (unsigned long long)total);
             if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;  // exclusive warp prefix
             if (lane == 0) {
                 s_excl = excl;
-                if (tile == n_tiles - 1) {  // the last tile knows M
+                if (range == n_ranges - 1) {  // the last range knows M
                     const unsigned long long Mtot = excl + total;
                     if (Mtot > (unsigned long long)sp.capacity) { st.m = sp.capacity; st.flags_step |= 1u; }
                     else st.m = (uint32_t)Mtot;
@@ -189,19 +224,26 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
             }
         }
         __syncthreads();
-        unsigned long long o = s_excl + s_warp[warp] + (incl - sum);
-#pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
-            const uint32_t i = base + k;
-            if (i < N) {
-                sp.off[i] = (uint32_t)min(o, (unsigned long long)0xFFFFFFFFull);
-                sp.f[i] = (uint8_t)f[k];
-                const uint32_t mval = (sp.phys_parents && f[k]) ? rowptr[i] : i;
-                for (uint32_t c = 0; c < f[k]; ++c) {
+        {
+            const uint32_t tbase = s_warp[warp] + (incl - sum);
+            for (uint32_t k = 0; k < per; ++k) s_off[tid * per + k] += tbase;
+        }
+        __syncthreads();
+        // ---- pass 2 (coalesced in i): offsets, f[], mother[]
+        const unsigned long long rbase = s_excl;
+        for (uint32_t k = tid; k < R; k += SCAN_THREADS) {
+            const uint32_t i = r0 + k;
+            if (i >= N) break;
+            const uint32_t f = s_f[k];
+            const unsigned long long o = rbase + s_off[k];
+            sp.off[i] = (uint32_t)min(o, (unsigned long long)0xFFFFFFFFull);
+            sp.f[i] = (uint8_t)f;
+            if (f) {
+                const uint32_t mval = sp.phys_parents ? rowptr[i] : i;
+                for (uint32_t c = 0; c < f; ++c) {
                     const unsigned long long j = o + c;
                     if (j < (unsigned long long)sp.capacity) sp.mother[j] = mval;
                 }
-                o += f[k];
             }
         }
         __syncthreads();
@@ -649,24 +691,6 @@ __global__ void __launch_bounds__(256) k_patch_pos(const __grid_constant__ SpK s
         atomicAdd((unsigned long long *)&st.acc_zi, (unsigned long long)a1);
         atomicAdd((unsigned long long *)&st.acc_zi2, (unsigned long long)a2);
     }
-}
-
-// a9: counts stay on the device; log entry; buffer flip
-__global__ void k_end(const __grid_constant__ SpK sp) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    DevSpecies &st = *sp.st;
-    const uint32_t nn = st.n_next;
-    LogEntry &e = sp.log[st.log_pos % sp.log_capacity];
-    e.n_t = st.n0; e.m_t = st.m; e.n_next = nn;
-    e.sum_zi = st.acc_zi; e.sum_zi2 = st.acc_zi2;
-    e.captures = st.captures; e.near_ties = st.near_ties;
-    e.flags = st.flags_step; e.step = sp.glob->step;
-    st.log_pos += 1;
-    if (st.flags_step) atomicOr(&sp.glob->flags, st.flags_step);
-    st.n = nn;
-    st.sum_zi = st.acc_zi;
-    st.cur ^= 1u;
-    if (sp.P == 1) { uint32_t *psn = sp.patch_start[st.cur]; psn[0] = 0; psn[1] = nn; }
 }
 
 }  // namespace spegg
