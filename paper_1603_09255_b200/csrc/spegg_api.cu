@@ -194,8 +194,8 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.offbuf = c.take(cap * l.row_bytes);
         l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
         l.table_len = c.take((uint64_t)l.n_tables * 4);
-        l.status_fec = c.take((cap / SCAN_THREADS + 2) * 8);
-        l.status_cmp = c.take((cap / 32 + 2) * 8);  // fused tiles are 32 offspring
+        l.status_fec = c.take((cap / SCAN_THREADS + 2 + (cap / SCAN_THREADS + 2) / 32 + 2) * 8);
+        l.status_cmp = c.take((cap / SCAN_TILE + 2 + (cap / SCAN_TILE + 2) / 32 + 2) * 8);
         l.patch_cnt = c.take(P * 5 * 4);
         l.patch_base = c.take(P * 5 * 4);
         l.log = c.take((uint64_t)logcap * sizeof(LogEntry));
@@ -301,8 +301,11 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             k_cmp_scatter<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
         }
     }
-    k_finish_all<<<1, 32, 0, s->stream>>>(s->d_spk, s->p.n_species); ++nl;
-    if (!s->debug) { launch_prepare(s); ++nl; }  // debug: prepared at the start, so the view stays valid
+    const bool solo = s->sp.size() == 1 && s->sp[0].k.solo;  // k_index closes the step itself
+    if (!solo) {
+        k_finish_all<<<1, 32, 0, s->stream>>>(s->d_spk, s->p.n_species); ++nl;
+        if (!s->debug) { launch_prepare(s); ++nl; }  // debug: prepared at the start, so the view stays valid
+    }
     CU(cudaGetLastError());
     if (n_launch) *n_launch = nl;
     return SPEGG_OK;
@@ -455,11 +458,13 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.cap = at<uint32_t>(s, l.cap);
         k.tables = at<uint32_t>(s, l.tables); k.table_len = at<uint32_t>(s, l.table_len);
         k.status_fec = at<unsigned long long>(s, l.status_fec); k.status_cmp = at<unsigned long long>(s, l.status_cmp);
+        k.status_fec_n = (uint32_t)(q.capacity / SCAN_THREADS + 2); k.status_cmp_n = (uint32_t)(q.capacity / SCAN_TILE + 2);
         k.patch_cnt = at<uint32_t>(s, l.patch_cnt); k.patch_base = at<uint32_t>(s, l.patch_base);
         k.st = s->d_st + si; k.st_all = s->d_st; k.glob = s->d_glob;
         k.log = at<LogEntry>(s, l.log); k.log_capacity = s->log_capacity;
         k.debug = p->debug;
         k.phys_parents = fused_ok(s, h) ? 1u : 0u;
+        k.solo = (k.phys_parents && p->n_species == 1) ? 1u : 0u;
     }
     for (uint32_t si = 0; si < p->n_species; ++si)
         if (s->sp[si].p.sel_predation) s->sp[si].k.cap_pred = s->sp[s->sp[si].p.predator_species].k.cap;

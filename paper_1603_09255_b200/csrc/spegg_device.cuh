@@ -126,9 +126,9 @@ __device__ __forceinline__ int normal_delta(const uint32_t *__restrict__ T, int 
 }
 
 // ------------------------------------------------------------ decoupled look-back (one warp)
-// status word = flag(2 bits) << 62 | value; flag 0 = not ready, 1 = tile aggregate, 2 = inclusive
-// prefix.  One 64-bit store publishes value and flag together, so no fence is needed.  Tiles are
-// handed out by an atomic ticket, so every lower-numbered tile has already started.
+// status word = flag(2 bits) << 62 | value; flag 0 = not ready, 1 = tile aggregate.  One 64-bit
+// store publishes value and flag together, so no fence is needed.  Tiles are handed out by an
+// atomic ticket, so every lower-numbered tile has already started (forward progress).
 constexpr unsigned long long LB_MASK = (1ull << 62) - 1ull;
 
 __device__ __forceinline__ unsigned long long ld_status(const unsigned long long *p) {
@@ -140,34 +140,36 @@ __device__ __forceinline__ void st_status(unsigned long long *p, unsigned long l
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-// Called by all 32 lanes of one warp; returns the exclusive prefix of `tile` to every lane.
-__device__ __forceinline__ unsigned long long lookback(unsigned long long *status, uint32_t tile,
-                                                       unsigned long long aggregate) {
+// Two-level counted look-back.  Tiles are numbered by an atomic ticket; groups of 32 consecutive
+// tiles share a counter word gsum[g] = (tiles arrived << 40) | (sum of their aggregates), updated
+// with ONE atomicAdd per tile.  The exclusive prefix of tile r is
+//     sum over complete groups g' < r/32 of gsum[g']  +  aggregates of tiles [32*(r/32), r)
+// so a tile reads at most one 32-wide window of each kind, in parallel, however many tiles are in
+// flight and even when they all finish at the same moment (the usual chained look-back then walks
+// back window by window).  Called by all 32 lanes of one warp; returns the prefix to every lane.
+// status[0..n_tiles_max) holds the per-tile aggregates, gsum = status + n_tiles_max.
+__device__ __forceinline__ unsigned long long lookback(unsigned long long *status, uint32_t n_tiles_max,
+                                                       uint32_t tile, unsigned long long aggregate) {
     const uint32_t lane = threadIdx.x & 31u;
-    if (tile == 0) {
-        if (lane == 0) st_status(status, (2ull << 62) | aggregate);
-        return 0ull;
+    unsigned long long *gsum = status + n_tiles_max;
+    const uint32_t g = tile >> 5, k = tile & 31u;
+    if (lane == 0) {
+        st_status(status + tile, (1ull << 62) | aggregate);
+        atomicAdd(gsum + g, (1ull << 40) | aggregate);
     }
-    if (lane == 0) st_status(status + tile, (1ull << 62) | aggregate);
-    unsigned long long excl = 0ull;
-    int look = (int)tile - 1;
-    for (;;) {
-        const int idx = look - (int)lane;
-        unsigned long long v = (idx >= 0) ? ld_status(status + idx) : (2ull << 62);
-        while (__any_sync(0xffffffffu, (v >> 62) == 0ull)) {
-            if ((v >> 62) == 0ull) v = ld_status(status + idx);
-        }
-        const uint32_t incl = __ballot_sync(0xffffffffu, (v >> 62) == 2ull);
-        const int first = incl ? (__ffs(incl) - 1) : 32;
-        unsigned long long val = ((int)lane <= first) ? (v & LB_MASK) : 0ull;
+    unsigned long long v = 0ull;
+    if (lane < k) {
+        do { v = ld_status(status + (g << 5) + lane); } while ((v >> 62) == 0ull);
+        v &= LB_MASK;
+    }
+    for (uint32_t gg = lane; gg < g; gg += 32) {
+        unsigned long long t;
+        do { t = ld_status(gsum + gg); } while ((t >> 40) != 32ull);
+        v += t & ((1ull << 40) - 1ull);
+    }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xffffffffu, val, o);
-        excl += val;
-        if (incl) break;
-        look -= 32;
-    }
-    if (lane == 0) st_status(status + tile, (2ull << 62) | ((excl + aggregate) & LB_MASK));
-    return excl;
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
 }
 
 __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v) {

@@ -166,9 +166,9 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             const uint32_t src = it * 4 + sub;
             const uint32_t j = j0 + src;
             const bool valid = j < M;
-            const uint32_t pm = __shfl_sync(0xffffffffu, mo, src), pf = __shfl_sync(0xffffffffu, fa, src);
             const float u01 = __shfl_sync(0xffffffffu, ul, src);
             const uint32_t mflag = (__shfl_sync(0xffffffffu, mf, src) >> g) & 1u;
+            const uint32_t pm = __shfl_sync(0xffffffffu, mo, src), pf = __shfl_sync(0xffffffffu, fa, src);
             const uint32_t parent = g ? pf : pm;
             const uint4 *row = pop + (size_t)parent * ROW4 + c * 2;
             const uint4 a = ldg_u4(row), b = ldg_u4(row + 1), d = ldg_u4(row + ROW4 / 2), e = ldg_u4(row + ROW4 / 2 + 1);
@@ -302,7 +302,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_index(const __grid_constant__ 
             uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
             const uint32_t wi = warp_incl_scan(w);
             const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
-            const unsigned long long excl = lookback(sp.status_cmp, tile, (unsigned long long)total);
+            const unsigned long long excl = lookback(sp.status_cmp, sp.status_cmp_n, tile, (unsigned long long)total);
             if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;
             if (lane == 0) {
                 s_excl = excl;
@@ -319,6 +319,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_index(const __grid_constant__ 
         }
         __syncthreads();
     }
+    if (sp.solo) solo_tail(sp, &s_tile);
 }
 
 __host__ inline bool fused_bit_supported(const SpK &k) {

@@ -77,6 +77,7 @@ struct SpK {
     uint32_t *rowptr[2];        // logical adult index -> physical row of pop[]
     uint32_t *chunk_mask;       // fused path: survivor bitmask of each 32-offspring chunk
     uint32_t phys_parents;      // 1: mother[] / father[] hold physical rows (fused path)
+    uint32_t solo;              // 1: single-species simulation (k_index finishes and prepares the step)
     uint8_t *f;
     uint32_t *off, *mother, *father, *dest, *pos;
     float *u01, *s;
@@ -86,7 +87,8 @@ struct SpK {
     uint32_t *cap;              // capture counts of THIS species' adults (CAPTURES model)
     uint32_t *cap_pred;         // capture counts of the predator species (predation term)
     uint32_t *tables, *table_len;
-    unsigned long long *status_fec, *status_cmp;
+    unsigned long long *status_fec, *status_cmp;  // [n] tile aggregates + [n/32+2] group counters
+    uint32_t status_fec_n, status_cmp_n;
     uint32_t *patch_cnt, *patch_base;  // [P][5]
     DevSpecies *st;             // this species
     DevSpecies *st_all;         // all species

@@ -80,45 +80,52 @@ __device__ __forceinline__ float survival_prob(const SpK &sp, float z, float the
 }
 
 // ------------------------------------------------------------------------ step bookkeeping
-// a9: end of step for every species (one thread each): counts stay on the device, log entry,
-// buffer flip; then the step counter advances.  Single block, so nothing races on glob->step.
-__global__ void k_finish_all(const SpK *__restrict__ spk, uint32_t n_species) {
-    if (threadIdx.x < n_species) {
-        const SpK &sp = spk[threadIdx.x];
-        DevSpecies &st = *sp.st;
-        const uint32_t nn = st.n_next;
-        if (st.n0 == 0) st.flags_step |= 2u;
-        LogEntry &e = sp.log[st.log_pos % sp.log_capacity];
-        e.n_t = st.n0; e.m_t = st.m; e.n_next = nn;
-        e.sum_zi = st.acc_zi; e.sum_zi2 = st.acc_zi2;
-        e.captures = st.captures; e.near_ties = st.near_ties;
-        e.flags = st.flags_step; e.step = sp.glob->step;
-        st.log_pos += 1;
-        if (st.flags_step) atomicOr(&sp.glob->flags, st.flags_step);
-        st.n = nn;
-        st.sum_zi = st.acc_zi;
-        st.cur ^= 1u;
-        if (sp.P == 1) { uint32_t *psn = sp.patch_start[st.cur]; psn[0] = 0; psn[1] = nn; }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) spk[0].glob->step += 1;
+__device__ __forceinline__ uint32_t ld_u32(const uint32_t *p) {
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long ld_u64(const void *p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// a9: end of step for one species (one thread): counts stay on the device, log entry, buffer flip.
+// Reads go through L2 (ld.relaxed.gpu) because the caller may be the last CTA of another kernel.
+__device__ __forceinline__ void finish_species(const SpK &sp) {
+    DevSpecies &st = *sp.st;
+    const uint32_t nn = ld_u32(&st.n_next), n0 = ld_u32(&st.n0);
+    uint32_t fl = ld_u32(&st.flags_step);
+    if (n0 == 0) fl |= 2u;
+    const uint32_t lp = ld_u32(&st.log_pos);
+    const long long a1 = (long long)ld_u64(&st.acc_zi), a2 = (long long)ld_u64(&st.acc_zi2);
+    LogEntry &e = sp.log[lp % sp.log_capacity];
+    e.n_t = n0; e.m_t = ld_u32(&st.m); e.n_next = nn;
+    e.sum_zi = a1; e.sum_zi2 = a2;
+    e.captures = ld_u64(&st.captures); e.near_ties = ld_u64(&st.near_ties);
+    e.flags = fl; e.step = ld_u32(&sp.glob->step);
+    st.log_pos = lp + 1;
+    if (fl) atomicOr(&sp.glob->flags, fl);
+    st.n = nn;
+    st.sum_zi = a1;
+    const uint32_t cur = ld_u32(&st.cur) ^ 1u;
+    st.cur = cur;
+    if (sp.P == 1) { uint32_t *psn = sp.patch_start[cur]; psn[0] = 0; psn[1] = nn; }
 }
 
 // a0: everything the next step needs before its first kernel (Fig. 1 F -> A): start-of-step
 // snapshots, fecundity tables from the device-resident counts, theta_t, predation scalars, cleared
-// look-back statuses / tickets / capture counts.  grid = (blocks, n_species).
-__global__ void __launch_bounds__(256) k_prepare_all(const SpK *__restrict__ spk) {
-    const SpK &sp = spk[blockIdx.y];
-    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
-    const uint32_t n_status_fec = sp.capacity / SCAN_THREADS + 2, n_status_cmp = sp.capacity / 32 / SCAN_THREADS + 2;
-    const uint32_t n_status_gen = sp.capacity / SCAN_TILE + 2;
-    for (uint32_t i = g; i < n_status_fec; i += stride) sp.status_fec[i] = 0ull;
-    for (uint32_t i = g; i < max(n_status_cmp, n_status_gen); i += stride) sp.status_cmp[i] = 0ull;
+// look-back statuses / tickets / capture counts.  g / stride: this thread's index and the number
+// of threads sharing the work; N, cur, sum_zi, step: the species' finished state.
+__device__ __forceinline__ void prepare_species(const SpK &sp, uint32_t g, uint32_t stride, uint32_t N,
+                                                uint32_t cur, long long sum_zi, uint32_t step) {
+    const uint32_t nf = sp.status_fec_n + sp.status_fec_n / 32 + 2, nc = sp.status_cmp_n + sp.status_cmp_n / 32 + 2;
+    for (uint32_t i = g; i < nf; i += stride) sp.status_fec[i] = 0ull;
+    for (uint32_t i = g; i < nc; i += stride) sp.status_cmp[i] = 0ull;
     if (sp.fec_model == 2)
         for (uint32_t i = g; i < sp.capacity; i += stride) sp.cap[i] = 0u;
-    DevSpecies &st = *sp.st;
-    const uint32_t N = st.n;
-    const uint32_t *ps = sp.patch_start[st.cur];
+    const uint32_t *ps = sp.patch_start[cur];
     for (uint32_t tab = g; tab < sp.n_tables; tab += stride) {
         double lam;
         if (sp.fec_model == 2) lam = fecundity_mean(sp, (double)N, sp.K, tab);
@@ -127,13 +134,14 @@ __global__ void __launch_bounds__(256) k_prepare_all(const SpK *__restrict__ spk
         sp.table_len[tab] = (uint32_t)build_poisson_table(lam, sp.tables + (size_t)tab * TMAX, TMAX);
     }
     if (g == 0) {
+        DevSpecies &st = *sp.st;
         st.n0 = N;
-        st.sum_zi0 = st.sum_zi;
+        st.sum_zi0 = sum_zi;
         st.m = 0; st.n_next = 0; st.flags_step = 0;
         st.ticket_fec = 0; st.ticket_cmp = 0; st.ticket_fused = 0; st.done_fused = 0;
         st.acc_zi = 0; st.acc_zi2 = 0; st.captures = 0; st.near_ties = 0;
         // R6: theta_t = fp32(theta0 + t*dtheta), fp64, never accumulated
-        st.theta_t = __double2float_rn(__dadd_rn(sp.theta0, __dmul_rn((double)sp.glob->step, sp.dtheta)));
+        st.theta_t = __double2float_rn(__dadd_rn(sp.theta0, __dmul_rn((double)step, sp.dtheta)));
         if (sp.sel_predation) {
             const DevSpecies &pr = sp.st_all[sp.predator];
             const uint32_t NC = pr.n;
@@ -143,6 +151,43 @@ __global__ void __launch_bounds__(256) k_prepare_all(const SpK *__restrict__ spk
             st.attack_n = __double2float_rn(__dmul_rn(sp.attack, (double)NC));
         }
     }
+}
+
+// Single block, so nothing races on glob->step.
+__global__ void k_finish_all(const SpK *__restrict__ spk, uint32_t n_species) {
+    if (threadIdx.x < n_species) finish_species(spk[threadIdx.x]);
+    __syncthreads();
+    if (threadIdx.x == 0) spk[0].glob->step += 1;
+}
+
+// grid = (blocks, n_species)
+__global__ void __launch_bounds__(256) k_prepare_all(const SpK *__restrict__ spk) {
+    const SpK &sp = spk[blockIdx.y];
+    const DevSpecies &st = *sp.st;
+    prepare_species(sp, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, st.n, st.cur, st.sum_zi,
+                    sp.glob->step);
+}
+
+// Tail of the last kernel of a single-species step: the CTA that finishes last closes the step and
+// prepares the next one, saving two launches.  Call from every CTA after its work is done.
+__device__ __forceinline__ void solo_tail(const SpK &sp, uint32_t *s_flag) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        *s_flag = (atomicAdd(&sp.st->done_fused, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!*s_flag) return;
+    __threadfence();
+    if (threadIdx.x == 0) {
+        finish_species(sp);
+        sp.glob->step = ld_u32(&sp.glob->step) + 1;
+        __threadfence();
+    }
+    __syncthreads();
+    DevSpecies &st = *sp.st;
+    prepare_species(sp, threadIdx.x, blockDim.x, ld_u32(&st.n), ld_u32(&st.cur), (long long)ld_u64(&st.sum_zi),
+                    ld_u32(&sp.glob->step));
 }
 
 // a1-a3: fecundity (one FEC block per adult), exclusive scan by decoupled look-back, mother fill.
@@ -212,7 +257,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
             uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
             const uint32_t wi = warp_incl_scan(w);
             const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
-            const unsigned long long excl = lookback(sp.status_fec, range, (unsigned long long)total);
+            const unsigned long long excl = lookback(sp.status_fec, sp.status_fec_n, range, (unsigned long long)total);
             if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;  // exclusive warp prefix
             if (lane == 0) {
                 s_excl = excl;
@@ -515,7 +560,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cmp_scan(const __grid_constant
             uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
             const uint32_t wi = warp_incl_scan(w);
             const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
-            const unsigned long long excl = lookback(sp.status_cmp, tile, (unsigned long long)total);
+            const unsigned long long excl = lookback(sp.status_cmp, sp.status_cmp_n, tile, (unsigned long long)total);
             if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;
             if (lane == 0) {
                 s_excl = excl;
