@@ -275,13 +275,13 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
         HostSpecies &h = s->sp[si];
         const SpK &k = h.k;
         const bool time_this = timed && si == 0 && s->ev_used + 2 <= s->ev.size();
-        k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
         if (fused_ok(s, h)) {
+            launch_scan_fused(k, G, s->stream, 0); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             launch_fused_bit(k, G, s->stream); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
-            launch_index(k, G, s->stream); ++nl;
         } else {
+            k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
             k_scalar<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             if (k.kind == 0) k_gamete_bit<<<G * 8, 256, 0, s->stream>>>(k);
@@ -467,6 +467,8 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.solo = (k.phys_parents && p->n_species == 1) ? 1u : 0u;
     }
     for (uint32_t si = 0; si < p->n_species; ++si)
+        if (s->sp[si].k.phys_parents && fused_bit_configure() != cudaSuccess) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }
+    for (uint32_t si = 0; si < p->n_species; ++si)
         if (s->sp[si].p.sel_predation) s->sp[si].k.cap_pred = s->sp[s->sp[si].p.predator_species].k.cap;
 
     for (uint32_t si = 0; si < p->n_species; ++si)
@@ -515,6 +517,7 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
     std::memset(&st, 0, sizeof st);
     st.cur = cur;
     st.n = (uint32_t)n;
+    st.m_phys = (uint32_t)n;
     CU(cudaMemcpyAsync(s->d_st + species, &st, sizeof st, cudaMemcpyHostToDevice, s->stream));
     DevGlobal g;
     CU(cudaMemcpy(&g, s->d_glob, sizeof g, cudaMemcpyDeviceToHost));
@@ -522,6 +525,7 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
     CU(cudaMemcpyAsync(s->d_glob, &g, sizeof g, cudaMemcpyHostToDevice, s->stream));
     if (n) {
         k_iota<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k.rowptr[cur], (uint32_t)n);
+        if (h.k.phys_parents) k_fill_masks<<<s->n_sms, 256, 0, s->stream>>>(h.k.chunk_mask, (uint32_t)n);
         k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1);
     }
     launch_prepare(s);
@@ -555,6 +559,11 @@ int spegg_read_state(spegg_sim *s, uint32_t species, uint64_t *n, uint32_t *step
     CU(cudaMemcpy(&g, s->d_glob, sizeof g, cudaMemcpyDeviceToHost));
     if (n) *n = st.n;
     if (step) *step = g.step;
+    if ((genomes_out || zi_out) && st.n && h.k.phys_parents) {
+        // fused path: the index (rowptr) of the current buffer is built on demand
+        launch_scan_fused(h.k, s->n_sms, s->stream, 1);
+        launch_prepare(s);   // clears the look-back words and tickets the scan used
+    }
     if (genomes_out) {
         if (cap_bytes < (uint64_t)st.n * h.k.row_bytes) return SPEGG_ERANGE;
         if (st.n) {  // rows in logical order: gather through rowptr into the staging buffer

@@ -1,27 +1,26 @@
-// spegg_fused.cuh -- fused single-pass kernels of the hot configuration (sm_100a).
+// spegg_fused.cuh -- fused two-kernel step of the hot configuration (sm_100a).
 //
 // Bit-packed genomes with NC chromosomes of WPC 32-bit words each (config 3: 4 x 8 words = 1,024
-// loci, 256-byte rows).  After k_fec_scan (fecundity, scan, mother[]) the step is two kernels:
+// loci, 256-byte rows).  One time step is TWO launches:
 //
-//   k_fused_bit   a3-a8 in one pass: father draw, gather of both parents' rows, crossover masks
-//                 from the RECOMB blocks (R8), select, mutate, popcount -> phenotype -> survival,
-//                 survivors stored once into the other population buffer.  Offspring rows never
-//                 touch memory unless they survive.
-//   k_index       stable order of the next generation from 4-byte chunk masks (rowptr).
+//   k_scan_fused  a1-a3 + the index half of a7: one pass over the physical rows of the current
+//                 buffer (32-row slabs, one survivor bitmask per slab): logical adult index by a
+//                 look-back over the alive counts -> rowptr[], Poisson fecundity of every adult,
+//                 second look-back over the fecundities -> mother[] (physical rows), M_t.
+//   k_fused_bit   a3-a8 in one pass: father draw, asynchronous gather of both parents' rows into
+//                 shared memory (cp.async, issued before the recombination draws are computed so
+//                 the gather latency hides behind the Philox work), crossover masks from the
+//                 RECOMB blocks (R8), select, mutate, popcount -> phenotype -> survival; every
+//                 offspring row is stored exactly once at row j of the other buffer, and only the
+//                 4-byte survivor mask of each 32-offspring chunk says which rows are the next
+//                 generation.  Its last CTA closes the step and prepares the next one (a0, a9).
 //
-// Thread mapping of k_fused_bit: 8 consecutive lanes own one offspring, lane q = (gamete g = q/4,
-// chromosome c = q%4): it loads the 8 words of chromosome c of both haplotypes of parent g with
-// four 128-bit loads, computes that chromosome's Philox block, builds its 8 mask words in
-// registers, and stores its 32 bytes of the surviving row with two 128-bit stores.  A warp handles
-// 4 offspring, a 256-thread CTA a tile of 32; tiles come from an atomic ticket and the survivors'
-// positions from the same decoupled look-back as the fecundity scan (stable order in j).
-// Every draw is addressed by (stream, offspring j, block, step), never by thread, so the result is
+// Every draw is addressed by (stream, entity, block, step), never by thread, so the result is
 // bit-identical to the materialised pipeline and to the oracle.
 #pragma once
 #include "spegg_kernels.cuh"
 
 namespace spegg {
-
 
 __device__ __forceinline__ uint32_t shl_clamp(uint32_t v, uint32_t n) {
     uint32_t r;
@@ -29,38 +28,56 @@ __device__ __forceinline__ uint32_t shl_clamp(uint32_t v, uint32_t n) {
     return r;
 }
 
-__device__ __forceinline__ uint4 ldg_u4(const uint4 *p) {
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
     uint4 v;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
 }
 
-// Warp-autonomous fused kernel.  A warp takes a chunk of FUSED_CHUNK = 32 consecutive offspring
-// from an atomic ticket.
-//   prologue (dense, every lane busy, independent Philox chains interleave):
-//     - lane = offspring: mother row, SCALAR block (father -> rowptr -> row, survival uniform),
-//       the two MUT blocks' counts
-//     - lane = (gamete g, chromosome c) of offspring it*4+sub, it = 0..7: the 8 RECOMB blocks this
-//       lane will need, decoded to a packed word (count, start phase, first two positions)
-//     - the few chromosomes with more than two crossovers (8 % at mean 1) are queued and their
-//       extra blocks / mask contributions computed one per lane, so no divergent Philox later
-//   8 passes of 4 offspring (8 lanes each): four 128-bit loads of the lane's 8-word chromosome
-//   from both haplotypes of its parent, mask words from the packed draw (+ queued extras), select,
-//   rare mutation, popcount -> phenotype -> fp32 survival, and the surviving rows are stored,
-//   packed and in j order, at the start of the chunk's own 32-row slab of the other buffer.
-// Nothing waits on another warp: the stable order of the next generation is established
-// afterwards by k_index, which scans the 4-byte chunk masks and writes rowptr (logical adult index
-// -> physical row).  The 256-byte rows are written exactly once; only indices are compacted.
-constexpr int FUSED_CHUNK = 32;
-constexpr int FUSED_WARPS = 8;
+// ones from bit s upward within word w of a 256-bit chromosome: (~0 << clamp(s - 32w, 0, 32))
+__device__ __forceinline__ uint32_t mask_from(int s, int w) {
+    return shl_clamp(0xFFFFFFFFu, (uint32_t)__viaddmax_s32(s, -32 * w, 0));
+}
 
+constexpr int FUSED_CHUNK = 32;                 // offspring per warp iteration = rows per slab
+constexpr int FUSED_WARPS = 4;                  // warps per CTA; 3 CTAs per SM by shared memory
+constexpr uint32_t FUSED_ROW = 256;             // bytes per row (config 3)
+constexpr uint32_t FUSED_FA_OFF = FUSED_CHUNK * FUSED_ROW + 16;  // fathers' rows: +16 B rotates the banks
+constexpr uint32_t FUSED_STAGE = FUSED_FA_OFF + FUSED_CHUNK * FUSED_ROW;
+constexpr uint32_t FUSED_SP_OFF = FUSED_STAGE;                   // packed recombination draws [8][32]
+constexpr uint32_t FUSED_XM_OFF = FUSED_SP_OFF + 8 * 32 * 4;     // extra-crossover masks [32][2] uint4
+constexpr uint32_t FUSED_Q_OFF = FUSED_XM_OFF + 32 * 32;         // queue [32]
+constexpr uint32_t FUSED_WARP_BYTES = FUSED_Q_OFF + 32 * 4;
+constexpr uint32_t FUSED_SMEM = FUSED_WARPS * FUSED_WARP_BYTES;
+
+// Warp-autonomous fused kernel.  A warp takes a chunk of 32 consecutive offspring from an atomic
+// ticket (the next ticket is fetched while the current chunk is processed).
+//   (a) lane = offspring: mother row, SCALAR block (father -> rowptr -> row, survival uniform), the
+//       two MUT blocks' counts.
+//   (b) 32 cp.async instructions start the gather of the chunk's 64 parent rows (16 KB) into this
+//       warp's stage: half a warp copies one 256-byte row with 16-byte pieces.
+//   (c) lane = (gamete g, chromosome c) of offspring it*4+sub, it = 0..7: the 8 RECOMB blocks this
+//       lane will need, decoded to a packed word (count, start phase, first two positions); the few
+//       chromosomes with more than two crossovers (8 % at mean 1) are queued and their extra
+//       blocks / mask contributions computed one per lane.  The gather lands meanwhile.
+//   (d) 8 passes of 4 offspring (8 lanes each): four conflict-free 128-bit shared loads of the
+//       lane's 8-word chromosome from both haplotypes of its parent, mask words from the packed
+//       draw (+ queued extras), select, rare mutation, popcount, two 128-bit stores of the lane's
+//       32 bytes of offspring row j.
+//   (e) lane = offspring: phenotype -> fp32 survival -> decision; the ballot is the chunk's mask.
 template <int NC, int WPC>
 __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_constant__ SpK sp) {
     static_assert(NC == 4 && WPC == 8, "lane group of 8 = 2 gametes x 4 chromosomes of 8 words");
-    __shared__ uint4 s_xmask[FUSED_WARPS][32][2];   // mask contribution of queued extra crossovers
-    __shared__ uint32_t s_P[FUSED_WARPS][8][32];    // packed recombination draws of the chunk
-    __shared__ uint32_t s_q[FUSED_WARPS][32];       // queue of chromosomes with > 2 crossovers
+    extern __shared__ __align__(128) uint8_t s_dyn[];
+    __shared__ uint32_t s_flag;
     DevSpecies &st = *sp.st;
     const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
     const uint32_t n_chunks = (M + FUSED_CHUNK - 1) / FUSED_CHUNK;
@@ -68,7 +85,12 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
     const uint32_t sub = lane >> 3, q = lane & 7u, g = q >> 2, c = q & 3u;
     constexpr uint32_t ROW4 = 2 * NC * WPC / 4;   // uint4 per row (16)
     constexpr uint32_t L = NC * WPC * 32;
-    const uint4 *pop = (const uint4 *)sp.pop[st.cur];
+    uint8_t *wbase = s_dyn + warp * FUSED_WARP_BYTES;
+    const uint32_t stage = smem_u32(wbase);
+    uint32_t *s_P = (uint32_t *)(wbase + FUSED_SP_OFF);
+    uint4 *s_xmask = (uint4 *)(wbase + FUSED_XM_OFF);
+    uint32_t *s_q = (uint32_t *)(wbase + FUSED_Q_OFF);
+    const uint8_t *pop = sp.pop[st.cur];
     uint4 *nxt = (uint4 *)sp.pop[st.cur ^ 1u];
     const uint32_t *rowptr = sp.rowptr[st.cur];
     const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
@@ -83,20 +105,25 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
     const uint32_t Tm0 = sp.mut_len ? sp.T_mut[0] : 0xFFFFFFFFu;
     const bool has_mut = sp.mut_len != 0;
     const float theta = st.theta_t;
+    // per-lane constant parts of the stage addresses
+    const uint32_t cp_dst = stage + (lane >> 4) * FUSED_ROW + (lane & 15u) * 16u;   // + k * 512 (+ FA_OFF)
+    const uint32_t cp_src = (lane & 15u) * 16u;
+    const uint32_t ld_src = stage + g * FUSED_FA_OFF + sub * FUSED_ROW + c * 32u;   // + it * 1024
     long long acc1 = 0, acc2 = 0;
-    uint32_t ties = 0;
+    uint32_t ties = 0, n_alive = 0;
 
-    for (;;) {
-        uint32_t chunk = 0;
-        if (lane == 0) chunk = atomicAdd(&st.ticket_fused, 1u);
-        chunk = __shfl_sync(0xffffffffu, chunk, 0);
-        if (chunk >= n_chunks) break;
+    uint32_t chunk = 0;
+    if (lane == 0) chunk = atomicAdd(&st.ticket_fused, 1u);
+    chunk = __shfl_sync(0xffffffffu, chunk, 0);
+    while (chunk < n_chunks) {
+        uint32_t next_chunk = 0;
+        if (lane == 0) next_chunk = atomicAdd(&st.ticket_fused, 1u);   // consumed at the loop end
         const uint32_t j0 = chunk * FUSED_CHUNK;
-        // ---- prologue (a): lane = offspring j0 + lane
+        // ---- (a) lane = offspring j0 + lane
         uint32_t mo = 0, fa = 0, mf = 0;
         float ul = 2.0f;
+        const uint32_t jl = j0 + lane;
         {
-            const uint32_t jl = j0 + lane;
             uint32_t x[4], a[4], b[4];
             draw(sp.key, sp.species, ST_SCALAR, jl, 0, step, x);
             draw(sp.key, sp.species, ST_MUT_M, jl, 0, step, a);
@@ -108,7 +135,19 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
                 if (has_mut) mf = (a[0] >= Tm0 ? 1u : 0u) | (b[0] >= Tm0 ? 2u : 0u);
             }
         }
-        // ---- prologue (b): the 8 RECOMB blocks of this lane's (gamete, chromosome) role
+        // ---- (b) start the gather: half-warp h copies the row of offspring 2k+h
+#pragma unroll
+        for (int k = 0; k < FUSED_CHUNK / 2; ++k) {
+            const uint32_t pm = __shfl_sync(0xffffffffu, mo, 2 * k + (lane >> 4));
+            cp_async16(cp_dst + k * 2 * FUSED_ROW, pop + (size_t)pm * FUSED_ROW + cp_src);
+        }
+#pragma unroll
+        for (int k = 0; k < FUSED_CHUNK / 2; ++k) {
+            const uint32_t pf = __shfl_sync(0xffffffffu, fa, 2 * k + (lane >> 4));
+            cp_async16(cp_dst + FUSED_FA_OFF + k * 2 * FUSED_ROW, pop + (size_t)pf * FUSED_ROW + cp_src);
+        }
+        cp_async_commit();
+        // ---- (c) the 8 RECOMB blocks of this lane's (gamete, chromosome) role
         uint32_t qn = 0;
 #pragma unroll
         for (int it = 0; it < 8; ++it) {
@@ -126,15 +165,15 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             uint32_t id = 63;
             if (need) {
                 const uint32_t e = qn + __popc(bal & ((1u << lane) - 1u));
-                if (e < 32) { id = e; s_q[warp][e] = (nc << 8) | ((uint32_t)it << 5) | lane; }
+                if (e < 32) { id = e; s_q[e] = (nc << 8) | ((uint32_t)it << 5) | lane; }
             }
             qn += __popc(bal);
-            s_P[warp][it][lane] = P | (id << 24);
+            s_P[it * 32 + lane] = P | (id << 24);
         }
         __syncwarp();
-        // ---- prologue (c): one lane per queued chromosome computes its extra crossovers
+        // one lane per queued chromosome computes its extra crossovers
         if (lane < min(qn, 32u)) {
-            const uint32_t e = s_q[warp][lane];
+            const uint32_t e = s_q[lane];
             const uint32_t e_nc = e >> 8, e_it = (e >> 5) & 7u, e_ln = e & 31u;
             const uint32_t e_c = e_ln & 3u, e_g = (e_ln >> 2) & 1u;
             const uint32_t e_j = j0 + e_it * 4 + (e_ln >> 3);
@@ -151,44 +190,38 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
                     if (b * 4 + i < extra) {
                         const int s = (int)__umulhi(y[i], e_clen1) + 1;
 #pragma unroll
-                        for (int w = 0; w < 8; ++w) xm[w] ^= shl_clamp(0xFFFFFFFFu, (uint32_t)max(s - 32 * w, 0));
+                        for (int w = 0; w < 8; ++w) xm[w] ^= mask_from(s, w);
                     }
                 }
             }
-            s_xmask[warp][lane][0] = make_uint4(xm[0], xm[1], xm[2], xm[3]);
-            s_xmask[warp][lane][1] = make_uint4(xm[4], xm[5], xm[6], xm[7]);
+            s_xmask[lane * 2] = make_uint4(xm[0], xm[1], xm[2], xm[3]);
+            s_xmask[lane * 2 + 1] = make_uint4(xm[4], xm[5], xm[6], xm[7]);
         }
+        cp_async_wait_all();
         __syncwarp();
 
-        uint32_t cnt = 0, cmask = 0;  // survivors stored so far / survivor bitmask (warp-uniform)
-#pragma unroll 1
+        // ---- (d) 8 passes of 4 offspring
+        int myzi = 0;
+#pragma unroll 2
         for (uint32_t it = 0; it < FUSED_CHUNK / 4; ++it) {
-            const uint32_t src = it * 4 + sub;
-            const uint32_t j = j0 + src;
-            const bool valid = j < M;
-            const float u01 = __shfl_sync(0xffffffffu, ul, src);
-            const uint32_t mflag = (__shfl_sync(0xffffffffu, mf, src) >> g) & 1u;
-            const uint32_t pm = __shfl_sync(0xffffffffu, mo, src), pf = __shfl_sync(0xffffffffu, fa, src);
-            const uint32_t parent = g ? pf : pm;
-            const uint4 *row = pop + (size_t)parent * ROW4 + c * 2;
-            const uint4 a = ldg_u4(row), b = ldg_u4(row + 1), d = ldg_u4(row + ROW4 / 2), e = ldg_u4(row + ROW4 / 2 + 1);
+            const uint32_t j = j0 + it * 4 + sub;
+            const uint32_t a_ = ld_src + it * 4 * FUSED_ROW;
+            const uint4 a = lds128(a_), b = lds128(a_ + 16), d = lds128(a_ + 128), e = lds128(a_ + 144);
             const uint32_t h0[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
             const uint32_t h1[8] = {d.x, d.y, d.z, d.w, e.x, e.y, e.z, e.w};
-            // ---- R8: crossover mask of chromosome c of gamete g from the packed draw
-            const uint32_t P = s_P[warp][it][lane];
+            // R8: crossover mask of chromosome c of gamete g from the packed draw
+            const uint32_t P = s_P[it * 32 + lane];
             const uint32_t nc = P & 63u;
             const uint32_t phi = ((P >> 6) & 1u) ? 0xFFFFFFFFu : 0u;
             const int s0 = nc > 0 ? (int)((P >> 8) & 0xFFu) : 4096;
             const int s1 = nc > 1 ? (int)((P >> 16) & 0xFFu) : 4096;
             uint32_t m[8];
 #pragma unroll
-            for (int w = 0; w < 8; ++w)
-                m[w] = phi ^ shl_clamp(0xFFFFFFFFu, (uint32_t)max(s0 - 32 * w, 0)) ^
-                       shl_clamp(0xFFFFFFFFu, (uint32_t)max(s1 - 32 * w, 0));
+            for (int w = 0; w < 8; ++w) m[w] = phi ^ mask_from(s0, w) ^ mask_from(s1, w);
             if (nc > 2) {
                 const uint32_t id = (P >> 24) & 63u;
                 if (id < 32) {
-                    const uint4 xa = s_xmask[warp][id][0], xb = s_xmask[warp][id][1];
+                    const uint4 xa = s_xmask[id * 2], xb = s_xmask[id * 2 + 1];
                     m[0] ^= xa.x; m[1] ^= xa.y; m[2] ^= xa.z; m[3] ^= xa.w;
                     m[4] ^= xb.x; m[5] ^= xb.y; m[6] ^= xb.z; m[7] ^= xb.w;
                 } else {  // queue overflow (> 32 such chromosomes in one chunk): compute in place
@@ -201,17 +234,18 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
                             if (bb * 4 + i < extra) {
                                 const int s = (int)__umulhi(y[i], clen1) + 1;
 #pragma unroll
-                                for (int w = 0; w < 8; ++w) m[w] ^= shl_clamp(0xFFFFFFFFu, (uint32_t)max(s - 32 * w, 0));
+                                for (int w = 0; w < 8; ++w) m[w] ^= mask_from(s, w);
                             }
                         }
                     }
                 }
             }
-            // ---- select: gamete word = hap[phase] word
+            // select: gamete word = hap[phase] word
             uint32_t gw[8];
 #pragma unroll
             for (int w = 0; w < 8; ++w) gw[w] = (h0[w] & ~m[w]) | (h1[w] & m[w]);
-            // ---- R9: mutation (rare; flagged per gamete in the prologue)
+            // R9: mutation (rare; flagged per gamete in (a))
+            const uint32_t mflag = (__shfl_sync(0xffffffffu, mf, it * 4 + sub) >> g) & 1u;
             if (mflag) {
                 const uint32_t ms = g ? ST_MUT_P : ST_MUT_M;
                 uint32_t x[4];
@@ -228,36 +262,35 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
                     }
                 }
             }
-            // ---- a5: additive phenotype, exact integer (R10)
+            // a7: the row is stored once, at row j of the other buffer (alive or not)
+            if (j < M) {
+                uint4 *o = nxt + (size_t)j * ROW4 + g * (ROW4 / 2) + c * 2;
+                o[0] = make_uint4(gw[0], gw[1], gw[2], gw[3]);
+                o[1] = make_uint4(gw[4], gw[5], gw[6], gw[7]);
+            }
+            // a5: additive phenotype, exact integer (R10); handed to the lane that owns offspring j
             int ones = 0;
 #pragma unroll
             for (int w = 0; w < 8; ++w) ones += __popc(gw[w]);
             ones += __shfl_xor_sync(0xffffffffu, ones, 1);
             ones += __shfl_xor_sync(0xffffffffu, ones, 2);
             ones += __shfl_xor_sync(0xffffffffu, ones, 4);
-            const int zi = 2 * ones - 2 * (int)L;
-            // ---- a6: survival (R11), same fp32 sequence as the materialised path
-            bool captured;
-            const float z = __fmul_rn((float)zi, sp.pheno_scale);
-            const float s = survival_prob(sp, z, theta, u01, captured);
-            const bool alive = valid && (u01 < s);
-            if (valid && q == 0) {
-                if (fabsf(__fsub_rn(u01, s)) < 1e-6f) ++ties;
-                if (alive) { acc1 += zi; acc2 += (long long)zi * zi; }
-            }
-            // ---- a7: store the surviving row at its rank within the chunk's slab
-            const uint32_t bal = __ballot_sync(0xffffffffu, alive && q == 0);
-            if (alive) {
-                const uint32_t slot = j0 + cnt + __popc(bal & ((1u << (lane & 24u)) - 1u));
-                uint4 *o = nxt + (size_t)slot * ROW4 + g * (ROW4 / 2) + c * 2;
-                o[0] = make_uint4(gw[0], gw[1], gw[2], gw[3]);
-                o[1] = make_uint4(gw[4], gw[5], gw[6], gw[7]);
-            }
-            cnt += __popc(bal);
-            cmask |= ((bal & 1u) | ((bal >> 7) & 2u) | ((bal >> 14) & 4u) | ((bal >> 21) & 8u)) << (it * 4);
+            const int zo = __shfl_sync(0xffffffffu, ones, (lane & 3u) * 8u);
+            if ((lane >> 2) == it) myzi = 2 * zo - 2 * (int)L;
         }
-        if (lane == 0) sp.chunk_mask[chunk] = cmask;
-        __syncwarp();
+        // ---- (e) a6: survival (R11), lane = offspring; same fp32 sequence as the materialised path
+        {
+            bool captured;
+            const float z = __fmul_rn((float)myzi, sp.pheno_scale);
+            const float s = survival_prob(sp, z, theta, ul, captured);
+            const bool valid = jl < M;
+            const bool alive = valid && (ul < s);
+            if (valid && fabsf(__fsub_rn(ul, s)) < 1e-6f) ++ties;
+            if (alive) { acc1 += myzi; acc2 += (long long)myzi * myzi; ++n_alive; }
+            const uint32_t bal = __ballot_sync(0xffffffffu, alive);
+            if (lane == 0) sp.chunk_mask[chunk] = bal;
+        }
+        chunk = __shfl_sync(0xffffffffu, next_chunk, 0);   // also orders the stage reuse
     }
     // ---- a8: survivor reductions (exact integers)
 #pragma unroll
@@ -265,6 +298,7 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
         acc1 += __shfl_xor_sync(0xffffffffu, acc1, o);
         acc2 += __shfl_xor_sync(0xffffffffu, acc2, o);
         ties += __shfl_xor_sync(0xffffffffu, ties, o);
+        n_alive += __shfl_xor_sync(0xffffffffu, n_alive, o);
     }
     if (lane == 0) {
         if (acc1 != 0 || acc2 != 0) {
@@ -272,54 +306,114 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             atomicAdd((unsigned long long *)&st.acc_zi2, (unsigned long long)acc2);
         }
         if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
+        if (n_alive) atomicAdd(&st.n_next, n_alive);
     }
+    if (sp.solo) solo_tail(sp, &s_flag);
 }
 
-// a7: stable order of the next generation.  One thread per chunk: exclusive scan of the chunks'
-// survivor counts (decoupled look-back over tiles of 256 chunks), then one warp per chunk writes
-// rowptr_next[base + r] = 32*chunk + r (coalesced).  Moves 4 bytes per survivor instead of rows.
-__global__ void __launch_bounds__(SCAN_THREADS) k_index(const __grid_constant__ SpK sp) {
+// a1-a3 and the index half of a7 for a species on the fused path.  The current buffer holds
+// m_phys physical rows in 32-row slabs; chunk_mask says which are adults.  A CTA takes a range of
+// 2,048 rows (8 per thread):
+//   look-back 1 over the alive counts  -> logical index i of every adult, rowptr[i] = row
+//   FEC draw of adult i                -> fecundity f_i  (R5)
+//   look-back 2 over the fecundities   -> offspring base off_i, mother[off_i .. off_i+f_i) = row
+// index_only = 1 builds rowptr alone (spegg_read_state).
+constexpr int SCANF_ROWS = 8;
+constexpr int SCANF_RANGE = SCAN_THREADS * SCANF_ROWS;
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_constant__ SpK sp, int index_only) {
+    __shared__ uint32_t s_tab[TMAX];
     __shared__ uint32_t s_warp[SCAN_THREADS / 32];
-    __shared__ uint32_t s_base[SCAN_THREADS], s_cnt[SCAN_THREADS];
     __shared__ uint32_t s_tile;
     __shared__ unsigned long long s_excl;
     DevSpecies &st = *sp.st;
-    const uint32_t n_chunks = (st.m + FUSED_CHUNK - 1) / FUSED_CHUNK;
-    const uint32_t n_tiles = (n_chunks + SCAN_THREADS - 1) / SCAN_THREADS;
+    const uint32_t mp = st.m_phys, step = sp.glob->step;
+    const uint32_t n_ranges = (mp + SCANF_RANGE - 1) / SCANF_RANGE;
+    const uint32_t n_chunks = (mp + FUSED_CHUNK - 1) / FUSED_CHUNK;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    uint32_t *rp = sp.rowptr[st.cur ^ 1u];
+    const uint32_t len0 = sp.table_len[0];
+    for (uint32_t i = tid; i < len0; i += SCAN_THREADS) s_tab[i] = sp.tables[i];
+    uint32_t *rp = sp.rowptr[st.cur];
     for (;;) {
         if (tid == 0) s_tile = atomicAdd(&st.ticket_cmp, 1u);
         __syncthreads();
-        const uint32_t tile = s_tile;
-        if (tile >= n_tiles) break;
-        const uint32_t ch = tile * SCAN_THREADS + tid;
-        const uint32_t cnt = ch < n_chunks ? __popc(sp.chunk_mask[ch]) : 0u;
+        const uint32_t range = s_tile;
+        if (range >= n_ranges) break;
+        const uint32_t row0 = range * SCANF_RANGE + tid * SCANF_ROWS;
+        const uint32_t ch = row0 >> 5;
+        const uint32_t bits = ch < n_chunks ? (sp.chunk_mask[ch] >> (row0 & 31u)) & 0xFFu : 0u;
+        // ---- look-back 1: adults before this thread's rows
+        const uint32_t cnt = __popc(bits);
         const uint32_t incl = warp_incl_scan(cnt);
         if (lane == 31) s_warp[warp] = incl;
         __syncthreads();
         if (warp == 0) {
-            uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
+            const uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
             const uint32_t wi = warp_incl_scan(w);
             const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
-            const unsigned long long excl = lookback(sp.status_cmp, sp.status_cmp_n, tile, (unsigned long long)total);
+            const unsigned long long excl = lookback(sp.status_cmp, sp.status_cmp_n, range, (unsigned long long)total);
+            if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;
+            if (lane == 0) s_excl = excl;
+        }
+        __syncthreads();
+        uint32_t i = (uint32_t)s_excl + s_warp[warp] + (incl - cnt);
+        // ---- rowptr and fecundity of this thread's adults
+        uint32_t fsum = 0;
+        unsigned long long fpack = 0ull;
+#pragma unroll
+        for (int k = 0; k < SCANF_ROWS; ++k) {
+            if ((bits >> k) & 1u) {
+                rp[i] = row0 + k;
+                if (!index_only) {
+                    uint32_t x[4];
+                    draw(sp.key, sp.species, ST_FEC, i, 0, step, x);
+                    const uint32_t f = poisson_count(s_tab, len0, x[0]);
+                    fpack |= (unsigned long long)f << (8 * k);
+                    fsum += f;
+                }
+                ++i;
+            }
+        }
+        __syncthreads();   // s_warp / s_excl are reused
+        if (index_only) continue;
+        // ---- look-back 2: offspring before this thread's adults
+        const uint32_t fincl = warp_incl_scan(fsum);
+        if (lane == 31) s_warp[warp] = fincl;
+        __syncthreads();
+        if (warp == 0) {
+            const uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
+            const uint32_t wi = warp_incl_scan(w);
+            const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
+            const unsigned long long excl = lookback(sp.status_fec, sp.status_fec_n, range, (unsigned long long)total);
             if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;
             if (lane == 0) {
                 s_excl = excl;
-                if (tile == n_tiles - 1) st.n_next = (uint32_t)(excl + total);
+                if (range == n_ranges - 1) {  // the last range knows M
+                    const unsigned long long Mtot = excl + total;
+                    if (Mtot > (unsigned long long)sp.capacity) { st.m = sp.capacity; st.flags_step |= 1u; }
+                    else st.m = (uint32_t)Mtot;
+                }
             }
         }
         __syncthreads();
-        s_base[tid] = (uint32_t)s_excl + s_warp[warp] + (incl - cnt);
-        s_cnt[tid] = cnt;
-        __syncthreads();
-        for (uint32_t k = 0; k < 32; ++k) {
-            const uint32_t t = warp * 32 + k;
-            if (lane < s_cnt[t]) rp[s_base[t] + lane] = (tile * SCAN_THREADS + t) * FUSED_CHUNK + lane;
+        unsigned long long o = s_excl + s_warp[warp] + (fincl - fsum);
+#pragma unroll
+        for (int k = 0; k < SCANF_ROWS; ++k) {
+            const uint32_t f = (uint32_t)(fpack >> (8 * k)) & 0xFFu;
+            for (uint32_t cpy = 0; cpy < f; ++cpy, ++o)
+                if (o < (unsigned long long)sp.capacity) sp.mother[o] = row0 + k;
         }
         __syncthreads();
     }
-    if (sp.solo) solo_tail(sp, &s_tile);
+}
+
+// chunk masks of a freshly written, dense population of n rows
+__global__ void __launch_bounds__(256) k_fill_masks(uint32_t *mask, uint32_t n) {
+    const uint32_t n_chunks = (n + 31) / 32;
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < n_chunks; c += gridDim.x * blockDim.x) {
+        const uint32_t r = n - c * 32;
+        mask[c] = r >= 32 ? 0xFFFFFFFFu : ((1u << r) - 1u);
+    }
 }
 
 __host__ inline bool fused_bit_supported(const SpK &k) {
@@ -327,12 +421,16 @@ __host__ inline bool fused_bit_supported(const SpK &k) {
            k.fec_model != 2 && k.theta_patch == nullptr;
 }
 
-inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
-    k_fused_bit<4, 8><<<n_sms * 3, FUSED_WARPS * 32, 0, stream>>>(k);
+inline cudaError_t fused_bit_configure() {
+    return cudaFuncSetAttribute(k_fused_bit<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSED_SMEM);
 }
 
-inline void launch_index(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
-    k_index<<<n_sms * 2, SCAN_THREADS, 0, stream>>>(k);
+inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
+    k_fused_bit<4, 8><<<n_sms * 3, FUSED_WARPS * 32, FUSED_SMEM, stream>>>(k);
+}
+
+inline void launch_scan_fused(const SpK &k, uint32_t n_sms, cudaStream_t stream, int index_only) {
+    k_scan_fused<<<n_sms * 2, SCAN_THREADS, 0, stream>>>(k, index_only);
 }
 
 }  // namespace spegg

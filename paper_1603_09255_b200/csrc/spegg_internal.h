@@ -24,7 +24,7 @@ struct DevSpecies {
     uint32_t flags_step;   // flags raised during the current step
     uint32_t ticket_fec, ticket_cmp, ticket_fused, done_fused;
     uint32_t log_pos;      // entries written to the log ring
-    uint32_t pad0;
+    uint32_t m_phys;       // fused path: physical rows of the current buffer (32-row slabs + chunk_mask)
     long long sum_zi;      // over the current adults (survivors of the last step)
     long long sum_zi0;     // snapshot at the start of the step
     long long acc_zi, acc_zi2;  // accumulators of the current step's survivors

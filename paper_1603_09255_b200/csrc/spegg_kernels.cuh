@@ -108,6 +108,7 @@ __device__ __forceinline__ void finish_species(const SpK &sp) {
     st.log_pos = lp + 1;
     if (fl) atomicOr(&sp.glob->flags, fl);
     st.n = nn;
+    if (sp.phys_parents) st.m_phys = ld_u32(&st.m);   // every offspring row was stored; the masks say which live
     st.sum_zi = a1;
     const uint32_t cur = ld_u32(&st.cur) ^ 1u;
     st.cur = cur;
