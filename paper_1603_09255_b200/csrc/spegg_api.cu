@@ -440,6 +440,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.T_mig = h_bernoulli_T(q.migration);
         k.n_tables = l.n_tables;
         k.key.k0 = (uint32_t)p->seed; k.key.k1 = (uint32_t)(p->seed >> 32);
+        for (uint32_t r = 0; r < 10; ++r) { k.rk[2 * r] = k.key.k0 + r * 0x9E3779B9u; k.rk[2 * r + 1] = k.key.k1 + r * 0xBB67AE85u; }
         k.T_recomb = at<uint32_t>(s, l.T_recomb);
         k.T_xover = at<uint32_t>(s, l.T_xover); k.xover_len = at<uint32_t>(s, l.xover_len);
         k.chrom_start = at<uint32_t>(s, l.chrom_start); k.chrom_len = at<uint32_t>(s, l.chrom_len);

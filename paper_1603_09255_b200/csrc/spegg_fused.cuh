@@ -58,20 +58,43 @@ constexpr uint32_t FUSED_Q_OFF = FUSED_XM_OFF + 32 * 32;         // queue [32]
 constexpr uint32_t FUSED_WARP_BYTES = FUSED_Q_OFF + 32 * 4;
 constexpr uint32_t FUSED_SMEM = FUSED_WARPS * FUSED_WARP_BYTES;
 
-// Warp-autonomous fused kernel.  A warp takes a chunk of 32 consecutive offspring from an atomic
-// ticket (the next ticket is fetched while the current chunk is processed).
-//   (a) lane = offspring: mother row, SCALAR block (father -> rowptr -> row, survival uniform), the
-//       two MUT blocks' counts.
+// Philox4x32-10 (R3) with the ten round keys taken from the kernel parameter block: the key
+// schedule k_r = k_0 + r * Weyl is the same for every draw of a simulation, so the host computes it
+// once (SpK::rk) and the XORs read it straight from the constant bank -- four instructions a round.
+__device__ __forceinline__ void draw_rk(const SpK &sp, uint32_t stream, uint32_t entity, uint32_t block,
+                                        uint32_t step, uint32_t (&o)[4]) {
+    uint32_t c0 = entity, c1 = block, c2 = step, c3 = (sp.species << 8) | stream;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ sp.rk[2 * r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ sp.rk[2 * r + 1];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
+}
+
+// Warp-autonomous fused kernel.  A warp takes chunks of 32 consecutive offspring from an atomic
+// ticket; the scalar work of a chunk is done one chunk ahead so that no index load is waited for.
+//   (a) lane = offspring: SCALAR block (father -> rowptr -> row, survival uniform), the two MUT
+//       blocks' counts, mother row.  Computed for the NEXT chunk while the current one is gathered.
 //   (b) 32 cp.async instructions start the gather of the chunk's 64 parent rows (16 KB) into this
 //       warp's stage: half a warp copies one 256-byte row with 16-byte pieces.
 //   (c) lane = (gamete g, chromosome c) of offspring it*4+sub, it = 0..7: the 8 RECOMB blocks this
 //       lane will need, decoded to a packed word (count, start phase, first two positions); the few
 //       chromosomes with more than two crossovers (8 % at mean 1) are queued and their extra
 //       blocks / mask contributions computed one per lane.  The gather lands meanwhile.
+//   (m) rare: a lane whose offspring carries a mutation flips that bit in BOTH haplotypes of the
+//       staged copy of the parent's row (the copy is private to the offspring), which flips it in
+//       the gamete whatever the phase is (R9) and keeps mutation out of the inner loop.
 //   (d) 8 passes of 4 offspring (8 lanes each): four conflict-free 128-bit shared loads of the
 //       lane's 8-word chromosome from both haplotypes of its parent, mask words from the packed
-//       draw (+ queued extras), select, rare mutation, popcount, two 128-bit stores of the lane's
-//       32 bytes of offspring row j.
+//       draw (+ queued extras), select, popcount, two 128-bit stores of the lane's 32 bytes of
+//       offspring row j.
 //   (e) lane = offspring: phenotype -> fp32 survival -> decision; the ballot is the chunk's mask.
 template <int NC, int WPC>
 __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_constant__ SpK sp) {
@@ -112,48 +135,57 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
     long long acc1 = 0, acc2 = 0;
     uint32_t ties = 0, n_alive = 0;
 
-    uint32_t chunk = 0;
-    if (lane == 0) chunk = atomicAdd(&st.ticket_fused, 1u);
-    chunk = __shfl_sync(0xffffffffu, chunk, 0);
-    while (chunk < n_chunks) {
-        uint32_t next_chunk = 0;
-        if (lane == 0) next_chunk = atomicAdd(&st.ticket_fused, 1u);   // consumed at the loop end
-        const uint32_t j0 = chunk * FUSED_CHUNK;
-        // ---- (a) lane = offspring j0 + lane
-        uint32_t mo = 0, fa = 0, mf = 0;
-        float ul = 2.0f;
-        const uint32_t jl = j0 + lane;
-        {
-            uint32_t x[4], a[4], b[4];
-            draw(sp.key, sp.species, ST_SCALAR, jl, 0, step, x);
-            draw(sp.key, sp.species, ST_MUT_M, jl, 0, step, a);
-            draw(sp.key, sp.species, ST_MUT_P, jl, 0, step, b);
-            if (jl < M) {
-                mo = sp.mother[jl];                        // physical row (phys_parents)
-                fa = rowptr[uniform_index(x[0], N)];       // R2: uniform mate, selfing allowed
-                ul = u01_of(x[3]);
-                if (has_mut) mf = (a[0] >= Tm0 ? 1u : 0u) | (b[0] >= Tm0 ? 2u : 0u);
-            }
+    // (a): scalar draws and index loads of offspring jl; the loads are consumed a chunk later
+    auto scalar_stage = [&](uint32_t jl, uint32_t &mo, uint32_t &fa, float &ul, uint32_t &mf) {
+        uint32_t x[4], a[4], b[4];
+        draw_rk(sp, ST_SCALAR, jl, 0, step, x);
+        draw_rk(sp, ST_MUT_M, jl, 0, step, a);
+        draw_rk(sp, ST_MUT_P, jl, 0, step, b);
+        mo = 0; fa = 0; mf = 0; ul = 2.0f;
+        if (jl < M) {
+            // physical rows (phys_parents) as 32-bit byte offsets into the buffer (capacity * 256 < 2^32)
+            mo = sp.mother[jl] * FUSED_ROW;
+            fa = rowptr[uniform_index(x[0], N)] * FUSED_ROW;   // R2: uniform mate, selfing allowed
+            ul = u01_of(x[3]);
+            if (has_mut) mf = (a[0] >= Tm0 ? 1u : 0u) | (b[0] >= Tm0 ? 2u : 0u);
         }
+    };
+
+    uint32_t chunk = 0, chunk1 = 0;
+    if (lane == 0) { chunk = atomicAdd(&st.ticket_fused, 1u); chunk1 = atomicAdd(&st.ticket_fused, 1u); }
+    chunk = __shfl_sync(0xffffffffu, chunk, 0);
+    chunk1 = __shfl_sync(0xffffffffu, chunk1, 0);
+    uint32_t mo, fa, mf;
+    float ul;
+    scalar_stage(chunk * FUSED_CHUNK + lane, mo, fa, ul, mf);
+    while (chunk < n_chunks) {
+        uint32_t chunk2 = 0;
+        if (lane == 0) chunk2 = atomicAdd(&st.ticket_fused, 1u);   // consumed at the loop end
+        const uint32_t j0 = chunk * FUSED_CHUNK;
+        const uint32_t jl = j0 + lane;
         // ---- (b) start the gather: half-warp h copies the row of offspring 2k+h
 #pragma unroll
         for (int k = 0; k < FUSED_CHUNK / 2; ++k) {
-            const uint32_t pm = __shfl_sync(0xffffffffu, mo, 2 * k + (lane >> 4));
-            cp_async16(cp_dst + k * 2 * FUSED_ROW, pop + (size_t)pm * FUSED_ROW + cp_src);
+            const uint32_t pm = __shfl_sync(0xffffffffu, mo, 2 * k + (lane >> 4));   // byte offset of the row
+            cp_async16(cp_dst + k * 2 * FUSED_ROW, pop + (pm | cp_src));
         }
 #pragma unroll
         for (int k = 0; k < FUSED_CHUNK / 2; ++k) {
             const uint32_t pf = __shfl_sync(0xffffffffu, fa, 2 * k + (lane >> 4));
-            cp_async16(cp_dst + FUSED_FA_OFF + k * 2 * FUSED_ROW, pop + (size_t)pf * FUSED_ROW + cp_src);
+            cp_async16(cp_dst + FUSED_FA_OFF + k * 2 * FUSED_ROW, pop + (pf | cp_src));
         }
         cp_async_commit();
+        // ---- (a) of the next chunk: its index loads land while this chunk is worked on
+        uint32_t mo1, fa1, mf1;
+        float ul1;
+        scalar_stage(chunk1 * FUSED_CHUNK + lane, mo1, fa1, ul1, mf1);
         // ---- (c) the 8 RECOMB blocks of this lane's (gamete, chromosome) role
         uint32_t qn = 0;
 #pragma unroll
         for (int it = 0; it < 8; ++it) {
             const uint32_t j = j0 + it * 4 + sub;
             uint32_t x[4];
-            draw(sp.key, sp.species, stream, j, c * 16, step, x);
+            draw_rk(sp, stream, j, c * 16, step, x);
             uint32_t nc = 0;
 #pragma unroll
             for (int i = 0; i < 6; ++i) nc += (x[0] >= T[i]) ? 1u : 0u;
@@ -184,7 +216,7 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             const uint32_t extra = e_nc - 2;
             for (uint32_t b = 0; b * 4 < extra; ++b) {
                 uint32_t y[4];
-                draw(sp.key, sp.species, e_g ? ST_RECOMB_P : ST_RECOMB_M, e_j, e_c * 16 + 1 + b, step, y);
+                draw_rk(sp, e_g ? ST_RECOMB_P : ST_RECOMB_M, e_j, e_c * 16 + 1 + b, step, y);
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
                     if (b * 4 + i < extra) {
@@ -199,9 +231,30 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
         }
         cp_async_wait_all();
         __syncwarp();
+        // ---- (m) R9: rare mutations, applied to the staged private copies of the parents' rows
+        if (__any_sync(0xffffffffu, mf != 0)) {
+            if (mf) {
+#pragma unroll
+                for (uint32_t gg = 0; gg < 2; ++gg) {
+                    if (!((mf >> gg) & 1u)) continue;
+                    const uint32_t ms = gg ? ST_MUT_P : ST_MUT_M;
+                    uint32_t *prow = (uint32_t *)(wbase + gg * FUSED_FA_OFF + lane * FUSED_ROW);
+                    uint32_t x[4];
+                    draw_rk(sp, ms, jl, 0, step, x);
+                    const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
+                    for (uint32_t k = 0; k < nm; ++k) {
+                        if (k > 0) draw_rk(sp, ms, jl, k, step, x);
+                        const uint32_t pos = __umulhi(x[1], L);
+                        const uint32_t bit = 1u << (pos & 31u);
+                        prow[pos >> 5] ^= bit;
+                        prow[L / 32 + (pos >> 5)] ^= bit;
+                    }
+                }
+            }
+            __syncwarp();
+        }
 
         // ---- (d) 8 passes of 4 offspring
-        int myzi = 0;
 #pragma unroll 2
         for (uint32_t it = 0; it < FUSED_CHUNK / 4; ++it) {
             const uint32_t j = j0 + it * 4 + sub;
@@ -228,7 +281,7 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
                     const uint32_t extra = nc - 2;
                     for (uint32_t bb = 0; bb * 4 < extra; ++bb) {
                         uint32_t y[4];
-                        draw(sp.key, sp.species, stream, j, c * 16 + 1 + bb, step, y);
+                        draw_rk(sp, stream, j, c * 16 + 1 + bb, step, y);
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
                             if (bb * 4 + i < extra) {
@@ -244,42 +297,24 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             uint32_t gw[8];
 #pragma unroll
             for (int w = 0; w < 8; ++w) gw[w] = (h0[w] & ~m[w]) | (h1[w] & m[w]);
-            // R9: mutation (rare; flagged per gamete in (a))
-            const uint32_t mflag = (__shfl_sync(0xffffffffu, mf, it * 4 + sub) >> g) & 1u;
-            if (mflag) {
-                const uint32_t ms = g ? ST_MUT_P : ST_MUT_M;
-                uint32_t x[4];
-                draw(sp.key, sp.species, ms, j, 0, step, x);
-                const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
-                for (uint32_t k = 0; k < nm; ++k) {
-                    if (k > 0) draw(sp.key, sp.species, ms, j, k, step, x);
-                    const uint32_t pos = __umulhi(x[1], L);
-                    const uint32_t wi = pos >> 5;
-                    if ((wi >> 3) == c) {
-#pragma unroll
-                        for (int w = 0; w < 8; ++w)
-                            if ((wi & 7u) == (uint32_t)w) gw[w] ^= 1u << (pos & 31u);
-                    }
-                }
-            }
             // a7: the row is stored once, at row j of the other buffer (alive or not)
             if (j < M) {
                 uint4 *o = nxt + (size_t)j * ROW4 + g * (ROW4 / 2) + c * 2;
                 o[0] = make_uint4(gw[0], gw[1], gw[2], gw[3]);
                 o[1] = make_uint4(gw[4], gw[5], gw[6], gw[7]);
             }
-            // a5: additive phenotype, exact integer (R10); handed to the lane that owns offspring j
-            int ones = 0;
+            // a5: this lane's share of the additive phenotype (R10), left where its draw was
+            uint32_t ones = 0;
 #pragma unroll
             for (int w = 0; w < 8; ++w) ones += __popc(gw[w]);
-            ones += __shfl_xor_sync(0xffffffffu, ones, 1);
-            ones += __shfl_xor_sync(0xffffffffu, ones, 2);
-            ones += __shfl_xor_sync(0xffffffffu, ones, 4);
-            const int zo = __shfl_sync(0xffffffffu, ones, (lane & 3u) * 8u);
-            if ((lane >> 2) == it) myzi = 2 * zo - 2 * (int)L;
+            s_P[it * 32 + lane] = ones;
         }
-        // ---- (e) a6: survival (R11), lane = offspring; same fp32 sequence as the materialised path
+        __syncwarp();
+        // ---- (e) a5-a6: lane = offspring: exact integer phenotype, survival (R11) in the same fp32
+        // sequence as the materialised path
         {
+            const uint4 oa = ((const uint4 *)s_P)[lane * 2], ob = ((const uint4 *)s_P)[lane * 2 + 1];
+            const int myzi = 2 * (int)(oa.x + oa.y + oa.z + oa.w + ob.x + ob.y + ob.z + ob.w) - 2 * (int)L;
             bool captured;
             const float z = __fmul_rn((float)myzi, sp.pheno_scale);
             const float s = survival_prob(sp, z, theta, ul, captured);
@@ -290,7 +325,10 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
             const uint32_t bal = __ballot_sync(0xffffffffu, alive);
             if (lane == 0) sp.chunk_mask[chunk] = bal;
         }
-        chunk = __shfl_sync(0xffffffffu, next_chunk, 0);   // also orders the stage reuse
+        __syncwarp();   // the stage and the draw words are reused by the next chunk
+        chunk = chunk1;
+        chunk1 = __shfl_sync(0xffffffffu, chunk2, 0);
+        mo = mo1; fa = fa1; ul = ul1; mf = mf1;
     }
     // ---- a8: survivor reductions (exact integers)
 #pragma unroll
@@ -418,7 +456,8 @@ __global__ void __launch_bounds__(256) k_fill_masks(uint32_t *mask, uint32_t n) 
 
 __host__ inline bool fused_bit_supported(const SpK &k) {
     return k.kind == 0 && k.linkage == 1 && k.n_chrom == 4 && k.L == 1024 && k.P == 1 && !k.sel_predation &&
-           k.fec_model != 2 && k.theta_patch == nullptr;
+           k.fec_model != 2 && k.theta_patch == nullptr &&
+           (unsigned long long)(k.capacity + 32) * FUSED_ROW < (1ull << 32);
 }
 
 inline cudaError_t fused_bit_configure() {

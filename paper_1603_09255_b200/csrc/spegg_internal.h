@@ -62,6 +62,7 @@ struct SpK {
     unsigned long long T_mig;
     uint32_t n_tables;
     Key key;
+    uint32_t rk[20];            // Philox round keys (k0_r, k1_r), r = 0..9: key + r * Weyl constants
     // constant tables
     const uint32_t *T_recomb;   // [L] INTERVAL switch thresholds (T_0 = 2^31)
     const uint32_t *T_xover;    // [n_chrom][XMAX]
