@@ -6,6 +6,7 @@
 // there is no CPU fallback.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -233,6 +234,7 @@ struct spegg_sim {
     uint32_t P = 1, n_sms = 148, launches = 0;
     uint32_t log_capacity = 4096;
     bool debug = false;
+    int fused_variant = 1;
     // kernel timing (direct launches bracketed by events)
     bool timing = false;
     std::vector<cudaEvent_t> ev;
@@ -253,7 +255,12 @@ int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
 
 // true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
 bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
-    return !s->debug && s->P == 1 && fused_bit_supported(h.k);
+    if (s->debug || s->P != 1 || !fused_bit_supported(h.k)) return false;
+    // the fused kernel tests u >= T as u > T - 1 (see spegg_fused.cuh): every threshold must be >= 1
+    for (uint32_t c = 0; c < h.p.n_chrom; ++c)
+        for (uint32_t k = 0; k < h.xover_len[c]; ++k)
+            if (h.T_xover[(size_t)c * XMAX + k] == 0) return false;
+    return h.k.mut_len == 0 || h.T_mut[0] != 0;
 }
 
 void launch_prepare(spegg_sim *s) {
@@ -278,7 +285,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
         if (fused_ok(s, h)) {
             launch_scan_fused(k, G, s->stream, 0); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
-            launch_fused_bit(k, G, s->stream); ++nl;
+            launch_fused_bit(k, G, s->stream, s->fused_variant); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
         } else {
             k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
@@ -358,6 +365,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     s->ws = (uint8_t *)d_workspace;
     s->ws_bytes = bytes;
     s->debug = p->debug != 0;
+    if (const char *v = std::getenv("SPEGG_FUSED_VARIANT")) s->fused_variant = std::atoi(v);
     s->log_capacity = p->log_capacity ? p->log_capacity : 4096;
     const uint32_t gw = p->grid_w ? p->grid_w : 1, gh = p->grid_h ? p->grid_h : 1;
     s->P = gw * gh;

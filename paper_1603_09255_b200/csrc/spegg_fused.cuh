@@ -349,6 +349,319 @@ __global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_
     if (sp.solo) solo_tail(sp, &s_flag);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Father-staged variant.  Only the fathers' rows (random gather, full DRAM latency) go through
+// shared memory; the mothers' rows (ascending, shared by siblings, prefetched into L2 at the start
+// of the chunk) are loaded straight into registers one pass ahead.  Half the stage means twice the
+// resident warps.  In pass (d) a lane owns HALF a chromosome (4 words = one uint4) of BOTH gametes
+// of offspring it*4+sub, so that every global access of a quarter warp is 128 contiguous bytes.
+constexpr int FUSEDF_WARPS = 4;
+#ifndef SPEGG_UNROLL_C
+#define SPEGG_UNROLL_C 2
+#endif
+#ifndef SPEGG_CTAS
+#define SPEGG_CTAS 5
+#endif
+constexpr int FUSEDF_UNROLL_C = SPEGG_UNROLL_C;   // decode passes in flight per lane
+constexpr int FUSEDF_CTAS = SPEGG_CTAS;           // resident CTAs per SM (shared memory allows 5)
+constexpr uint32_t FUSEDF_SP_OFF = FUSED_CHUNK * FUSED_ROW;        // packed draws [8][4][4][2] / partial sums
+constexpr uint32_t FUSEDF_Q_OFF = FUSEDF_SP_OFF + 8 * 32 * 4;      // queue of chromosomes with > 2 crossovers: draw [32], (pass, lane) [32]
+constexpr uint32_t FUSEDF_MO_OFF = FUSEDF_Q_OFF + 64 * 4;          // mothers' row offsets [32]
+constexpr uint32_t FUSEDF_WARP_BYTES = FUSEDF_MO_OFF + 32 * 4;
+constexpr uint32_t FUSEDF_SMEM = FUSEDF_WARPS * FUSEDF_WARP_BYTES;
+
+__device__ __forceinline__ uint4 ldg128(const void *p) {
+    uint4 v;
+    asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// packed draw of one (gamete, chromosome): s0 | s1 << 9 | phase << 31; positions 1..255,
+// 256 = no crossover
+__device__ __forceinline__ void half_masks(uint32_t P, uint32_t half, uint32_t (&m)[4]) {
+    const int s0 = (int)(P & 0x1FFu) - 128 * (int)half, s1 = (int)((P >> 9) & 0x1FFu) - 128 * (int)half;
+    const uint32_t phi = (uint32_t)((int)P >> 31);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) m[i] = phi ^ mask_from(s0, i) ^ mask_from(s1, i);
+}
+
+template <int NC, int WPC>
+__global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(const __grid_constant__ SpK sp) {
+    static_assert(NC == 4 && WPC == 8, "lane group of 8 = 2 gametes x 4 chromosomes of 8 words");
+    extern __shared__ __align__(128) uint8_t s_dyn[];
+    __shared__ uint32_t s_flag;
+    DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
+    const uint32_t n_chunks = (M + FUSED_CHUNK - 1) / FUSED_CHUNK;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t sub = lane >> 3, q = lane & 7u;
+    const uint32_t g = q >> 2, c = q & 3u;        // role in (c): one (gamete, chromosome)
+    const uint32_t hc = q >> 1, half = q & 1u;    // role in (d): half `half` of chromosome hc, both gametes
+    constexpr uint32_t L = NC * WPC * 32;
+    uint8_t *wbase = s_dyn + warp * FUSEDF_WARP_BYTES;
+    const uint32_t stage = smem_u32(wbase);
+    uint32_t *s_P = (uint32_t *)(wbase + FUSEDF_SP_OFF);
+    uint32_t *s_q = (uint32_t *)(wbase + FUSEDF_Q_OFF);
+    uint32_t *s_mo = (uint32_t *)(wbase + FUSEDF_MO_OFF);
+    const uint8_t *pop = sp.pop[st.cur];
+    uint8_t *nxt = sp.pop[st.cur ^ 1u];
+    const uint32_t *rowptr = sp.rowptr[st.cur];
+    const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
+    // the hot path only needs "at least 1 / 2 / 3 crossovers": x >= T_k written as x > T_k - 1 so that a
+    // missing threshold (table shorter than k+1; T_k >= 1 is checked at create time) is never reached
+    const uint32_t xl = sp.xover_len[c];
+    const uint32_t *XT = sp.T_xover + c * XMAX;
+    const uint32_t U0 = xl > 0 ? XT[0] - 1u : 0xFFFFFFFFu, U1 = xl > 1 ? XT[1] - 1u : 0xFFFFFFFFu,
+                   U2 = xl > 2 ? XT[2] - 1u : 0xFFFFFFFFu;
+    const uint32_t clen1 = sp.chrom_len[c] - 1;
+    const uint32_t Um0 = sp.mut_len ? sp.T_mut[0] - 1u : 0xFFFFFFFFu;
+    const float theta = st.theta_t;
+    const uint32_t cp_dst = stage + (lane >> 4) * FUSED_ROW + (lane & 15u) * 16u;   // + k * 512
+    const uint32_t cp_src = (lane & 15u) * 16u;
+    const uint32_t ld_fa = stage + sub * FUSED_ROW + q * 16u;                       // + it * 1024 (+ 128)
+    const uint32_t sp_slot = sub * 8u + hc * 2u;                                    // + it * 32: (g=0, g=1) pair
+    long long acc1 = 0, acc2 = 0;
+    uint32_t ties = 0, n_alive = 0;
+
+    auto scalar_stage = [&](uint32_t jl, uint32_t &mo, uint32_t &fa, float &ul, uint32_t &mf) {
+        uint32_t x[4], a[4], b[4];
+        draw_rk(sp, ST_SCALAR, jl, 0, step, x);
+        draw_rk(sp, ST_MUT_M, jl, 0, step, a);
+        draw_rk(sp, ST_MUT_P, jl, 0, step, b);
+        mo = 0; fa = 0; mf = 0; ul = 2.0f;
+        if (jl < M) {
+            mo = sp.mother[jl] * FUSED_ROW;
+            fa = rowptr[uniform_index(x[0], N)] * FUSED_ROW;   // R2
+            ul = u01_of(x[3]);
+            mf = (a[0] > Um0 ? 1u : 0u) | (b[0] > Um0 ? 2u : 0u);
+        }
+    };
+    // R9 for one gamete of offspring jl: calls flip(word index 0..31, bit) for every mutation
+    auto mutate = [&](uint32_t ms, uint32_t jl, auto &&flip) {
+        uint32_t x[4];
+        draw_rk(sp, ms, jl, 0, step, x);
+        const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
+        for (uint32_t k = 0; k < nm; ++k) {
+            if (k > 0) draw_rk(sp, ms, jl, k, step, x);
+            const uint32_t pos = __umulhi(x[1], L);
+            flip(pos >> 5, 1u << (pos & 31u));
+        }
+    };
+
+    uint32_t j0 = 0;
+    // (x) for chromosome e_c of gamete e_g of offspring j0 + e_o, which drew e_nc > 2 crossovers
+    auto fix_extra = [&](uint32_t e_o, uint32_t e_g, uint32_t e_c, uint32_t e_nc) {
+        const uint32_t e_j = j0 + e_o;
+        if (e_j >= M) return;
+        const uint32_t e_clen1 = sp.chrom_len[e_c] - 1;
+        uint32_t xm[8];
+#pragma unroll
+        for (int w = 0; w < 8; ++w) xm[w] = 0;
+        const uint32_t extra = e_nc - 2;
+        for (uint32_t b = 0; b * 4 < extra; ++b) {
+            uint32_t y[4];
+            draw_rk(sp, e_g ? ST_RECOMB_P : ST_RECOMB_M, e_j, e_c * 16 + 1 + b, step, y);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                if (b * 4 + i < extra) {
+                    const int s = (int)__umulhi(y[i], e_clen1) + 1;
+#pragma unroll
+                    for (int w = 0; w < 8; ++w) xm[w] ^= mask_from(s, w);
+                }
+            }
+        }
+        // the parent's two haplotypes of this chromosome: father from the stage, mother from global
+        uint4 h[4];
+        if (e_g) {
+            const uint32_t a_ = stage + e_o * FUSED_ROW + e_c * 32u;
+            h[0] = lds128(a_); h[1] = lds128(a_ + 16); h[2] = lds128(a_ + FUSED_ROW / 2); h[3] = lds128(a_ + FUSED_ROW / 2 + 16);
+        } else {
+            const uint8_t *a_ = pop + (s_mo[e_o] | (e_c * 32u));
+            h[0] = ldg128(a_); h[1] = ldg128(a_ + 16); h[2] = ldg128(a_ + FUSED_ROW / 2); h[3] = ldg128(a_ + FUSED_ROW / 2 + 16);
+        }
+        uint4 *orow = (uint4 *)(nxt + (size_t)e_j * FUSED_ROW + e_g * (FUSED_ROW / 2) + e_c * 32u);
+        uint4 o0 = orow[0], o1 = orow[1];
+        const int before = __popc(o0.x) + __popc(o0.y) + __popc(o0.z) + __popc(o0.w) + __popc(o1.x) + __popc(o1.y) + __popc(o1.z) + __popc(o1.w);
+        o0.x ^= (h[0].x ^ h[2].x) & xm[0]; o0.y ^= (h[0].y ^ h[2].y) & xm[1];
+        o0.z ^= (h[0].z ^ h[2].z) & xm[2]; o0.w ^= (h[0].w ^ h[2].w) & xm[3];
+        o1.x ^= (h[1].x ^ h[3].x) & xm[4]; o1.y ^= (h[1].y ^ h[3].y) & xm[5];
+        o1.z ^= (h[1].z ^ h[3].z) & xm[6]; o1.w ^= (h[1].w ^ h[3].w) & xm[7];
+        const int after = __popc(o0.x) + __popc(o0.y) + __popc(o0.z) + __popc(o0.w) + __popc(o1.x) + __popc(o1.y) + __popc(o1.z) + __popc(o1.w);
+        orow[0] = o0; orow[1] = o1;
+        atomicAdd(&s_P[e_o * 8], (uint32_t)(after - before));
+    };
+
+    // software pipeline over chunks: the first trip only runs stage (a) of the first chunk
+    constexpr uint32_t NONE = 0xFFFFFFFFu;
+    uint32_t chunk = NONE, chunk1 = 0;
+    if (lane == 0) chunk1 = atomicAdd(&st.ticket_fused, 1u);
+    chunk1 = __shfl_sync(0xffffffffu, chunk1, 0);
+    uint32_t mo = 0, fa = 0, mf = 0;
+    float ul = 2.0f;
+    for (;;) {
+        uint32_t chunk2 = 0;
+        if (lane == 0) chunk2 = atomicAdd(&st.ticket_fused, 1u);   // consumed at the loop end
+        const bool active = chunk != NONE;
+        j0 = chunk * FUSED_CHUNK;
+        const uint32_t jl = j0 + lane;
+        // ---- (b) fathers: half-warp h copies the row of offspring 2k+h into the stage
+        if (active) {
+#pragma unroll
+            for (int k = 0; k < FUSED_CHUNK / 2; ++k) {
+                const uint32_t pf = __shfl_sync(0xffffffffu, fa, 2 * k + (lane >> 4));
+                cp_async16(cp_dst + k * 2 * FUSED_ROW, pop + (pf | cp_src));
+            }
+            cp_async_commit();
+            //  mothers: every 32-byte sector of the 32 rows is asked into L2 (lane -> sector lane&7 of
+            //  the rows of offspring (lane>>3) + 4k)
+            s_mo[lane] = mo;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const uint32_t pm = __shfl_sync(0xffffffffu, mo, 4 * k + (lane >> 3));
+                prefetch_l2(pop + (pm | ((lane & 7u) * 32u)));
+            }
+        }
+        const uint32_t matmask = __ballot_sync(0xffffffffu, (mf & 1u) != 0);
+        // ---- (a) of the next chunk
+        uint32_t mo1, fa1, mf1;
+        float ul1;
+        scalar_stage(chunk1 * FUSED_CHUNK + lane, mo1, fa1, ul1, mf1);
+        if (active) {
+        // ---- (c) the 8 RECOMB blocks of this lane's (gamete, chromosome) role
+        uint32_t qn = 0;
+#pragma unroll FUSEDF_UNROLL_C
+        for (int it = 0; it < 8; ++it) {
+            const uint32_t j = j0 + it * 4 + sub;
+            uint32_t x[4];
+            draw_rk(sp, stream, j, c * 16, step, x);
+            const uint32_t s0 = x[0] > U0 ? __umulhi(x[2], clen1) + 1 : 256u;
+            const uint32_t s1 = x[0] > U1 ? __umulhi(x[3], clen1) + 1 : 256u;
+            const uint32_t P = (s0 + (s1 << 9)) | (x[1] & 0x80000000u);
+            // chromosomes with crossovers beyond the first two are queued for the fix-up pass (x)
+            const bool need = x[0] > U2;
+            const uint32_t bal = __ballot_sync(0xffffffffu, need);
+            if (need) {
+                const uint32_t e = qn + __popc(bal & ((1u << lane) - 1u));
+                if (e < 32) { s_q[e] = x[0]; s_q[32 + e] = ((uint32_t)it << 5) | lane; }
+            }
+            qn += __popc(bal);
+            s_P[it * 32 + sub * 8 + c * 2 + g] = P;
+        }
+        cp_async_wait_all();
+        __syncwarp();
+        // ---- (m) R9, paternal gamete: flips in the staged private copy of the father's row
+        if (__any_sync(0xffffffffu, (mf & 2u) != 0)) {
+            if (mf & 2u) {
+                uint32_t *prow = (uint32_t *)(wbase + lane * FUSED_ROW);
+                mutate(ST_MUT_P, jl, [&](uint32_t wi, uint32_t bit) { prow[wi] ^= bit; prow[L / 32 + wi] ^= bit; });
+            }
+            __syncwarp();
+        }
+
+        // ---- (d) 8 passes of 4 offspring; mothers' words are loaded one pass ahead
+        const uint8_t *mrow = pop + (s_mo[sub] | (q * 16u));
+        uint4 ma = ldg128(mrow), mb = ldg128(mrow + FUSED_ROW / 2);
+#pragma unroll 2
+        for (uint32_t it = 0; it < FUSED_CHUNK / 4; ++it) {
+            const uint32_t o = it * 4 + sub, j = j0 + o;
+            const uint4 ca = ma, cb = mb;
+            if (it + 1 < FUSED_CHUNK / 4) {
+                mrow = pop + (s_mo[o + 4] | (q * 16u));
+                ma = ldg128(mrow); mb = ldg128(mrow + FUSED_ROW / 2);
+            }
+            const uint4 fa0 = lds128(ld_fa + it * 4 * FUSED_ROW), fa1_ = lds128(ld_fa + it * 4 * FUSED_ROW + FUSED_ROW / 2);
+            const uint2 PP = *(const uint2 *)(s_P + it * 32 + sp_slot);
+            // R8: masks of this lane's four words of chromosome hc, maternal and paternal gamete
+            uint32_t mm[4], mp[4];
+            half_masks(PP.x, half, mm);
+            half_masks(PP.y, half, mp);
+            // select: gamete word = hap[phase] word
+            uint4 gm, gp;
+            gm.x = (ca.x & ~mm[0]) | (cb.x & mm[0]); gm.y = (ca.y & ~mm[1]) | (cb.y & mm[1]);
+            gm.z = (ca.z & ~mm[2]) | (cb.z & mm[2]); gm.w = (ca.w & ~mm[3]) | (cb.w & mm[3]);
+            gp.x = (fa0.x & ~mp[0]) | (fa1_.x & mp[0]); gp.y = (fa0.y & ~mp[1]) | (fa1_.y & mp[1]);
+            gp.z = (fa0.z & ~mp[2]) | (fa1_.z & mp[2]); gp.w = (fa0.w & ~mp[3]) | (fa1_.w & mp[3]);
+            // R9, maternal gamete (rare): flip in the registers of the lane that owns the word
+            if ((matmask >> o) & 1u) {
+                mutate(ST_MUT_M, j, [&](uint32_t wi, uint32_t bit) {
+                    if ((wi >> 2) == q) {
+                        const uint32_t k = wi & 3u;
+                        if (k == 0) gm.x ^= bit; else if (k == 1) gm.y ^= bit; else if (k == 2) gm.z ^= bit; else gm.w ^= bit;
+                    }
+                });
+            }
+            // a7: the row is stored once, at row j of the other buffer (alive or not)
+            if (j < M) {
+                uint4 *orow = (uint4 *)(nxt + (size_t)j * FUSED_ROW) + q;
+                orow[0] = gm;
+                orow[FUSED_ROW / 32] = gp;
+            }
+            // a5: this lane's share of the additive phenotype (R10), left where the draws were
+            const uint32_t ones = __popc(gm.x) + __popc(gm.y) + __popc(gm.z) + __popc(gm.w) +
+                                  __popc(gp.x) + __popc(gp.y) + __popc(gp.z) + __popc(gp.w);
+            __syncwarp();
+            s_P[it * 32 + lane] = ones;
+        }
+        __syncwarp();
+        // ---- (x) R8, crossovers beyond the second (8 % of the chromosomes at mean 1): one lane per
+        // queued chromosome.  A further crossover at s swaps the source haplotype of every locus >= s,
+        // i.e. XORs the gamete with (hap0 ^ hap1) there -- applied to the row this warp just stored.
+        if (qn <= 32) {
+            if (lane < qn) {
+                const uint32_t e = s_q[32 + lane], e_ln = e & 31u, e_c = e_ln & 3u;
+                const uint32_t e_nc = poisson_count(sp.T_xover + e_c * XMAX, sp.xover_len[e_c], s_q[lane]);
+                fix_extra((e >> 5) * 4 + (e_ln >> 3), (e_ln >> 2) & 1u, e_c, e_nc);
+            }
+        }
+        else {   // queue overflow, rare beyond measure: every lane walks its own eight draws again
+            for (uint32_t it = 0; it < 8; ++it) {
+                uint32_t x[4];
+                draw_rk(sp, stream, j0 + it * 4 + sub, c * 16, step, x);
+                const uint32_t nc = poisson_count(XT, xl, x[0]);
+                if (nc > 2) fix_extra(it * 4 + sub, g, c, nc);
+            }
+        }
+        __syncwarp();
+        // ---- (e) a5-a6: lane = offspring
+        {
+            const uint4 oa = ((const uint4 *)s_P)[lane * 2], ob = ((const uint4 *)s_P)[lane * 2 + 1];
+            const int myzi = 2 * (int)(oa.x + oa.y + oa.z + oa.w + ob.x + ob.y + ob.z + ob.w) - 2 * (int)L;
+            bool captured;
+            const float z = __fmul_rn((float)myzi, sp.pheno_scale);
+            const float s = survival_prob(sp, z, theta, ul, captured);
+            const bool valid = jl < M;
+            const bool alive = valid && (ul < s);
+            if (valid && fabsf(__fsub_rn(ul, s)) < 1e-6f) ++ties;
+            if (alive) { acc1 += myzi; acc2 += (long long)myzi * myzi; ++n_alive; }
+            const uint32_t bal = __ballot_sync(0xffffffffu, alive);
+            if (lane == 0) sp.chunk_mask[chunk] = bal;
+        }
+        __syncwarp();   // the stage and the draw words are reused by the next chunk
+        }
+        chunk = chunk1;
+        chunk1 = __shfl_sync(0xffffffffu, chunk2, 0);
+        mo = mo1; fa = fa1; ul = ul1; mf = mf1;
+        if (chunk >= n_chunks) break;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        acc1 += __shfl_xor_sync(0xffffffffu, acc1, o);
+        acc2 += __shfl_xor_sync(0xffffffffu, acc2, o);
+        ties += __shfl_xor_sync(0xffffffffu, ties, o);
+        n_alive += __shfl_xor_sync(0xffffffffu, n_alive, o);
+    }
+    if (lane == 0) {
+        if (acc1 != 0 || acc2 != 0) {
+            atomicAdd((unsigned long long *)&st.acc_zi, (unsigned long long)acc1);
+            atomicAdd((unsigned long long *)&st.acc_zi2, (unsigned long long)acc2);
+        }
+        if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
+        if (n_alive) atomicAdd(&st.n_next, n_alive);
+    }
+    if (sp.solo) solo_tail(sp, &s_flag);
+}
+
 // a1-a3 and the index half of a7 for a species on the fused path.  The current buffer holds
 // m_phys physical rows in 32-row slabs; chunk_mask says which are adults.  A CTA takes a range of
 // 2,048 rows (8 per thread):
@@ -461,11 +774,14 @@ __host__ inline bool fused_bit_supported(const SpK &k) {
 }
 
 inline cudaError_t fused_bit_configure() {
-    return cudaFuncSetAttribute(k_fused_bit<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSED_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_fused_bit<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSED_SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_fused_bit_f<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
 }
 
-inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
-    k_fused_bit<4, 8><<<n_sms * 3, FUSED_WARPS * 32, FUSED_SMEM, stream>>>(k);
+inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream, int variant) {
+    if (variant == 0) k_fused_bit<4, 8><<<n_sms * 3, FUSED_WARPS * 32, FUSED_SMEM, stream>>>(k);
+    else k_fused_bit_f<4, 8><<<n_sms * FUSEDF_CTAS, FUSEDF_WARPS * 32, FUSEDF_SMEM, stream>>>(k);
 }
 
 inline void launch_scan_fused(const SpK &k, uint32_t n_sms, cudaStream_t stream, int index_only) {
