@@ -90,10 +90,8 @@ class ClockSampler:
 
 
 def workload(which, seed_offset=0):
-    from paper_1603_09255_b200 import workloads
-    cfg = workloads.config(which)
-    cfg["seed"] = cfg["seed"] + 1000 * seed_offset
-    return cfg
+    from paper_1603_09255_b200 import replicas, workloads
+    return replicas.replica_config(workloads.config(which), seed_offset)
 
 
 def describe(cfg):
@@ -144,7 +142,7 @@ def run_reference(args):
     from paper_1603_09255_b200 import workloads
     full = workload(args.config)
     # bounded sample: shrink the population so that K+W oracle steps end within ~2 minutes
-    per_step_s = 120.0 / max(1, args.steps + args.warmup)
+    per_step_s = args.ref_budget_s / max(1, args.steps + args.warmup)
     scale = min(1.0, max(0.001, per_step_s * 7.0e4 / full["n0"][0]))
     cfg = workloads.config(args.config, scale=scale)
     units, dt = oracle_run(cfg, args.steps, warm=args.warmup)
@@ -165,11 +163,9 @@ def run_reference(args):
 def run_ours(args):
     import numpy as np
     import torch
-    from paper_1603_09255_b200 import binding, workloads
+    from paper_1603_09255_b200 import binding, replicas, workloads
 
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank, local, world = replicas.env_rank()
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -249,13 +245,8 @@ def run_ours(args):
     e2e_s = time.perf_counter() - t0
 
     # ---- reduce over ranks: max time, summed units
-    if dist is not None:
-        t = torch.tensor([ms, e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        u = torch.tensor([units, e_units, offspring], device=dev, dtype=torch.float64)
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        ms, e2e_s = float(t[0]), float(t[1])
-        units, e_units, offspring = float(u[0]), float(u[1]), float(u[2])
+    (ms, e2e_s), (units, e_units, offspring) = replicas.reduce_over_ranks(
+        dist, [ms, e2e_s], [units, e_units, offspring], device=dev)
     launches = sim.launches_per_step() * args.steps
 
     if rank == 0:
@@ -308,6 +299,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--ref-budget-s", type=float, default=120.0,
+                    help="--impl reference: CPU seconds the K+W oracle steps are sized for")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

@@ -128,3 +128,27 @@ def test_bad_parameters_are_rejected(binding):
     cfg["species"][0]["mu"] = 1.5
     with pytest.raises(binding.SpeggError):
         binding.workspace_bytes(cfg)
+
+
+# ---- BASELINE.json's FULL sizes, in the launch configuration bench.py times (debug off, the
+# production kernels, the captured graph).  The oracle finishes a full-size step in seconds
+# (C3 ~6 s, C4 ~9 s, C5 ~17 s), so the comparison is complete -- every row of the next
+# generation, every log field -- rather than sampled.
+@pytest.mark.parametrize("which,steps", [(3, 3), (2, 6), (4, 1), (5, 1)])
+def test_full_size_bench_configuration(oracle_mod, binding, which, steps):
+    cfg = workloads.config(which)                     # scale 1.0: N0, K, capacity as benchmarked
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    for s in range(len(cfg["species"])):
+        rows = workloads.initial_rows(cfg, s)
+        ps = workloads.initial_patch_start(cfg, s)
+        orc.write_state(s, rows, ps, 0)
+        sim.write_state(s, rows, ps, 0)
+        del rows
+    orc.step(steps)
+    sim.step(steps)                                   # free-running: step t+1 consumes the GPU's own step t
+    for s in range(len(cfg["species"])):
+        parity.assert_logs_equal(sim.read_log(s), orc.log(s), tag="C%d species %d" % (which, s))
+    parity.assert_state_equal(sim, orc, cfg, tag="C%d full size" % which)
+    assert sim.status() == orc.flags
+    sim.close()
