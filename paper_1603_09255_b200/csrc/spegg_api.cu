@@ -92,7 +92,7 @@ struct Carver {
 };
 
 struct SpeciesLayout {
-    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask, f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
+    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask, range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
     uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, K_patch, theta_patch;
     uint32_t norm_len, n_tables, row_bytes;
@@ -178,6 +178,8 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.rowptr[0] = c.take(cap32 * 4);
         l.rowptr[1] = c.take(cap32 * 4);
         l.chunk_mask = c.take((cap / 32 + 2) * 4);
+        l.range_cnt[0] = c.take((cap32 / SCANF_RANGE + 2) * 4);
+        l.range_cnt[1] = c.take((cap32 / SCANF_RANGE + 2) * 4);
         l.patch_start[0] = c.take((P + 1) * 4);
         l.patch_start[1] = c.take((P + 1) * 4);
         l.f = c.take(cap);
@@ -234,7 +236,6 @@ struct spegg_sim {
     uint32_t P = 1, n_sms = 148, launches = 0;
     uint32_t log_capacity = 4096;
     bool debug = false;
-    int fused_variant = 1;
     // kernel timing (direct launches bracketed by events)
     bool timing = false;
     std::vector<cudaEvent_t> ev;
@@ -285,7 +286,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
         if (fused_ok(s, h)) {
             launch_scan_fused(k, G, s->stream, 0); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
-            launch_fused_bit(k, G, s->stream, s->fused_variant); ++nl;
+            launch_fused_bit(k, G, s->stream); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
         } else {
             k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
@@ -365,7 +366,6 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     s->ws = (uint8_t *)d_workspace;
     s->ws_bytes = bytes;
     s->debug = p->debug != 0;
-    if (const char *v = std::getenv("SPEGG_FUSED_VARIANT")) s->fused_variant = std::atoi(v);
     s->log_capacity = p->log_capacity ? p->log_capacity : 4096;
     const uint32_t gw = p->grid_w ? p->grid_w : 1, gh = p->grid_h ? p->grid_h : 1;
     s->P = gw * gh;
@@ -458,6 +458,8 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.patch_start[0] = at<uint32_t>(s, l.patch_start[0]); k.patch_start[1] = at<uint32_t>(s, l.patch_start[1]);
         k.rowptr[0] = at<uint32_t>(s, l.rowptr[0]); k.rowptr[1] = at<uint32_t>(s, l.rowptr[1]);
         k.chunk_mask = at<uint32_t>(s, l.chunk_mask);
+        k.range_cnt[0] = at<uint32_t>(s, l.range_cnt[0]);
+        k.range_cnt[1] = at<uint32_t>(s, l.range_cnt[1]);
         k.f = at<uint8_t>(s, l.f); k.off = at<uint32_t>(s, l.off);
         k.mother = at<uint32_t>(s, l.mother); k.father = at<uint32_t>(s, l.father);
         k.dest = at<uint32_t>(s, l.dest); k.pos = at<uint32_t>(s, l.pos);
@@ -534,7 +536,7 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
     CU(cudaMemcpyAsync(s->d_glob, &g, sizeof g, cudaMemcpyHostToDevice, s->stream));
     if (n) {
         k_iota<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k.rowptr[cur], (uint32_t)n);
-        if (h.k.phys_parents) k_fill_masks<<<s->n_sms, 256, 0, s->stream>>>(h.k.chunk_mask, (uint32_t)n);
+        if (h.k.phys_parents) k_fill_masks<<<s->n_sms, 256, 0, s->stream>>>(h.k.chunk_mask, h.k.range_cnt[cur], (uint32_t)n);
         k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1);
     }
     launch_prepare(s);

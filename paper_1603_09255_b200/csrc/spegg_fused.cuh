@@ -4,16 +4,17 @@
 // loci, 256-byte rows).  One time step is TWO launches:
 //
 //   k_scan_fused  a1-a3 + the index half of a7: one pass over the physical rows of the current
-//                 buffer (32-row slabs, one survivor bitmask per slab): logical adult index by a
-//                 look-back over the alive counts -> rowptr[], Poisson fecundity of every adult,
-//                 second look-back over the fecundities -> mother[] (physical rows), M_t.
-//   k_fused_bit   a3-a8 in one pass: father draw, asynchronous gather of both parents' rows into
+//                 buffer (32-row slabs, one survivor bitmask per slab, one adult count per 2,048-row
+//                 range): logical adult index from the range counts -> rowptr[], Poisson fecundity
+//                 of every adult, ONE look-back over the fecundities -> mother[] (physical rows), M_t.
+//   k_fused_bit_f a3-a8 in one pass: father draw, asynchronous gather of the fathers' rows into
 //                 shared memory (cp.async, issued before the recombination draws are computed so
-//                 the gather latency hides behind the Philox work), crossover masks from the
-//                 RECOMB blocks (R8), select, mutate, popcount -> phenotype -> survival; every
-//                 offspring row is stored exactly once at row j of the other buffer, and only the
-//                 4-byte survivor mask of each 32-offspring chunk says which rows are the next
-//                 generation.  Its last CTA closes the step and prepares the next one (a0, a9).
+//                 the gather latency hides behind the Philox work), mothers' rows prefetched into L2
+//                 and loaded a pass ahead, crossover masks from the RECOMB blocks (R8), select,
+//                 mutate, popcount -> phenotype -> survival; every offspring row is stored exactly
+//                 once at row j of the other buffer, and only the 4-byte survivor mask of each
+//                 32-offspring chunk says which rows are the next generation.  Its last CTA closes
+//                 the step and prepares the next one (a0, a9).
 //
 // Every draw is addressed by (stream, entity, block, step), never by thread, so the result is
 // bit-identical to the materialised pipeline and to the oracle.
@@ -48,15 +49,10 @@ __device__ __forceinline__ uint32_t mask_from(int s, int w) {
 }
 
 constexpr int FUSED_CHUNK = 32;                 // offspring per warp iteration = rows per slab
-constexpr int FUSED_WARPS = 4;                  // warps per CTA; 3 CTAs per SM by shared memory
 constexpr uint32_t FUSED_ROW = 256;             // bytes per row (config 3)
-constexpr uint32_t FUSED_FA_OFF = FUSED_CHUNK * FUSED_ROW + 16;  // fathers' rows: +16 B rotates the banks
-constexpr uint32_t FUSED_STAGE = FUSED_FA_OFF + FUSED_CHUNK * FUSED_ROW;
-constexpr uint32_t FUSED_SP_OFF = FUSED_STAGE;                   // packed recombination draws [8][32]
-constexpr uint32_t FUSED_XM_OFF = FUSED_SP_OFF + 8 * 32 * 4;     // extra-crossover masks [32][2] uint4
-constexpr uint32_t FUSED_Q_OFF = FUSED_XM_OFF + 32 * 32;         // queue [32]
-constexpr uint32_t FUSED_WARP_BYTES = FUSED_Q_OFF + 32 * 4;
-constexpr uint32_t FUSED_SMEM = FUSED_WARPS * FUSED_WARP_BYTES;
+constexpr int SCANF_ROWS = 8;                   // rows per thread of k_scan_fused
+constexpr int SCANF_RANGE = SCAN_THREADS * SCANF_ROWS;          // rows per range (2,048 = 64 chunks)
+constexpr int SCANF_CHUNKS = SCANF_RANGE / FUSED_CHUNK;
 
 // Philox4x32-10 (R3) with the ten round keys taken from the kernel parameter block: the key
 // schedule k_r = k_0 + r * Weyl is the same for every draw of a simulation, so the host computes it
@@ -78,292 +74,29 @@ __device__ __forceinline__ void draw_rk(const SpK &sp, uint32_t stream, uint32_t
     o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
 }
 
-// Warp-autonomous fused kernel.  A warp takes chunks of 32 consecutive offspring from an atomic
-// ticket; the scalar work of a chunk is done one chunk ahead so that no index load is waited for.
-//   (a) lane = offspring: SCALAR block (father -> rowptr -> row, survival uniform), the two MUT
-//       blocks' counts, mother row.  Computed for the NEXT chunk while the current one is gathered.
-//   (b) 32 cp.async instructions start the gather of the chunk's 64 parent rows (16 KB) into this
-//       warp's stage: half a warp copies one 256-byte row with 16-byte pieces.
-//   (c) lane = (gamete g, chromosome c) of offspring it*4+sub, it = 0..7: the 8 RECOMB blocks this
-//       lane will need, decoded to a packed word (count, start phase, first two positions); the few
-//       chromosomes with more than two crossovers (8 % at mean 1) are queued and their extra
-//       blocks / mask contributions computed one per lane.  The gather lands meanwhile.
-//   (m) rare: a lane whose offspring carries a mutation flips that bit in BOTH haplotypes of the
-//       staged copy of the parent's row (the copy is private to the offspring), which flips it in
-//       the gamete whatever the phase is (R9) and keeps mutation out of the inner loop.
-//   (d) 8 passes of 4 offspring (8 lanes each): four conflict-free 128-bit shared loads of the
-//       lane's 8-word chromosome from both haplotypes of its parent, mask words from the packed
-//       draw (+ queued extras), select, popcount, two 128-bit stores of the lane's 32 bytes of
-//       offspring row j.
-//   (e) lane = offspring: phenotype -> fp32 survival -> decision; the ballot is the chunk's mask.
-template <int NC, int WPC>
-__global__ void __launch_bounds__(FUSED_WARPS * 32, 3) k_fused_bit(const __grid_constant__ SpK sp) {
-    static_assert(NC == 4 && WPC == 8, "lane group of 8 = 2 gametes x 4 chromosomes of 8 words");
-    extern __shared__ __align__(128) uint8_t s_dyn[];
-    __shared__ uint32_t s_flag;
-    DevSpecies &st = *sp.st;
-    const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
-    const uint32_t n_chunks = (M + FUSED_CHUNK - 1) / FUSED_CHUNK;
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t sub = lane >> 3, q = lane & 7u, g = q >> 2, c = q & 3u;
-    constexpr uint32_t ROW4 = 2 * NC * WPC / 4;   // uint4 per row (16)
-    constexpr uint32_t L = NC * WPC * 32;
-    uint8_t *wbase = s_dyn + warp * FUSED_WARP_BYTES;
-    const uint32_t stage = smem_u32(wbase);
-    uint32_t *s_P = (uint32_t *)(wbase + FUSED_SP_OFF);
-    uint4 *s_xmask = (uint4 *)(wbase + FUSED_XM_OFF);
-    uint32_t *s_q = (uint32_t *)(wbase + FUSED_Q_OFF);
-    const uint8_t *pop = sp.pop[st.cur];
-    uint4 *nxt = (uint4 *)sp.pop[st.cur ^ 1u];
-    const uint32_t *rowptr = sp.rowptr[st.cur];
-    const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
-    // this chromosome's crossover-count thresholds in registers (count <= 6 without a loop)
-    const uint32_t xl = sp.xover_len[c];
-    const uint32_t *XT = sp.T_xover + c * XMAX;
-    uint32_t T[6];
-#pragma unroll
-    for (int i = 0; i < 6; ++i) T[i] = (uint32_t)i < xl ? XT[i] : 0xFFFFFFFFu;
-    const bool short_table = xl <= 6;
-    const uint32_t clen1 = sp.chrom_len[c] - 1;
-    const uint32_t Tm0 = sp.mut_len ? sp.T_mut[0] : 0xFFFFFFFFu;
-    const bool has_mut = sp.mut_len != 0;
-    const float theta = st.theta_t;
-    // per-lane constant parts of the stage addresses
-    const uint32_t cp_dst = stage + (lane >> 4) * FUSED_ROW + (lane & 15u) * 16u;   // + k * 512 (+ FA_OFF)
-    const uint32_t cp_src = (lane & 15u) * 16u;
-    const uint32_t ld_src = stage + g * FUSED_FA_OFF + sub * FUSED_ROW + c * 32u;   // + it * 1024
-    long long acc1 = 0, acc2 = 0;
-    uint32_t ties = 0, n_alive = 0;
-
-    // (a): scalar draws and index loads of offspring jl; the loads are consumed a chunk later
-    auto scalar_stage = [&](uint32_t jl, uint32_t &mo, uint32_t &fa, float &ul, uint32_t &mf) {
-        uint32_t x[4], a[4], b[4];
-        draw_rk(sp, ST_SCALAR, jl, 0, step, x);
-        draw_rk(sp, ST_MUT_M, jl, 0, step, a);
-        draw_rk(sp, ST_MUT_P, jl, 0, step, b);
-        mo = 0; fa = 0; mf = 0; ul = 2.0f;
-        if (jl < M) {
-            // physical rows (phys_parents) as 32-bit byte offsets into the buffer (capacity * 256 < 2^32)
-            mo = sp.mother[jl] * FUSED_ROW;
-            fa = rowptr[uniform_index(x[0], N)] * FUSED_ROW;   // R2: uniform mate, selfing allowed
-            ul = u01_of(x[3]);
-            if (has_mut) mf = (a[0] >= Tm0 ? 1u : 0u) | (b[0] >= Tm0 ? 2u : 0u);
-        }
-    };
-
-    uint32_t chunk = 0, chunk1 = 0;
-    if (lane == 0) { chunk = atomicAdd(&st.ticket_fused, 1u); chunk1 = atomicAdd(&st.ticket_fused, 1u); }
-    chunk = __shfl_sync(0xffffffffu, chunk, 0);
-    chunk1 = __shfl_sync(0xffffffffu, chunk1, 0);
-    uint32_t mo, fa, mf;
-    float ul;
-    scalar_stage(chunk * FUSED_CHUNK + lane, mo, fa, ul, mf);
-    while (chunk < n_chunks) {
-        uint32_t chunk2 = 0;
-        if (lane == 0) chunk2 = atomicAdd(&st.ticket_fused, 1u);   // consumed at the loop end
-        const uint32_t j0 = chunk * FUSED_CHUNK;
-        const uint32_t jl = j0 + lane;
-        // ---- (b) start the gather: half-warp h copies the row of offspring 2k+h
-#pragma unroll
-        for (int k = 0; k < FUSED_CHUNK / 2; ++k) {
-            const uint32_t pm = __shfl_sync(0xffffffffu, mo, 2 * k + (lane >> 4));   // byte offset of the row
-            cp_async16(cp_dst + k * 2 * FUSED_ROW, pop + (pm | cp_src));
-        }
-#pragma unroll
-        for (int k = 0; k < FUSED_CHUNK / 2; ++k) {
-            const uint32_t pf = __shfl_sync(0xffffffffu, fa, 2 * k + (lane >> 4));
-            cp_async16(cp_dst + FUSED_FA_OFF + k * 2 * FUSED_ROW, pop + (pf | cp_src));
-        }
-        cp_async_commit();
-        // ---- (a) of the next chunk: its index loads land while this chunk is worked on
-        uint32_t mo1, fa1, mf1;
-        float ul1;
-        scalar_stage(chunk1 * FUSED_CHUNK + lane, mo1, fa1, ul1, mf1);
-        // ---- (c) the 8 RECOMB blocks of this lane's (gamete, chromosome) role
-        uint32_t qn = 0;
-#pragma unroll
-        for (int it = 0; it < 8; ++it) {
-            const uint32_t j = j0 + it * 4 + sub;
-            uint32_t x[4];
-            draw_rk(sp, stream, j, c * 16, step, x);
-            uint32_t nc = 0;
-#pragma unroll
-            for (int i = 0; i < 6; ++i) nc += (x[0] >= T[i]) ? 1u : 0u;
-            if (!short_table && nc == 6) nc = poisson_count(XT, xl, x[0]);
-            uint32_t P = nc | ((x[1] >> 31) << 6) | ((__umulhi(x[2], clen1) + 1) << 8) | ((__umulhi(x[3], clen1) + 1) << 16);
-            // queue the chromosomes that need crossovers beyond the first two
-            const bool need = nc > 2;
-            const uint32_t bal = __ballot_sync(0xffffffffu, need);
-            uint32_t id = 63;
-            if (need) {
-                const uint32_t e = qn + __popc(bal & ((1u << lane) - 1u));
-                if (e < 32) { id = e; s_q[e] = (nc << 8) | ((uint32_t)it << 5) | lane; }
-            }
-            qn += __popc(bal);
-            s_P[it * 32 + lane] = P | (id << 24);
-        }
-        __syncwarp();
-        // one lane per queued chromosome computes its extra crossovers
-        if (lane < min(qn, 32u)) {
-            const uint32_t e = s_q[lane];
-            const uint32_t e_nc = e >> 8, e_it = (e >> 5) & 7u, e_ln = e & 31u;
-            const uint32_t e_c = e_ln & 3u, e_g = (e_ln >> 2) & 1u;
-            const uint32_t e_j = j0 + e_it * 4 + (e_ln >> 3);
-            const uint32_t e_clen1 = sp.chrom_len[e_c] - 1;
-            uint32_t xm[8];
-#pragma unroll
-            for (int w = 0; w < 8; ++w) xm[w] = 0;
-            const uint32_t extra = e_nc - 2;
-            for (uint32_t b = 0; b * 4 < extra; ++b) {
-                uint32_t y[4];
-                draw_rk(sp, e_g ? ST_RECOMB_P : ST_RECOMB_M, e_j, e_c * 16 + 1 + b, step, y);
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    if (b * 4 + i < extra) {
-                        const int s = (int)__umulhi(y[i], e_clen1) + 1;
-#pragma unroll
-                        for (int w = 0; w < 8; ++w) xm[w] ^= mask_from(s, w);
-                    }
-                }
-            }
-            s_xmask[lane * 2] = make_uint4(xm[0], xm[1], xm[2], xm[3]);
-            s_xmask[lane * 2 + 1] = make_uint4(xm[4], xm[5], xm[6], xm[7]);
-        }
-        cp_async_wait_all();
-        __syncwarp();
-        // ---- (m) R9: rare mutations, applied to the staged private copies of the parents' rows
-        if (__any_sync(0xffffffffu, mf != 0)) {
-            if (mf) {
-#pragma unroll
-                for (uint32_t gg = 0; gg < 2; ++gg) {
-                    if (!((mf >> gg) & 1u)) continue;
-                    const uint32_t ms = gg ? ST_MUT_P : ST_MUT_M;
-                    uint32_t *prow = (uint32_t *)(wbase + gg * FUSED_FA_OFF + lane * FUSED_ROW);
-                    uint32_t x[4];
-                    draw_rk(sp, ms, jl, 0, step, x);
-                    const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
-                    for (uint32_t k = 0; k < nm; ++k) {
-                        if (k > 0) draw_rk(sp, ms, jl, k, step, x);
-                        const uint32_t pos = __umulhi(x[1], L);
-                        const uint32_t bit = 1u << (pos & 31u);
-                        prow[pos >> 5] ^= bit;
-                        prow[L / 32 + (pos >> 5)] ^= bit;
-                    }
-                }
-            }
-            __syncwarp();
-        }
-
-        // ---- (d) 8 passes of 4 offspring
-#pragma unroll 2
-        for (uint32_t it = 0; it < FUSED_CHUNK / 4; ++it) {
-            const uint32_t j = j0 + it * 4 + sub;
-            const uint32_t a_ = ld_src + it * 4 * FUSED_ROW;
-            const uint4 a = lds128(a_), b = lds128(a_ + 16), d = lds128(a_ + 128), e = lds128(a_ + 144);
-            const uint32_t h0[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-            const uint32_t h1[8] = {d.x, d.y, d.z, d.w, e.x, e.y, e.z, e.w};
-            // R8: crossover mask of chromosome c of gamete g from the packed draw
-            const uint32_t P = s_P[it * 32 + lane];
-            const uint32_t nc = P & 63u;
-            const uint32_t phi = ((P >> 6) & 1u) ? 0xFFFFFFFFu : 0u;
-            const int s0 = nc > 0 ? (int)((P >> 8) & 0xFFu) : 4096;
-            const int s1 = nc > 1 ? (int)((P >> 16) & 0xFFu) : 4096;
-            uint32_t m[8];
-#pragma unroll
-            for (int w = 0; w < 8; ++w) m[w] = phi ^ mask_from(s0, w) ^ mask_from(s1, w);
-            if (nc > 2) {
-                const uint32_t id = (P >> 24) & 63u;
-                if (id < 32) {
-                    const uint4 xa = s_xmask[id * 2], xb = s_xmask[id * 2 + 1];
-                    m[0] ^= xa.x; m[1] ^= xa.y; m[2] ^= xa.z; m[3] ^= xa.w;
-                    m[4] ^= xb.x; m[5] ^= xb.y; m[6] ^= xb.z; m[7] ^= xb.w;
-                } else {  // queue overflow (> 32 such chromosomes in one chunk): compute in place
-                    const uint32_t extra = nc - 2;
-                    for (uint32_t bb = 0; bb * 4 < extra; ++bb) {
-                        uint32_t y[4];
-                        draw_rk(sp, stream, j, c * 16 + 1 + bb, step, y);
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            if (bb * 4 + i < extra) {
-                                const int s = (int)__umulhi(y[i], clen1) + 1;
-#pragma unroll
-                                for (int w = 0; w < 8; ++w) m[w] ^= mask_from(s, w);
-                            }
-                        }
-                    }
-                }
-            }
-            // select: gamete word = hap[phase] word
-            uint32_t gw[8];
-#pragma unroll
-            for (int w = 0; w < 8; ++w) gw[w] = (h0[w] & ~m[w]) | (h1[w] & m[w]);
-            // a7: the row is stored once, at row j of the other buffer (alive or not)
-            if (j < M) {
-                uint4 *o = nxt + (size_t)j * ROW4 + g * (ROW4 / 2) + c * 2;
-                o[0] = make_uint4(gw[0], gw[1], gw[2], gw[3]);
-                o[1] = make_uint4(gw[4], gw[5], gw[6], gw[7]);
-            }
-            // a5: this lane's share of the additive phenotype (R10), left where its draw was
-            uint32_t ones = 0;
-#pragma unroll
-            for (int w = 0; w < 8; ++w) ones += __popc(gw[w]);
-            s_P[it * 32 + lane] = ones;
-        }
-        __syncwarp();
-        // ---- (e) a5-a6: lane = offspring: exact integer phenotype, survival (R11) in the same fp32
-        // sequence as the materialised path
-        {
-            const uint4 oa = ((const uint4 *)s_P)[lane * 2], ob = ((const uint4 *)s_P)[lane * 2 + 1];
-            const int myzi = 2 * (int)(oa.x + oa.y + oa.z + oa.w + ob.x + ob.y + ob.z + ob.w) - 2 * (int)L;
-            bool captured;
-            const float z = __fmul_rn((float)myzi, sp.pheno_scale);
-            const float s = survival_prob(sp, z, theta, ul, captured);
-            const bool valid = jl < M;
-            const bool alive = valid && (ul < s);
-            if (valid && fabsf(__fsub_rn(ul, s)) < 1e-6f) ++ties;
-            if (alive) { acc1 += myzi; acc2 += (long long)myzi * myzi; ++n_alive; }
-            const uint32_t bal = __ballot_sync(0xffffffffu, alive);
-            if (lane == 0) sp.chunk_mask[chunk] = bal;
-        }
-        __syncwarp();   // the stage and the draw words are reused by the next chunk
-        chunk = chunk1;
-        chunk1 = __shfl_sync(0xffffffffu, chunk2, 0);
-        mo = mo1; fa = fa1; ul = ul1; mf = mf1;
-    }
-    // ---- a8: survivor reductions (exact integers)
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        acc1 += __shfl_xor_sync(0xffffffffu, acc1, o);
-        acc2 += __shfl_xor_sync(0xffffffffu, acc2, o);
-        ties += __shfl_xor_sync(0xffffffffu, ties, o);
-        n_alive += __shfl_xor_sync(0xffffffffu, n_alive, o);
-    }
-    if (lane == 0) {
-        if (acc1 != 0 || acc2 != 0) {
-            atomicAdd((unsigned long long *)&st.acc_zi, (unsigned long long)acc1);
-            atomicAdd((unsigned long long *)&st.acc_zi2, (unsigned long long)acc2);
-        }
-        if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
-        if (n_alive) atomicAdd(&st.n_next, n_alive);
-    }
-    if (sp.solo) solo_tail(sp, &s_flag);
-}
-
 // ---------------------------------------------------------------------------------------------
-// Father-staged variant.  Only the fathers' rows (random gather, full DRAM latency) go through
-// shared memory; the mothers' rows (ascending, shared by siblings, prefetched into L2 at the start
-// of the chunk) are loaded straight into registers one pass ahead.  Half the stage means twice the
-// resident warps.  In pass (d) a lane owns HALF a chromosome (4 words = one uint4) of BOTH gametes
-// of offspring it*4+sub, so that every global access of a quarter warp is 128 contiguous bytes.
+// The fused kernel.  A warp takes chunks of 32 consecutive offspring from an atomic ticket and runs
+// a software pipeline over them:
+//   (a) lane = offspring: SCALAR block (father -> rowptr -> row, survival uniform), the two MUT
+//       blocks' counts, mother row -- for the NEXT chunk, so that no index load is ever waited for.
+//   (b) 16 cp.async instructions start the gather of the chunk's 32 fathers' rows (8 KB) into this
+//       warp's stage (random rows, full DRAM latency); the mothers' rows (ascending, shared by
+//       siblings) are only prefetched into L2.  A stage of 8 KB instead of 16 doubles the warps.
+//   (c) lane = (gamete g, chromosome c) of offspring it*4+sub, it = 0..7: the 8 RECOMB blocks,
+//       decoded to a packed word (start phase, first two crossover positions); the few chromosomes
+//       with more than two crossovers (8 % at mean 1) are queued for pass (x).
+//   (m) rare: paternal mutations flip the bit in BOTH haplotypes of the staged private copy of the
+//       father's row, which flips it in the gamete whatever the phase is (R9).
+//   (d) 8 passes of 4 offspring: a lane owns HALF a chromosome (4 words = one uint4) of BOTH gametes,
+//       so that every global access of a quarter warp is 128 contiguous bytes; mothers' words come
+//       straight from global one pass ahead, fathers' from the stage; select, popcount, two 128-bit
+//       stores of offspring row j.
+//   (x) extra crossovers as a fix-up of the rows just stored.
+//   (e) lane = offspring: phenotype -> fp32 survival -> decision; the ballot is the chunk's mask.
 constexpr int FUSEDF_WARPS = 4;
-#ifndef SPEGG_UNROLL_C
-#define SPEGG_UNROLL_C 2
-#endif
-#ifndef SPEGG_CTAS
-#define SPEGG_CTAS 5
-#endif
-constexpr int FUSEDF_UNROLL_C = SPEGG_UNROLL_C;   // decode passes in flight per lane
-constexpr int FUSEDF_CTAS = SPEGG_CTAS;           // resident CTAs per SM (shared memory allows 5)
+constexpr int FUSEDF_UNROLL_C = 2;                // decode passes in flight per lane
+constexpr int FUSEDF_CTAS = 5;                    // resident CTAs per SM (shared memory and registers allow 5)
+constexpr int FUSEDF_AHEAD = 1;                   // passes the mothers' loads run ahead
 constexpr uint32_t FUSEDF_SP_OFF = FUSED_CHUNK * FUSED_ROW;        // packed draws [8][4][4][2] / partial sums
 constexpr uint32_t FUSEDF_Q_OFF = FUSEDF_SP_OFF + 8 * 32 * 4;      // queue of chromosomes with > 2 crossovers: draw [32], (pass, lane) [32]
 constexpr uint32_t FUSEDF_MO_OFF = FUSEDF_Q_OFF + 64 * 4;          // mothers' row offsets [32]
@@ -376,6 +109,13 @@ __device__ __forceinline__ uint4 ldg128(const void *p) {
     return v;
 }
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// ticket counter: written as PTX so that nvcc does not turn it into its warp-aggregated form, whose
+// broadcast shuffle waits for the atomic's round trip on the spot; the result is consumed a chunk later
+__device__ __forceinline__ uint32_t atom_inc_u32(uint32_t *p) {
+    uint32_t r;
+    asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(r) : "l"(p));
+    return r;
+}
 
 // packed draw of one (gamete, chromosome): s0 | s1 << 9 | phase << 31; positions 1..255,
 // 256 = no crossover
@@ -407,6 +147,7 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     const uint8_t *pop = sp.pop[st.cur];
     uint8_t *nxt = sp.pop[st.cur ^ 1u];
     const uint32_t *rowptr = sp.rowptr[st.cur];
+    uint32_t *range_cnt = sp.range_cnt[st.cur ^ 1u];   // zeroed by this step's k_scan_fused
     const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
     // the hot path only needs "at least 1 / 2 / 3 crossovers": x >= T_k written as x > T_k - 1 so that a
     // missing threshold (table shorter than k+1; T_k >= 1 is checked at create time) is never reached
@@ -424,6 +165,8 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     long long acc1 = 0, acc2 = 0;
     uint32_t ties = 0, n_alive = 0;
 
+    // mo / fa are the parents' physical ROW numbers exactly as loaded: nothing here depends on the
+    // two index loads, so they stay in flight until the rows are needed one chunk later
     auto scalar_stage = [&](uint32_t jl, uint32_t &mo, uint32_t &fa, float &ul, uint32_t &mf) {
         uint32_t x[4], a[4], b[4];
         draw_rk(sp, ST_SCALAR, jl, 0, step, x);
@@ -431,8 +174,8 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
         draw_rk(sp, ST_MUT_P, jl, 0, step, b);
         mo = 0; fa = 0; mf = 0; ul = 2.0f;
         if (jl < M) {
-            mo = sp.mother[jl] * FUSED_ROW;
-            fa = rowptr[uniform_index(x[0], N)] * FUSED_ROW;   // R2
+            mo = sp.mother[jl];
+            fa = rowptr[uniform_index(x[0], N)];   // R2
             ul = u01_of(x[3]);
             mf = (a[0] > Um0 ? 1u : 0u) | (b[0] > Um0 ? 2u : 0u);
         }
@@ -495,13 +238,13 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     // software pipeline over chunks: the first trip only runs stage (a) of the first chunk
     constexpr uint32_t NONE = 0xFFFFFFFFu;
     uint32_t chunk = NONE, chunk1 = 0;
-    if (lane == 0) chunk1 = atomicAdd(&st.ticket_fused, 1u);
+    if (lane == 0) chunk1 = atom_inc_u32(&st.ticket_fused);
     chunk1 = __shfl_sync(0xffffffffu, chunk1, 0);
     uint32_t mo = 0, fa = 0, mf = 0;
     float ul = 2.0f;
     for (;;) {
         uint32_t chunk2 = 0;
-        if (lane == 0) chunk2 = atomicAdd(&st.ticket_fused, 1u);   // consumed at the loop end
+        if (lane == 0) chunk2 = atom_inc_u32(&st.ticket_fused);   // consumed at the loop end
         const bool active = chunk != NONE;
         j0 = chunk * FUSED_CHUNK;
         const uint32_t jl = j0 + lane;
@@ -509,16 +252,16 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
         if (active) {
 #pragma unroll
             for (int k = 0; k < FUSED_CHUNK / 2; ++k) {
-                const uint32_t pf = __shfl_sync(0xffffffffu, fa, 2 * k + (lane >> 4));
+                const uint32_t pf = __shfl_sync(0xffffffffu, fa, 2 * k + (lane >> 4)) * FUSED_ROW;
                 cp_async16(cp_dst + k * 2 * FUSED_ROW, pop + (pf | cp_src));
             }
             cp_async_commit();
             //  mothers: every 32-byte sector of the 32 rows is asked into L2 (lane -> sector lane&7 of
             //  the rows of offspring (lane>>3) + 4k)
-            s_mo[lane] = mo;
+            s_mo[lane] = mo * FUSED_ROW;
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
-                const uint32_t pm = __shfl_sync(0xffffffffu, mo, 4 * k + (lane >> 3));
+                const uint32_t pm = __shfl_sync(0xffffffffu, mo, 4 * k + (lane >> 3)) * FUSED_ROW;
                 prefetch_l2(pop + (pm | ((lane & 7u) * 32u)));
             }
         }
@@ -559,16 +302,20 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
             __syncwarp();
         }
 
-        // ---- (d) 8 passes of 4 offspring; mothers' words are loaded one pass ahead
-        const uint8_t *mrow = pop + (s_mo[sub] | (q * 16u));
-        uint4 ma = ldg128(mrow), mb = ldg128(mrow + FUSED_ROW / 2);
-#pragma unroll 2
-        for (uint32_t it = 0; it < FUSED_CHUNK / 4; ++it) {
+        // ---- (d) 8 passes of 4 offspring; mothers' words are loaded TWO passes ahead (an L2 round trip
+        // is several passes long)
+        uint4 ma[FUSEDF_AHEAD], mb[FUSEDF_AHEAD];
+#pragma unroll
+        for (int p = 0; p < FUSEDF_AHEAD; ++p) {
+            const uint8_t *mrow = pop + (s_mo[p * 4 + sub] | (q * 16u));
+            ma[p] = ldg128(mrow); mb[p] = ldg128(mrow + FUSED_ROW / 2);
+        }
+        auto pass = [&](const uint32_t it, uint4 &ma_, uint4 &mb_) {
             const uint32_t o = it * 4 + sub, j = j0 + o;
-            const uint4 ca = ma, cb = mb;
-            if (it + 1 < FUSED_CHUNK / 4) {
-                mrow = pop + (s_mo[o + 4] | (q * 16u));
-                ma = ldg128(mrow); mb = ldg128(mrow + FUSED_ROW / 2);
+            const uint4 ca = ma_, cb = mb_;
+            if (it + FUSEDF_AHEAD < FUSED_CHUNK / 4) {
+                const uint8_t *mrow = pop + (s_mo[o + 4 * FUSEDF_AHEAD] | (q * 16u));
+                ma_ = ldg128(mrow); mb_ = ldg128(mrow + FUSED_ROW / 2);
             }
             const uint4 fa0 = lds128(ld_fa + it * 4 * FUSED_ROW), fa1_ = lds128(ld_fa + it * 4 * FUSED_ROW + FUSED_ROW / 2);
             const uint2 PP = *(const uint2 *)(s_P + it * 32 + sp_slot);
@@ -602,6 +349,11 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
                                   __popc(gp.x) + __popc(gp.y) + __popc(gp.z) + __popc(gp.w);
             __syncwarp();
             s_P[it * 32 + lane] = ones;
+        };
+#pragma unroll(FUSEDF_AHEAD == 1 ? 2 : 1)
+        for (uint32_t it = 0; it < FUSED_CHUNK / 4; it += FUSEDF_AHEAD) {
+#pragma unroll
+            for (int p = 0; p < FUSEDF_AHEAD; ++p) pass(it + p, ma[p], mb[p]);
         }
         __syncwarp();
         // ---- (x) R8, crossovers beyond the second (8 % of the chromosomes at mean 1): one lane per
@@ -635,7 +387,10 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
             if (valid && fabsf(__fsub_rn(ul, s)) < 1e-6f) ++ties;
             if (alive) { acc1 += myzi; acc2 += (long long)myzi * myzi; ++n_alive; }
             const uint32_t bal = __ballot_sync(0xffffffffu, alive);
-            if (lane == 0) sp.chunk_mask[chunk] = bal;
+            if (lane == 0) {
+                sp.chunk_mask[chunk] = bal;
+                if (bal) atomicAdd(range_cnt + chunk / SCANF_CHUNKS, (uint32_t)__popc(bal));
+            }
         }
         __syncwarp();   // the stage and the draw words are reused by the next chunk
         }
@@ -663,51 +418,58 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
 }
 
 // a1-a3 and the index half of a7 for a species on the fused path.  The current buffer holds
-// m_phys physical rows in 32-row slabs; chunk_mask says which are adults.  A CTA takes a range of
-// 2,048 rows (8 per thread):
-//   look-back 1 over the alive counts  -> logical index i of every adult, rowptr[i] = row
+// m_phys physical rows in 32-row slabs; chunk_mask says which are adults and range_cnt how many
+// adults each 2,048-row range holds (both left by the previous step's fused kernel, or by
+// spegg_write_state).  A CTA takes one range (8 rows per thread):
+//   sum of range_cnt[0 .. range)       -> logical index i of every adult, rowptr[i] = row
 //   FEC draw of adult i                -> fecundity f_i  (R5)
-//   look-back 2 over the fecundities   -> offspring base off_i, mother[off_i .. off_i+f_i) = row
-// index_only = 1 builds rowptr alone (spegg_read_state).
-constexpr int SCANF_ROWS = 8;
-constexpr int SCANF_RANGE = SCAN_THREADS * SCANF_ROWS;
-
+//   look-back over the fecundities     -> offspring base off_i, mother[off_i .. off_i+f_i) = row
+// so the only chain between CTAs is ONE look-back.  It also zeroes the other buffer's range counts,
+// which the fused kernel of this step accumulates.  index_only = 1 builds rowptr alone
+// (spegg_read_state).
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_constant__ SpK sp, int index_only) {
+    constexpr uint32_t NW = SCAN_THREADS / 32;
     __shared__ uint32_t s_tab[TMAX];
-    __shared__ uint32_t s_warp[SCAN_THREADS / 32];
-    __shared__ uint32_t s_tile;
-    __shared__ unsigned long long s_excl;
+    __shared__ uint32_t s_cnt[2][NW], s_pre[2][NW], s_f[2][NW];
+    __shared__ uint32_t s_tile[2];
+    __shared__ unsigned long long s_excl[2];
     DevSpecies &st = *sp.st;
-    const uint32_t mp = st.m_phys, step = sp.glob->step;
+    const uint32_t mp = st.m_phys, step = sp.glob->step, cur = st.cur;
     const uint32_t n_ranges = (mp + SCANF_RANGE - 1) / SCANF_RANGE;
     const uint32_t n_chunks = (mp + FUSED_CHUNK - 1) / FUSED_CHUNK;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t *cnt = sp.range_cnt[cur];
+    uint32_t *rp = sp.rowptr[cur];
+    if (tid == 0) s_tile[0] = atomicAdd(&st.ticket_cmp, 1u);
+    if (!index_only) {
+        uint32_t *cnt_next = sp.range_cnt[cur ^ 1u];
+        const uint32_t n_max = (sp.capacity + 31u) / 32u * 32u / SCANF_RANGE + 2u;
+        for (uint32_t i = blockIdx.x * SCAN_THREADS + tid; i < n_max; i += gridDim.x * SCAN_THREADS) cnt_next[i] = 0u;
+    }
     const uint32_t len0 = sp.table_len[0];
     for (uint32_t i = tid; i < len0; i += SCAN_THREADS) s_tab[i] = sp.tables[i];
-    uint32_t *rp = sp.rowptr[st.cur];
-    for (;;) {
-        if (tid == 0) s_tile = atomicAdd(&st.ticket_cmp, 1u);
-        __syncthreads();
-        const uint32_t range = s_tile;
+    __syncthreads();
+    for (uint32_t trip = 0;; ++trip) {
+        const uint32_t b = trip & 1u;            // shared scratch alternates, so one barrier less per trip
+        const uint32_t range = s_tile[b];
         if (range >= n_ranges) break;
         const uint32_t row0 = range * SCANF_RANGE + tid * SCANF_ROWS;
         const uint32_t ch = row0 >> 5;
         const uint32_t bits = ch < n_chunks ? (sp.chunk_mask[ch] >> (row0 & 31u)) & 0xFFu : 0u;
-        // ---- look-back 1: adults before this thread's rows
-        const uint32_t cnt = __popc(bits);
-        const uint32_t incl = warp_incl_scan(cnt);
-        if (lane == 31) s_warp[warp] = incl;
+        // ---- adults before this range (from the range counts) and before this thread's rows
+        uint32_t pre = 0;
+        for (uint32_t k = tid; k < range; k += SCAN_THREADS) pre += cnt[k];
+        const uint32_t c8 = __popc(bits);
+        const uint32_t incl = warp_incl_scan(c8);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) pre += __shfl_xor_sync(0xffffffffu, pre, o);
+        if (lane == 31) s_cnt[b][warp] = incl;
+        if (lane == 0) s_pre[b][warp] = pre;
+        if (tid == 0) s_tile[b ^ 1u] = atomicAdd(&st.ticket_cmp, 1u);   // next trip's range
         __syncthreads();
-        if (warp == 0) {
-            const uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
-            const uint32_t wi = warp_incl_scan(w);
-            const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
-            const unsigned long long excl = lookback(sp.status_cmp, sp.status_cmp_n, range, (unsigned long long)total);
-            if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;
-            if (lane == 0) s_excl = excl;
-        }
-        __syncthreads();
-        uint32_t i = (uint32_t)s_excl + s_warp[warp] + (incl - cnt);
+        uint32_t i = incl - c8;
+#pragma unroll
+        for (uint32_t w = 0; w < NW; ++w) i += s_pre[b][w] + (w < warp ? s_cnt[b][w] : 0u);
         // ---- rowptr and fecundity of this thread's adults
         uint32_t fsum = 0;
         unsigned long long fpack = 0ull;
@@ -725,20 +487,18 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
                 ++i;
             }
         }
-        __syncthreads();   // s_warp / s_excl are reused
         if (index_only) continue;
-        // ---- look-back 2: offspring before this thread's adults
+        // ---- look-back over the fecundities: offspring before this thread's adults
         const uint32_t fincl = warp_incl_scan(fsum);
-        if (lane == 31) s_warp[warp] = fincl;
+        if (lane == 31) s_f[b][warp] = fincl;
         __syncthreads();
+        uint32_t total = 0, wbase = 0;
+#pragma unroll
+        for (uint32_t w = 0; w < NW; ++w) { const uint32_t v = s_f[b][w]; total += v; if (w < warp) wbase += v; }
         if (warp == 0) {
-            const uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
-            const uint32_t wi = warp_incl_scan(w);
-            const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
             const unsigned long long excl = lookback(sp.status_fec, sp.status_fec_n, range, (unsigned long long)total);
-            if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;
             if (lane == 0) {
-                s_excl = excl;
+                s_excl[b] = excl;
                 if (range == n_ranges - 1) {  // the last range knows M
                     const unsigned long long Mtot = excl + total;
                     if (Mtot > (unsigned long long)sp.capacity) { st.m = sp.capacity; st.flags_step |= 1u; }
@@ -747,24 +507,25 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
             }
         }
         __syncthreads();
-        unsigned long long o = s_excl + s_warp[warp] + (fincl - fsum);
+        unsigned long long o = s_excl[b] + wbase + (fincl - fsum);
 #pragma unroll
         for (int k = 0; k < SCANF_ROWS; ++k) {
             const uint32_t f = (uint32_t)(fpack >> (8 * k)) & 0xFFu;
             for (uint32_t cpy = 0; cpy < f; ++cpy, ++o)
                 if (o < (unsigned long long)sp.capacity) sp.mother[o] = row0 + k;
         }
-        __syncthreads();
     }
 }
 
-// chunk masks of a freshly written, dense population of n rows
-__global__ void __launch_bounds__(256) k_fill_masks(uint32_t *mask, uint32_t n) {
-    const uint32_t n_chunks = (n + 31) / 32;
+// chunk masks and range counts of a freshly written, dense population of n rows
+__global__ void __launch_bounds__(256) k_fill_masks(uint32_t *mask, uint32_t *range_cnt, uint32_t n) {
+    const uint32_t n_chunks = (n + 31) / 32, n_ranges = (n + SCANF_RANGE - 1) / SCANF_RANGE;
     for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < n_chunks; c += gridDim.x * blockDim.x) {
         const uint32_t r = n - c * 32;
         mask[c] = r >= 32 ? 0xFFFFFFFFu : ((1u << r) - 1u);
     }
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < n_ranges; c += gridDim.x * blockDim.x)
+        range_cnt[c] = min(n - c * SCANF_RANGE, (uint32_t)SCANF_RANGE);
 }
 
 __host__ inline bool fused_bit_supported(const SpK &k) {
@@ -774,18 +535,16 @@ __host__ inline bool fused_bit_supported(const SpK &k) {
 }
 
 inline cudaError_t fused_bit_configure() {
-    cudaError_t e = cudaFuncSetAttribute(k_fused_bit<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSED_SMEM);
-    if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_fused_bit_f<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
 }
 
-inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream, int variant) {
-    if (variant == 0) k_fused_bit<4, 8><<<n_sms * 3, FUSED_WARPS * 32, FUSED_SMEM, stream>>>(k);
-    else k_fused_bit_f<4, 8><<<n_sms * FUSEDF_CTAS, FUSEDF_WARPS * 32, FUSEDF_SMEM, stream>>>(k);
+inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
+    k_fused_bit_f<4, 8><<<n_sms * FUSEDF_CTAS, FUSEDF_WARPS * 32, FUSEDF_SMEM, stream>>>(k);
 }
 
+// one range per CTA in a single wave at the bench sizes (capacity / 2,048 = 576 ranges <= 4 per SM)
 inline void launch_scan_fused(const SpK &k, uint32_t n_sms, cudaStream_t stream, int index_only) {
-    k_scan_fused<<<n_sms * 2, SCAN_THREADS, 0, stream>>>(k, index_only);
+    k_scan_fused<<<n_sms * 4, SCAN_THREADS, 0, stream>>>(k, index_only);
 }
 
 }  // namespace spegg

@@ -77,6 +77,7 @@ struct SpK {
     uint32_t *patch_start[2];   // [P+1] each
     uint32_t *rowptr[2];        // logical adult index -> physical row of pop[]
     uint32_t *chunk_mask;       // fused path: survivor bitmask of each 32-offspring chunk
+    uint32_t *range_cnt[2];     // fused path: adults per 2,048-row range of pop[0] / pop[1]
     uint32_t phys_parents;      // 1: mother[] / father[] hold physical rows (fused path)
     uint32_t solo;              // 1: single-species simulation (k_index finishes and prepares the step)
     uint8_t *f;
