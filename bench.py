@@ -289,7 +289,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` capture summarised under profiles/ (None until a capture exists).
-TRAFFIC_BYTES = {}
+TRAFFIC_BYTES = {"C3": 550.2e6}   # profiles/r01_fused_full.md: 344.7 MB read + 205.5 MB written
 
 
 def main():
