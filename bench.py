@@ -217,7 +217,8 @@ def run_ours(args):
     sim.step(kt_steps)
     k_ms, k_n = sim.kernel_timing(False)
     klog = sim.read_log(0)[kl0:kl0 + kt_steps]
-    k_bytes = alg_bytes(cfg, klog, kernel_only=True) / max(1, len(klog))
+    # a one-launch step does the scan too: the kernel is charged the whole step's bytes
+    k_bytes = alg_bytes(cfg, klog, kernel_only=sim.launches_per_step() > 1) / max(1, len(klog))
 
     # ---- end to end through the C ABI with HOST buffers: upload, K x (step + read of the step's
     # result), download -- all inside the timed region
@@ -275,7 +276,7 @@ def run_ours(args):
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": TRAFFIC_BYTES.get(cfg["name"]),
-                         "kernel": "fused gamete+phenotype+survival+compaction" if k_n else "none",
+                         "kernel": ("fused step kernel: scan+parents+gametes+phenotype+survival+compaction" if sim.launches_per_step() == 1 else "gamete kernel") if k_n else "none",
                          "kernel_ms": k_ms, "kernel_launches_timed": k_n, "alg_bytes_per_launch": k_bytes,
                          "peak_source": peak_src},
             "cpu_baseline": {"value": cb_units / cb_dt, "unit": UNIT, "cores": 1, "kind": "oracle",

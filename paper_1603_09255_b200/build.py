@@ -24,7 +24,7 @@ def build(force=False, verbose=False):
     if not force and not _stale():
         return SO
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + ["-o", SO] + [os.path.join(CSRC, f) for f in SOURCES]
+    cmd = [nvcc] + NVCC_FLAGS + os.environ.get("SPEGG_NVCC_FLAGS", "").split() + ["-o", SO] + [os.path.join(CSRC, f) for f in SOURCES]
     if verbose:
         cmd += ["-Xptxas", "-v"]
     subprocess.run(cmd, check=True, cwd=CSRC)

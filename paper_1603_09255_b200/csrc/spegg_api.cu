@@ -82,6 +82,8 @@ int h_normal_table(double sq, std::vector<uint32_t> &T) {
 }
 
 // ------------------------------------------------------------------------------ layout
+constexpr uint64_t HEADER_SPK = 8192;   // workspace header: DevGlobal at 0, DevSpecies[] at 256, SpK[] here
+
 struct Carver {
     uint64_t off = 0;
     uint64_t take(uint64_t bytes) {
@@ -92,7 +94,7 @@ struct Carver {
 };
 
 struct SpeciesLayout {
-    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask, range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
+    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
     uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, K_patch, theta_patch;
     uint32_t norm_len, n_tables, row_bytes;
@@ -161,7 +163,7 @@ uint32_t row_bytes_of(const spegg_species_params &q) {
 // Lays out the whole workspace; returns total bytes.  Header: DevGlobal + DevSpecies[MAX].
 uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
     Carver c;
-    c.take(4096 + MAX_SPECIES * sizeof(SpK));  // header: DevGlobal, DevSpecies[], SpK[]
+    c.take(HEADER_SPK + MAX_SPECIES * sizeof(SpK));  // header: DevGlobal, DevSpecies[], SpK[]
     const uint32_t gw = p->grid_w ? p->grid_w : 1, gh = p->grid_h ? p->grid_h : 1;
     const uint64_t P = (uint64_t)gw * gh;
     const uint32_t logcap = p->log_capacity ? p->log_capacity : 4096;
@@ -177,14 +179,15 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.pop[1] = c.take(cap32 * l.row_bytes);
         l.rowptr[0] = c.take(cap32 * 4);
         l.rowptr[1] = c.take(cap32 * 4);
-        l.chunk_mask = c.take((cap / 32 + 2) * 4);
+        l.chunk_mask[0] = c.take((cap / 32 + 2) * 4);
+        l.chunk_mask[1] = c.take((cap / 32 + 2) * 4);
         l.range_cnt[0] = c.take((cap32 / SCANF_RANGE + 2) * 4);
         l.range_cnt[1] = c.take((cap32 / SCANF_RANGE + 2) * 4);
         l.patch_start[0] = c.take((P + 1) * 4);
         l.patch_start[1] = c.take((P + 1) * 4);
         l.f = c.take(cap);
         l.off = c.take(cap * 4);
-        l.mother = c.take(cap * 4);
+        l.mother = c.take(cap32 * 4);
         l.father = c.take(cap * 4);
         l.dest = c.take(cap * 4);
         l.pos = c.take(cap * 4);
@@ -233,7 +236,7 @@ struct spegg_sim {
     DevGlobal *d_glob = nullptr;
     DevSpecies *d_st = nullptr;
     SpK *d_spk = nullptr;
-    uint32_t P = 1, n_sms = 148, launches = 0;
+    uint32_t P = 1, n_sms = 148, launches = 0, scan_ctas = 1;
     uint32_t log_capacity = 4096;
     bool debug = false;
     // kernel timing (direct launches bracketed by events)
@@ -284,7 +287,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
         const SpK &k = h.k;
         const bool time_this = timed && si == 0 && s->ev_used + 2 <= s->ev.size();
         if (fused_ok(s, h)) {
-            launch_scan_fused(k, G, s->stream, 0); ++nl;
+            CU(launch_scan_fused(k, G, s->scan_ctas, s->stream)); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             launch_fused_bit(k, G, s->stream); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
@@ -384,8 +387,9 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     }
     s->d_glob = at<DevGlobal>(s, 0);
     s->d_st = at<DevSpecies>(s, 256);
-    s->d_spk = at<SpK>(s, 4096);
-    if (cudaMemsetAsync(s->ws, 0, 4096 + MAX_SPECIES * sizeof(SpK), s->stream) != cudaSuccess) return fail(SPEGG_ECUDA);
+    s->d_spk = at<SpK>(s, HEADER_SPK);
+    static_assert(256 + MAX_SPECIES * sizeof(DevSpecies) <= HEADER_SPK, "header too small");
+    if (cudaMemsetAsync(s->ws, 0, HEADER_SPK + MAX_SPECIES * sizeof(SpK), s->stream) != cudaSuccess) return fail(SPEGG_ECUDA);
 
     s->sp.resize(p->n_species);
     for (uint32_t si = 0; si < p->n_species; ++si) {
@@ -457,7 +461,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.pop[0] = at<uint8_t>(s, l.pop[0]); k.pop[1] = at<uint8_t>(s, l.pop[1]);
         k.patch_start[0] = at<uint32_t>(s, l.patch_start[0]); k.patch_start[1] = at<uint32_t>(s, l.patch_start[1]);
         k.rowptr[0] = at<uint32_t>(s, l.rowptr[0]); k.rowptr[1] = at<uint32_t>(s, l.rowptr[1]);
-        k.chunk_mask = at<uint32_t>(s, l.chunk_mask);
+        k.chunk_mask[0] = at<uint32_t>(s, l.chunk_mask[0]); k.chunk_mask[1] = at<uint32_t>(s, l.chunk_mask[1]);
         k.range_cnt[0] = at<uint32_t>(s, l.range_cnt[0]);
         k.range_cnt[1] = at<uint32_t>(s, l.range_cnt[1]);
         k.f = at<uint8_t>(s, l.f); k.off = at<uint32_t>(s, l.off);
@@ -479,6 +483,11 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     }
     for (uint32_t si = 0; si < p->n_species; ++si)
         if (s->sp[si].k.phys_parents && fused_bit_configure() != cudaSuccess) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }
+    {
+        const int n = scan_fused_ctas_per_sm();
+        if (n < 1) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }
+        s->scan_ctas = (uint32_t)n;
+    }
     for (uint32_t si = 0; si < p->n_species; ++si)
         if (s->sp[si].p.sel_predation) s->sp[si].k.cap_pred = s->sp[s->sp[si].p.predator_species].k.cap;
 
@@ -536,7 +545,7 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
     CU(cudaMemcpyAsync(s->d_glob, &g, sizeof g, cudaMemcpyHostToDevice, s->stream));
     if (n) {
         k_iota<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k.rowptr[cur], (uint32_t)n);
-        if (h.k.phys_parents) k_fill_masks<<<s->n_sms, 256, 0, s->stream>>>(h.k.chunk_mask, h.k.range_cnt[cur], (uint32_t)n);
+        if (h.k.phys_parents) k_fill_masks<<<s->n_sms, 256, 0, s->stream>>>(h.k.chunk_mask[cur], h.k.range_cnt[cur], (uint32_t)n);
         k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1);
     }
     launch_prepare(s);
@@ -572,8 +581,7 @@ int spegg_read_state(spegg_sim *s, uint32_t species, uint64_t *n, uint32_t *step
     if (step) *step = g.step;
     if ((genomes_out || zi_out) && st.n && h.k.phys_parents) {
         // fused path: the index (rowptr) of the current buffer is built on demand
-        launch_scan_fused(h.k, s->n_sms, s->stream, 1);
-        launch_prepare(s);   // clears the look-back words and tickets the scan used
+        launch_rowptr_fused(h.k, s->n_sms, s->stream);
     }
     if (genomes_out) {
         if (cap_bytes < (uint64_t)st.n * h.k.row_bytes) return SPEGG_ERANGE;
@@ -656,5 +664,12 @@ int spegg_kernel_timing(spegg_sim *s, int enable, float *mean_ms, uint32_t *n_la
     s->timing = enable != 0;
     return SPEGG_OK;
 }
+
+#ifdef SPEGG_PROBE
+// development build only (-DSPEGG_PROBE): the timing probes of the step kernel
+int spegg_probe_read(unsigned long long *out, uint32_t n_words) {
+    return cudaMemcpyFromSymbol(out, spegg::g_probe, (size_t)n_words * 8) == cudaSuccess ? 0 : -3;
+}
+#endif
 
 }  // extern "C"

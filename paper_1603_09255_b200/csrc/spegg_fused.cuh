@@ -4,7 +4,7 @@
 // loci, 256-byte rows).  One time step is TWO launches:
 //
 //   k_scan_fused  a1-a3 + the index half of a7: one pass over the physical rows of the current
-//                 buffer (32-row slabs, one survivor bitmask per slab, one adult count per 2,048-row
+//                 buffer (32-row slabs, one survivor bitmask per slab, one adult count per 1,024-row
 //                 range): logical adult index from the range counts -> rowptr[], Poisson fecundity
 //                 of every adult, ONE look-back over the fecundities -> mother[] (physical rows), M_t.
 //   k_fused_bit_f a3-a8 in one pass: father draw, asynchronous gather of the fathers' rows into
@@ -15,6 +15,10 @@
 //                 once at row j of the other buffer, and only the 4-byte survivor mask of each
 //                 32-offspring chunk says which rows are the next generation.  Its last CTA closes
 //                 the step and prepares the next one (a0, a9).
+//
+// (A one-launch variant -- the scan as a first phase of the gamete kernel, which then polled the
+// index words -- measured slower: the scan is latency-bound and wants the whole machine's warps,
+// which the gamete kernel's 20 warps per SM do not give it.)
 //
 // Every draw is addressed by (stream, entity, block, step), never by thread, so the result is
 // bit-identical to the materialised pipeline and to the oracle.
@@ -50,8 +54,7 @@ __device__ __forceinline__ uint32_t mask_from(int s, int w) {
 
 constexpr int FUSED_CHUNK = 32;                 // offspring per warp iteration = rows per slab
 constexpr uint32_t FUSED_ROW = 256;             // bytes per row (config 3)
-constexpr int SCANF_ROWS = 8;                   // rows per thread of k_scan_fused
-constexpr int SCANF_RANGE = SCAN_THREADS * SCANF_ROWS;          // rows per range (2,048 = 64 chunks)
+constexpr int SCANF_RANGE = FUSED_RANGE;         // rows per scan range (1,024 = 32 chunks)
 constexpr int SCANF_CHUNKS = SCANF_RANGE / FUSED_CHUNK;
 
 // Philox4x32-10 (R3) with the ten round keys taken from the kernel parameter block: the key
@@ -126,6 +129,30 @@ __device__ __forceinline__ void half_masks(uint32_t P, uint32_t half, uint32_t (
     for (int i = 0; i < 4; ++i) m[i] = phi ^ mask_from(s0, i) ^ mask_from(s1, i);
 }
 
+#ifdef SPEGG_PROBE
+// timing probes of a development build (-DSPEGG_PROBE): globaltimer at the phase boundaries of every warp
+__device__ unsigned long long g_probe[8192 * 8];
+__device__ __forceinline__ void probe_cta(uint32_t slot) {   // scan kernel: one row per CTA after the gamete kernel's rows
+    if (threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+        g_probe[((4096u + blockIdx.x) & 8191u) * 8 + slot] = t;
+    }
+}
+#define PROBE_CTA(slot) probe_cta(slot)
+__device__ __forceinline__ void probe(uint32_t slot) {
+    if ((threadIdx.x & 31u) == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+        g_probe[((blockIdx.x * FUSEDF_WARPS + (threadIdx.x >> 5)) & 4095u) * 8 + slot] = t;
+    }
+}
+#define PROBE(slot) probe(slot)
+#else
+#define PROBE(slot)
+#define PROBE_CTA(slot)
+#endif
+
 template <int NC, int WPC>
 __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(const __grid_constant__ SpK sp) {
     static_assert(NC == 4 && WPC == 8, "lane group of 8 = 2 gametes x 4 chromosomes of 8 words");
@@ -147,7 +174,8 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     const uint8_t *pop = sp.pop[st.cur];
     uint8_t *nxt = sp.pop[st.cur ^ 1u];
     const uint32_t *rowptr = sp.rowptr[st.cur];
-    uint32_t *range_cnt = sp.range_cnt[st.cur ^ 1u];   // zeroed by this step's k_scan_fused
+    uint32_t *mask_nxt = sp.chunk_mask[st.cur ^ 1u];
+    uint32_t *range_cnt = sp.range_cnt[st.cur ^ 1u];   // zeroed when the previous step was closed
     const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
     // the hot path only needs "at least 1 / 2 / 3 crossovers": x >= T_k written as x > T_k - 1 so that a
     // missing threshold (table shorter than k+1; T_k >= 1 is checked at create time) is never reached
@@ -164,6 +192,8 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     const uint32_t sp_slot = sub * 8u + hc * 2u;                                    // + it * 32: (g=0, g=1) pair
     long long acc1 = 0, acc2 = 0;
     uint32_t ties = 0, n_alive = 0;
+
+    PROBE(0);
 
     // mo / fa are the parents' physical ROW numbers exactly as loaded: nothing here depends on the
     // two index loads, so they stay in flight until the rows are needed one chunk later
@@ -237,15 +267,16 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
 
     // software pipeline over chunks: the first trip only runs stage (a) of the first chunk
     constexpr uint32_t NONE = 0xFFFFFFFFu;
-    uint32_t chunk = NONE, chunk1 = 0;
-    if (lane == 0) chunk1 = atom_inc_u32(&st.ticket_fused);
-    chunk1 = __shfl_sync(0xffffffffu, chunk1, 0);
+    // the first two chunks of every warp are fixed (a burst of same-address atomics at the start of
+    // the kernel would be served one by one), the later ones come from the ticket
+    const uint32_t gwarp = blockIdx.x * FUSEDF_WARPS + warp, n_warps = gridDim.x * FUSEDF_WARPS;
+    uint32_t chunk = NONE, chunk1 = gwarp;
     uint32_t mo = 0, fa = 0, mf = 0;
     float ul = 2.0f;
     for (;;) {
         uint32_t chunk2 = 0;
-        if (lane == 0) chunk2 = atom_inc_u32(&st.ticket_fused);   // consumed at the loop end
         const bool active = chunk != NONE;
+        if (lane == 0) chunk2 = active ? 2u * n_warps + atom_inc_u32(&st.ticket_fused) : gwarp + n_warps;   // consumed at the loop end
         j0 = chunk * FUSED_CHUNK;
         const uint32_t jl = j0 + lane;
         // ---- (b) fathers: half-warp h copies the row of offspring 2k+h into the stage
@@ -388,7 +419,7 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
             if (alive) { acc1 += myzi; acc2 += (long long)myzi * myzi; ++n_alive; }
             const uint32_t bal = __ballot_sync(0xffffffffu, alive);
             if (lane == 0) {
-                sp.chunk_mask[chunk] = bal;
+                mask_nxt[chunk] = bal;
                 if (bal) atomicAdd(range_cnt + chunk / SCANF_CHUNKS, (uint32_t)__popc(bal));
             }
         }
@@ -414,91 +445,100 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
         if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
         if (n_alive) atomicAdd(&st.n_next, n_alive);
     }
+    PROBE(3);
     if (sp.solo) solo_tail(sp, &s_flag);
+    PROBE(4);
 }
 
-// a1-a3 and the index half of a7 for a species on the fused path.  The current buffer holds
-// m_phys physical rows in 32-row slabs; chunk_mask says which are adults and range_cnt how many
-// adults each 2,048-row range holds (both left by the previous step's fused kernel, or by
-// spegg_write_state).  A CTA takes one range (8 rows per thread):
+// a1-a3 and the index half of a7 for a species on the fused path.  The current buffer holds m_phys
+// physical rows in 32-row slabs; chunk_mask[cur] says which are adults and range_cnt[cur] how many
+// adults each 1,024-row range holds (both left by the previous step's gamete kernel, or by
+// spegg_write_state).  CTA b takes ranges b, b + gridDim.x, ... (4 rows per thread, so that the
+// whole machine shares the FEC draws):
 //   sum of range_cnt[0 .. range)       -> logical index i of every adult, rowptr[i] = row
 //   FEC draw of adult i                -> fecundity f_i  (R5)
 //   look-back over the fecundities     -> offspring base off_i, mother[off_i .. off_i+f_i) = row
-// so the only chain between CTAs is ONE look-back.  It also zeroes the other buffer's range counts,
-// which the fused kernel of this step accumulates.  index_only = 1 builds rowptr alone
-// (spegg_read_state).
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_constant__ SpK sp, int index_only) {
-    constexpr uint32_t NW = SCAN_THREADS / 32;
+// so the only dependence between CTAs is ONE counted look-back.  rowptr[] and mother[] are staged in
+// shared memory and stored coalesced.  The launch is cooperative: every CTA of the grid is resident,
+// so the look-back never waits for a range nobody has started (no ticket: a thousand same-address
+// atomics at the start of a kernel are served one by one).
+constexpr uint32_t SCANF_ROWS = SCANF_RANGE / SCAN_THREADS;   // rows per thread (4)
+constexpr uint32_t SCANF_STAGE = 4096;                        // index words staged per range
+static_assert(SCANF_ROWS == 4 && 32 % SCANF_ROWS == 0, "a thread's rows are one nibble of a slab mask");
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_constant__ SpK sp) {
+    constexpr uint32_t NW = SCAN_THREADS / 32, NT = SCAN_THREADS;
     __shared__ uint32_t s_tab[TMAX];
-    __shared__ uint32_t s_cnt[2][NW], s_pre[2][NW], s_f[2][NW];
-    __shared__ uint32_t s_tile[2];
-    __shared__ unsigned long long s_excl[2];
+    __shared__ uint32_t s_cnt[NW], s_pre[NW], s_f[NW];
+    __shared__ unsigned long long s_excl;
+    __shared__ uint32_t s_stage[SCANF_STAGE];
     DevSpecies &st = *sp.st;
     const uint32_t mp = st.m_phys, step = sp.glob->step, cur = st.cur;
     const uint32_t n_ranges = (mp + SCANF_RANGE - 1) / SCANF_RANGE;
-    const uint32_t n_chunks = (mp + FUSED_CHUNK - 1) / FUSED_CHUNK;
+    const uint32_t n_slabs = (mp + FUSED_CHUNK - 1) / FUSED_CHUNK;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t *cnt = sp.range_cnt[cur];
+    const uint32_t *mask = sp.chunk_mask[cur];
     uint32_t *rp = sp.rowptr[cur];
-    if (tid == 0) s_tile[0] = atomicAdd(&st.ticket_cmp, 1u);
-    if (!index_only) {
-        uint32_t *cnt_next = sp.range_cnt[cur ^ 1u];
-        const uint32_t n_max = (sp.capacity + 31u) / 32u * 32u / SCANF_RANGE + 2u;
-        for (uint32_t i = blockIdx.x * SCAN_THREADS + tid; i < n_max; i += gridDim.x * SCAN_THREADS) cnt_next[i] = 0u;
-    }
+    PROBE_CTA(0);
+    if (blockIdx.x >= n_ranges) return;   // (no adults at all: M_t stays 0)
     const uint32_t len0 = sp.table_len[0];
-    for (uint32_t i = tid; i < len0; i += SCAN_THREADS) s_tab[i] = sp.tables[i];
-    __syncthreads();
-    for (uint32_t trip = 0;; ++trip) {
-        const uint32_t b = trip & 1u;            // shared scratch alternates, so one barrier less per trip
-        const uint32_t range = s_tile[b];
-        if (range >= n_ranges) break;
+    if (tid < TMAX) s_tab[tid] = sp.tables[tid];
+    for (uint32_t range = blockIdx.x; range < n_ranges; range += gridDim.x) {
         const uint32_t row0 = range * SCANF_RANGE + tid * SCANF_ROWS;
         const uint32_t ch = row0 >> 5;
-        const uint32_t bits = ch < n_chunks ? (sp.chunk_mask[ch] >> (row0 & 31u)) & 0xFFu : 0u;
+        const uint32_t bits = ch < n_slabs ? (mask[ch] >> (row0 & 31u)) & ((1u << SCANF_ROWS) - 1u) : 0u;
         // ---- adults before this range (from the range counts) and before this thread's rows
         uint32_t pre = 0;
-        for (uint32_t k = tid; k < range; k += SCAN_THREADS) pre += cnt[k];
-        const uint32_t c8 = __popc(bits);
-        const uint32_t incl = warp_incl_scan(c8);
+        for (uint32_t k = tid; k < range; k += NT) pre += cnt[k];
+        const uint32_t c4 = __popc(bits);
+        const uint32_t incl = warp_incl_scan(c4);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) pre += __shfl_xor_sync(0xffffffffu, pre, o);
-        if (lane == 31) s_cnt[b][warp] = incl;
-        if (lane == 0) s_pre[b][warp] = pre;
-        if (tid == 0) s_tile[b ^ 1u] = atomicAdd(&st.ticket_cmp, 1u);   // next trip's range
+        __syncthreads();   // the previous range's stage has been written out
+        if (lane == 31) s_cnt[warp] = incl;
+        if (lane == 0) s_pre[warp] = pre;
         __syncthreads();
-        uint32_t i = incl - c8;
+        uint32_t ibase = 0, li0 = incl - c4, n_r = 0;   // adults before the range / before this thread in it / in it
 #pragma unroll
-        for (uint32_t w = 0; w < NW; ++w) i += s_pre[b][w] + (w < warp ? s_cnt[b][w] : 0u);
-        // ---- rowptr and fecundity of this thread's adults
-        uint32_t fsum = 0;
-        unsigned long long fpack = 0ull;
+        for (uint32_t w = 0; w < NW; ++w) { ibase += s_pre[w]; n_r += s_cnt[w]; if (w < warp) li0 += s_cnt[w]; }
+        // ---- rowptr
+        {
+            uint32_t li = li0;
 #pragma unroll
-        for (int k = 0; k < SCANF_ROWS; ++k) {
-            if ((bits >> k) & 1u) {
-                rp[i] = row0 + k;
-                if (!index_only) {
+            for (uint32_t k = 0; k < SCANF_ROWS; ++k)
+                if ((bits >> k) & 1u) s_stage[li++] = row0 + k;
+        }
+        __syncthreads();
+        for (uint32_t k = tid; k < n_r; k += NT) rp[ibase + k] = s_stage[k];
+        PROBE_CTA(5);
+        // ---- fecundity of this thread's adults
+        uint32_t fsum = 0, fpack = 0;
+        {
+            uint32_t i = ibase + li0;
+#pragma unroll
+            for (uint32_t k = 0; k < SCANF_ROWS; ++k) {
+                if ((bits >> k) & 1u) {
                     uint32_t x[4];
-                    draw(sp.key, sp.species, ST_FEC, i, 0, step, x);
+                    draw_rk(sp, ST_FEC, i++, 0, step, x);
                     const uint32_t f = poisson_count(s_tab, len0, x[0]);
-                    fpack |= (unsigned long long)f << (8 * k);
+                    fpack |= f << (8u * k);
                     fsum += f;
                 }
-                ++i;
             }
         }
-        if (index_only) continue;
-        // ---- look-back over the fecundities: offspring before this thread's adults
+        PROBE_CTA(6);
+        // ---- look-back over the fecundities: offspring before this range
         const uint32_t fincl = warp_incl_scan(fsum);
-        if (lane == 31) s_f[b][warp] = fincl;
-        __syncthreads();
+        if (lane == 31) s_f[warp] = fincl;
+        __syncthreads();   // (also: the staged rowptr words have been read)
         uint32_t total = 0, wbase = 0;
 #pragma unroll
-        for (uint32_t w = 0; w < NW; ++w) { const uint32_t v = s_f[b][w]; total += v; if (w < warp) wbase += v; }
+        for (uint32_t w = 0; w < NW; ++w) { const uint32_t v = s_f[w]; total += v; if (w < warp) wbase += v; }
         if (warp == 0) {
             const unsigned long long excl = lookback(sp.status_fec, sp.status_fec_n, range, (unsigned long long)total);
             if (lane == 0) {
-                s_excl[b] = excl;
+                s_excl = excl;
                 if (range == n_ranges - 1) {  // the last range knows M
                     const unsigned long long Mtot = excl + total;
                     if (Mtot > (unsigned long long)sp.capacity) { st.m = sp.capacity; st.flags_step |= 1u; }
@@ -506,14 +546,68 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
                 }
             }
         }
-        __syncthreads();
-        unsigned long long o = s_excl[b] + wbase + (fincl - fsum);
+        // ---- mother[]: staged per range like rowptr (a range with more offspring than the stage holds
+        // -- fecundities far above the table means of any configuration -- writes them directly)
+        const bool staged = total <= SCANF_STAGE;
+        uint32_t lo = wbase + (fincl - fsum);
+        if (staged) {
 #pragma unroll
-        for (int k = 0; k < SCANF_ROWS; ++k) {
-            const uint32_t f = (uint32_t)(fpack >> (8 * k)) & 0xFFu;
-            for (uint32_t cpy = 0; cpy < f; ++cpy, ++o)
-                if (o < (unsigned long long)sp.capacity) sp.mother[o] = row0 + k;
+            for (uint32_t k = 0; k < SCANF_ROWS; ++k) {
+                const uint32_t f = (fpack >> (8u * k)) & 0xFFu;
+                for (uint32_t cpy = 0; cpy < f; ++cpy) s_stage[lo++] = row0 + k;
+            }
         }
+        __syncthreads();
+        PROBE_CTA(7);
+        const unsigned long long obase = s_excl;
+        if (staged) {
+            for (uint32_t k = tid; k < total; k += NT)
+                if (obase + k < (unsigned long long)sp.capacity) sp.mother[obase + k] = s_stage[k];
+        } else {
+            unsigned long long o = obase + lo;
+#pragma unroll
+            for (uint32_t k = 0; k < SCANF_ROWS; ++k) {
+                const uint32_t f = (fpack >> (8u * k)) & 0xFFu;
+                for (uint32_t cpy = 0; cpy < f; ++cpy, ++o)
+                    if (o < (unsigned long long)sp.capacity) sp.mother[o] = row0 + k;
+            }
+        }
+    }
+    PROBE_CTA(1);
+}
+
+// rowptr[] of the current buffer alone (spegg_read_state): the index half of k_scan_fused.
+__global__ void __launch_bounds__(SCAN_THREADS) k_rowptr_fused(const __grid_constant__ SpK sp) {
+    constexpr uint32_t NW = SCAN_THREADS / 32;
+    __shared__ uint32_t s_cnt[NW], s_pre[NW];
+    const DevSpecies &st = *sp.st;
+    const uint32_t mp = st.m_phys, cur = st.cur;
+    const uint32_t n_ranges = (mp + SCANF_RANGE - 1) / SCANF_RANGE;
+    const uint32_t n_slabs = (mp + FUSED_CHUNK - 1) / FUSED_CHUNK;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t *cnt = sp.range_cnt[cur];
+    const uint32_t *mask = sp.chunk_mask[cur];
+    uint32_t *rp = sp.rowptr[cur];
+    for (uint32_t range = blockIdx.x; range < n_ranges; range += gridDim.x) {
+        const uint32_t row0 = range * SCANF_RANGE + tid * SCANF_ROWS;
+        const uint32_t ch = row0 >> 5;
+        const uint32_t bits = ch < n_slabs ? (mask[ch] >> (row0 & 31u)) & ((1u << SCANF_ROWS) - 1u) : 0u;
+        uint32_t pre = 0;
+        for (uint32_t k = tid; k < range; k += SCAN_THREADS) pre += cnt[k];
+        const uint32_t c = __popc(bits);
+        const uint32_t incl = warp_incl_scan(c);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) pre += __shfl_xor_sync(0xffffffffu, pre, o);
+        __syncthreads();
+        if (lane == 31) s_cnt[warp] = incl;
+        if (lane == 0) s_pre[warp] = pre;
+        __syncthreads();
+        uint32_t i = incl - c;
+#pragma unroll
+        for (uint32_t w = 0; w < NW; ++w) i += s_pre[w] + (w < warp ? s_cnt[w] : 0u);
+#pragma unroll
+        for (uint32_t k = 0; k < SCANF_ROWS; ++k)
+            if ((bits >> k) & 1u) rp[i++] = row0 + k;
     }
 }
 
@@ -542,9 +636,30 @@ inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) 
     k_fused_bit_f<4, 8><<<n_sms * FUSEDF_CTAS, FUSEDF_WARPS * 32, FUSEDF_SMEM, stream>>>(k);
 }
 
-// one range per CTA in a single wave at the bench sizes (capacity / 2,048 = 576 ranges <= 4 per SM)
-inline void launch_scan_fused(const SpK &k, uint32_t n_sms, cudaStream_t stream, int index_only) {
-    k_scan_fused<<<n_sms * 4, SCAN_THREADS, 0, stream>>>(k, index_only);
+// Cooperative launch: the whole grid is resident at once (or the launch fails), which the fixed
+// range -> CTA assignment of the look-back relies on.  ctas_per_sm comes from the occupancy query.
+inline cudaError_t launch_scan_fused(const SpK &k, uint32_t n_sms, uint32_t ctas_per_sm, cudaStream_t stream) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(n_sms * ctas_per_sm);
+    cfg.blockDim = dim3(SCAN_THREADS);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_scan_fused, k);
+}
+
+inline int scan_fused_ctas_per_sm() {
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_scan_fused, SCAN_THREADS, 0) != cudaSuccess) return 0;
+    return n;
+}
+
+inline void launch_rowptr_fused(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
+    k_rowptr_fused<<<n_sms * 4, SCAN_THREADS, 0, stream>>>(k);
 }
 
 }  // namespace spegg

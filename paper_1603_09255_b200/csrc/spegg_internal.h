@@ -13,6 +13,7 @@ constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 4;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 constexpr int MAX_SPECIES = 8;
+constexpr uint32_t FUSED_RANGE = 1024;            // fused path: rows per scan range (32 slabs of 32 rows)
 
 // Device-resident per-species state: counts never leave the GPU between steps.
 struct DevSpecies {
@@ -22,7 +23,7 @@ struct DevSpecies {
     uint32_t m;            // offspring of the current step (after capacity truncation)
     uint32_t n_next;       // survivors of the current step
     uint32_t flags_step;   // flags raised during the current step
-    uint32_t ticket_fec, ticket_cmp, ticket_fused, done_fused;
+    uint32_t ticket_fec, done_fused;
     uint32_t log_pos;      // entries written to the log ring
     uint32_t m_phys;       // fused path: physical rows of the current buffer (32-row slabs + chunk_mask)
     long long sum_zi;      // over the current adults (survivors of the last step)
@@ -31,6 +32,11 @@ struct DevSpecies {
     unsigned long long captures, near_ties;
     float theta_t, zbar_pred, attack_n;
     uint32_t n_pred0;      // predator count snapshot used by this step
+    // work tickets of the step kernels, each on a cache line of its own: hundreds of CTAs draw from
+    // them at the same moment, and same-line atomics are served one after the other by L2
+    alignas(128) uint32_t ticket_cmp;
+    alignas(128) uint32_t ticket_fused;
+    alignas(128) uint32_t ticket_pad;
 };
 
 struct DevGlobal {
@@ -76,7 +82,7 @@ struct SpK {
     uint8_t *pop[2];
     uint32_t *patch_start[2];   // [P+1] each
     uint32_t *rowptr[2];        // logical adult index -> physical row of pop[]
-    uint32_t *chunk_mask;       // fused path: survivor bitmask of each 32-offspring chunk
+    uint32_t *chunk_mask[2];    // fused path: survivor bitmask of each 32-row slab of pop[0] / pop[1]
     uint32_t *range_cnt[2];     // fused path: adults per 2,048-row range of pop[0] / pop[1]
     uint32_t phys_parents;      // 1: mother[] / father[] hold physical rows (fused path)
     uint32_t solo;              // 1: single-species simulation (k_index finishes and prepares the step)

@@ -126,6 +126,11 @@ __device__ __forceinline__ void prepare_species(const SpK &sp, uint32_t g, uint3
     for (uint32_t i = g; i < nc; i += stride) sp.status_cmp[i] = 0ull;
     if (sp.fec_model == 2)
         for (uint32_t i = g; i < sp.capacity; i += stride) sp.cap[i] = 0u;
+    if (sp.phys_parents) {  // fused path: the coming step counts its survivors per range of the other buffer
+        uint32_t *cnt_next = sp.range_cnt[cur ^ 1u];
+        const uint32_t n_max = (sp.capacity + 31u) / 32u * 32u / FUSED_RANGE + 2u;
+        for (uint32_t i = g; i < n_max; i += stride) cnt_next[i] = 0u;
+    }
     const uint32_t *ps = sp.patch_start[cur];
     for (uint32_t tab = g; tab < sp.n_tables; tab += stride) {
         double lam;
@@ -180,15 +185,16 @@ __device__ __forceinline__ void solo_tail(const SpK &sp, uint32_t *s_flag) {
     __syncthreads();
     if (!*s_flag) return;
     __threadfence();
+    // every thread reads what the next step's preparation needs straight from L2, in one round trip,
+    // while thread 0 closes the step: nothing below waits for a value another thread wrote
+    DevSpecies &st = *sp.st;
+    const uint32_t nn = ld_u32(&st.n_next), cur1 = ld_u32(&st.cur) ^ 1u, step1 = ld_u32(&sp.glob->step) + 1u;
+    const long long a1 = (long long)ld_u64(&st.acc_zi);
     if (threadIdx.x == 0) {
         finish_species(sp);
-        sp.glob->step = ld_u32(&sp.glob->step) + 1;
-        __threadfence();
+        sp.glob->step = step1;
     }
-    __syncthreads();
-    DevSpecies &st = *sp.st;
-    prepare_species(sp, threadIdx.x, blockDim.x, ld_u32(&st.n), ld_u32(&st.cur), (long long)ld_u64(&st.sum_zi),
-                    ld_u32(&sp.glob->step));
+    prepare_species(sp, threadIdx.x, blockDim.x, nn, cur1, a1, step1);
 }
 
 // a1-a3: fecundity (one FEC block per adult), exclusive scan by decoupled look-back, mother fill.
