@@ -295,12 +295,16 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
             k_scalar<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
+            // production q10 path: vectorised gamete kernel that also takes the phenotype (debug keeps
+            // the plain kernels, so the two can be compared with each other and with the oracle)
+            const bool q10v = !s->debug && gamete_q10v_supported(k);
             if (k.kind == 0) k_gamete_bit<<<G * 8, 256, 0, s->stream>>>(k);
+            else if (q10v) k_gamete_q10v<<<G * 8, 256, 0, s->stream>>>(k);
             else k_gamete_q10<<<G * 8, 256, 0, s->stream>>>(k);
             ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
-            k_mutate<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
-            k_phenotype<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+            k_mutate<<<G * 8, 256, 0, s->stream>>>(k, q10v ? 1 : 0); ++nl;
+            if (!q10v) { k_phenotype<<<G * 8, 256, 0, s->stream>>>(k); ++nl; }
             k_survival<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
             if (s->P == 1) {
                 k_cmp_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;

@@ -57,26 +57,6 @@ constexpr uint32_t FUSED_ROW = 256;             // bytes per row (config 3)
 constexpr int SCANF_RANGE = FUSED_RANGE;         // rows per scan range (1,024 = 32 chunks)
 constexpr int SCANF_CHUNKS = SCANF_RANGE / FUSED_CHUNK;
 
-// Philox4x32-10 (R3) with the ten round keys taken from the kernel parameter block: the key
-// schedule k_r = k_0 + r * Weyl is the same for every draw of a simulation, so the host computes it
-// once (SpK::rk) and the XORs read it straight from the constant bank -- four instructions a round.
-__device__ __forceinline__ void draw_rk(const SpK &sp, uint32_t stream, uint32_t entity, uint32_t block,
-                                        uint32_t step, uint32_t (&o)[4]) {
-    uint32_t c0 = entity, c1 = block, c2 = step, c3 = (sp.species << 8) | stream;
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
-        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
-        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ sp.rk[2 * r];
-        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ sp.rk[2 * r + 1];
-        c1 = (uint32_t)p1;
-        c3 = (uint32_t)p0;
-        c0 = n0;
-        c2 = n2;
-    }
-    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
-}
-
 // ---------------------------------------------------------------------------------------------
 // The fused kernel.  A warp takes chunks of 32 consecutive offspring from an atomic ticket and runs
 // a software pipeline over them:

@@ -39,6 +39,26 @@ __device__ __forceinline__ uint32_t neighbour(uint32_t p, uint32_t dir, uint32_t
     return py * gw + px;
 }
 
+// Philox4x32-10 (R3) with the ten round keys taken from the kernel parameter block: the key
+// schedule k_r = k_0 + r * Weyl is the same for every draw of a simulation, so the host computes it
+// once (SpK::rk) and the XORs read it straight from the constant bank -- four instructions a round.
+__device__ __forceinline__ void draw_rk(const SpK &sp, uint32_t stream, uint32_t entity, uint32_t block,
+                                        uint32_t step, uint32_t (&o)[4]) {
+    uint32_t c0 = entity, c1 = block, c2 = step, c3 = (sp.species << 8) | stream;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ sp.rk[2 * r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ sp.rk[2 * r + 1];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    o[0] = c0; o[1] = c1; o[2] = c2; o[3] = c3;
+}
+
 // R13/R14: fecundity mean, fp64 with the stated op order
 __device__ __forceinline__ double fecundity_mean(const SpK &sp, double n, double K, uint32_t cap_index) {
     if (sp.fec_model == 0) {  // Beverton-Holt
@@ -422,8 +442,83 @@ __global__ void __launch_bounds__(256) k_gamete_q10(const __grid_constant__ SpK 
     }
 }
 
+// a4 + a5 (q10 genomes, R7 + R10) for L = 8 ... 256 a power of two: a lane owns 8 consecutive loci of
+// one gamete (two RECOMB blocks, one 128-bit load from each parental haplotype, one 128-bit store),
+// GS = L / 8 lanes make a gamete, and a warp works on whole offspring: both gametes side by side
+// (L <= 128; several offspring per warp when L <= 64) or one after the other (L = 256).  The phase
+// is the XOR prefix of the switch bits: within the lane in registers, across the lanes of the gamete
+// by a ballot.  The lane's share of the additive phenotype (sum of the 8 alleles it selected) is
+// reduced over the offspring's lanes, so the offspring row is never read again for a5.
+__host__ __device__ inline bool gamete_q10v_supported(const SpK &k) {
+    return k.kind == 1 && k.L >= 8 && k.L <= 256 && (k.L & (k.L - 1)) == 0;
+}
+
+__global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK sp) {
+    const DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, step = sp.glob->step, L = sp.L;
+    const uint32_t GS = L >> 3;                         // lanes per gamete
+    const uint32_t LPO = min(32u, 2u * GS);             // lanes per offspring in one pass
+    const uint32_t npass = (2u * GS) / LPO;             // 2 when L = 256, else 1
+    const uint32_t opw = 32u / LPO;                     // offspring per warp iteration
+    const uint32_t lane = threadIdx.x & 31u, li = lane % LPO, osub = lane / LPO;
+    const uint32_t lt = (1u << lane) - 1u;
+    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    const uint8_t *pop = sp.pop[st.cur];
+    const uint32_t *rowptr = sp.rowptr[st.cur];
+    const uint4 *Tr = (const uint4 *)sp.T_recomb;
+    for (unsigned long long ob = (unsigned long long)gw * opw; ob < M; ob += (unsigned long long)n_warps * opw) {
+        const uint32_t j = (uint32_t)ob + osub;
+        const bool live = j < M;
+        uint32_t par0 = 0u, par1 = 0u;
+        if (live) { par0 = rowptr[sp.mother[j]]; par1 = rowptr[sp.father[j]]; }
+        int acc = 0;
+        for (uint32_t p = 0; p < npass; ++p) {
+            const uint32_t t = p * LPO + li, g = t / GS, slot = t % GS;
+            const uint4 *h0 = (const uint4 *)(pop + (size_t)(g ? par1 : par0) * sp.row_bytes) + slot;
+            uint4 a = make_uint4(0, 0, 0, 0), b = a;
+            if (live) { a = h0[0]; b = h0[GS]; }
+            // R7: switch bits of this lane's 8 loci and their running parity
+            uint32_t x[4], y[4];
+            const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
+            draw_rk(sp, stream, j, 2u * slot, step, x);
+            draw_rk(sp, stream, j, 2u * slot + 1u, step, y);
+            const uint4 t0 = Tr[2u * slot], t1 = Tr[2u * slot + 1u];
+            uint32_t run = 0, ph = 0;   // ph bit k = parity of the switch bits of loci 0..k of the lane
+            run ^= x[0] < t0.x ? 1u : 0u; ph |= run;
+            run ^= x[1] < t0.y ? 1u : 0u; ph |= run << 1;
+            run ^= x[2] < t0.z ? 1u : 0u; ph |= run << 2;
+            run ^= x[3] < t0.w ? 1u : 0u; ph |= run << 3;
+            run ^= y[0] < t1.x ? 1u : 0u; ph |= run << 4;
+            run ^= y[1] < t1.y ? 1u : 0u; ph |= run << 5;
+            run ^= y[2] < t1.z ? 1u : 0u; ph |= run << 6;
+            run ^= y[3] < t1.w ? 1u : 0u; ph |= run << 7;
+            const uint32_t bal = __ballot_sync(0xffffffffu, run != 0);
+            const uint32_t gmask = (GS == 32u ? 0xFFFFFFFFu : ((1u << GS) - 1u)) << (lane - slot);
+            if (__popc(bal & gmask & lt) & 1u) ph ^= 0xFFu;
+            // select: allele from hap1 where the phase bit is set
+            uint4 o;
+            {
+                const uint32_t m0 = ((ph & 1u) ? 0x0000FFFFu : 0u) | ((ph & 2u) ? 0xFFFF0000u : 0u);
+                const uint32_t m1 = ((ph & 4u) ? 0x0000FFFFu : 0u) | ((ph & 8u) ? 0xFFFF0000u : 0u);
+                const uint32_t m2 = ((ph & 16u) ? 0x0000FFFFu : 0u) | ((ph & 32u) ? 0xFFFF0000u : 0u);
+                const uint32_t m3 = ((ph & 64u) ? 0x0000FFFFu : 0u) | ((ph & 128u) ? 0xFFFF0000u : 0u);
+                o.x = (a.x & ~m0) | (b.x & m0); o.y = (a.y & ~m1) | (b.y & m1);
+                o.z = (a.z & ~m2) | (b.z & m2); o.w = (a.w & ~m3) | (b.w & m3);
+            }
+            if (live) {
+                ((uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes))[g * GS + slot] = o;
+                // R10: both int16 halves of a word summed by one dp2a
+                acc = __dp2a_lo((int)o.x, 0x0101, acc); acc = __dp2a_lo((int)o.y, 0x0101, acc);
+                acc = __dp2a_lo((int)o.z, 0x0101, acc); acc = __dp2a_lo((int)o.w, 0x0101, acc);
+            }
+        }
+        for (uint32_t off = LPO >> 1; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+        if (live && li == 0) sp.zi[j] = acc;
+    }
+}
+
 // a4: sparse mutation (R9), one thread per (offspring, gamete), applied after recombination
-__global__ void __launch_bounds__(256) k_mutate(const __grid_constant__ SpK sp) {
+__global__ void __launch_bounds__(256) k_mutate(const __grid_constant__ SpK sp, int zi_delta) {
     const DevSpecies &st = *sp.st;
     const uint32_t M = st.m, step = sp.glob->step, L = sp.L;
     const unsigned long long total = 2ull * M;
@@ -442,9 +537,11 @@ __global__ void __launch_bounds__(256) k_mutate(const __grid_constant__ SpK sp) 
                 row[pos >> 5] ^= 1u << (pos & 31u);
             } else {
                 int16_t *row = (int16_t *)sp.offbuf + (size_t)j * 2 * L + (size_t)g * L;
-                int v = (int)row[pos] + normal_delta(sp.T_norm, sp.R_norm, x[2]);
+                const int v0 = (int)row[pos];
+                int v = v0 + normal_delta(sp.T_norm, sp.R_norm, x[2]);
                 v = max(-32767, min(32767, v));
                 row[pos] = (int16_t)v;
+                if (zi_delta && v != v0) atomicAdd(&sp.zi[j], v - v0);   // a5 was taken before the mutation
             }
         }
     }
