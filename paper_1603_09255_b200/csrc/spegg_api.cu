@@ -484,6 +484,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.debug = p->debug;
         k.phys_parents = fused_ok(s, h) ? 1u : 0u;
         k.solo = (k.phys_parents && p->n_species == 1) ? 1u : 0u;
+        k.index_only = (!s->debug && !k.phys_parents && gamete_q10v_supported(k)) ? 1u : 0u;
     }
     for (uint32_t si = 0; si < p->n_species; ++si)
         if (s->sp[si].k.phys_parents && fused_bit_configure() != cudaSuccess) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }

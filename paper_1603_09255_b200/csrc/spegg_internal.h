@@ -85,7 +85,8 @@ struct SpK {
     uint32_t *chunk_mask[2];    // fused path: survivor bitmask of each 32-row slab of pop[0] / pop[1]
     uint32_t *range_cnt[2];     // fused path: adults per 2,048-row range of pop[0] / pop[1]
     uint32_t phys_parents;      // 1: mother[] / father[] hold physical rows (fused path)
-    uint32_t solo;              // 1: single-species simulation (k_index finishes and prepares the step)
+    uint32_t solo;              // 1: single-species simulation (the gamete kernel's last CTA closes and prepares the step)
+    uint32_t index_only;        // 1: offspring rows are written once, at row j of the other buffer; compaction writes rowptr[] only
     uint8_t *f;
     uint32_t *off, *mother, *father, *dest, *pos;
     float *u01, *s;

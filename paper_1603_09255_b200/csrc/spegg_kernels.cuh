@@ -99,6 +99,12 @@ __device__ __forceinline__ float survival_prob(const SpK &sp, float z, float the
     return s;
 }
 
+// where the offspring rows of the current step live: row j of the other population buffer when the
+// compaction is index-only (they are never moved again), else the staging buffer
+__device__ __forceinline__ uint8_t *offspring_rows(const SpK &sp) {
+    return sp.index_only ? sp.pop[sp.st->cur ^ 1u] : sp.offbuf;
+}
+
 // ------------------------------------------------------------------------ step bookkeeping
 __device__ __forceinline__ uint32_t ld_u32(const uint32_t *p) {
     uint32_t v;
@@ -466,17 +472,31 @@ __global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK
     const uint8_t *pop = sp.pop[st.cur];
     const uint32_t *rowptr = sp.rowptr[st.cur];
     const uint4 *Tr = (const uint4 *)sp.T_recomb;
-    for (unsigned long long ob = (unsigned long long)gw * opw; ob < M; ob += (unsigned long long)n_warps * opw) {
+    uint8_t *out = offspring_rows(sp);
+    // the parents' rows of the NEXT iteration are looked up (mother[] / father[] -> rowptr[]) while this
+    // one computes, so the two dependent index loads are never waited for
+    auto parents = [&](unsigned long long ob_, uint32_t &p0, uint32_t &p1) {
+        const unsigned long long j_ = ob_ + osub;
+        p0 = 0u; p1 = 0u;
+        if (j_ < M) { p0 = rowptr[sp.mother[j_]]; p1 = rowptr[sp.father[j_]]; }
+    };
+    const unsigned long long stride = (unsigned long long)n_warps * opw;
+    uint32_t par0, par1;
+    parents((unsigned long long)gw * opw, par0, par1);
+    for (unsigned long long ob = (unsigned long long)gw * opw; ob < M; ob += stride) {
         const uint32_t j = (uint32_t)ob + osub;
         const bool live = j < M;
-        uint32_t par0 = 0u, par1 = 0u;
-        if (live) { par0 = rowptr[sp.mother[j]]; par1 = rowptr[sp.father[j]]; }
+        uint32_t nx0, nx1;
+        parents(ob + stride, nx0, nx1);
         int acc = 0;
         for (uint32_t p = 0; p < npass; ++p) {
             const uint32_t t = p * LPO + li, g = t / GS, slot = t % GS;
             const uint4 *h0 = (const uint4 *)(pop + (size_t)(g ? par1 : par0) * sp.row_bytes) + slot;
-            uint4 a = make_uint4(0, 0, 0, 0), b = a;
-            if (live) { a = h0[0]; b = h0[GS]; }
+            // (volatile asm: the loads are issued HERE, ahead of the draws, not sunk to their first use;
+            // a dead lane reads row 0)
+            uint4 a, b;
+            asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w) : "l"(h0));
+            asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(h0 + GS));
             // R7: switch bits of this lane's 8 loci and their running parity
             uint32_t x[4], y[4];
             const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
@@ -506,14 +526,19 @@ __global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK
                 o.z = (a.z & ~m2) | (b.z & m2); o.w = (a.w & ~m3) | (b.w & m3);
             }
             if (live) {
-                ((uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes))[g * GS + slot] = o;
+                ((uint4 *)(out + (size_t)j * sp.row_bytes))[g * GS + slot] = o;
                 // R10: both int16 halves of a word summed by one dp2a
                 acc = __dp2a_lo((int)o.x, 0x0101, acc); acc = __dp2a_lo((int)o.y, 0x0101, acc);
                 acc = __dp2a_lo((int)o.z, 0x0101, acc); acc = __dp2a_lo((int)o.w, 0x0101, acc);
             }
         }
-        for (uint32_t off = LPO >> 1; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+#pragma unroll
+        for (uint32_t off = 16; off > 0; off >>= 1) {
+            const int v = __shfl_xor_sync(0xffffffffu, acc, off);
+            if (off < LPO) acc += v;
+        }
         if (live && li == 0) sp.zi[j] = acc;
+        par0 = nx0; par1 = nx1;
     }
 }
 
@@ -533,10 +558,10 @@ __global__ void __launch_bounds__(256) k_mutate(const __grid_constant__ SpK sp, 
             if (k > 0) draw(sp.key, sp.species, stream, j, k, step, x);
             const uint32_t pos = uniform_index(x[1], L);
             if (sp.kind == 0) {
-                uint32_t *row = (uint32_t *)sp.offbuf + (size_t)j * 2 * sp.W + (size_t)g * sp.W;
+                uint32_t *row = (uint32_t *)offspring_rows(sp) + (size_t)j * 2 * sp.W + (size_t)g * sp.W;
                 row[pos >> 5] ^= 1u << (pos & 31u);
             } else {
-                int16_t *row = (int16_t *)sp.offbuf + (size_t)j * 2 * L + (size_t)g * L;
+                int16_t *row = (int16_t *)offspring_rows(sp) + (size_t)j * 2 * L + (size_t)g * L;
                 const int v0 = (int)row[pos];
                 int v = v0 + normal_delta(sp.T_norm, sp.R_norm, x[2]);
                 v = max(-32767, min(32767, v));
@@ -571,7 +596,7 @@ __global__ void __launch_bounds__(256) k_phenotype(const __grid_constant__ SpK s
     const uint32_t M = sp.st->m;
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     for (uint32_t j = warp0; j < M; j += nw) {
-        const int32_t zi = warp_row_zi(sp, sp.offbuf + (size_t)j * sp.row_bytes);
+        const int32_t zi = warp_row_zi(sp, offspring_rows(sp) + (size_t)j * sp.row_bytes);
         if ((threadIdx.x & 31u) == 0) sp.zi[j] = zi;
     }
 }
@@ -695,6 +720,13 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     uint8_t *dst = sp.pop[st.cur ^ 1u];
     uint32_t *rp = sp.rowptr[st.cur ^ 1u];
+    if (sp.index_only) {   // the rows stay where the gamete kernel stored them: only the index is written
+        for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
+            const uint32_t p = sp.pos[j];
+            if (p != 0xFFFFFFFFu) rp[p] = j;
+        }
+        return;
+    }
     for (uint32_t j = warp0; j < M; j += nw) {
         const uint32_t p = sp.pos[j];
         if (p == 0xFFFFFFFFu) continue;
