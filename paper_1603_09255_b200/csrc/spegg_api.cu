@@ -292,31 +292,38 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             launch_fused_bit(k, G, s->stream); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
         } else {
-            k_fec_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
-            k_scalar<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+            // grids are fixed at capture time: sized for the capacity (a thousand idle CTAs cost a small
+            // population more than its work), capped at a few CTAs per SM; the kernels loop over the counts
+            const uint64_t cap = k.capacity;
+            auto ctas = [&](uint64_t items, uint64_t per_cta, uint32_t per_sm) {
+                return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>((items + per_cta - 1) / per_cta, (uint64_t)G * per_sm));
+            };
+            const uint32_t g_thread = ctas(cap, 256, 8), g_warp = ctas(cap, 8, 8);   // thread / warp per offspring
+            k_fec_scan<<<ctas(cap, SCAN_THREADS, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
+            k_scalar<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             // production q10 path: vectorised gamete kernel that also takes the phenotype (debug keeps
             // the plain kernels, so the two can be compared with each other and with the oracle)
             const bool q10v = !s->debug && gamete_q10v_supported(k);
-            if (k.kind == 0) k_gamete_bit<<<G * 8, 256, 0, s->stream>>>(k);
-            else if (q10v) k_gamete_q10v<<<G * 8, 256, 0, s->stream>>>(k);
-            else k_gamete_q10<<<G * 8, 256, 0, s->stream>>>(k);
+            if (k.kind == 0) k_gamete_bit<<<ctas(cap * 2 * k.n_chrom, 256, 8), 256, 0, s->stream>>>(k);
+            else if (q10v) k_gamete_q10v<<<g_warp, 256, 0, s->stream>>>(k);
+            else k_gamete_q10<<<ctas(cap * 2, 8, 8), 256, 0, s->stream>>>(k);
             ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
-            k_mutate<<<G * 8, 256, 0, s->stream>>>(k, q10v ? 1 : 0); ++nl;
-            if (!q10v) { k_phenotype<<<G * 8, 256, 0, s->stream>>>(k); ++nl; }
-            k_survival<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+            k_mutate<<<ctas(cap * 2, 256, 8), 256, 0, s->stream>>>(k, q10v ? 1 : 0); ++nl;
+            if (!q10v) { k_phenotype<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }
+            k_survival<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
             if (s->P == 1) {
-                k_cmp_scan<<<G * 4, SCAN_THREADS, 0, s->stream>>>(k); ++nl;
+                k_cmp_scan<<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
             } else {
                 k_patch_count<<<std::min(s->P, G * 8), 256, 0, s->stream>>>(k); ++nl;
                 k_patch_base<<<1, 1024, 0, s->stream>>>(k); ++nl;
                 k_patch_pos<<<std::min(s->P, G * 8), 256, 0, s->stream>>>(k); ++nl;
             }
-            k_cmp_scatter<<<G * 8, 256, 0, s->stream>>>(k); ++nl;
+            k_cmp_scatter<<<k.index_only ? g_thread : g_warp, 256, 0, s->stream>>>(k); ++nl;
         }
     }
-    const bool solo = s->sp.size() == 1 && s->sp[0].k.solo;  // k_index closes the step itself
+    const bool solo = s->sp.size() == 1 && s->sp[0].k.solo;  // the last kernel closes the step itself
     if (!solo) {
         k_finish_all<<<1, 32, 0, s->stream>>>(s->d_spk, s->p.n_species); ++nl;
         if (!s->debug) { launch_prepare(s); ++nl; }  // debug: prepared at the start, so the view stays valid
@@ -483,7 +490,9 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.log = at<LogEntry>(s, l.log); k.log_capacity = s->log_capacity;
         k.debug = p->debug;
         k.phys_parents = fused_ok(s, h) ? 1u : 0u;
-        k.solo = (k.phys_parents && p->n_species == 1) ? 1u : 0u;
+        // single unstructured species, production kernels: the step's last kernel closes it and prepares
+        // the next one itself (one Poisson table; per-patch tables are a grid's work, not a CTA's)
+        k.solo = (!s->debug && p->n_species == 1 && s->P == 1) ? 1u : 0u;
         k.index_only = (!s->debug && !k.phys_parents && gamete_q10v_supported(k)) ? 1u : 0u;
     }
     for (uint32_t si = 0; si < p->n_species; ++si)

@@ -466,7 +466,8 @@ __global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK
     const uint32_t LPO = min(32u, 2u * GS);             // lanes per offspring in one pass
     const uint32_t npass = (2u * GS) / LPO;             // 2 when L = 256, else 1
     const uint32_t opw = 32u / LPO;                     // offspring per warp iteration
-    const uint32_t lane = threadIdx.x & 31u, li = lane % LPO, osub = lane / LPO;
+    const uint32_t gs_log = (uint32_t)__ffs((int)GS) - 1u, lpo_log = (uint32_t)__ffs((int)LPO) - 1u;   // both powers of two
+    const uint32_t lane = threadIdx.x & 31u, li = lane & (LPO - 1u), osub = lane >> lpo_log;
     const uint32_t lt = (1u << lane) - 1u;
     const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
     const uint8_t *pop = sp.pop[st.cur];
@@ -490,7 +491,7 @@ __global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK
         parents(ob + stride, nx0, nx1);
         int acc = 0;
         for (uint32_t p = 0; p < npass; ++p) {
-            const uint32_t t = p * LPO + li, g = t / GS, slot = t % GS;
+            const uint32_t t = p * LPO + li, g = t >> gs_log, slot = t & (GS - 1u);
             const uint4 *h0 = (const uint4 *)(pop + (size_t)(g ? par1 : par0) * sp.row_bytes) + slot;
             // (volatile asm: the loads are issued HERE, ahead of the draws, not sunk to their first use;
             // a dead lane reads row 0)
@@ -518,10 +519,10 @@ __global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK
             // select: allele from hap1 where the phase bit is set
             uint4 o;
             {
-                const uint32_t m0 = ((ph & 1u) ? 0x0000FFFFu : 0u) | ((ph & 2u) ? 0xFFFF0000u : 0u);
-                const uint32_t m1 = ((ph & 4u) ? 0x0000FFFFu : 0u) | ((ph & 8u) ? 0xFFFF0000u : 0u);
-                const uint32_t m2 = ((ph & 16u) ? 0x0000FFFFu : 0u) | ((ph & 32u) ? 0xFFFF0000u : 0u);
-                const uint32_t m3 = ((ph & 64u) ? 0x0000FFFFu : 0u) | ((ph & 128u) ? 0xFFFF0000u : 0u);
+                // phase bit 2w -> low half, 2w+1 -> high half of word w: (b0 | b1 << 16) * 0xFFFF
+                const uint32_t sp2 = ph | (ph << 15);
+                const uint32_t m0 = (sp2 & 0x00010001u) * 0xFFFFu, m1 = ((sp2 >> 2) & 0x00010001u) * 0xFFFFu;
+                const uint32_t m2 = ((sp2 >> 4) & 0x00010001u) * 0xFFFFu, m3 = ((sp2 >> 6) & 0x00010001u) * 0xFFFFu;
                 o.x = (a.x & ~m0) | (b.x & m0); o.y = (a.y & ~m1) | (b.y & m1);
                 o.z = (a.z & ~m2) | (b.z & m2); o.w = (a.w & ~m3) | (b.w & m3);
             }
@@ -720,21 +721,23 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     uint8_t *dst = sp.pop[st.cur ^ 1u];
     uint32_t *rp = sp.rowptr[st.cur ^ 1u];
+    __shared__ uint32_t s_flag;
     if (sp.index_only) {   // the rows stay where the gamete kernel stored them: only the index is written
         for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
             const uint32_t p = sp.pos[j];
             if (p != 0xFFFFFFFFu) rp[p] = j;
         }
-        return;
+    } else {
+        for (uint32_t j = warp0; j < M; j += nw) {
+            const uint32_t p = sp.pos[j];
+            if (p == 0xFFFFFFFFu) continue;
+            if (lane == 0) rp[p] = p;  // materialised path: rows are dense, rowptr is the identity
+            const uint4 *src = (const uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes);
+            uint4 *d = (uint4 *)(dst + (size_t)p * sp.row_bytes);
+            for (uint32_t i = lane; i < sp.row_u4; i += 32) d[i] = src[i];
+        }
     }
-    for (uint32_t j = warp0; j < M; j += nw) {
-        const uint32_t p = sp.pos[j];
-        if (p == 0xFFFFFFFFu) continue;
-        if (lane == 0) rp[p] = p;  // materialised path: rows are dense, rowptr is the identity
-        const uint4 *src = (const uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes);
-        uint4 *d = (uint4 *)(dst + (size_t)p * sp.row_bytes);
-        for (uint32_t i = lane; i < sp.row_u4; i += 32) d[i] = src[i];
-    }
+    if (sp.solo) solo_tail(sp, &s_flag);   // single unstructured species: the last CTA closes the step
 }
 
 // ---- a7 (patches, R15): the next generation is ordered by (destination patch, j).  Offspring of

@@ -152,3 +152,34 @@ def test_full_size_bench_configuration(oracle_mod, binding, which, steps):
     parity.assert_state_equal(sim, orc, cfg, tag="C%d full size" % which)
     assert sim.status() == orc.flags
     sim.close()
+
+
+def _q10_variant(n_loci, chrom_len, r_within, mu, n0=3000):
+    """C1 with another genetic architecture: exercises the lane layouts of the vectorised q10
+    gamete kernel (L / 8 lanes per gamete) and, with a high mutation rate, the phenotype
+    correction applied by the mutation kernel."""
+    cfg = workloads.config(1, scale=n0 / 1000.0)
+    sp = cfg["species"][0]
+    sp.update(n_loci=n_loci, chrom_len=list(chrom_len), r=workloads._interval_r(list(chrom_len), r_within), mu=mu)
+    return cfg
+
+
+@pytest.mark.parametrize("n_loci,chrom_len,r,mu", [
+    (8, [8], 0.5, 0.02),              # one lane per gamete pair of blocks: 16 offspring per warp
+    (32, [16, 16], 0.1, 0.05),        # 4 lanes per gamete, many mutations per step
+    (256, [256], 0.02, 1e-3),         # 32 lanes per gamete: the two gametes in successive passes
+    (128, [100, 28], 0.3, 1e-2),      # chromosome boundary inside a lane's 8 loci
+    (24, [24], 0.25, 1e-2),           # not a power of two: the plain kernels
+])
+def test_q10_lane_layouts_free_running(oracle_mod, binding, n_loci, chrom_len, r, mu):
+    cfg = _q10_variant(n_loci, chrom_len, r, mu)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(3):            # compare along the way too, so that a first divergence is localised
+        orc.step(5)
+        sim.step(5)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+        parity.assert_state_equal(sim, orc, cfg)
+    sim.close()
