@@ -289,7 +289,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
         if (fused_ok(s, h)) {
             CU(launch_scan_fused(k, G, s->scan_ctas, s->stream)); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
-            launch_fused_bit(k, G, s->stream); ++nl;
+            CU(launch_fused_bit(k, G, s->stream)); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
         } else {
             // grids are fixed at capture time: sized for the capacity (a thousand idle CTAs cost a small

@@ -52,6 +52,14 @@ __device__ __forceinline__ uint32_t mask_from(int s, int w) {
     return shl_clamp(0xFFFFFFFFu, (uint32_t)__viaddmax_s32(s, -32 * w, 0));
 }
 
+// Programmatic dependent launch: the two kernels of a step are launched with programmatic stream
+// serialization, so the next kernel's CTAs are scheduled while the previous grid drains and wait
+// here (before their first global access) until it has completed and its writes are visible.
+__device__ __forceinline__ void pdl_prologue() {
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 constexpr int FUSED_CHUNK = 32;                 // offspring per warp iteration = rows per slab
 constexpr uint32_t FUSED_ROW = 256;             // bytes per row (config 3)
 constexpr int SCANF_RANGE = FUSED_RANGE;         // rows per scan range (1,024 = 32 chunks)
@@ -138,6 +146,7 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     static_assert(NC == 4 && WPC == 8, "lane group of 8 = 2 gametes x 4 chromosomes of 8 words");
     extern __shared__ __align__(128) uint8_t s_dyn[];
     __shared__ uint32_t s_flag;
+    pdl_prologue();
     DevSpecies &st = *sp.st;
     const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
     const uint32_t n_chunks = (M + FUSED_CHUNK - 1) / FUSED_CHUNK;
@@ -452,6 +461,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
     __shared__ uint32_t s_cnt[NW], s_pre[NW], s_f[NW];
     __shared__ unsigned long long s_excl;
     __shared__ uint32_t s_stage[SCANF_STAGE];
+    pdl_prologue();
     DevSpecies &st = *sp.st;
     const uint32_t mp = st.m_phys, step = sp.glob->step, cur = st.cur;
     const uint32_t n_ranges = (mp + SCANF_RANGE - 1) / SCANF_RANGE;
@@ -612,8 +622,18 @@ inline cudaError_t fused_bit_configure() {
     return cudaFuncSetAttribute(k_fused_bit_f<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
 }
 
-inline void launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
-    k_fused_bit_f<4, 8><<<n_sms * FUSEDF_CTAS, FUSEDF_WARPS * 32, FUSEDF_SMEM, stream>>>(k);
+inline cudaError_t launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(n_sms * FUSEDF_CTAS);
+    cfg.blockDim = dim3(FUSEDF_WARPS * 32);
+    cfg.dynamicSmemBytes = FUSEDF_SMEM;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8>, k);
 }
 
 // Cooperative launch: the whole grid is resident at once (or the launch fails), which the fixed
@@ -624,11 +644,13 @@ inline cudaError_t launch_scan_fused(const SpK &k, uint32_t n_sms, uint32_t ctas
     cfg.blockDim = dim3(SCAN_THREADS);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = stream;
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeCooperative;
     at[0].val.cooperative = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = 2;
     return cudaLaunchKernelEx(&cfg, k_scan_fused, k);
 }
 
