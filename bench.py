@@ -89,8 +89,12 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def workload(which, seed_offset=0):
+def workload(which, seed_offset=0, world=1):
+    """Rank `seed_offset`'s workload.  Configs 1-5: an independent replica (own seed).  Config 6 (the
+    sweep of unlinked patches): the rank's block of 16 patches out of a 16 x world sweep."""
     from paper_1603_09255_b200 import replicas, workloads
+    if which == 6:
+        return replicas.sweep_shard(16 * world, seed_offset, world)
     return replicas.replica_config(workloads.config(which), seed_offset)
 
 
@@ -176,7 +180,7 @@ def run_ours(args):
     torch.cuda.set_device(dev)
     binding.load()  # fails loudly if the CUDA extension is missing
 
-    cfg = workload(args.config, seed_offset=rank)
+    cfg = workload(args.config, seed_offset=rank, world=world)
     n_sp = len(cfg["species"])
     sim = binding.Sim(cfg, debug=False, log_capacity=max(4096, args.steps * 3 + args.warmup + 64), device=str(dev))
     rows0 = [workloads.initial_rows(cfg, s) for s in range(n_sp)]
@@ -262,7 +266,7 @@ def run_ours(args):
             "metric": METRIC, "value": units / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-            "config": {"workload": describe(cfg), "parallelism": "replicas only x%d" % world,
+            "config": {"workload": describe(cfg), "parallelism": ("patches sharded x%d, no collective" if args.config == 6 else "replicas only x%d") % world,
                        "l2": "inputs larger than L2 (two %d MB population buffers vs 126 MB L2)" % (
                            cfg["species"][0]["capacity"] * row_bytes(cfg["species"][0]) // 2 ** 20),
                        "mean_N_t": units / args.steps / world, "mean_M_t": offspring / args.steps / world,

@@ -24,6 +24,25 @@ def replica_config(cfg, rank):
     return out
 
 
+def patch_block(n_patches, rank, world):
+    """Contiguous block [first, first + count) of a sweep's patches owned by `rank`: unlinked patches
+    (m = 0) are independent replicates, so a sweep shards by patch with no data-path
+    collective.  Blocks differ in size by at most one patch."""
+    base, extra = divmod(int(n_patches), int(world))
+    first = rank * base + min(rank, extra)
+    return first, base + (1 if rank < extra else 0)
+
+
+def sweep_shard(n_patches, rank, world, **kw):
+    """The rank's share of an `n_patches` sweep (workloads.sweep_config), with the parameters the
+    patches have in the whole sweep and a seed of its own."""
+    from . import workloads
+    first, count = patch_block(n_patches, rank, world)
+    seed = kw.pop("seed", 6)
+    return workloads.sweep_config(n_patches=count, first_patch=first, total_patches=n_patches,
+                                  seed=seed + SEED_STRIDE * rank, **kw)
+
+
 def reduce_over_ranks(dist, times, units, device="cpu"):
     """times -> element-wise MAX over ranks, units -> element-wise SUM over ranks.
     `dist` is torch.distributed (initialised) or None for a single process."""

@@ -89,7 +89,35 @@ def config(which, scale=1.0, grid=None, seed=None):
                   predation=None, migration=0.05,
                   capacity=4_718_592 if (scale == 1.0 and grid is None) else cap(per * P))
         return dict(name="C5", seed=sd, grid=(gw, gh), species=[sp], n0=[per * P], steps=200, init_sd=0.1)
+    if which == 6:
+        return sweep_config(scale=scale, seed=seed, n_patches=None if grid is None else grid[0] * grid[1])
     raise ValueError(which)
+
+
+def sweep_config(n_patches=None, per_patch=50_000, scale=1.0, seed=None, first_patch=0, total_patches=None):
+    """S6, the paper-shaped sweep (Fig. S5): P UNLINKED
+    patches (m = 0), i.e. independent replicates, each governed by its own parameter combination
+    (carrying capacity K_p and optimum theta_p), about 50,000 individuals per patch, few freely
+    recombining loci with mutation (case study 1 has 5; rows are 16-byte multiples, so 8 here), 250
+    steps.  `first_patch` / `total_patches` cut a block of patches out of a larger sweep (the
+    parameters of patch p do not depend on how the sweep is split), which is how it shards."""
+    P = 16 if n_patches is None else int(n_patches)
+    T = P if total_patches is None else int(total_patches)
+    per = max(int(round(per_patch * scale)), 4)
+    sd = 6 if seed is None else seed
+    idx = np.arange(first_patch, first_patch + P, dtype=np.float64)
+    # the sweep's parameter grid: optimum from -1 to 1 across the sweep, capacity 60-100 % of the start size
+    theta = (-1.0 + 2.0 * (idx + 0.5) / T).astype(np.float32)
+    Kp = np.floor(per * (0.6 + 0.4 * ((idx * 7.0) % 10.0) / 9.0))
+    cl = [1] * 8
+    n0 = per * P
+    cap = int(np.ceil(n0 * 1.125 / 1024.0)) * 1024
+    sp = dict(n_loci=8, kind="q10", chrom_len=cl, linkage="interval", r=_interval_r(cl, 0.5),
+              xover_mean=None, mu=1e-3, mut_sd=0.05, pheno_scale=2.0 ** -11, fecundity="bh", fec_a=2.0,
+              K=float(per), K_patch=Kp, gaussian=dict(theta0=0.0, dtheta=0.0, omega=1.0, theta_patch=theta),
+              predation=None, migration=0.0, capacity=max(cap, 2048))
+    return dict(name="S6", seed=sd, grid=(P, 1), species=[sp], n0=[n0], steps=250, init_sd=0.1,
+                first_patch=first_patch, total_patches=T)
 
 
 def initial_rows(cfg, species, n=None, seed=None):

@@ -183,3 +183,36 @@ def test_q10_lane_layouts_free_running(oracle_mod, binding, n_loci, chrom_len, r
         parity.assert_logs_equal(sim.read_log(0), orc.log(0))
         parity.assert_state_equal(sim, orc, cfg)
     sim.close()
+
+
+def test_sweep_of_unlinked_patches(oracle_mod, binding):
+    """S6: with m = 0 the patches are independent replicates
+    with their own parameters.  Parity with the oracle, and the metamorphic properties SURVEY.md
+    section 4 lists: no individual ever changes patch, and an emptied patch stays empty."""
+    cfg = workloads.config(6, scale=0.01, grid=(6, 1))
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=True)
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=False)
+    rows = workloads.initial_rows(cfg, 0)
+    ps = workloads.initial_patch_start(cfg, 0).astype(np.int64)
+    a, b = ps[2], ps[3]                                  # patch 2 starts empty
+    rows = np.concatenate([rows[:a], rows[b:]])
+    ps2 = ps.copy()
+    ps2[3:] -= b - a
+    ps2 = ps2.astype(np.uint32)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=True)
+    for o in (orc, sim):
+        o.write_state(0, rows, ps2, 0)
+    for t in range(4):
+        before = sim.read_state(0)[1].astype(np.int64)   # patch_start of the adults
+        orc.step(1)
+        sim.step(1)
+        d = sim.read_debug(0)
+        natal = np.searchsorted(before, d["mother"].astype(np.int64), side="right") - 1
+        assert np.array_equal(natal, d["dest"].astype(np.int64)), "an offspring left its natal patch"
+        parity.assert_debug_equal(d, orc.debug(0), cfg["species"][0], tag="step %d" % t)
+    parity.assert_state_equal(sim, orc, cfg)
+    after = sim.read_state(0)[1].astype(np.int64)
+    sizes = np.diff(after)
+    assert sizes[2] == 0 and (np.delete(sizes, 2) > 0).all()
+    sim.close()
