@@ -482,9 +482,6 @@ __global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK
         if (j_ < M) { p0 = rowptr[sp.mother[j_]]; p1 = rowptr[sp.father[j_]]; }
     };
     const unsigned long long stride = (unsigned long long)n_warps * opw;
-    // the switch thresholds of the lane's 8 loci do not change from offspring to offspring (pass 0)
-    const uint32_t slot0 = li & (GS - 1u);
-    const uint4 tp0 = Tr[2u * slot0], tp1 = Tr[2u * slot0 + 1u];
     uint32_t par0, par1;
     parents((unsigned long long)gw * opw, par0, par1);
     for (unsigned long long ob = (unsigned long long)gw * opw; ob < M; ob += stride) {
@@ -506,8 +503,7 @@ __global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK
             const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
             draw_rk(sp, stream, j, 2u * slot, step, x);
             draw_rk(sp, stream, j, 2u * slot + 1u, step, y);
-            uint4 t0 = tp0, t1 = tp1;
-            if (p) { t0 = Tr[2u * slot]; t1 = Tr[2u * slot + 1u]; }
+            const uint4 t0 = Tr[2u * slot], t1 = Tr[2u * slot + 1u];
             uint32_t run = 0, ph = 0;   // ph bit k = parity of the switch bits of loci 0..k of the lane
             run ^= x[0] < t0.x ? 1u : 0u; ph |= run;
             run ^= x[1] < t0.y ? 1u : 0u; ph |= run << 1;
