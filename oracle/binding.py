@@ -43,7 +43,7 @@ class _SpeciesParams(C.Structure):
         ("theta0", C.c_double), ("dtheta", C.c_double), ("omega", C.c_double),
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
-        ("capacity", C.c_uint64),
+        ("capacity", C.c_uint64), ("resid_sd", C.c_double),
     ]
 
 
@@ -225,6 +225,7 @@ class Oracle:
                 p.predator_species = pr["predator"]
             p.migration = sp.get("migration", 0.0)
             p.capacity = sp["capacity"]
+            p.resid_sd = sp.get("resid_sd", 0.0)
             if sp["kind"] == "bit":
                 self.row_shape.append(2 * (L // 32))
                 self.row_dtype.append(np.uint32)

@@ -12,7 +12,8 @@
  *                    probability mu; Gaussian step about the old value; fusion;
  *                    midpoint additive map
  *   PAPER.md:329     eq. S2-14 additive genotype -> phenotype
- *   DESIGN.md "Readings" R1-R16 for everything the paper leaves open.
+ *   PAPER.md:327-330 eq. S2-14 residual phenotype noise z ~ Normal(genetic value, rho) (R17)
+ *   DESIGN.md "Readings" R1-R17 for everything the paper leaves open.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors, exp
  * specs vs libm, Poisson/normal table moments, brute-force gamete enumeration at
@@ -169,6 +170,7 @@ inline int normal_delta(const uint32_t *T, int R, uint32_t u) {
 
 /* ---------------------------------------------------------------- simulator */
 const int NORMAL_CAP = 8192;
+const int ENV_CAP = 65536;   /* R17: residual-noise table, sd up to 4096 phenotype quanta */
 
 struct SpeciesDebug {
     uint64_t n_t = 0, m_t = 0;
@@ -193,6 +195,7 @@ struct Species {
     std::vector<std::vector<uint32_t>> T_xover;   /* POISSON: per chromosome */
     std::vector<uint32_t> T_mut;                  /* Poisson(L*mu) */
     std::vector<uint32_t> T_norm; int R_norm = 0; /* Q10 effects */
+    std::vector<uint32_t> T_env; int R_env = 0;   /* R17: residual phenotype noise, in phenotype quanta; R_env = 0: none */
     uint64_t T_mig = 0;
     float sel_c = 0.0f; /* fp32(1/(2 omega^2)) */
     /* state */
@@ -460,7 +463,16 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         }
         /* ---- a5: genotype -> phenotype (Fig. 1C) ---- */
         const int32_t zi = phenotype_int(S, ob, oq);
-        const float z = (float)zi * S.p.pheno_scale;
+        /* R17, eq. S2-14: z ~ Normal(genetic value, resid_sd).  The residual is a
+         * whole number k of phenotype quanta from the discrete-normal table (the sampler of R9) on
+         * word 1 of SCALAR block 1; it acts on this individual's selection only and is not inherited. */
+        int32_t zp = zi;
+        if (S.R_env > 0) {
+            uint32_t y[4];
+            draw(sim.seed, si, SCALAR, (uint32_t)j, 1, t, y);
+            zp += normal_delta(S.T_env.data(), S.R_env, y[1]);
+        }
+        const float z = (float)zp * S.p.pheno_scale;
         D.zi[j] = zi; D.z[j] = z;
         /* ---- a6: selection (Fig. 1D), fp32 in this order (R11, R14) ---- */
         float s = 1.0f;
@@ -588,6 +600,11 @@ orc_sim *orc_create(const orc_params *p) {
             /* sigma/q with q = 2^-10 */
             S.R_norm = normal_table(S.p.mut_sd * 1024.0, S.T_norm.data(), NORMAL_CAP);
             if (S.R_norm < 0) { delete sim; return nullptr; }
+        }
+        if (S.p.resid_sd > 0.0) {
+            S.T_env.resize(ENV_CAP);
+            S.R_env = normal_table(S.p.resid_sd / (double)S.p.pheno_scale, S.T_env.data(), ENV_CAP);
+            if (S.R_env < 0) { delete sim; return nullptr; }
         }
         if (S.p.K_patch) S.K_patch.assign(S.p.K_patch, S.p.K_patch + sim->P);
         if (S.p.theta_patch) S.theta_patch.assign(S.p.theta_patch, S.p.theta_patch + sim->P);

@@ -48,6 +48,8 @@ typedef struct {
     uint32_t predator_species;
     double migration;           /* m                                               */
     uint64_t capacity;          /* max rows per population buffer                  */
+    double resid_sd;            /* R17: sd of the residual (environmental) phenotype noise, eq. S2-14
+                                   (PAPER.md:327-330), phenotype units; 0 = none      */
 } orc_species_params;
 
 typedef struct {

@@ -325,3 +325,45 @@ def test_c4_reading_persists_at_small_scale(oracle_mod):
     c = workloads.config(4, scale=0.005)
     o = run(oracle_mod, c, n_steps=60)
     assert o.n(0) > 0.5 * c["n0"][0] and o.n(1) > 0.2 * c["n0"][1]
+
+
+def test_residual_phenotype_noise_closed_forms(oracle_mod):
+    """R17, eq. S2-14: z ~ Normal(genetic value, rho).  Pins: the residual is a
+    whole number of phenotype quanta with mean 0 and variance rho^2 (+ q^2/12, Sheppard), is
+    independent of the genetic value and normal; selection then sees V_P = V_G + rho^2 (survivor
+    fraction: the Gaussian integral) and moves the GENETIC mean by h^2 = V_G/V_P of the phenotypic
+    selection differential (breeder's equation); rho = 0 is the path without noise."""
+    rho, theta = 0.5, 0.8
+    c = workloads.config(2, scale=0.3)
+    sp = c["species"][0]
+    sp["gaussian"].update(theta0=theta, dtheta=0.0)
+    sp["mu"] = 0.0
+    sp["resid_sd"] = rho
+    d = run(oracle_mod, c).debug(0)
+    q = sp["pheno_scale"]
+    g = d["zi"].astype(np.float64) * q
+    z = d["z"].astype(np.float64)
+    k = (z - g) / q
+    assert np.array_equal(k, np.rint(k))                         # whole quanta, exact in fp32
+    e = k * q
+    m = len(e)
+    assert abs(e.mean()) < 5 * rho / math.sqrt(m)
+    assert abs(e.var() / (rho * rho + q * q / 12) - 1) < 5 * math.sqrt(2.0 / m)
+    assert abs(np.corrcoef(e, g)[0, 1]) < 5 / math.sqrt(m)
+    assert stats.kstest(e / rho, "norm").pvalue > 1e-3
+    # the survival probability is the Gaussian of the PHENOTYPE
+    assert np.allclose(d["s"], np.exp(-(z - theta) ** 2 / 2.0), rtol=2e-6, atol=1e-12)
+    alive = d["alive"].astype(bool)
+    VG, VP = g.var(), g.var() + rho * rho
+    w = 1.0 / math.sqrt(VP + 1.0) * math.exp(-(theta - g.mean()) ** 2 / (2 * (VP + 1.0)))
+    assert abs(alive.mean() - w) < 4.5 * math.sqrt(w * (1 - w) / m) + 0.002
+    resp = g[alive].mean() - g.mean()
+    assert abs(resp - (theta - g.mean()) * VG / (VP + 1.0)) < 5 * math.sqrt(VG / alive.sum())
+    # without the noise the response would be (theta - gbar) VG / (VG + 1): a dropped term fails here
+    assert abs(resp - (theta - g.mean()) * VG / (VG + 1.0)) > 5 * math.sqrt(VG / alive.sum())
+    # rho = 0 is bit-identical to a configuration without the field
+    c0 = workloads.config(2, scale=0.01)
+    c1 = workloads.config(2, scale=0.01)
+    c1["species"][0]["resid_sd"] = 0.0
+    a, b = run(oracle_mod, c0, 3), run(oracle_mod, c1, 3)
+    assert a.log(0) == b.log(0) and np.array_equal(a.read_state(0)[0], b.read_state(0)[0])
