@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SPEGG_ABI_VERSION 1u
+#define SPEGG_ABI_VERSION 2u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
        SPEGG_ESTATE = -5 };
@@ -80,6 +80,10 @@ typedef struct spegg_species_params {
     double migration;           /* m: probability that a newborn disperses to one of the 4
                                    torus neighbours of its natal patch (R15)                 */
     uint64_t capacity;          /* rows per population buffer (>= any N_t, M_t), < 2^31      */
+    double resid_sd;            /* rho: sd of the residual (environmental) phenotype noise,
+                                   z ~ Normal(genetic value, rho), eq. S2-14,
+                                   in phenotype units; 0 = none.  Sampled as whole phenotype
+                                   quanta (pheno_scale); rho / pheno_scale <= 4096           */
 } spegg_species_params;
 
 typedef struct spegg_params {

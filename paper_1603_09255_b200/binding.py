@@ -18,6 +18,9 @@ OK, EINVAL, ENOMEM, ECUDA, ERANGE, ESTATE = 0, -1, -2, -3, -4, -5
 FLAG_OVERFLOW, FLAG_EXTINCT = 1, 2
 
 
+ABI_VERSION = 2   # SPEGG_ABI_VERSION of include/spegg.h
+
+
 class SpeciesParams(C.Structure):
     _fields_ = [
         ("n_loci", C.c_uint32), ("genome_kind", C.c_uint32), ("n_chrom", C.c_uint32),
@@ -29,7 +32,7 @@ class SpeciesParams(C.Structure):
         ("theta0", C.c_double), ("dtheta", C.c_double), ("omega", C.c_double),
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
-        ("capacity", C.c_uint64),
+        ("capacity", C.c_uint64), ("resid_sd", C.c_double),
     ]
 
 
@@ -138,6 +141,7 @@ def make_params(cfg, debug=False, log_capacity=0):
             keep.append(xm)
             p.xover_mean = _ptr(xm, C.c_double)
         p.mu, p.mut_sd, p.pheno_scale = sp["mu"], sp.get("mut_sd", 0.0), sp["pheno_scale"]
+        p.resid_sd = sp.get("resid_sd", 0.0)
         p.fecundity_model, p.fec_a, p.K = _FEC[sp["fecundity"]], sp["fec_a"], sp["K"]
         if sp.get("K_patch") is not None:
             kp = np.ascontiguousarray(sp["K_patch"], dtype=np.float64)
@@ -158,7 +162,7 @@ def make_params(cfg, debug=False, log_capacity=0):
             p.sel_predation, p.attack, p.predator_species = 1, pr["attack"], pr["predator"]
         p.migration, p.capacity = sp.get("migration", 0.0), sp["capacity"]
     keep.append(arr)
-    prm = Params(C.sizeof(Params), 1, cfg["seed"], ns, w, h, 1 if debug else 0, log_capacity, 0, arr)
+    prm = Params(C.sizeof(Params), ABI_VERSION, cfg["seed"], ns, w, h, 1 if debug else 0, log_capacity, 0, arr)
     return prm, keep
 
 

@@ -96,16 +96,16 @@ struct Carver {
 struct SpeciesLayout {
     uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
-    uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, K_patch, theta_patch;
-    uint32_t norm_len, n_tables, row_bytes;
+    uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, T_env, K_patch, theta_patch;
+    uint32_t norm_len, env_len, n_tables, row_bytes;
 };
 
 struct HostSpecies {
     spegg_species_params p;
-    std::vector<uint32_t> chrom_len, chrom_start, T_recomb, T_xover, xover_len, T_mut, T_norm;
+    std::vector<uint32_t> chrom_len, chrom_start, T_recomb, T_xover, xover_len, T_mut, T_norm, T_env;
     std::vector<double> K_patch;
     std::vector<float> theta_patch;
-    int R_norm = 0;
+    int R_norm = 0, R_env = 0;
     SpeciesLayout lay;
     SpK k;
 };
@@ -146,6 +146,7 @@ int validate(const spegg_params *p) {
         if (q.genome_kind == SPEGG_Q10 && !(q.mut_sd > 0.0 && q.mut_sd * 1024.0 * 8.0 < 32000.0)) return SPEGG_EINVAL;
         if (!(q.K > 0.0) || !(q.fec_a >= 0.0)) return SPEGG_EINVAL;
         if (q.capacity == 0 || q.capacity >= (1ull << 31)) return SPEGG_EINVAL;
+        if (!(q.resid_sd >= 0.0) || !(q.pheno_scale > 0.0f) || q.resid_sd / (double)q.pheno_scale > 4096.0) return SPEGG_EINVAL;
         if (q.fecundity_model == SPEGG_FEC_CAPTURES && P != 1) return SPEGG_EINVAL;
         if (q.sel_predation) {
             if (q.predator_species >= p->n_species || q.predator_species <= s) return SPEGG_EINVAL;
@@ -213,6 +214,8 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.T_mut = c.take(TMAX * 4);
         l.norm_len = q.genome_kind == SPEGG_Q10 ? 2 * (uint32_t)std::max(1.0, std::ceil(8.0 * q.mut_sd * 1024.0)) : 0;
         l.T_norm = c.take((uint64_t)l.norm_len * 4 + 16);
+        l.env_len = q.resid_sd > 0.0 ? 2 * (uint32_t)std::max(1.0, std::ceil(8.0 * q.resid_sd / (double)q.pheno_scale)) : 0;
+        l.T_env = c.take((uint64_t)l.env_len * 4 + 16);
         l.K_patch = c.take(P * 8);
         l.theta_patch = c.take(P * 4);
     }
@@ -424,6 +427,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         h.T_mut.assign(TMAX, 0);
         const uint32_t mut_len = (uint32_t)h_poisson_table((double)L * q.mu, h.T_mut.data(), TMAX);
         if (q.genome_kind == SPEGG_Q10) h.R_norm = h_normal_table(q.mut_sd * 1024.0, h.T_norm);
+        if (q.resid_sd > 0.0) h.R_env = h_normal_table(q.resid_sd / (double)q.pheno_scale, h.T_env);   // R17
         if (q.K_patch) h.K_patch.assign(q.K_patch, q.K_patch + s->P);
         if (q.theta_patch) h.theta_patch.assign(q.theta_patch, q.theta_patch + s->P);
         h.p.chrom_len = nullptr; h.p.r = nullptr; h.p.xover_mean = nullptr; h.p.K_patch = nullptr; h.p.theta_patch = nullptr;
@@ -436,6 +440,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
             (rc = upload(s, l.chrom_len, h.chrom_len.data(), h.chrom_len.size() * 4)) ||
             (rc = upload(s, l.T_mut, h.T_mut.data(), TMAX * 4)) ||
             (rc = upload(s, l.T_norm, h.T_norm.data(), h.T_norm.size() * 4)) ||
+            (rc = upload(s, l.T_env, h.T_env.data(), h.T_env.size() * 4)) ||
             (rc = upload(s, l.K_patch, h.K_patch.data(), h.K_patch.size() * 8)) ||
             (rc = upload(s, l.theta_patch, h.theta_patch.data(), h.theta_patch.size() * 4)))
             return fail(rc);
@@ -469,6 +474,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.chrom_start = at<uint32_t>(s, l.chrom_start); k.chrom_len = at<uint32_t>(s, l.chrom_len);
         k.T_mut = at<uint32_t>(s, l.T_mut); k.mut_len = mut_len;
         k.T_norm = at<uint32_t>(s, l.T_norm); k.R_norm = h.R_norm;
+        k.T_env = at<uint32_t>(s, l.T_env); k.R_env = h.R_env;
         k.pop[0] = at<uint8_t>(s, l.pop[0]); k.pop[1] = at<uint8_t>(s, l.pop[1]);
         k.patch_start[0] = at<uint32_t>(s, l.patch_start[0]); k.patch_start[1] = at<uint32_t>(s, l.patch_start[1]);
         k.rowptr[0] = at<uint32_t>(s, l.rowptr[0]); k.rowptr[1] = at<uint32_t>(s, l.rowptr[1]);

@@ -78,6 +78,8 @@ struct SpK {
     uint32_t mut_len;
     const uint32_t *T_norm;
     int R_norm;
+    const uint32_t *T_env;      // R17: residual phenotype noise, whole phenotype quanta (discrete-normal table)
+    int R_env;                  // 0: no noise
     // state
     uint8_t *pop[2];
     uint32_t *patch_start[2];   // [P+1] each

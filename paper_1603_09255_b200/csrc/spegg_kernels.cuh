@@ -637,7 +637,13 @@ __global__ void __launch_bounds__(256) k_survival(const __grid_constant__ SpK sp
     const uint32_t M = st.m, step = sp.glob->step;
     unsigned int ties = 0, caps = 0;
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
-        const float z = __fmul_rn((float)sp.zi[j], sp.pheno_scale);
+        int32_t zp = sp.zi[j];
+        if (sp.R_env > 0) {   // R17, eq. S2-14: residual phenotype noise, k quanta from word 1 of SCALAR block 1
+            uint32_t y[4];
+            draw_rk(sp, ST_SCALAR, j, 1, step, y);
+            zp += normal_delta(sp.T_env, sp.R_env, y[1]);
+        }
+        const float z = __fmul_rn((float)zp, sp.pheno_scale);
         const float u = sp.u01[j];
         const float theta = sp.theta_patch ? sp.theta_patch[sp.dest[j]] : st.theta_t;
         bool captured;

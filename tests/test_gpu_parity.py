@@ -216,3 +216,22 @@ def test_sweep_of_unlinked_patches(oracle_mod, binding):
     sizes = np.diff(after)
     assert sizes[2] == 0 and (np.delete(sizes, 2) > 0).all()
     sim.close()
+
+
+@pytest.mark.parametrize("which,scale,rho", [(2, 0.05, 0.3), (1, 2.0, 1.0), (3, 0.01, 0.75), (5, 0.02, 0.25)])
+def test_residual_phenotype_noise(oracle_mod, binding, which, scale, rho):
+    """R17, eq. S2-14: residual phenotype noise.  Per-step parity of every
+    intermediate (debug), then a free-running trajectory on the production kernels (the bit
+    configuration leaves the fused kernel for the general pipeline when rho > 0)."""
+    cfg = workloads.config(which, scale=scale, grid=(4, 3) if which == 5 else None)
+    cfg["species"][0]["resid_sd"] = rho
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    orc.step(8)
+    sim.step(8)
+    parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+    parity.assert_state_equal(sim, orc, cfg)
+    sim.close()
