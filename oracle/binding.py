@@ -43,7 +43,7 @@ class _SpeciesParams(C.Structure):
         ("theta0", C.c_double), ("dtheta", C.c_double), ("omega", C.c_double),
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
-        ("capacity", C.c_uint64), ("resid_sd", C.c_double),
+        ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
     ]
 
 
@@ -69,6 +69,7 @@ class _DebugView(C.Structure):
         ("tables", C.POINTER(C.c_uint32)), ("table_len", C.POINTER(C.c_uint32)),
         ("n_tables", C.c_uint32), ("theta_t", C.c_float), ("zbar_pred", C.c_float),
         ("attack_n", C.c_float), ("cap", C.POINTER(C.c_uint32)),
+        ("a_alive", C.POINTER(C.c_uint8)), ("a_u", C.POINTER(C.c_float)), ("a_s", C.POINTER(C.c_float)),
     ]
 
 
@@ -226,6 +227,7 @@ class Oracle:
             p.migration = sp.get("migration", 0.0)
             p.capacity = sp["capacity"]
             p.resid_sd = sp.get("resid_sd", 0.0)
+            p.adult_survival = sp.get("adult_survival", 0.0)
             if sp["kind"] == "bit":
                 self.row_shape.append(2 * (L // 32))
                 self.row_dtype.append(np.uint32)
@@ -308,6 +310,7 @@ class Oracle:
             "s": arr(v.s, m, np.float32), "z": arr(v.z, m, np.float32),
             "zi": arr(v.zi, m, np.int32), "alive": arr(v.alive, m, np.uint8),
             "captured": arr(v.captured, m, np.uint8),
+            "a_alive": arr(v.a_alive, n, np.uint8), "a_u": arr(v.a_u, n, np.float32), "a_s": arr(v.a_s, n, np.float32),
             "theta_t": float(v.theta_t), "zbar_pred": float(v.zbar_pred), "attack_n": float(v.attack_n),
         }
         nt = int(v.n_tables)

@@ -13,7 +13,8 @@
  *                    midpoint additive map
  *   PAPER.md:329     eq. S2-14 additive genotype -> phenotype
  *   PAPER.md:327-330 eq. S2-14 residual phenotype noise z ~ Normal(genetic value, rho) (R17)
- *   DESIGN.md "Readings" R1-R17 for everything the paper leaves open.
+ *   PAPER.md:56,170,182 overlapping generations, maximum per-step survivorship 0.975 (R18)
+ *   DESIGN.md "Readings" R1-R18 for everything the paper leaves open.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors, exp
  * specs vs libm, Poisson/normal table moments, brute-force gamete enumeration at
@@ -174,9 +175,9 @@ const int ENV_CAP = 65536;   /* R17: residual-noise table, sd up to 4096 phenoty
 
 struct SpeciesDebug {
     uint64_t n_t = 0, m_t = 0;
-    std::vector<uint8_t> f, alive, captured;
+    std::vector<uint8_t> f, alive, captured, a_alive;
     std::vector<uint32_t> off, mother, father, dest, tables, table_len, cap;
-    std::vector<float> u01, s, z;
+    std::vector<float> u01, s, z, a_u, a_s;
     std::vector<int32_t> zi;
     std::vector<uint32_t> off_bits; /* offspring rows, BIT */
     std::vector<int16_t> off_q;     /* offspring rows, Q10 */
@@ -402,8 +403,10 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
     /* ---- a2: exclusive scan ---- */
     uint64_t M = 0;
     for (uint64_t i = 0; i < N; ++i) { D.off[i] = (uint32_t)M; M += D.f[i]; }
-    if (M > S.p.capacity) { /* offspring j >= capacity do not exist */
-        M = S.p.capacity;
+    /* R18: with overlapping generations every adult may stay, so the offspring get what is left */
+    const uint64_t m_cap = S.p.adult_survival > 0.0 ? S.p.capacity - N : S.p.capacity;
+    if (M > m_cap) { /* offspring j >= m_cap do not exist */
+        M = m_cap;
         le.flags |= ORC_FLAG_OVERFLOW;
         sim.flags |= ORC_FLAG_OVERFLOW;
     }
@@ -505,19 +508,57 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         }
     }
 
-    /* ---- a7: survivors (Fig. 1E): all adults die (R1); next adults = surviving offspring
-     *      in increasing (dest, j) ---- */
+    /* ---- R18: overlapping generations.  After reproducing, adult i stays
+     *      alive with probability s_A * w(z_i): s_A the maximum per-step survivorship (the paper's
+     *      0.975 gives a lifespan of 1/(1-0.975) = 40 steps), w the Gaussian term of
+     *      R11 at the adult's GENETIC value (the residual of R17 is a juvenile effect).  The uniform
+     *      is word 1 of the adult's FEC block.  fp32, this order: p = s_A * w. ---- */
+    D.a_alive.assign(N, 0); D.a_u.assign(N, 0.0f); D.a_s.assign(N, 0.0f);
+    std::vector<uint32_t> stay;
+    if (S.p.adult_survival > 0.0) {
+        const float sA = (float)S.p.adult_survival;
+        for (uint64_t i = 0; i < N; ++i) {
+            uint32_t x[4];
+            draw(sim.seed, si, FEC, (uint32_t)i, 0, t, x);
+            const float u = u01_of(x[1]);
+            float w = 1.0f;
+            if (S.p.sel_gaussian) {
+                const float z = (float)S.zi[i] * S.p.pheno_scale;
+                const float th = S.theta_patch.empty() ? D.theta_t : S.theta_patch[0];
+                const float d = z - th;
+                const float sq = d * d;
+                w = expf_spec(-(sq * S.sel_c));
+            }
+            const float p = sA * w;
+            D.a_u[i] = u; D.a_s[i] = p;
+            D.a_alive[i] = (u < p) ? 1 : 0;
+            if (std::fabs(u - p) < 1e-6f) le.near_ties++;
+            if (D.a_alive[i]) stay.push_back((uint32_t)i);
+        }
+    }
+
+    /* ---- a7: survivors (Fig. 1E): next adults = the adults that stay (R18; none under R1), in
+     *      increasing i, then the surviving offspring in increasing (dest, j) ---- */
     std::vector<uint32_t> order;
     order.reserve(M);
     for (uint64_t j = 0; j < M; ++j) if (D.alive[j]) order.push_back((uint32_t)j);
     if (P > 1) std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) { return D.dest[a] < D.dest[b]; });
-    const uint64_t Nn = order.size();
+    const uint64_t Na = stay.size(), Nn = Na + order.size();
     std::vector<uint32_t> nb; std::vector<int16_t> nq;
     if (S.p.genome_kind == ORC_BIT) nb.resize(Nn * S.row_elems); else nq.resize(Nn * S.row_elems);
     std::vector<int32_t> nzi(Nn);
     std::vector<uint32_t> nps(P + 1, 0);
-    for (uint64_t k = 0; k < Nn; ++k) {
-        uint32_t j = order[k];
+    for (uint64_t k = 0; k < Na; ++k) {   /* R18: the adults that stay keep their rows */
+        const uint32_t i = stay[k];
+        if (S.p.genome_kind == ORC_BIT) std::memcpy(&nb[k * S.row_elems], &S.bits[(size_t)i * S.row_elems], S.row_elems * 4);
+        else std::memcpy(&nq[k * S.row_elems], &S.q[(size_t)i * S.row_elems], S.row_elems * 2);
+        nzi[k] = S.zi[i];
+        nps[1]++;
+        le.sum_zi += S.zi[i];
+        le.sum_zi2 += (int64_t)S.zi[i] * S.zi[i];
+    }
+    for (uint64_t k = Na; k < Nn; ++k) {
+        uint32_t j = order[k - Na];
         if (S.p.genome_kind == ORC_BIT) std::memcpy(&nb[k * S.row_elems], &D.off_bits[(size_t)j * S.row_elems], S.row_elems * 4);
         else std::memcpy(&nq[k * S.row_elems], &D.off_q[(size_t)j * S.row_elems], S.row_elems * 2);
         nzi[k] = D.zi[j];
@@ -601,6 +642,8 @@ orc_sim *orc_create(const orc_params *p) {
             S.R_norm = normal_table(S.p.mut_sd * 1024.0, S.T_norm.data(), NORMAL_CAP);
             if (S.R_norm < 0) { delete sim; return nullptr; }
         }
+        /* R18 is defined for an unstructured species (one patch) */
+        if (!(S.p.adult_survival >= 0.0 && S.p.adult_survival <= 1.0) || (S.p.adult_survival > 0.0 && sim->P != 1)) { delete sim; return nullptr; }
         if (S.p.resid_sd > 0.0) {
             S.T_env.resize(ENV_CAP);
             S.R_env = normal_table(S.p.resid_sd / (double)S.p.pheno_scale, S.T_env.data(), ENV_CAP);
@@ -703,6 +746,7 @@ int orc_debug(const orc_sim *sim, uint32_t species, orc_debug_view *o) {
     o->tables = D.tables.data(); o->table_len = D.table_len.data(); o->n_tables = (uint32_t)D.table_len.size();
     o->theta_t = D.theta_t; o->zbar_pred = D.zbar_pred; o->attack_n = D.attack_n;
     o->cap = D.cap.data();
+    o->a_alive = D.a_alive.data(); o->a_u = D.a_u.data(); o->a_s = D.a_s.data();
     return 0;
 }
 

@@ -50,6 +50,8 @@ typedef struct {
     uint64_t capacity;          /* max rows per population buffer                  */
     double resid_sd;            /* R17: sd of the residual (environmental) phenotype noise, eq. S2-14
                                    (PAPER.md:327-330), phenotype units; 0 = none      */
+    double adult_survival;      /* R18: overlapping generations: maximum per-step
+                                   survivorship of an adult, e.g. 0.975; 0 = discrete generations */
 } orc_species_params;
 
 typedef struct {
@@ -114,6 +116,8 @@ typedef struct {
     uint32_t n_tables;
     float theta_t, zbar_pred, attack_n; /* derived scalars                         */
     const uint32_t *cap;       /* predator capture counts (species with CAPTURES)  */
+    const uint8_t *a_alive;    /* [n_t] R18: adult i survives to the next step     */
+    const float *a_u, *a_s;    /* [n_t] its uniform and survival probability       */
 } orc_debug_view;
 int orc_debug(const orc_sim *s, uint32_t species, orc_debug_view *out);
 

@@ -367,3 +367,85 @@ def test_residual_phenotype_noise_closed_forms(oracle_mod):
     c1["species"][0]["resid_sd"] = 0.0
     a, b = run(oracle_mod, c0, 3), run(oracle_mod, c1, 3)
     assert a.log(0) == b.log(0) and np.array_equal(a.read_state(0)[0], b.read_state(0)[0])
+
+
+def _overlap_cfg(n0=2000, sA=0.975, omega=0.0, fec_a=0.0, K=1e9, L=16, capacity=8192):
+    sp = species(L=L, kind="q10", r=0.5, mu=0.0, fec_a=fec_a, K=K, omega=omega, capacity=capacity)
+    sp["adult_survival"] = sA
+    c = cfg(sp, seed=11)
+    c["n0"] = [n0]
+    c["init_sd"] = 0.1
+    return c
+
+
+def test_overlapping_generations_lifespan(oracle_mod):
+    """R18.  Pin from the paper itself: at the maximum per-step survivorship
+    0.975 the average lifespan is about 40 steps (tests/golden/lifespan.txt).  A cohort
+    that neither reproduces (fec_a = 0) nor is selected (omega = inf) decays as N_t ~ N_0 s^t, and
+    the lifespan of its members, sum_t N_t / N_0 counting the step of birth, is 1/(1-s)."""
+    sA, life = [float(x) for x in open(os.path.join(HERE, "golden", "lifespan.txt")).read().split("\n")[-2].split()]
+    assert abs(1.0 / (1.0 - sA) - life) < 1e-9            # the textbook geometric mean, retyped
+    n0 = 3000
+    c = _overlap_cfg(n0=n0, sA=sA)
+    o = oracle_mod.Oracle(c)
+    o.write_state(0, workloads.initial_rows(c, 0), None, 0)
+    o.step(600)
+    lg = o.log(0)
+    N = np.array([e["n_t"] for e in lg] + [lg[-1]["n_next"]], dtype=np.float64)
+    assert all(e["m_t"] == 0 for e in lg) and N[-1] == 0   # nobody is born, everybody dies in the end
+    assert (np.diff(N) <= 0).all()
+    # binomial chain: N_t | N_0 has mean N_0 s^t and variance N_0 s^t (1 - s^t)
+    for t in (10, 40, 100):
+        mu = n0 * sA ** t
+        assert abs(N[t] - mu) < 5 * math.sqrt(mu * (1 - sA ** t))
+    lifespan = N[:-1].sum() / n0                           # steps lived per individual
+    assert abs(lifespan - life) < 5 * math.sqrt(sA) / (1 - sA) / math.sqrt(n0)   # sd of a geometric lifetime
+    # s_A = 0 is the discrete-generation path, bit for bit
+    a, b = workloads.config(1), workloads.config(1)
+    b["species"][0]["adult_survival"] = 0.0
+    ra, rb = run(oracle_mod, a, 3), run(oracle_mod, b, 3)
+    assert ra.log(0) == rb.log(0) and np.array_equal(ra.read_state(0)[0], rb.read_state(0)[0])
+
+
+def test_overlapping_generations_order_selection_and_regulation(oracle_mod):
+    """R18: the next generation is the staying adults (in order, rows unchanged) followed by the
+    surviving offspring; an adult stays with probability s_A w(z); with overlap the Beverton-Holt
+    population settles where births balance deaths."""
+    sA, om = 0.6, 1.0
+    c = _overlap_cfg(n0=4000, sA=sA, omega=om, fec_a=2.0, K=4000.0, L=64, capacity=32768)
+    c["species"][0]["gaussian"]["theta0"] = 0.5
+    o = oracle_mod.Oracle(c)
+    rows0 = workloads.initial_rows(c, 0)
+    o.write_state(0, rows0, None, 0)
+    o.step(1)
+    d = o.debug(0)
+    stay = d["a_alive"].astype(bool)
+    alive = d["alive"].astype(bool)
+    rows1 = o.read_state(0)[0]
+    assert len(rows1) == stay.sum() + alive.sum() == o.log(0)[0]["n_next"]
+    assert np.array_equal(rows1[:stay.sum()], rows0[stay])
+    assert np.array_equal(rows1[stay.sum():], d["offspring"][alive])
+    # probability and decision
+    z = rows0.astype(np.int64).sum(axis=1) * 2.0 ** -11
+    assert np.allclose(d["a_s"], sA * np.exp(-(z - 0.5) ** 2 / (2 * om * om)), rtol=2e-6)
+    assert np.array_equal(stay, d["a_u"] < d["a_s"])
+    # the adults' uniforms are independent of their fecundity draws (two words of one block)
+    assert abs(np.corrcoef(d["a_u"], d["f"].astype(np.float64))[0, 1]) < 5 / math.sqrt(len(z))
+    assert stats.kstest(d["a_u"], "uniform").pvalue > 1e-3
+    V = z.var()
+    w = om / math.sqrt(V + om * om) * math.exp(-(0.5 - z.mean()) ** 2 / (2 * (V + om * om)))
+    assert abs(stay.mean() - sA * w) < 4.5 * math.sqrt(sA * w * (1 - sA * w) / len(z))
+    # regulation without selection: N* solves 1 = s_A + R0/(1 + N*/K)  =>  N* = K (R0/(1 - s_A) - 1)
+    c = _overlap_cfg(n0=1000, sA=0.5, fec_a=2.0, K=1000.0, capacity=16384)
+    o = oracle_mod.Oracle(c)
+    o.write_state(0, workloads.initial_rows(c, 0), None, 0)
+    o.step(120)
+    N = np.array([e["n_t"] for e in o.log(0)[40:]], dtype=np.float64)
+    assert abs(N.mean() / (1000.0 * (2.0 / 0.5 - 1.0)) - 1) < 0.03
+    # the offspring get the room the adults leave: M_t <= capacity - N_t
+    c = _overlap_cfg(n0=1500, sA=0.9, fec_a=2.0, K=1e9, capacity=2048)
+    o = oracle_mod.Oracle(c)
+    o.write_state(0, workloads.initial_rows(c, 0), None, 0)
+    o.step(1)
+    e = o.log(0)[0]
+    assert e["m_t"] == 2048 - 1500 and e["flags"] & 1 and e["n_next"] <= 2048
