@@ -84,6 +84,13 @@ typedef struct spegg_species_params {
                                    z ~ Normal(genetic value, rho), eq. S2-14,
                                    in phenotype units; 0 = none.  Sampled as whole phenotype
                                    quanta (pheno_scale); rho / pheno_scale <= 4096           */
+    double adult_survival;      /* s_A: overlapping generations.  After
+                                   reproducing, an adult stays alive with probability
+                                   s_A * w(z) (w: the Gaussian term at its genetic value; the
+                                   paper's maximum survivorship is 0.975 = a lifespan of 40
+                                   steps); the next generation is the staying adults, in order,
+                                   then the surviving offspring, and M_t <= capacity - N_t.
+                                   0 = discrete generations.  Unstructured species (1x1) only */
 } spegg_species_params;
 
 typedef struct spegg_params {
@@ -122,6 +129,8 @@ typedef struct spegg_debug_view {
     uint32_t n_tables;
     float theta_t, zbar_pred, attack_n;
     const uint32_t *d_cap;      /* [n_t] capture counts (SPEGG_FEC_CAPTURES species)          */
+    const uint8_t *d_a_alive;   /* [n_t] adult stays alive (adult_survival > 0)               */
+    const float *d_a_u, *d_a_s; /* [n_t] its uniform and survival probability                 */
 } spegg_debug_view;
 
 typedef struct spegg_sim spegg_sim;

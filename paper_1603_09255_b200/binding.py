@@ -32,7 +32,7 @@ class SpeciesParams(C.Structure):
         ("theta0", C.c_double), ("dtheta", C.c_double), ("omega", C.c_double),
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
-        ("capacity", C.c_uint64), ("resid_sd", C.c_double),
+        ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
     ]
 
 
@@ -57,6 +57,7 @@ class DebugView(C.Structure):
         ("d_captured", C.c_void_p), ("d_offspring", C.c_void_p), ("d_tables", C.c_void_p),
         ("d_table_len", C.c_void_p), ("n_tables", C.c_uint32), ("theta_t", C.c_float),
         ("zbar_pred", C.c_float), ("attack_n", C.c_float), ("d_cap", C.c_void_p),
+        ("d_a_alive", C.c_void_p), ("d_a_u", C.c_void_p), ("d_a_s", C.c_void_p),
     ]
 
 
@@ -142,6 +143,7 @@ def make_params(cfg, debug=False, log_capacity=0):
             p.xover_mean = _ptr(xm, C.c_double)
         p.mu, p.mut_sd, p.pheno_scale = sp["mu"], sp.get("mut_sd", 0.0), sp["pheno_scale"]
         p.resid_sd = sp.get("resid_sd", 0.0)
+        p.adult_survival = sp.get("adult_survival", 0.0)
         p.fecundity_model, p.fec_a, p.K = _FEC[sp["fecundity"]], sp["fec_a"], sp["K"]
         if sp.get("K_patch") is not None:
             kp = np.ascontiguousarray(sp["K_patch"], dtype=np.float64)
@@ -314,5 +316,7 @@ class Sim:
             "table_len": arr(v.d_table_len, nt, np.uint32),
             "theta_t": float(v.theta_t), "zbar_pred": float(v.zbar_pred), "attack_n": float(v.attack_n),
             "cap": arr(v.d_cap, n, np.uint32),
+            "a_alive": arr(v.d_a_alive, n, np.uint8), "a_u": arr(v.d_a_u, n, np.float32),
+            "a_s": arr(v.d_a_s, n, np.float32),
         }
         return d

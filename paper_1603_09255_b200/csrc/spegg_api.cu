@@ -94,7 +94,7 @@ struct Carver {
 };
 
 struct SpeciesLayout {
-    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured,
+    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
     uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, T_env, K_patch, theta_patch;
     uint32_t norm_len, env_len, n_tables, row_bytes;
@@ -146,6 +146,7 @@ int validate(const spegg_params *p) {
         if (q.genome_kind == SPEGG_Q10 && !(q.mut_sd > 0.0 && q.mut_sd * 1024.0 * 8.0 < 32000.0)) return SPEGG_EINVAL;
         if (!(q.K > 0.0) || !(q.fec_a >= 0.0)) return SPEGG_EINVAL;
         if (q.capacity == 0 || q.capacity >= (1ull << 31)) return SPEGG_EINVAL;
+        if (!(q.adult_survival >= 0.0 && q.adult_survival <= 1.0) || (q.adult_survival > 0.0 && P != 1)) return SPEGG_EINVAL;
         if (!(q.resid_sd >= 0.0) || !(q.pheno_scale > 0.0f) || q.resid_sd / (double)q.pheno_scale > 4096.0) return SPEGG_EINVAL;
         if (q.fecundity_model == SPEGG_FEC_CAPTURES && P != 1) return SPEGG_EINVAL;
         if (q.sel_predation) {
@@ -197,6 +198,9 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.zi = c.take(cap * 4);
         l.alive = c.take(cap);
         l.captured = c.take(cap);
+        const uint64_t acap = q.adult_survival > 0.0 ? cap : 1;   // R18 arrays only when generations overlap
+        l.a_alive = c.take(acap); l.a_u = c.take(acap * 4); l.a_s = c.take(acap * 4);
+        l.a_zi = c.take(acap * 4); l.a_pos = c.take(acap * 4);
         l.cap = c.take(cap * 4);
         l.offbuf = c.take(cap * l.row_bytes);
         l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
@@ -316,6 +320,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             k_mutate<<<ctas(cap * 2, 256, 8), 256, 0, s->stream>>>(k, q10v ? 1 : 0); ++nl;
             if (!q10v) { k_phenotype<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }
             k_survival<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
+            if (k.adult_surv > 0.0f) { k_adult_survive<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }   // R18
             if (s->P == 1) {
                 k_cmp_scan<<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
             } else {
@@ -323,7 +328,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
                 k_patch_base<<<1, 1024, 0, s->stream>>>(k); ++nl;
                 k_patch_pos<<<std::min(s->P, G * 8), 256, 0, s->stream>>>(k); ++nl;
             }
-            k_cmp_scatter<<<k.index_only ? g_thread : g_warp, 256, 0, s->stream>>>(k); ++nl;
+            k_cmp_scatter<<<(k.index_only && k.adult_surv == 0.0f) ? g_thread : g_warp, 256, 0, s->stream>>>(k); ++nl;
         }
     }
     const bool solo = s->sp.size() == 1 && s->sp[0].k.solo;  // the last kernel closes the step itself
@@ -487,6 +492,9 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.u01 = at<float>(s, l.u01); k.s = at<float>(s, l.s);
         k.offbuf = at<uint8_t>(s, l.offbuf); k.zi = at<int32_t>(s, l.zi);
         k.alive = at<uint8_t>(s, l.alive); k.captured = at<uint8_t>(s, l.captured);
+        k.adult_surv = (float)q.adult_survival;
+        k.a_alive = at<uint8_t>(s, l.a_alive); k.a_u = at<float>(s, l.a_u); k.a_s = at<float>(s, l.a_s);
+        k.a_zi = at<int32_t>(s, l.a_zi); k.a_pos = at<uint32_t>(s, l.a_pos);
         k.cap = at<uint32_t>(s, l.cap);
         k.tables = at<uint32_t>(s, l.tables); k.table_len = at<uint32_t>(s, l.table_len);
         k.status_fec = at<unsigned long long>(s, l.status_fec); k.status_cmp = at<unsigned long long>(s, l.status_cmp);
@@ -652,6 +660,7 @@ int spegg_read_debug(spegg_sim *s, uint32_t species, spegg_debug_view *o) {
     o->d_offspring = k.offbuf; o->d_tables = k.tables; o->d_table_len = k.table_len; o->n_tables = k.n_tables;
     o->theta_t = st.theta_t; o->zbar_pred = st.zbar_pred; o->attack_n = st.attack_n;
     o->d_cap = k.cap;
+    o->d_a_alive = k.a_alive; o->d_a_u = k.a_u; o->d_a_s = k.a_s;
     return SPEGG_OK;
 }
 

@@ -613,7 +613,7 @@ __global__ void __launch_bounds__(256) k_fill_masks(uint32_t *mask, uint32_t *ra
 }
 
 __host__ inline bool fused_bit_supported(const SpK &k) {
-    return k.kind == 0 && k.linkage == 1 && k.n_chrom == 4 && k.L == 1024 && k.P == 1 && !k.sel_predation && k.R_env == 0 &&
+    return k.kind == 0 && k.linkage == 1 && k.n_chrom == 4 && k.L == 1024 && k.P == 1 && !k.sel_predation && k.R_env == 0 && k.adult_surv == 0.0f &&
            k.fec_model != 2 && k.theta_patch == nullptr &&
            (unsigned long long)(k.capacity + 32) * FUSED_ROW < (1ull << 32);
 }

@@ -95,6 +95,12 @@ struct SpK {
     uint8_t *offbuf;
     int32_t *zi;
     uint8_t *alive, *captured;
+    // R18, overlapping generations (adult_surv > 0): per adult i of the current step
+    float adult_surv;           // s_A as fp32; 0 = discrete generations
+    uint8_t *a_alive;           // stays alive
+    float *a_u, *a_s;           // its uniform and survival probability
+    int32_t *a_zi;              // its integer genetic value
+    uint32_t *a_pos;            // its position in the next generation (0xFFFFFFFF: dies)
     uint32_t *cap;              // capture counts of THIS species' adults (CAPTURES model)
     uint32_t *cap_pred;         // capture counts of the predator species (predation term)
     uint32_t *tables, *table_len;

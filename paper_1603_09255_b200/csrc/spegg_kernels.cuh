@@ -245,6 +245,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
     __shared__ unsigned long long s_excl;
     DevSpecies &st = *sp.st;
     const uint32_t N = st.n0, step = sp.glob->step;
+    // R18: with overlapping generations every adult may stay, so the offspring get the room that is left
+    const uint32_t m_cap = sp.adult_surv > 0.0f ? sp.capacity - N : sp.capacity;
     const uint32_t R = fec_range_size(N, gridDim.x);
     const uint32_t n_ranges = (N + R - 1) / R;
     const uint32_t per = R / SCAN_THREADS;  // adults per thread in pass 2 (<= 32)
@@ -296,7 +298,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
                 s_excl = excl;
                 if (range == n_ranges - 1) {  // the last range knows M
                     const unsigned long long Mtot = excl + total;
-                    if (Mtot > (unsigned long long)sp.capacity) { st.m = sp.capacity; st.flags_step |= 1u; }
+                    if (Mtot > (unsigned long long)m_cap) { st.m = m_cap; st.flags_step |= 1u; }
                     else st.m = (uint32_t)Mtot;
                 }
             }
@@ -320,7 +322,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
                 const uint32_t mval = sp.phys_parents ? rowptr[i] : i;
                 for (uint32_t c = 0; c < f; ++c) {
                     const unsigned long long j = o + c;
-                    if (j < (unsigned long long)sp.capacity) sp.mother[j] = mval;
+                    if (j < (unsigned long long)m_cap) sp.mother[j] = mval;
                 }
             }
         }
@@ -665,16 +667,50 @@ __global__ void __launch_bounds__(256) k_survival(const __grid_constant__ SpK sp
     if (caps) atomicAdd(&st.captures, (unsigned long long)caps);
 }
 
+// R18, overlapping generations: adult i stays alive with probability
+// s_A * w(z_i) -- w the Gaussian term of R11 at its genetic value, the uniform word 1 of its FEC
+// block; fp32 in this order: p = s_A * w.  One warp per adult (the genetic value is re-read from its row).
+__global__ void __launch_bounds__(256) k_adult_survive(const __grid_constant__ SpK sp) {
+    DevSpecies &st = *sp.st;
+    const uint32_t N = st.n0, step = sp.glob->step, lane = threadIdx.x & 31u;
+    const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    const uint8_t *pop = sp.pop[st.cur];
+    const uint32_t *rowptr = sp.rowptr[st.cur];
+    const float theta = sp.theta_patch ? sp.theta_patch[0] : st.theta_t;
+    unsigned int ties = 0;
+    for (uint32_t i = warp0; i < N; i += nw) {
+        const int32_t zi = warp_row_zi(sp, pop + (size_t)rowptr[i] * sp.row_bytes);
+        if (lane == 0) {
+            uint32_t x[4];
+            draw_rk(sp, ST_FEC, i, 0, step, x);
+            const float u = u01_of(x[1]);
+            float w = 1.0f;
+            if (sp.sel_gaussian) {
+                const float d = __fsub_rn(__fmul_rn((float)zi, sp.pheno_scale), theta);
+                w = expf_spec(-__fmul_rn(__fmul_rn(d, d), sp.sel_c));
+            }
+            const float p = __fmul_rn(sp.adult_surv, w);
+            sp.a_zi[i] = zi; sp.a_u[i] = u; sp.a_s[i] = p;
+            sp.a_alive[i] = (u < p) ? 1 : 0;
+            if (fabsf(__fsub_rn(u, p)) < 1e-6f) ++ties;
+        }
+    }
+    if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
+}
+
 // a7 (unstructured): stable compaction positions by decoupled look-back + survivor reductions
 __global__ void __launch_bounds__(SCAN_THREADS) k_cmp_scan(const __grid_constant__ SpK sp) {
     __shared__ uint32_t s_warp[SCAN_THREADS / 32];
     __shared__ uint32_t s_tile;
     __shared__ unsigned long long s_excl;
     DevSpecies &st = *sp.st;
-    const uint32_t M = st.m;
+    // items: the NA adults (R18; none when generations are discrete), then the M offspring -- which is
+    // the order of the next generation
+    const uint32_t NA = sp.adult_surv > 0.0f ? st.n0 : 0u, M = NA + st.m;
     const uint32_t n_tiles = (M + SCAN_TILE - 1) / SCAN_TILE;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     long long a1 = 0, a2 = 0;
+    if (M == 0 && blockIdx.x == 0 && tid == 0) st.n_next = 0;
     for (;;) {
         if (tid == 0) s_tile = atomicAdd(&st.ticket_cmp, 1u);
         __syncthreads();
@@ -685,9 +721,9 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cmp_scan(const __grid_constant
 #pragma unroll
         for (int k = 0; k < SCAN_ITEMS; ++k) {
             const uint32_t j = base + k;
-            a[k] = (j < M) ? sp.alive[j] : 0u;
+            a[k] = (j < M) ? (j < NA ? sp.a_alive[j] : sp.alive[j - NA]) : 0u;
             sum += a[k];
-            if (a[k]) { const long long z = sp.zi[j]; a1 += z; a2 += z * z; }
+            if (a[k]) { const long long z = j < NA ? sp.a_zi[j] : sp.zi[j - NA]; a1 += z; a2 += z * z; }
         }
         const uint32_t incl = warp_incl_scan(sum);
         if (lane == 31) s_warp[warp] = incl;
@@ -708,7 +744,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cmp_scan(const __grid_constant
 #pragma unroll
         for (int k = 0; k < SCAN_ITEMS; ++k) {
             const uint32_t j = base + k;
-            if (j < M) { sp.pos[j] = a[k] ? o : 0xFFFFFFFFu; o += a[k]; }
+            if (j < M) { (j < NA ? sp.a_pos[j] : sp.pos[j - NA]) = a[k] ? o : 0xFFFFFFFFu; o += a[k]; }
         }
         __syncthreads();
     }
@@ -741,6 +777,22 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
             const uint4 *src = (const uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes);
             uint4 *d = (uint4 *)(dst + (size_t)p * sp.row_bytes);
             for (uint32_t i = lane; i < sp.row_u4; i += 32) d[i] = src[i];
+        }
+    }
+    // R18: the adults that stay are copied into the other buffer, one warp per row -- behind the
+    // offspring rows (row M + rank) when the compaction is index-only, else at their position
+    if (sp.adult_surv > 0.0f) {
+        const uint32_t N = st.n0, cur = st.cur;
+        const uint8_t *src_pop = sp.pop[cur];
+        const uint32_t *rp_cur = sp.rowptr[cur];
+        for (uint32_t i = warp0; i < N; i += nw) {
+            const uint32_t p = sp.a_pos[i];
+            if (p == 0xFFFFFFFFu) continue;
+            const uint32_t row = sp.index_only ? M + p : p;
+            if (lane == 0) rp[p] = row;
+            const uint4 *src = (const uint4 *)(src_pop + (size_t)rp_cur[i] * sp.row_bytes);
+            uint4 *d = (uint4 *)(dst + (size_t)row * sp.row_bytes);
+            for (uint32_t k = lane; k < sp.row_u4; k += 32) d[k] = src[k];
         }
     }
     if (sp.solo) solo_tail(sp, &s_flag);   // single unstructured species: the last CTA closes the step

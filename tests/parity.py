@@ -30,6 +30,10 @@ def assert_debug_equal(dg, do, species_cfg, tag=""):
         assert np.float32(dg[k]) == np.float32(do[k]), (tag, k)
     if species_cfg["fecundity"] == "captures":
         assert np.array_equal(dg["cap"], do["cap"]), (tag, "cap")
+    if species_cfg.get("adult_survival", 0.0) > 0.0:   # R18: the adults' own survival
+        assert np.array_equal(dg["a_alive"], do["a_alive"]), (tag, "a_alive")
+        assert np.array_equal(dg["a_u"].view(np.uint32), do["a_u"].view(np.uint32)), (tag, "a_u")
+        assert np.array_equal(dg["a_s"].view(np.uint32), do["a_s"].view(np.uint32)), (tag, "a_s")
 
 
 def assert_state_equal(sim, orc, cfg, tag=""):

@@ -235,3 +235,37 @@ def test_residual_phenotype_noise(oracle_mod, binding, which, scale, rho):
     parity.assert_logs_equal(sim.read_log(0), orc.log(0))
     parity.assert_state_equal(sim, orc, cfg)
     sim.close()
+
+
+@pytest.mark.parametrize("which,scale,sA,rho", [(1, 1.0, 0.975, 0.0), (2, 0.04, 0.6, 0.0), (3, 0.008, 0.5, 0.0),
+                                                 (2, 0.03, 0.8, 0.2)])
+def test_overlapping_generations(oracle_mod, binding, which, scale, sA, rho):
+    """R18: adults stay alive with probability s_A w(z); the next generation is
+    the staying adults followed by the surviving offspring.  Per-step parity of every intermediate
+    (debug), then a free-running trajectory on the production kernels."""
+    cfg = workloads.config(which, scale=scale)
+    sp = cfg["species"][0]
+    sp["adult_survival"] = sA
+    sp["resid_sd"] = rho
+    sp["capacity"] = 4 * sp["capacity"]          # generations pile up: N* = K (2 w / (1 - s_A w) - 1)
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(2):
+        orc.step(6)
+        sim.step(6)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+        parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags
+    sim.close()
+
+
+def test_overlapping_generations_room_for_offspring(oracle_mod, binding):
+    # M_t <= capacity - N_t: the overflow flag and the truncation agree with the oracle
+    cfg = workloads.config(1, scale=1.5)
+    sp = cfg["species"][0]
+    sp.update(adult_survival=0.9, K=1e9, capacity=2048)
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=True)
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
