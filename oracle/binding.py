@@ -44,6 +44,7 @@ class _SpeciesParams(C.Structure):
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
+        ("mate_skew", C.c_double),
     ]
 
 
@@ -70,6 +71,7 @@ class _DebugView(C.Structure):
         ("n_tables", C.c_uint32), ("theta_t", C.c_float), ("zbar_pred", C.c_float),
         ("attack_n", C.c_float), ("cap", C.POINTER(C.c_uint32)),
         ("a_alive", C.POINTER(C.c_uint8)), ("a_u", C.POINTER(C.c_float)), ("a_s", C.POINTER(C.c_float)),
+        ("mate_cum", C.POINTER(C.c_uint64)), ("zbar_self", C.c_float),
     ]
 
 
@@ -228,6 +230,7 @@ class Oracle:
             p.capacity = sp["capacity"]
             p.resid_sd = sp.get("resid_sd", 0.0)
             p.adult_survival = sp.get("adult_survival", 0.0)
+            p.mate_skew = sp.get("mate_skew", 0.0)
             if sp["kind"] == "bit":
                 self.row_shape.append(2 * (L // 32))
                 self.row_dtype.append(np.uint32)
@@ -312,6 +315,9 @@ class Oracle:
             "captured": arr(v.captured, m, np.uint8),
             "a_alive": arr(v.a_alive, n, np.uint8), "a_u": arr(v.a_u, n, np.float32), "a_s": arr(v.a_s, n, np.float32),
             "theta_t": float(v.theta_t), "zbar_pred": float(v.zbar_pred), "attack_n": float(v.attack_n),
+            "zbar_self": float(v.zbar_self),
+            "mate_cum": (arr(v.mate_cum, n, np.uint64) if self.cfg["species"][species].get("mate_skew", 0.0) != 0.0
+                         else np.zeros(0, np.uint64)),
         }
         nt = int(v.n_tables)
         d["table_len"] = arr(v.table_len, nt, np.uint32)

@@ -178,6 +178,8 @@ struct SpeciesDebug {
     std::vector<uint8_t> f, alive, captured, a_alive;
     std::vector<uint32_t> off, mother, father, dest, tables, table_len, cap;
     std::vector<float> u01, s, z, a_u, a_s;
+    std::vector<uint64_t> mate_cum; /* R19 */
+    float zbar_self = 0;
     std::vector<int32_t> zi;
     std::vector<uint32_t> off_bits; /* offspring rows, BIT */
     std::vector<int16_t> off_q;     /* offspring rows, Q10 */
@@ -389,6 +391,30 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         D.attack_n = (float)(S.p.attack * (double)NC);
     }
 
+    /* ---- R19 ("shared preference"; eq. S2-10): the probability that
+     *      adult i fathers a given egg is X_i^{v_m} / sum_k X_k^{v_m}.  The trait is read as log size,
+     *      X_i = exp(z_i), so the weight is exp(v_m z_i); it is taken relative to the adults' mean
+     *      zbar (fp64 sum/N*scale rounded to fp32, as zbar_C in R14) and clamped to +-16 so that the
+     *      spec'd expf (x <= 0) serves: fp32, this order: d = z_i - zbar; e = v*d; e = min(max(e,-16),16);
+     *      x = e - 16; w = expf_spec(x); integer weight = trunc(w * 2^40) (exact scaling).  mate_cum is
+     *      the inclusive running sum in adult order (uint64, no rounding anywhere). ---- */
+    if (S.p.mate_skew != 0.0) {
+        const float v = (float)S.p.mate_skew;
+        D.zbar_self = (float)(((double)sumzi0[si] / (double)N) * (double)S.p.pheno_scale);
+        D.mate_cum.resize(N);
+        uint64_t run = 0;
+        for (uint64_t i = 0; i < N; ++i) {
+            const float z = (float)S.zi[i] * S.p.pheno_scale;
+            const float d = z - D.zbar_self;
+            float e = v * d;
+            e = std::min(std::max(e, -16.0f), 16.0f);
+            const float x = e - 16.0f;
+            const float w = expf_spec(x);
+            run += (uint64_t)(w * 0x1p40f);
+            D.mate_cum[i] = run;
+        }
+    }
+
     /* ---- a1: fecundity (Fig. 1A), one FEC block per adult ---- */
     D.f.resize(N);
     D.off.resize(N);
@@ -436,7 +462,23 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         /* R2: father uniform over the adults of the mother's patch, selfing allowed */
         const uint32_t base = (P == 1) ? 0 : S.patch_start[pm];
         const uint32_t np = (P == 1) ? (uint32_t)N : S.patch_start[pm + 1] - S.patch_start[pm];
-        const uint32_t fa = base + uniform_index(x[0], np);
+        uint32_t fa = base + uniform_index(x[0], np);
+        if (S.p.mate_skew != 0.0) {
+            /* R19: weighted draw among the adults of the mother's patch by running sum + search:
+             * total = weight of the patch; 64-bit uniform from words 2,3 of SCALAR block 1;
+             * target = floor(u * total / 2^64); father = first adult whose inclusive running sum
+             * exceeds (running sum before the patch) + target.  A patch of total weight 0 keeps R2. */
+            const uint64_t before = base ? D.mate_cum[base - 1] : 0;
+            const uint64_t total = D.mate_cum[base + np - 1] - before;
+            if (total > 0) {
+                uint32_t y[4];
+                draw(sim.seed, si, SCALAR, (uint32_t)j, 1, t, y);
+                const uint64_t u = ((uint64_t)y[2] << 32) | y[3];
+                const uint64_t target = before + (uint64_t)(((unsigned __int128)u * total) >> 64);
+                /* first index in the patch with mate_cum > target (library binary search) */
+                fa = (uint32_t)(std::upper_bound(D.mate_cum.begin() + base, D.mate_cum.begin() + base + np, target) - D.mate_cum.begin());
+            }
+        }
         D.father[j] = fa;
         /* R15: dispersal drawn at birth */
         uint32_t dest = pm;
@@ -642,6 +684,7 @@ orc_sim *orc_create(const orc_params *p) {
             S.R_norm = normal_table(S.p.mut_sd * 1024.0, S.T_norm.data(), NORMAL_CAP);
             if (S.R_norm < 0) { delete sim; return nullptr; }
         }
+        if (!(std::fabs(S.p.mate_skew) <= 1e6)) { delete sim; return nullptr; }
         /* R18 is defined for an unstructured species (one patch) */
         if (!(S.p.adult_survival >= 0.0 && S.p.adult_survival <= 1.0) || (S.p.adult_survival > 0.0 && sim->P != 1)) { delete sim; return nullptr; }
         if (S.p.resid_sd > 0.0) {
@@ -747,6 +790,7 @@ int orc_debug(const orc_sim *sim, uint32_t species, orc_debug_view *o) {
     o->theta_t = D.theta_t; o->zbar_pred = D.zbar_pred; o->attack_n = D.attack_n;
     o->cap = D.cap.data();
     o->a_alive = D.a_alive.data(); o->a_u = D.a_u.data(); o->a_s = D.a_s.data();
+    o->mate_cum = D.mate_cum.data(); o->zbar_self = D.zbar_self;
     return 0;
 }
 

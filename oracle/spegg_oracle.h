@@ -52,6 +52,10 @@ typedef struct {
                                    (PAPER.md:327-330), phenotype units; 0 = none      */
     double adult_survival;      /* R18: overlapping generations: maximum per-step
                                    survivorship of an adult, e.g. 0.975; 0 = discrete generations */
+    double mate_skew;           /* R19: shared-preference mating (eq. S2-10):
+                                   the father of each egg is drawn with probability proportional to
+                                   X_i^{v_m}, X_i = exp(z_i) the adult's size, v_m = mate_skew;
+                                   0 = uniform mate (R2)                              */
 } orc_species_params;
 
 typedef struct {
@@ -118,6 +122,8 @@ typedef struct {
     const uint32_t *cap;       /* predator capture counts (species with CAPTURES)  */
     const uint8_t *a_alive;    /* [n_t] R18: adult i survives to the next step     */
     const float *a_u, *a_s;    /* [n_t] its uniform and survival probability       */
+    const uint64_t *mate_cum;  /* [n_t] R19: inclusive running sum of the integer mating weights */
+    float zbar_self;           /* R19: mean genetic value of the adults, the weights' reference */
 } orc_debug_view;
 int orc_debug(const orc_sim *s, uint32_t species, orc_debug_view *out);
 
