@@ -11,7 +11,7 @@
  *   E  survivors identified, dead removed                    (stable stream compaction)
  *   F  environment updated from the survivors' phenotypes   (exact integer reductions, counts)
  * plus migration between patches.  What the paper leaves open (RNG, samplers,
- * density regulation, ...) is fixed by the readings R1-R16 in DESIGN.md.
+ * density regulation, ...) is fixed by the readings R1-R19 in DESIGN.md.
  *
  * Conventions
  *   - Plain C, no exceptions.  Every call returns an int: 0 = SPEGG_OK, <0 = error code
@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SPEGG_ABI_VERSION 2u
+#define SPEGG_ABI_VERSION 3u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
        SPEGG_ESTATE = -5 };
@@ -91,6 +91,12 @@ typedef struct spegg_species_params {
                                    steps); the next generation is the staying adults, in order,
                                    then the surviving offspring, and M_t <= capacity - N_t.
                                    0 = discrete generations.  Unstructured species (1x1) only */
+    double mate_skew;           /* v_m: shared-preference mating (eq. S2-10,
+                                   PAPER.md:281-283): the father of each egg is drawn, among
+                                   the adults of the mother's patch, with probability
+                                   proportional to X_i^{v_m}, X_i = exp(z_i) (z_i the adult's
+                                   genetic value), by integer running sum + search (R19).
+                                   0 = uniform mate (R2).  |v_m| <= 1e6                      */
 } spegg_species_params;
 
 typedef struct spegg_params {
@@ -131,6 +137,9 @@ typedef struct spegg_debug_view {
     const uint32_t *d_cap;      /* [n_t] capture counts (SPEGG_FEC_CAPTURES species)          */
     const uint8_t *d_a_alive;   /* [n_t] adult stays alive (adult_survival > 0)               */
     const float *d_a_u, *d_a_s; /* [n_t] its uniform and survival probability                 */
+    const uint64_t *d_mate_cum; /* [n_t] inclusive running sum of the integer mating weights
+                                   (mate_skew != 0, R19)                                      */
+    float zbar_self;            /* the weights' reference: mean genetic value of the adults   */
 } spegg_debug_view;
 
 typedef struct spegg_sim spegg_sim;

@@ -18,7 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ERANGE, ESTATE = 0, -1, -2, -3, -4, -5
 FLAG_OVERFLOW, FLAG_EXTINCT = 1, 2
 
 
-ABI_VERSION = 2   # SPEGG_ABI_VERSION of include/spegg.h
+ABI_VERSION = 3   # SPEGG_ABI_VERSION of include/spegg.h
 
 
 class SpeciesParams(C.Structure):
@@ -33,6 +33,7 @@ class SpeciesParams(C.Structure):
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
+        ("mate_skew", C.c_double),
     ]
 
 
@@ -58,6 +59,7 @@ class DebugView(C.Structure):
         ("d_table_len", C.c_void_p), ("n_tables", C.c_uint32), ("theta_t", C.c_float),
         ("zbar_pred", C.c_float), ("attack_n", C.c_float), ("d_cap", C.c_void_p),
         ("d_a_alive", C.c_void_p), ("d_a_u", C.c_void_p), ("d_a_s", C.c_void_p),
+        ("d_mate_cum", C.c_void_p), ("zbar_self", C.c_float),
     ]
 
 
@@ -144,6 +146,7 @@ def make_params(cfg, debug=False, log_capacity=0):
         p.mu, p.mut_sd, p.pheno_scale = sp["mu"], sp.get("mut_sd", 0.0), sp["pheno_scale"]
         p.resid_sd = sp.get("resid_sd", 0.0)
         p.adult_survival = sp.get("adult_survival", 0.0)
+        p.mate_skew = sp.get("mate_skew", 0.0)
         p.fecundity_model, p.fec_a, p.K = _FEC[sp["fecundity"]], sp["fec_a"], sp["K"]
         if sp.get("K_patch") is not None:
             kp = np.ascontiguousarray(sp["K_patch"], dtype=np.float64)
@@ -318,5 +321,8 @@ class Sim:
             "cap": arr(v.d_cap, n, np.uint32),
             "a_alive": arr(v.d_a_alive, n, np.uint8), "a_u": arr(v.d_a_u, n, np.float32),
             "a_s": arr(v.d_a_s, n, np.float32),
+            "zbar_self": float(v.zbar_self),
+            "mate_cum": (arr(v.d_mate_cum, n, np.uint64) if self.cfg["species"][species].get("mate_skew", 0.0) != 0.0
+                         else np.zeros(0, np.uint64)),
         }
         return d

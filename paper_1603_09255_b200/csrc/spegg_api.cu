@@ -94,7 +94,7 @@ struct Carver {
 };
 
 struct SpeciesLayout {
-    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos,
+    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos, mate_cum, mate_tile,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
     uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, T_env, K_patch, theta_patch;
     uint32_t norm_len, env_len, n_tables, row_bytes;
@@ -148,6 +148,7 @@ int validate(const spegg_params *p) {
         if (q.capacity == 0 || q.capacity >= (1ull << 31)) return SPEGG_EINVAL;
         if (!(q.adult_survival >= 0.0 && q.adult_survival <= 1.0) || (q.adult_survival > 0.0 && P != 1)) return SPEGG_EINVAL;
         if (!(q.resid_sd >= 0.0) || !(q.pheno_scale > 0.0f) || q.resid_sd / (double)q.pheno_scale > 4096.0) return SPEGG_EINVAL;
+        if (!(std::fabs(q.mate_skew) <= 1e6)) return SPEGG_EINVAL;
         if (q.fecundity_model == SPEGG_FEC_CAPTURES && P != 1) return SPEGG_EINVAL;
         if (q.sel_predation) {
             if (q.predator_species >= p->n_species || q.predator_species <= s) return SPEGG_EINVAL;
@@ -201,6 +202,8 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         const uint64_t acap = q.adult_survival > 0.0 ? cap : 1;   // R18 arrays only when generations overlap
         l.a_alive = c.take(acap); l.a_u = c.take(acap * 4); l.a_s = c.take(acap * 4);
         l.a_zi = c.take(acap * 4); l.a_pos = c.take(acap * 4);
+        l.mate_cum = c.take((q.mate_skew != 0.0 ? cap : 1) * 8);      // R19 arrays only with weighted mating
+        l.mate_tile = c.take((q.mate_skew != 0.0 ? cap / MATE_TILE + 2 : 1) * 8);
         l.cap = c.take(cap * 4);
         l.offbuf = c.take(cap * l.row_bytes);
         l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
@@ -266,7 +269,7 @@ int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
 
 // true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
 bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
-    if (s->debug || s->P != 1 || !fused_bit_supported(h.k)) return false;
+    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.mate_v != 0.0f) return false;
     // the fused kernel tests u >= T as u > T - 1 (see spegg_fused.cuh): every threshold must be >= 1
     for (uint32_t c = 0; c < h.p.n_chrom; ++c)
         for (uint32_t k = 0; k < h.xover_len[c]; ++k)
@@ -307,6 +310,10 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             };
             const uint32_t g_thread = ctas(cap, 256, 8), g_warp = ctas(cap, 8, 8);   // thread / warp per offspring
             k_fec_scan<<<ctas(cap, SCAN_THREADS, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
+            if (k.mate_v != 0.0f) {   // R19: mating weights of the adults and their running sum
+                k_mate_weight<<<g_warp, 256, 0, s->stream>>>(k); ++nl;
+                k_mate_scan<<<ctas(cap, MATE_TILE, 8), 256, 0, s->stream>>>(k); ++nl;
+            }
             k_scalar<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             // production q10 path: vectorised gamete kernel that also takes the phenotype (debug keeps
@@ -495,6 +502,8 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.adult_surv = (float)q.adult_survival;
         k.a_alive = at<uint8_t>(s, l.a_alive); k.a_u = at<float>(s, l.a_u); k.a_s = at<float>(s, l.a_s);
         k.a_zi = at<int32_t>(s, l.a_zi); k.a_pos = at<uint32_t>(s, l.a_pos);
+        k.mate_v = (float)q.mate_skew;
+        k.mate_cum = at<unsigned long long>(s, l.mate_cum); k.mate_tile = at<unsigned long long>(s, l.mate_tile);
         k.cap = at<uint32_t>(s, l.cap);
         k.tables = at<uint32_t>(s, l.tables); k.table_len = at<uint32_t>(s, l.table_len);
         k.status_fec = at<unsigned long long>(s, l.status_fec); k.status_cmp = at<unsigned long long>(s, l.status_cmp);
@@ -661,6 +670,7 @@ int spegg_read_debug(spegg_sim *s, uint32_t species, spegg_debug_view *o) {
     o->theta_t = st.theta_t; o->zbar_pred = st.zbar_pred; o->attack_n = st.attack_n;
     o->d_cap = k.cap;
     o->d_a_alive = k.a_alive; o->d_a_u = k.a_u; o->d_a_s = k.a_s;
+    o->d_mate_cum = (const uint64_t *)k.mate_cum; o->zbar_self = st.zbar_self;
     return SPEGG_OK;
 }
 

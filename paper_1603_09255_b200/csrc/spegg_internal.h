@@ -13,6 +13,7 @@ constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 4;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 constexpr int MAX_SPECIES = 8;
+constexpr uint32_t MATE_TILE = 1024;             // R19: adults per tile of the mating-weight running sum
 constexpr uint32_t FUSED_RANGE = 1024;            // fused path: rows per scan range (32 slabs of 32 rows)
 
 // Device-resident per-species state: counts never leave the GPU between steps.
@@ -30,7 +31,7 @@ struct DevSpecies {
     long long sum_zi0;     // snapshot at the start of the step
     long long acc_zi, acc_zi2;  // accumulators of the current step's survivors
     unsigned long long captures, near_ties;
-    float theta_t, zbar_pred, attack_n;
+    float theta_t, zbar_pred, attack_n, zbar_self;
     uint32_t n_pred0;      // predator count snapshot used by this step
     // work tickets of the step kernels, each on a cache line of its own: hundreds of CTAs draw from
     // them at the same moment, and same-line atomics are served one after the other by L2
@@ -101,6 +102,10 @@ struct SpK {
     float *a_u, *a_s;           // its uniform and survival probability
     int32_t *a_zi;              // its integer genetic value
     uint32_t *a_pos;            // its position in the next generation (0xFFFFFFFF: dies)
+    // R19, shared-preference mating (mate_v != 0): integer mating weights of the current adults
+    float mate_v;               // v_m as fp32; 0 = uniform mate (R2)
+    unsigned long long *mate_cum;   // [n] inclusive running sum of the weights, adult order
+    unsigned long long *mate_tile;  // [n / MATE_TILE + 2] weight of each tile of MATE_TILE adults
     uint32_t *cap;              // capture counts of THIS species' adults (CAPTURES model)
     uint32_t *cap_pred;         // capture counts of the predator species (predation term)
     uint32_t *tables, *table_len;

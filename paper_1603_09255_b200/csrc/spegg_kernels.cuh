@@ -152,6 +152,8 @@ __device__ __forceinline__ void prepare_species(const SpK &sp, uint32_t g, uint3
     for (uint32_t i = g; i < nc; i += stride) sp.status_cmp[i] = 0ull;
     if (sp.fec_model == 2)
         for (uint32_t i = g; i < sp.capacity; i += stride) sp.cap[i] = 0u;
+    if (sp.mate_v != 0.0f)   // R19: tile totals of the mating weights are accumulated with atomics
+        for (uint32_t i = g; i < sp.capacity / MATE_TILE + 2u; i += stride) sp.mate_tile[i] = 0ull;
     if (sp.phys_parents) {  // fused path: the coming step counts its survivors per range of the other buffer
         uint32_t *cnt_next = sp.range_cnt[cur ^ 1u];
         const uint32_t n_max = (sp.capacity + 31u) / 32u * 32u / FUSED_RANGE + 2u;
@@ -330,6 +332,73 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
     }
 }
 
+__device__ __forceinline__ int32_t warp_row_zi(const SpK &sp, const uint8_t *row);
+
+// R19 ("shared preference"; eq. S2-10): integer mating weight of every
+// adult, w_i = trunc(expf_spec(clamp(v (z_i - zbar), -16, 16) - 16) * 2^40), fp32 in this order, zbar the
+// adults' mean genetic value (fp64 sum / N * scale rounded to fp32, as zbar_C of R14).  One warp per
+// adult (the genetic value is re-read from its row); the raw weight goes to mate_cum[i] and is added
+// to its tile's total (integer atomics: exact in any order).
+__global__ void __launch_bounds__(256) k_mate_weight(const __grid_constant__ SpK sp) {
+    DevSpecies &st = *sp.st;
+    const uint32_t N = st.n0, lane = threadIdx.x & 31u;
+    const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    const uint8_t *pop = sp.pop[st.cur];
+    const uint32_t *rowptr = sp.rowptr[st.cur];
+    const float zbar = N ? __double2float_rn(__dmul_rn(__ddiv_rn((double)st.sum_zi0, (double)N), (double)sp.pheno_scale)) : 0.0f;
+    if (warp0 == 0 && lane == 0) st.zbar_self = zbar;
+    for (uint32_t i = warp0; i < N; i += nw) {
+        const int32_t zi = warp_row_zi(sp, pop + (size_t)rowptr[i] * sp.row_bytes);
+        if (lane == 0) {
+            const float d = __fsub_rn(__fmul_rn((float)zi, sp.pheno_scale), zbar);
+            float e = __fmul_rn(sp.mate_v, d);
+            e = fminf(fmaxf(e, -16.0f), 16.0f);
+            const float w = expf_spec(__fsub_rn(e, 16.0f));
+            const unsigned long long wi = (unsigned long long)__fmul_rn(w, 0x1p40f);
+            sp.mate_cum[i] = wi;
+            if (wi) atomicAdd(&sp.mate_tile[i / MATE_TILE], wi);
+        }
+    }
+}
+
+// R19: inclusive running sum of the weights in adult order.  One CTA per tile of MATE_TILE adults:
+// the tile's base is the sum of the tile totals before it (every CTA adds them up itself -- a few
+// thousand L2-resident words, no chain between CTAs), then a block scan of 4 adults per thread.
+__global__ void __launch_bounds__(256) k_mate_scan(const __grid_constant__ SpK sp) {
+    __shared__ unsigned long long s_red[8];
+    __shared__ unsigned long long s_base;
+    const uint32_t N = sp.st->n0, tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t n_tiles = (N + MATE_TILE - 1) / MATE_TILE;
+    for (uint32_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        unsigned long long b = 0;
+        for (uint32_t k = tid; k < t; k += 256) b += sp.mate_tile[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) b += __shfl_xor_sync(0xffffffffu, b, o);
+        if (lane == 0) s_red[warp] = b;
+        __syncthreads();
+        if (tid == 0) { unsigned long long a = 0; for (int k = 0; k < 8; ++k) a += s_red[k]; s_base = a; }
+        __syncthreads();
+        const uint32_t i0 = t * MATE_TILE + tid * 4;
+        unsigned long long w[4], sum = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { w[k] = (i0 + k < N) ? sp.mate_cum[i0 + k] : 0ull; sum += w[k]; w[k] = sum; }
+        unsigned long long incl = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= (uint32_t)o) incl += v;
+        }
+        __syncthreads();                       // s_red is reused
+        if (lane == 31) s_red[warp] = incl;
+        __syncthreads();
+        unsigned long long excl = s_base + (incl - sum);
+        for (uint32_t k = 0; k < warp; ++k) excl += s_red[k];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) if (i0 + k < N) sp.mate_cum[i0 + k] = excl + w[k];
+        __syncthreads();
+    }
+}
+
 // a3: scalar draws of each offspring: father (R2), dispersal (R15), survival uniform (R4)
 __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) {
     const DevSpecies &st = *sp.st;
@@ -341,7 +410,27 @@ __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) 
         draw(sp.key, sp.species, ST_SCALAR, j, 0, step, x);
         uint32_t pm = 0, base = 0, np = N;
         if (sp.P > 1) { pm = patch_of(ps, sp.P, mo); base = ps[pm]; np = ps[pm + 1] - base; }
-        sp.father[j] = base + uniform_index(x[0], np);
+        uint32_t fa = base + uniform_index(x[0], np);
+        if (sp.mate_v != 0.0f) {
+            // R19: weighted draw among the adults of the mother's patch: 64-bit uniform from words 2,3 of
+            // SCALAR block 1, target = floor(u * total / 2^64), father = first adult of the patch whose
+            // inclusive running sum exceeds (sum before the patch) + target; total 0 keeps the uniform mate
+            const unsigned long long before = base ? sp.mate_cum[base - 1] : 0ull;
+            const unsigned long long total = sp.mate_cum[base + np - 1] - before;
+            if (total) {
+                uint32_t y[4];
+                draw_rk(sp, ST_SCALAR, j, 1, step, y);
+                const unsigned long long u = ((unsigned long long)y[2] << 32) | y[3];
+                const unsigned long long target = before + __umul64hi(u, total);
+                uint32_t lo = base, hi = base + np - 1;   // first index with mate_cum > target; exists since target < before + total
+                while (lo < hi) {
+                    const uint32_t mid = (lo + hi) >> 1;
+                    if (sp.mate_cum[mid] > target) hi = mid; else lo = mid + 1;
+                }
+                fa = lo;
+            }
+        }
+        sp.father[j] = fa;
         uint32_t dest = pm;
         if (sp.P > 1 && (unsigned long long)x[1] < sp.T_mig) dest = neighbour(pm, x[2] >> 30, sp.grid_w, sp.grid_h);
         sp.dest[j] = dest;

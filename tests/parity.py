@@ -36,6 +36,11 @@ def assert_debug_equal(dg, do, species_cfg, tag=""):
         assert np.array_equal(dg["a_s"].view(np.uint32), do["a_s"].view(np.uint32)), (tag, "a_s")
 
 
+    if species_cfg.get("mate_skew", 0.0) != 0.0:        # R19: the integer mating weights' running sum
+        assert np.float32(dg["zbar_self"]) == np.float32(do["zbar_self"]), (tag, "zbar_self")
+        assert np.array_equal(dg["mate_cum"], do["mate_cum"]), (tag, "mate_cum")
+
+
 def assert_state_equal(sim, orc, cfg, tag=""):
     for s in range(len(cfg["species"])):
         rg, pg, zg = sim.read_state(s)

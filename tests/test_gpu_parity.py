@@ -269,3 +269,45 @@ def test_overlapping_generations_room_for_offspring(oracle_mod, binding):
     sp.update(adult_survival=0.9, K=1e9, capacity=2048)
     parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=True)
     parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+
+
+@pytest.mark.parametrize("which,scale,v,grid,extra", [
+    (1, 1.0, 2.0, None, {}),                        # C1, strong preference
+    (2, 0.06, 1.0, None, {}),                       # C2: 6,000 adults = several weight tiles and a ragged tail
+    (2, 0.04, -3.0, None, {"resid_sd": 0.2}),       # preference for small mates, with residual noise (same SCALAR block)
+    (3, 0.012, 0.5, None, {}),                      # bit genome: leaves the fused kernel for the general pipeline
+    (5, 0.03, 1.5, (5, 4), {}),                     # patches: the father comes from the mother's patch
+    (2, 0.04, 1.0, None, {"adult_survival": 0.6}),  # with overlapping generations
+    (1, 1.0, 400.0, None, {}),                      # clamp in play, most integer weights are 0
+])
+def test_shared_preference_mating(oracle_mod, binding, which, scale, v, grid, extra):
+    """R19 (eq. S2-10): the father is drawn with probability
+    proportional to exp(v_m z) by integer running sum + search.  Per-step parity of every
+    intermediate including the running sum (debug), then a free-running trajectory on the
+    production kernels."""
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    sp = cfg["species"][0]
+    sp["mate_skew"] = v
+    sp.update(extra)
+    if "adult_survival" in extra:
+        sp["capacity"] = 4 * sp["capacity"]
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(2):
+        orc.step(5)
+        sim.step(5)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+        parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags
+    sim.close()
+
+
+def test_shared_preference_mating_full_size(oracle_mod, binding):
+    """R19 at C2's full size (100,000 adults, ~100 weight tiles) on the production kernels: one step
+    from the oracle's state, fathers compared through the offspring that survive (state + log)."""
+    cfg = workloads.config(2)
+    cfg["species"][0]["mate_skew"] = 1.0
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
