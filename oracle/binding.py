@@ -44,7 +44,7 @@ class _SpeciesParams(C.Structure):
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
-        ("mate_skew", C.c_double),
+        ("mate_skew", C.c_double), ("encounters", C.c_uint32),
     ]
 
 
@@ -226,6 +226,7 @@ class Oracle:
                 p.sel_predation = 1
                 p.attack = pr["attack"]
                 p.predator_species = pr["predator"]
+                p.encounters = pr.get("encounters", 0)
             p.migration = sp.get("migration", 0.0)
             p.capacity = sp["capacity"]
             p.resid_sd = sp.get("resid_sd", 0.0)

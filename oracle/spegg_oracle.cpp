@@ -522,7 +522,29 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         /* ---- a6: selection (Fig. 1D), fp32 in this order (R11, R14) ---- */
         float s = 1.0f;
         bool captured = false;
-        if (S.p.sel_predation) {
+        int met = -1; /* R20: the consumer that captured this newborn */
+        if (S.p.sel_predation && S.p.encounters > 0) {
+            /* R20 ("for a given individual of either species we instead simulate a random
+             * subset of possible encounters"; eq. S3-2): meeting k = 0..E-1, in order, until
+             * the first capture: consumer i_k uniform over the N_C consumers (word 2(k%2) of SCALAR block
+             * 2 + k/2), matching m = e/(1+e), e = expf_spec(-(d*d)), d = z - z_{i_k} (the consumer's genetic
+             * value), capture probability p = v * m (v = fp32(attack)), captured iff u01(word 2(k%2)+1) < p.
+             * fp32, this order.  The stabilising term below is separate: alive iff not captured and u01 < s. */
+            const float v = (float)S.p.attack;
+            for (uint32_t k = 0; k < S.p.encounters && NC && !captured; ++k) {
+                uint32_t y[4];
+                draw(sim.seed, si, SCALAR, (uint32_t)j, 2 + k / 2, t, y);
+                const uint32_t ik = uniform_index(y[2 * (k & 1)], (uint32_t)NC);
+                const float zc = (float)pred->zi[ik] * pred->p.pheno_scale;
+                const float d = z - zc;
+                const float e = expf_spec(-(d * d));
+                const float m = e / (1.0f + e);
+                const float p = v * m;
+                const float u = u01_of(y[2 * (k & 1) + 1]);
+                if (std::fabs(u - p) < 1e-6f) le.near_ties++;
+                if (u < p) { captured = true; met = (int)ik; }
+            }
+        } else if (S.p.sel_predation) {
             float d = z - D.zbar_pred;
             float g = expf_spec(-(0.5f * (d * d)));
             float sp = expf_spec(-(D.attack_n * g));
@@ -534,15 +556,16 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
             float d = z - th;
             float sq = d * d;
             float ss = expf_spec(-(sq * S.sel_c));
-            s = S.p.sel_predation ? s * ss : ss;
+            s = (S.p.sel_predation && S.p.encounters == 0) ? s * ss : ss;
         }
         D.s[j] = s;
-        D.alive[j] = (D.u01[j] < s) ? 1 : 0;
+        D.alive[j] = (D.u01[j] < s && !(captured && S.p.encounters > 0)) ? 1 : 0;
         if (std::fabs(D.u01[j] - s) < 1e-6f) le.near_ties++;
         if (captured) {
             D.captured[j] = 1;
             le.captures++;
-            if (NC) { /* credit a uniformly drawn predator (SCALAR block 1 word 0) */
+            if (met >= 0) pred->cap[met] += 1; /* R20: the consumer met */
+            else if (NC) { /* credit a uniformly drawn predator (SCALAR block 1 word 0) */
                 uint32_t y[4];
                 draw(sim.seed, si, SCALAR, (uint32_t)j, 1, t, y);
                 pred->cap[uniform_index(y[0], (uint32_t)NC)] += 1;
@@ -685,6 +708,7 @@ orc_sim *orc_create(const orc_params *p) {
             if (S.R_norm < 0) { delete sim; return nullptr; }
         }
         if (!(std::fabs(S.p.mate_skew) <= 1e6)) { delete sim; return nullptr; }
+        if (S.p.encounters > 16 || (S.p.encounters && (!S.p.sel_predation || !(S.p.attack >= 0.0 && S.p.attack <= 2.0)))) { delete sim; return nullptr; }
         /* R18 is defined for an unstructured species (one patch) */
         if (!(S.p.adult_survival >= 0.0 && S.p.adult_survival <= 1.0) || (S.p.adult_survival > 0.0 && sim->P != 1)) { delete sim; return nullptr; }
         if (S.p.resid_sd > 0.0) {

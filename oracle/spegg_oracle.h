@@ -56,6 +56,12 @@ typedef struct {
                                    the father of each egg is drawn with probability proportional to
                                    X_i^{v_m}, X_i = exp(z_i) the adult's size, v_m = mate_skew;
                                    0 = uniform mate (R2)                              */
+    uint32_t encounters;        /* R20: individual-level interspecific encounters (eq. S3-2,
+                                   PAPER.md:464): with sel_predation, each newborn meets this many
+                                   randomly drawn individuals of predator_species; at each meeting it is
+                                   captured with probability attack * e/(1+e), e = exp(-(x - delta)^2),
+                                   x the consumer's and delta its own trait; the capture is credited to
+                                   the consumer met.  0 = the mean-field term of R14.  <= 16      */
 } orc_species_params;
 
 typedef struct {
