@@ -11,7 +11,7 @@
  *   E  survivors identified, dead removed                    (stable stream compaction)
  *   F  environment updated from the survivors' phenotypes   (exact integer reductions, counts)
  * plus migration between patches.  What the paper leaves open (RNG, samplers,
- * density regulation, ...) is fixed by the readings R1-R19 in DESIGN.md.
+ * density regulation, ...) is fixed by the readings R1-R20 in DESIGN.md.
  *
  * Conventions
  *   - Plain C, no exceptions.  Every call returns an int: 0 = SPEGG_OK, <0 = error code
@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SPEGG_ABI_VERSION 3u
+#define SPEGG_ABI_VERSION 4u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
        SPEGG_ESTATE = -5 };
@@ -97,6 +97,14 @@ typedef struct spegg_species_params {
                                    proportional to X_i^{v_m}, X_i = exp(z_i) (z_i the adult's
                                    genetic value), by integer running sum + search (R19).
                                    0 = uniform mate (R2).  |v_m| <= 1e6                      */
+    uint32_t encounters;        /* E: individual-level interspecific encounters (
+                                   eq. S3-2; R20).  With sel_predation, each
+                                   newborn meets E uniformly drawn adults of predator_species,
+                                   in order, until the first capture; a meeting captures with
+                                   probability attack * e/(1+e), e = exp(-(x - delta)^2), x the
+                                   consumer's and delta the newborn's trait (attack <= 2), and
+                                   the capture is credited to the consumer met.  0 = the
+                                   mean-field term of R14.  E <= 16                          */
 } spegg_species_params;
 
 typedef struct spegg_params {

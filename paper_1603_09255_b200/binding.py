@@ -18,7 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ERANGE, ESTATE = 0, -1, -2, -3, -4, -5
 FLAG_OVERFLOW, FLAG_EXTINCT = 1, 2
 
 
-ABI_VERSION = 3   # SPEGG_ABI_VERSION of include/spegg.h
+ABI_VERSION = 4   # SPEGG_ABI_VERSION of include/spegg.h
 
 
 class SpeciesParams(C.Structure):
@@ -33,7 +33,7 @@ class SpeciesParams(C.Structure):
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
-        ("mate_skew", C.c_double),
+        ("mate_skew", C.c_double), ("encounters", C.c_uint32),
     ]
 
 
@@ -165,6 +165,7 @@ def make_params(cfg, debug=False, log_capacity=0):
         pr = sp.get("predation")
         if pr is not None:
             p.sel_predation, p.attack, p.predator_species = 1, pr["attack"], pr["predator"]
+            p.encounters = pr.get("encounters", 0)
         p.migration, p.capacity = sp.get("migration", 0.0), sp["capacity"]
     keep.append(arr)
     prm = Params(C.sizeof(Params), ABI_VERSION, cfg["seed"], ns, w, h, 1 if debug else 0, log_capacity, 0, arr)

@@ -94,7 +94,7 @@ struct Carver {
 };
 
 struct SpeciesLayout {
-    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos, mate_cum, mate_tile,
+    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos, mate_cum, mate_tile, enc_zi,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
     uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, T_env, K_patch, theta_patch;
     uint32_t norm_len, env_len, n_tables, row_bytes;
@@ -154,7 +154,8 @@ int validate(const spegg_params *p) {
             if (q.predator_species >= p->n_species || q.predator_species <= s) return SPEGG_EINVAL;
             if (p->species[q.predator_species].fecundity_model != SPEGG_FEC_CAPTURES) return SPEGG_EINVAL;
             if (!(q.attack >= 0.0)) return SPEGG_EINVAL;
-        }
+            if (q.encounters > 16 || (q.encounters && !(q.attack <= 2.0))) return SPEGG_EINVAL;
+        } else if (q.encounters) return SPEGG_EINVAL;
     }
     return SPEGG_OK;
 }
@@ -204,6 +205,10 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.a_zi = c.take(acap * 4); l.a_pos = c.take(acap * 4);
         l.mate_cum = c.take((q.mate_skew != 0.0 ? cap : 1) * 8);      // R19 arrays only with weighted mating
         l.mate_tile = c.take((q.mate_skew != 0.0 ? cap / MATE_TILE + 2 : 1) * 8);
+        bool is_met = false;   // R20: some species meets this one individually
+        for (uint32_t o = 0; o < p->n_species; ++o)
+            if (p->species[o].sel_predation && p->species[o].encounters && p->species[o].predator_species == s) is_met = true;
+        l.enc_zi = c.take((is_met ? cap : 1) * 4);
         l.cap = c.take(cap * 4);
         l.offbuf = c.take(cap * l.row_bytes);
         l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
@@ -326,6 +331,10 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
             k_mutate<<<ctas(cap * 2, 256, 8), 256, 0, s->stream>>>(k, q10v ? 1 : 0); ++nl;
             if (!q10v) { k_phenotype<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }
+            if (k.enc_E) {   // R20: genetic values of the consumers this species' newborns meet
+                const SpK &kp = s->sp[h.p.predator_species].k;
+                k_enc_zi<<<ctas(kp.capacity, 8, 8), 256, 0, s->stream>>>(kp); ++nl;
+            }
             k_survival<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
             if (k.adult_surv > 0.0f) { k_adult_survive<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }   // R18
             if (s->P == 1) {
@@ -504,6 +513,8 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.a_zi = at<int32_t>(s, l.a_zi); k.a_pos = at<uint32_t>(s, l.a_pos);
         k.mate_v = (float)q.mate_skew;
         k.mate_cum = at<unsigned long long>(s, l.mate_cum); k.mate_tile = at<unsigned long long>(s, l.mate_tile);
+        k.enc_E = q.sel_predation ? q.encounters : 0u; k.enc_v = (float)q.attack;
+        k.enc_zi = at<int32_t>(s, l.enc_zi);
         k.cap = at<uint32_t>(s, l.cap);
         k.tables = at<uint32_t>(s, l.tables); k.table_len = at<uint32_t>(s, l.table_len);
         k.status_fec = at<unsigned long long>(s, l.status_fec); k.status_cmp = at<unsigned long long>(s, l.status_cmp);
@@ -526,7 +537,10 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         s->scan_ctas = (uint32_t)n;
     }
     for (uint32_t si = 0; si < p->n_species; ++si)
-        if (s->sp[si].p.sel_predation) s->sp[si].k.cap_pred = s->sp[s->sp[si].p.predator_species].k.cap;
+        if (s->sp[si].p.sel_predation) {
+            s->sp[si].k.cap_pred = s->sp[s->sp[si].p.predator_species].k.cap;
+            s->sp[si].k.pred_zi = s->sp[s->sp[si].p.predator_species].k.enc_zi;
+        }
 
     for (uint32_t si = 0; si < p->n_species; ++si)
         if (cudaMemcpyAsync(s->d_spk + si, &s->sp[si].k, sizeof(SpK), cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return fail(SPEGG_ECUDA);

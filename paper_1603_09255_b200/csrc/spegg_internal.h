@@ -106,6 +106,11 @@ struct SpK {
     float mate_v;               // v_m as fp32; 0 = uniform mate (R2)
     unsigned long long *mate_cum;   // [n] inclusive running sum of the weights, adult order
     unsigned long long *mate_tile;  // [n / MATE_TILE + 2] weight of each tile of MATE_TILE adults
+    // R20, individual-level encounters (enc_E > 0 on the prey; enc_zi filled on the species it meets)
+    uint32_t enc_E;             // meetings per newborn; 0 = mean-field predation term (R14)
+    float enc_v;                // v = fp32(attack)
+    int32_t *enc_zi;            // [n] integer genetic values of THIS species' adults (when another species meets them)
+    const int32_t *pred_zi;     // enc_zi of the predator species
     uint32_t *cap;              // capture counts of THIS species' adults (CAPTURES model)
     uint32_t *cap_pred;         // capture counts of the predator species (predation term)
     uint32_t *tables, *table_len;

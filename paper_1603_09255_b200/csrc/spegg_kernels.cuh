@@ -705,6 +705,16 @@ __global__ void __launch_bounds__(256) k_adult_zi(const __grid_constant__ SpK sp
         atomicAdd((unsigned long long *)&sp.st->sum_zi, (unsigned long long)acc);
 }
 
+// R20: integer genetic values of this species' current adults, for the species that meets them
+__global__ void __launch_bounds__(256) k_enc_zi(const __grid_constant__ SpK sp) {
+    const uint32_t N = sp.st->n0, cur = sp.st->cur;
+    const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t i = warp0; i < N; i += nw) {
+        const int32_t zi = warp_row_zi(sp, sp.pop[cur] + (size_t)sp.rowptr[cur][i] * sp.row_bytes);
+        if ((threadIdx.x & 31u) == 0) sp.enc_zi[i] = zi;
+    }
+}
+
 // rowptr = identity for a freshly written, dense population
 __global__ void __launch_bounds__(256) k_iota(uint32_t *p, uint32_t n) {
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = i;
@@ -738,14 +748,41 @@ __global__ void __launch_bounds__(256) k_survival(const __grid_constant__ SpK sp
         const float u = sp.u01[j];
         const float theta = sp.theta_patch ? sp.theta_patch[sp.dest[j]] : st.theta_t;
         bool captured;
-        const float s = survival_prob(sp, z, theta, u, captured);
+        float s;
+        uint32_t met = 0xFFFFFFFFu;
+        if (sp.enc_E) {
+            // R20 (eq. S3-2): meeting k = 0..E-1 until the first capture: consumer
+            // i_k uniform (word 2(k%2) of SCALAR block 2 + k/2), m = e/(1+e), e = expf_spec(-(d*d)),
+            // d = z - z_{i_k}; captured iff u01(word 2(k%2)+1) < v*m.  The stabilising term stays separate.
+            captured = false;
+            const uint32_t NC = st.n_pred0;
+            uint32_t y[4];
+            for (uint32_t k = 0; k < sp.enc_E && NC && !captured; ++k) {
+                if ((k & 1u) == 0) draw_rk(sp, ST_SCALAR, j, 2 + (k >> 1), step, y);
+                const uint32_t ik = uniform_index(y[2 * (k & 1u)], NC);
+                const float d = __fsub_rn(z, __fmul_rn((float)sp.pred_zi[ik], sp.pred_scale));
+                const float e = expf_spec(-__fmul_rn(d, d));
+                const float p = __fmul_rn(sp.enc_v, __fdiv_rn(e, __fadd_rn(1.0f, e)));
+                const float uk = u01_of(y[2 * (k & 1u) + 1]);
+                if (fabsf(__fsub_rn(uk, p)) < 1e-6f) ++ties;
+                if (uk < p) { captured = true; met = ik; }
+            }
+            s = 1.0f;
+            if (sp.sel_gaussian) {
+                const float d = __fsub_rn(z, theta);
+                s = expf_spec(-__fmul_rn(__fmul_rn(d, d), sp.sel_c));
+            }
+        } else {
+            s = survival_prob(sp, z, theta, u, captured);
+        }
         sp.s[j] = s;
-        sp.alive[j] = (u < s) ? 1 : 0;
+        sp.alive[j] = (u < s && met == 0xFFFFFFFFu) ? 1 : 0;
         sp.captured[j] = captured ? 1 : 0;
         if (fabsf(__fsub_rn(u, s)) < 1e-6f) ++ties;
         if (captured) {
             ++caps;
-            if (st.n_pred0) {
+            if (met != 0xFFFFFFFFu) atomicAdd(&sp.cap_pred[met], 1u);
+            else if (st.n_pred0) {
                 uint32_t y[4];
                 draw(sp.key, sp.species, ST_SCALAR, j, 1, step, y);
                 atomicAdd(&sp.cap_pred[uniform_index(y[0], st.n_pred0)], 1u);

@@ -311,3 +311,34 @@ def test_shared_preference_mating_full_size(oracle_mod, binding):
     cfg = workloads.config(2)
     cfg["species"][0]["mate_skew"] = 1.0
     parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+
+
+@pytest.mark.parametrize("scale,E,v,extra", [
+    (0.004, 3, 0.15, {}),                     # C4 shape: 4,000 prey, 400 consumers, three meetings each
+    (0.004, 1, 0.4, {}),                      # one meeting, strong
+    (0.004, 1, 1.0, {}),                      # so strong that the consumers overshoot and go extinct at step 2
+    (0.003, 16, 0.05, {}),                    # the maximum: eight SCALAR blocks per newborn
+    (0.004, 4, 0.3, {"resid_sd": 0.5}),       # with residual phenotype noise on the newborn's trait
+    (0.004, 2, 2.0, {"mate_skew": 1.0}),      # with weighted fathers (both use later SCALAR blocks)
+])
+def test_individual_encounters(oracle_mod, binding, scale, E, v, extra):
+    """R20 (PAPER.md:475; eq. S3-2, PAPER.md:464): each newborn meets E uniformly drawn consumers;
+    captures are credited to the consumer met.  Per-step parity of every intermediate of both
+    species (debug), then a free-running trajectory on the production kernels."""
+    cfg = workloads.config(4, scale=scale)
+    cfg["species"][0]["predation"].update(encounters=E, attack=v)
+    cfg["species"][0].update(extra)
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(2):
+        orc.step(6)
+        sim.step(6)
+        for s in range(2):
+            parity.assert_logs_equal(sim.read_log(s), orc.log(s), tag="species %d" % s)
+        parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags
+    assert sum(e["captures"] for e in orc.log(0)) > 0
+    sim.close()
