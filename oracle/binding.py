@@ -44,7 +44,7 @@ class _SpeciesParams(C.Structure):
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
-        ("mate_skew", C.c_double), ("encounters", C.c_uint32),
+        ("mate_skew", C.c_double), ("encounters", C.c_uint32), ("separate_sexes", C.c_uint32),
     ]
 
 
@@ -72,6 +72,7 @@ class _DebugView(C.Structure):
         ("attack_n", C.c_float), ("cap", C.POINTER(C.c_uint32)),
         ("a_alive", C.POINTER(C.c_uint8)), ("a_u", C.POINTER(C.c_float)), ("a_s", C.POINTER(C.c_float)),
         ("mate_cum", C.POINTER(C.c_uint64)), ("zbar_self", C.c_float),
+        ("sex_off", C.POINTER(C.c_uint8)),
     ]
 
 
@@ -88,6 +89,8 @@ def lib():
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_write_state.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p, C.c_void_p, C.c_uint32]
         L.orc_step.argtypes = [C.c_void_p, C.c_uint32]
+        L.orc_write_sex.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p]
+        L.orc_read_sex.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p]
         L.orc_n.restype = C.c_uint64
         L.orc_n.argtypes = [C.c_void_p, C.c_uint32]
         L.orc_step_counter.restype = C.c_uint32
@@ -232,6 +235,7 @@ class Oracle:
             p.resid_sd = sp.get("resid_sd", 0.0)
             p.adult_survival = sp.get("adult_survival", 0.0)
             p.mate_skew = sp.get("mate_skew", 0.0)
+            p.separate_sexes = 1 if sp.get("separate_sexes") else 0
             if sp["kind"] == "bit":
                 self.row_shape.append(2 * (L // 32))
                 self.row_dtype.append(np.uint32)
@@ -259,6 +263,16 @@ class Oracle:
                                    ps.ctypes.data if ps is not None else None, step)
         if rc != 0:
             raise ValueError("orc_write_state failed")
+
+    def write_sex(self, species, sex):
+        sex = np.ascontiguousarray(sex, dtype=np.uint8)
+        if lib().orc_write_sex(self._h, species, sex.shape[0], sex.ctypes.data) != 0:
+            raise ValueError("orc_write_sex failed")
+
+    def read_sex(self, species=0):
+        out = np.zeros(self.n(species), dtype=np.uint8)
+        lib().orc_read_sex(self._h, species, out.ctypes.data)
+        return out
 
     def step(self, n=1):
         lib().orc_step(self._h, n)
@@ -317,8 +331,10 @@ class Oracle:
             "a_alive": arr(v.a_alive, n, np.uint8), "a_u": arr(v.a_u, n, np.float32), "a_s": arr(v.a_s, n, np.float32),
             "theta_t": float(v.theta_t), "zbar_pred": float(v.zbar_pred), "attack_n": float(v.attack_n),
             "zbar_self": float(v.zbar_self),
-            "mate_cum": (arr(v.mate_cum, n, np.uint64) if self.cfg["species"][species].get("mate_skew", 0.0) != 0.0
-                         else np.zeros(0, np.uint64)),
+            "mate_cum": (arr(v.mate_cum, n, np.uint64)
+                         if (self.cfg["species"][species].get("mate_skew", 0.0) != 0.0
+                             or self.cfg["species"][species].get("separate_sexes")) else np.zeros(0, np.uint64)),
+            "sex_off": arr(v.sex_off, m, np.uint8),
         }
         nt = int(v.n_tables)
         d["table_len"] = arr(v.table_len, nt, np.uint32)

@@ -175,7 +175,7 @@ const int ENV_CAP = 65536;   /* R17: residual-noise table, sd up to 4096 phenoty
 
 struct SpeciesDebug {
     uint64_t n_t = 0, m_t = 0;
-    std::vector<uint8_t> f, alive, captured, a_alive;
+    std::vector<uint8_t> f, alive, captured, a_alive, sex_off;
     std::vector<uint32_t> off, mother, father, dest, tables, table_len, cap;
     std::vector<float> u01, s, z, a_u, a_s;
     std::vector<uint64_t> mate_cum; /* R19 */
@@ -207,6 +207,7 @@ struct Species {
     std::vector<int16_t> q;
     std::vector<uint32_t> patch_start;
     std::vector<int32_t> zi;
+    std::vector<uint8_t> sex;   /* R21: 1 = male; all 0 without separate sexes */
     std::vector<uint32_t> cap;
     std::vector<orc_log_entry> log;
     SpeciesDebug dbg;
@@ -398,7 +399,11 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
      *      spec'd expf (x <= 0) serves: fp32, this order: d = z_i - zbar; e = v*d; e = min(max(e,-16),16);
      *      x = e - 16; w = expf_spec(x); integer weight = trunc(w * 2^40) (exact scaling).  mate_cum is
      *      the inclusive running sum in adult order (uint64, no rounding anywhere). ---- */
-    if (S.p.mate_skew != 0.0) {
+    /* R21 (eqs. S2-9/S2-10): with separate sexes only males father eggs: a
+     * female's mating weight is 0, a male's is the weight above (with v_m = 0 every male weighs
+     * trunc(expf_spec(-16) * 2^40), i.e. the father is uniform over the males of the patch). */
+    const bool mate_on = S.p.mate_skew != 0.0 || S.p.separate_sexes;
+    if (mate_on) {
         const float v = (float)S.p.mate_skew;
         D.zbar_self = (float)(((double)sumzi0[si] / (double)N) * (double)S.p.pheno_scale);
         D.mate_cum.resize(N);
@@ -410,7 +415,7 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
             e = std::min(std::max(e, -16.0f), 16.0f);
             const float x = e - 16.0f;
             const float w = expf_spec(x);
-            run += (uint64_t)(w * 0x1p40f);
+            if (!S.p.separate_sexes || S.sex[i]) run += (uint64_t)(w * 0x1p40f);
             D.mate_cum[i] = run;
         }
     }
@@ -425,6 +430,7 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         if (S.p.fecundity_model == ORC_FEC_CAPTURES) tab = std::min<uint32_t>(S.cap[i], ORC_CAP_TABLES - 1);
         else tab = patch_of(S, P, i);
         D.f[i] = (uint8_t)poisson_count(&D.tables[(size_t)tab * ORC_TMAX], (int)D.table_len[tab], x[0]);
+        if (S.p.separate_sexes && S.sex[i]) D.f[i] = 0; /* R21: males lay no eggs (the draw is made and ignored) */
     }
     /* ---- a2: exclusive scan ---- */
     uint64_t M = 0;
@@ -442,7 +448,7 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
     /* ---- a3: parent assignment (Fig. 1B), mother order ---- */
     D.mother.resize(M); D.father.resize(M); D.dest.resize(M);
     D.u01.resize(M); D.s.resize(M); D.z.resize(M); D.zi.resize(M);
-    D.alive.resize(M); D.captured.assign(M, 0);
+    D.alive.resize(M); D.captured.assign(M, 0); D.sex_off.assign(M, 0);
     for (uint64_t i = 0; i < N; ++i)
         for (uint32_t k = 0; k < D.f[i]; ++k) {
             uint64_t j = (uint64_t)D.off[i] + k;
@@ -463,7 +469,7 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         const uint32_t base = (P == 1) ? 0 : S.patch_start[pm];
         const uint32_t np = (P == 1) ? (uint32_t)N : S.patch_start[pm + 1] - S.patch_start[pm];
         uint32_t fa = base + uniform_index(x[0], np);
-        if (S.p.mate_skew != 0.0) {
+        if (mate_on) {
             /* R19: weighted draw among the adults of the mother's patch by running sum + search:
              * total = weight of the patch; 64-bit uniform from words 2,3 of SCALAR block 1;
              * target = floor(u * total / 2^64); father = first adult whose inclusive running sum
@@ -494,6 +500,8 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         }
         D.dest[j] = dest;
         D.u01[j] = u01_of(x[3]);
+        /* R21: sex at birth = bit 0 of word 2 of SCALAR block 0 (bits 30-31 of it are the dispersal direction) */
+        D.sex_off[j] = S.p.separate_sexes ? (uint8_t)(x[2] & 1u) : 0;
 
         /* ---- a4: gametes; offspring hap0 = maternal gamete, hap1 = paternal gamete ---- */
         uint32_t *ob = nullptr; int16_t *oq = nullptr;
@@ -612,12 +620,14 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
     std::vector<uint32_t> nb; std::vector<int16_t> nq;
     if (S.p.genome_kind == ORC_BIT) nb.resize(Nn * S.row_elems); else nq.resize(Nn * S.row_elems);
     std::vector<int32_t> nzi(Nn);
+    std::vector<uint8_t> nsex(Nn, 0);
     std::vector<uint32_t> nps(P + 1, 0);
     for (uint64_t k = 0; k < Na; ++k) {   /* R18: the adults that stay keep their rows */
         const uint32_t i = stay[k];
         if (S.p.genome_kind == ORC_BIT) std::memcpy(&nb[k * S.row_elems], &S.bits[(size_t)i * S.row_elems], S.row_elems * 4);
         else std::memcpy(&nq[k * S.row_elems], &S.q[(size_t)i * S.row_elems], S.row_elems * 2);
         nzi[k] = S.zi[i];
+        nsex[k] = S.sex[i];
         nps[1]++;
         le.sum_zi += S.zi[i];
         le.sum_zi2 += (int64_t)S.zi[i] * S.zi[i];
@@ -627,13 +637,14 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         if (S.p.genome_kind == ORC_BIT) std::memcpy(&nb[k * S.row_elems], &D.off_bits[(size_t)j * S.row_elems], S.row_elems * 4);
         else std::memcpy(&nq[k * S.row_elems], &D.off_q[(size_t)j * S.row_elems], S.row_elems * 2);
         nzi[k] = D.zi[j];
+        nsex[k] = D.sex_off[j];
         nps[D.dest[j] + 1]++;
         /* ---- a8: environment reductions (Fig. 1F), exact integers ---- */
         le.sum_zi += D.zi[j];
         le.sum_zi2 += (int64_t)D.zi[j] * D.zi[j];
     }
     for (uint32_t p = 0; p < P; ++p) nps[p + 1] += nps[p];
-    S.bits.swap(nb); S.q.swap(nq); S.zi.swap(nzi); S.patch_start.swap(nps);
+    S.bits.swap(nb); S.q.swap(nq); S.zi.swap(nzi); S.sex.swap(nsex); S.patch_start.swap(nps);
     S.n = Nn;
     S.cap.assign(Nn, 0);
     le.n_next = Nn;
@@ -746,7 +757,20 @@ int orc_write_state(orc_sim *sim, uint32_t species, uint64_t n, const void *rows
     for (uint64_t i = 0; i < n; ++i)
         S.zi[i] = phenotype_int(S, S.bits.empty() ? nullptr : &S.bits[i * S.row_elems], S.q.empty() ? nullptr : &S.q[i * S.row_elems]);
     S.cap.assign(n, 0);
+    S.sex.assign(n, 0);
     sim->step = step;
+    return 0;
+}
+
+int orc_write_sex(orc_sim *sim, uint32_t species, uint64_t n, const uint8_t *sex) {
+    if (!sim || species >= sim->n_species || n != sim->sp[species].n || !sex) return -1;
+    for (uint64_t i = 0; i < n; ++i) sim->sp[species].sex[i] = sex[i] ? 1 : 0;
+    return 0;
+}
+
+int orc_read_sex(const orc_sim *sim, uint32_t species, uint8_t *sex) {
+    if (!sim || species >= sim->n_species || !sex) return -1;
+    std::memcpy(sex, sim->sp[species].sex.data(), sim->sp[species].n);
     return 0;
 }
 
@@ -815,6 +839,7 @@ int orc_debug(const orc_sim *sim, uint32_t species, orc_debug_view *o) {
     o->cap = D.cap.data();
     o->a_alive = D.a_alive.data(); o->a_u = D.a_u.data(); o->a_s = D.a_s.data();
     o->mate_cum = D.mate_cum.data(); o->zbar_self = D.zbar_self;
+    o->sex_off = D.sex_off.data();
     return 0;
 }
 

@@ -3,7 +3,7 @@
  *
  * TEST INFRASTRUCTURE ONLY.  This is the plain, slow, single-threaded, obviously
  * correct restatement of what the hot path computes (Fig. 1 A-F;
- * PAPER.md:321-330 genetics; the readings R1-R16 in DESIGN.md).  Only tests/,
+ * PAPER.md:321-330 genetics; the readings R1-R21 in DESIGN.md).  Only tests/,
  * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load it.  It shares no code, header, table or constant generator with the CUDA
  * library (include/spegg.h, paper_1603_09255_b200/csrc/): the structs below are
@@ -62,6 +62,10 @@ typedef struct {
                                    captured with probability attack * e/(1+e), e = exp(-(x - delta)^2),
                                    x the consumer's and delta its own trait; the capture is credited to
                                    the consumer met.  0 = the mean-field term of R14.  <= 16      */
+    uint32_t separate_sexes;    /* R21 (eqs. S2-9/S2-10: "the mother and father are drawn
+                                   at random from mature males and females"): 1 = every individual is
+                                   female (0) or male (1); only females lay eggs, only males father them.
+                                   0 = hermaphrodites (R2)                                       */
 } orc_species_params;
 
 typedef struct {
@@ -98,6 +102,9 @@ void orc_destroy(orc_sim *s);
 /* rows: BIT -> uint32 [n][2W]; Q10 -> int16 [n][2L]; patch_start: n_patches+1 or NULL */
 int orc_write_state(orc_sim *s, uint32_t species, uint64_t n, const void *rows,
                     const uint32_t *patch_start, uint32_t step);
+/* R21: sexes of the current adults (1 = male), in row order; write after orc_write_state (which makes everybody female) */
+int orc_write_sex(orc_sim *s, uint32_t species, uint64_t n, const uint8_t *sex);
+int orc_read_sex(const orc_sim *s, uint32_t species, uint8_t *sex);
 int orc_step(orc_sim *s, uint32_t n_steps);
 uint64_t orc_n(const orc_sim *s, uint32_t species);
 uint32_t orc_step_counter(const orc_sim *s);
@@ -130,6 +137,7 @@ typedef struct {
     const float *a_u, *a_s;    /* [n_t] its uniform and survival probability       */
     const uint64_t *mate_cum;  /* [n_t] R19: inclusive running sum of the integer mating weights */
     float zbar_self;           /* R19: mean genetic value of the adults, the weights' reference */
+    const uint8_t *sex_off;    /* [m_t] R21: sex of each offspring (1 = male)                 */
 } orc_debug_view;
 int orc_debug(const orc_sim *s, uint32_t species, orc_debug_view *out);
 
