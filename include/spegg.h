@@ -11,7 +11,7 @@
  *   E  survivors identified, dead removed                    (stable stream compaction)
  *   F  environment updated from the survivors' phenotypes   (exact integer reductions, counts)
  * plus migration between patches.  What the paper leaves open (RNG, samplers,
- * density regulation, ...) is fixed by the readings R1-R20 in DESIGN.md.
+ * density regulation, ...) is fixed by the readings R1-R21 in DESIGN.md.
  *
  * Conventions
  *   - Plain C, no exceptions.  Every call returns an int: 0 = SPEGG_OK, <0 = error code
@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SPEGG_ABI_VERSION 4u
+#define SPEGG_ABI_VERSION 5u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
        SPEGG_ESTATE = -5 };
@@ -105,6 +105,13 @@ typedef struct spegg_species_params {
                                    consumer's and delta the newborn's trait (attack <= 2), and
                                    the capture is credited to the consumer met.  0 = the
                                    mean-field term of R14.  E <= 16                          */
+    uint32_t separate_sexes;    /* 1: every individual is female (0) or male (1) (eqs. S2-9 /
+                                   S2-10; R21): only females lay eggs, only
+                                   males father them (uniform over the males of the mother's
+                                   patch, or by mate_skew's weights among them); sex at birth
+                                   is a fair coin; a patch without males mates as R2.
+                                   spegg_write_state makes everybody female: follow it with
+                                   spegg_write_sex.  0 = hermaphrodites (R2)                 */
 } spegg_species_params;
 
 typedef struct spegg_params {
@@ -148,6 +155,7 @@ typedef struct spegg_debug_view {
     const uint64_t *d_mate_cum; /* [n_t] inclusive running sum of the integer mating weights
                                    (mate_skew != 0, R19)                                      */
     float zbar_self;            /* the weights' reference: mean genetic value of the adults   */
+    const uint8_t *d_sex_off;   /* [m_t] sex of each offspring, 1 = male (separate_sexes, R21) */
 } spegg_debug_view;
 
 typedef struct spegg_sim spegg_sim;
@@ -168,6 +176,12 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
  * (rows, patch_start, step, seed) is a complete checkpoint.  Synchronises the stream. */
 int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *genomes,
                       int genomes_is_device, const uint32_t *patch_start, uint32_t step);
+
+/* Sexes of the current adults of `species` (separate_sexes = 1, else SPEGG_ESTATE), in the row order
+ * of spegg_write_state / spegg_read_state: HOST [n] bytes, 0 = female, non-zero = male; n must be
+ * the current population size (SPEGG_ERANGE).  Synchronises the stream. */
+int spegg_write_sex(spegg_sim *s, uint32_t species, uint64_t n, const uint8_t *sex);
+int spegg_read_sex(spegg_sim *s, uint32_t species, uint8_t *sex_out, uint64_t cap_bytes);
 
 /* Enqueues n_steps steps on the stream and returns; no host synchronisation.  Never fails for
  * model reasons: overflow / extinction set sticky device flags (spegg_status). */

@@ -18,7 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ERANGE, ESTATE = 0, -1, -2, -3, -4, -5
 FLAG_OVERFLOW, FLAG_EXTINCT = 1, 2
 
 
-ABI_VERSION = 4   # SPEGG_ABI_VERSION of include/spegg.h
+ABI_VERSION = 5   # SPEGG_ABI_VERSION of include/spegg.h
 
 
 class SpeciesParams(C.Structure):
@@ -33,7 +33,7 @@ class SpeciesParams(C.Structure):
         ("theta_patch", C.POINTER(C.c_float)), ("sel_predation", C.c_uint32),
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
-        ("mate_skew", C.c_double), ("encounters", C.c_uint32),
+        ("mate_skew", C.c_double), ("encounters", C.c_uint32), ("separate_sexes", C.c_uint32),
     ]
 
 
@@ -59,11 +59,11 @@ class DebugView(C.Structure):
         ("d_table_len", C.c_void_p), ("n_tables", C.c_uint32), ("theta_t", C.c_float),
         ("zbar_pred", C.c_float), ("attack_n", C.c_float), ("d_cap", C.c_void_p),
         ("d_a_alive", C.c_void_p), ("d_a_u", C.c_void_p), ("d_a_s", C.c_void_p),
-        ("d_mate_cum", C.c_void_p), ("zbar_self", C.c_float),
+        ("d_mate_cum", C.c_void_p), ("zbar_self", C.c_float), ("d_sex_off", C.c_void_p),
     ]
 
 
-EXPORTS = ["spegg_workspace_bytes", "spegg_create", "spegg_write_state", "spegg_step", "spegg_read_state",
+EXPORTS = ["spegg_workspace_bytes", "spegg_create", "spegg_write_state", "spegg_write_sex", "spegg_read_sex", "spegg_step", "spegg_read_state",
            "spegg_read_log", "spegg_read_debug", "spegg_status", "spegg_launches_per_step",
            "spegg_kernel_timing", "spegg_destroy", "spegg_strerror"]
 
@@ -83,6 +83,8 @@ def load():
     L.spegg_workspace_bytes.argtypes = [C.POINTER(Params), C.POINTER(u64)]
     L.spegg_create.argtypes = [C.POINTER(Params), vp, u64, vp, C.POINTER(vp)]
     L.spegg_write_state.argtypes = [vp, u32, u64, vp, C.c_int, vp, u32]
+    L.spegg_write_sex.argtypes = [vp, u32, u64, vp]
+    L.spegg_read_sex.argtypes = [vp, u32, vp, u64]
     L.spegg_step.argtypes = [vp, u32]
     L.spegg_read_state.argtypes = [vp, u32, C.POINTER(u64), C.POINTER(u32), vp, C.c_int, u64, vp, vp]
     L.spegg_read_log.argtypes = [vp, u32, u32, u32, C.POINTER(LogEntry), C.POINTER(u32)]
@@ -147,6 +149,7 @@ def make_params(cfg, debug=False, log_capacity=0):
         p.resid_sd = sp.get("resid_sd", 0.0)
         p.adult_survival = sp.get("adult_survival", 0.0)
         p.mate_skew = sp.get("mate_skew", 0.0)
+        p.separate_sexes = 1 if sp.get("separate_sexes") else 0
         p.fecundity_model, p.fec_a, p.K = _FEC[sp["fecundity"]], sp["fec_a"], sp["K"]
         if sp.get("K_patch") is not None:
             kp = np.ascontiguousarray(sp["K_patch"], dtype=np.float64)
@@ -239,6 +242,16 @@ class Sim:
             assert rows.ndim == 2 and rows.shape[1] == self.row_shape[species]
             _check(self.lib.spegg_write_state(self._h, species, rows.shape[0], rows.ctypes.data, 0, psp, step))
 
+    def write_sex(self, species, sex):
+        sex = np.ascontiguousarray(sex, dtype=np.uint8)
+        _check(self.lib.spegg_write_sex(self._h, species, sex.shape[0], sex.ctypes.data))
+
+    def read_sex(self, species=0):
+        out = np.zeros(self.n(species), dtype=np.uint8)
+        if len(out):
+            _check(self.lib.spegg_read_sex(self._h, species, out.ctypes.data, len(out)))
+        return out
+
     def step(self, n=1):
         _check(self.lib.spegg_step(self._h, n))
 
@@ -323,7 +336,10 @@ class Sim:
             "a_alive": arr(v.d_a_alive, n, np.uint8), "a_u": arr(v.d_a_u, n, np.float32),
             "a_s": arr(v.d_a_s, n, np.float32),
             "zbar_self": float(v.zbar_self),
-            "mate_cum": (arr(v.d_mate_cum, n, np.uint64) if self.cfg["species"][species].get("mate_skew", 0.0) != 0.0
-                         else np.zeros(0, np.uint64)),
+            "mate_cum": (arr(v.d_mate_cum, n, np.uint64)
+                         if (self.cfg["species"][species].get("mate_skew", 0.0) != 0.0
+                             or self.cfg["species"][species].get("separate_sexes")) else np.zeros(0, np.uint64)),
+            "sex_off": (arr(v.d_sex_off, m, np.uint8) if self.cfg["species"][species].get("separate_sexes")
+                        else np.zeros(m, np.uint8)),
         }
         return d

@@ -94,7 +94,7 @@ struct Carver {
 };
 
 struct SpeciesLayout {
-    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos, mate_cum, mate_tile, enc_zi,
+    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos, mate_cum, mate_tile, enc_zi, sex[2], sex_off,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
     uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, T_env, K_patch, theta_patch;
     uint32_t norm_len, env_len, n_tables, row_bytes;
@@ -148,7 +148,7 @@ int validate(const spegg_params *p) {
         if (q.capacity == 0 || q.capacity >= (1ull << 31)) return SPEGG_EINVAL;
         if (!(q.adult_survival >= 0.0 && q.adult_survival <= 1.0) || (q.adult_survival > 0.0 && P != 1)) return SPEGG_EINVAL;
         if (!(q.resid_sd >= 0.0) || !(q.pheno_scale > 0.0f) || q.resid_sd / (double)q.pheno_scale > 4096.0) return SPEGG_EINVAL;
-        if (!(std::fabs(q.mate_skew) <= 1e6)) return SPEGG_EINVAL;
+        if (!(std::fabs(q.mate_skew) <= 1e6) || q.separate_sexes > 1) return SPEGG_EINVAL;
         if (q.fecundity_model == SPEGG_FEC_CAPTURES && P != 1) return SPEGG_EINVAL;
         if (q.sel_predation) {
             if (q.predator_species >= p->n_species || q.predator_species <= s) return SPEGG_EINVAL;
@@ -203,8 +203,11 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         const uint64_t acap = q.adult_survival > 0.0 ? cap : 1;   // R18 arrays only when generations overlap
         l.a_alive = c.take(acap); l.a_u = c.take(acap * 4); l.a_s = c.take(acap * 4);
         l.a_zi = c.take(acap * 4); l.a_pos = c.take(acap * 4);
-        l.mate_cum = c.take((q.mate_skew != 0.0 ? cap : 1) * 8);      // R19 arrays only with weighted mating
-        l.mate_tile = c.take((q.mate_skew != 0.0 ? cap / MATE_TILE + 2 : 1) * 8);
+        const bool mate_on = q.mate_skew != 0.0 || q.separate_sexes;
+        l.mate_cum = c.take((mate_on ? cap : 1) * 8);      // R19 arrays only with weighted mating / separate sexes
+        l.mate_tile = c.take((mate_on ? cap / MATE_TILE + 2 : 1) * 8);
+        const uint64_t scap = q.separate_sexes ? cap32 : 1;         // R21
+        l.sex[0] = c.take(scap); l.sex[1] = c.take(scap); l.sex_off = c.take(scap);
         bool is_met = false;   // R20: some species meets this one individually
         for (uint32_t o = 0; o < p->n_species; ++o)
             if (p->species[o].sel_predation && p->species[o].encounters && p->species[o].predator_species == s) is_met = true;
@@ -274,7 +277,7 @@ int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
 
 // true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
 bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
-    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.mate_v != 0.0f) return false;
+    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.mate_on) return false;
     // the fused kernel tests u >= T as u > T - 1 (see spegg_fused.cuh): every threshold must be >= 1
     for (uint32_t c = 0; c < h.p.n_chrom; ++c)
         for (uint32_t k = 0; k < h.xover_len[c]; ++k)
@@ -315,7 +318,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             };
             const uint32_t g_thread = ctas(cap, 256, 8), g_warp = ctas(cap, 8, 8);   // thread / warp per offspring
             k_fec_scan<<<ctas(cap, SCAN_THREADS, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
-            if (k.mate_v != 0.0f) {   // R19: mating weights of the adults and their running sum
+            if (k.mate_on) {   // R19: mating weights of the adults and their running sum
                 k_mate_weight<<<g_warp, 256, 0, s->stream>>>(k); ++nl;
                 k_mate_scan<<<ctas(cap, MATE_TILE, 8), 256, 0, s->stream>>>(k); ++nl;
             }
@@ -512,6 +515,8 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.a_alive = at<uint8_t>(s, l.a_alive); k.a_u = at<float>(s, l.a_u); k.a_s = at<float>(s, l.a_s);
         k.a_zi = at<int32_t>(s, l.a_zi); k.a_pos = at<uint32_t>(s, l.a_pos);
         k.mate_v = (float)q.mate_skew;
+        k.sexes = q.separate_sexes; k.mate_on = (q.mate_skew != 0.0 || q.separate_sexes) ? 1u : 0u;
+        k.sex[0] = at<uint8_t>(s, l.sex[0]); k.sex[1] = at<uint8_t>(s, l.sex[1]); k.sex_off = at<uint8_t>(s, l.sex_off);
         k.mate_cum = at<unsigned long long>(s, l.mate_cum); k.mate_tile = at<unsigned long long>(s, l.mate_tile);
         k.enc_E = q.sel_predation ? q.encounters : 0u; k.enc_v = (float)q.attack;
         k.enc_zi = at<int32_t>(s, l.enc_zi);
@@ -594,6 +599,7 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
     CU(cudaMemcpy(&g, s->d_glob, sizeof g, cudaMemcpyDeviceToHost));
     g.step = step;
     CU(cudaMemcpyAsync(s->d_glob, &g, sizeof g, cudaMemcpyHostToDevice, s->stream));
+    if (h.k.sexes) CU(cudaMemsetAsync(h.k.sex[cur], 0, (size_t)n, s->stream));   // R21: everybody female until spegg_write_sex
     if (n) {
         k_iota<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k.rowptr[cur], (uint32_t)n);
         if (h.k.phys_parents) k_fill_masks<<<s->n_sms, 256, 0, s->stream>>>(h.k.chunk_mask[cur], h.k.range_cnt[cur], (uint32_t)n);
@@ -602,6 +608,38 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
     launch_prepare(s);
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(s->stream));
+    return SPEGG_OK;
+}
+
+int spegg_write_sex(spegg_sim *s, uint32_t species, uint64_t n, const uint8_t *sex) {
+    if (!s || species >= s->sp.size() || (n && !sex)) return SPEGG_EINVAL;
+    HostSpecies &h = s->sp[species];
+    if (!h.k.sexes) return SPEGG_ESTATE;
+    CU(cudaStreamSynchronize(s->stream));
+    DevSpecies st;
+    CU(cudaMemcpy(&st, s->d_st + species, sizeof st, cudaMemcpyDeviceToHost));
+    if (n != st.n) return SPEGG_ERANGE;
+    if (n == 0) return SPEGG_OK;
+    CU(cudaMemcpyAsync(h.k.sex_off, sex, (size_t)n, cudaMemcpyHostToDevice, s->stream));
+    k_sex_io<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k, (uint32_t)n, h.k.sex_off, 1);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(s->stream));
+    return SPEGG_OK;
+}
+
+int spegg_read_sex(spegg_sim *s, uint32_t species, uint8_t *sex_out, uint64_t cap_bytes) {
+    if (!s || species >= s->sp.size() || !sex_out) return SPEGG_EINVAL;
+    HostSpecies &h = s->sp[species];
+    if (!h.k.sexes) return SPEGG_ESTATE;
+    CU(cudaStreamSynchronize(s->stream));
+    DevSpecies st;
+    CU(cudaMemcpy(&st, s->d_st + species, sizeof st, cudaMemcpyDeviceToHost));
+    if (cap_bytes < st.n) return SPEGG_ERANGE;
+    if (st.n == 0) return SPEGG_OK;
+    k_sex_io<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k, st.n, h.k.sex_off, 0);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(s->stream));
+    CU(cudaMemcpy(sex_out, h.k.sex_off, (size_t)st.n, cudaMemcpyDeviceToHost));
     return SPEGG_OK;
 }
 
@@ -685,6 +723,7 @@ int spegg_read_debug(spegg_sim *s, uint32_t species, spegg_debug_view *o) {
     o->d_cap = k.cap;
     o->d_a_alive = k.a_alive; o->d_a_u = k.a_u; o->d_a_s = k.a_s;
     o->d_mate_cum = (const uint64_t *)k.mate_cum; o->zbar_self = st.zbar_self;
+    o->d_sex_off = k.sex_off;
     return SPEGG_OK;
 }
 

@@ -106,6 +106,11 @@ struct SpK {
     float mate_v;               // v_m as fp32; 0 = uniform mate (R2)
     unsigned long long *mate_cum;   // [n] inclusive running sum of the weights, adult order
     unsigned long long *mate_tile;  // [n / MATE_TILE + 2] weight of each tile of MATE_TILE adults
+    uint32_t mate_on;           // 1: the father comes from the running sum (mate_v != 0 or separate sexes)
+    // R21, separate sexes (sexes = 1): one byte per PHYSICAL row of pop[0] / pop[1], 1 = male
+    uint32_t sexes;
+    uint8_t *sex[2];
+    uint8_t *sex_off;           // [m] sex of each offspring of the current step (staging; also I/O staging)
     // R20, individual-level encounters (enc_E > 0 on the prey; enc_zi filled on the species it meets)
     uint32_t enc_E;             // meetings per newborn; 0 = mean-field predation term (R14)
     float enc_v;                // v = fp32(attack)

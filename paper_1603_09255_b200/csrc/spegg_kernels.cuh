@@ -152,7 +152,7 @@ __device__ __forceinline__ void prepare_species(const SpK &sp, uint32_t g, uint3
     for (uint32_t i = g; i < nc; i += stride) sp.status_cmp[i] = 0ull;
     if (sp.fec_model == 2)
         for (uint32_t i = g; i < sp.capacity; i += stride) sp.cap[i] = 0u;
-    if (sp.mate_v != 0.0f)   // R19: tile totals of the mating weights are accumulated with atomics
+    if (sp.mate_on)   // R19: tile totals of the mating weights are accumulated with atomics
         for (uint32_t i = g; i < sp.capacity / MATE_TILE + 2u; i += stride) sp.mate_tile[i] = 0ull;
     if (sp.phys_parents) {  // fused path: the coming step counts its survivors per range of the other buffer
         uint32_t *cnt_next = sp.range_cnt[cur ^ 1u];
@@ -280,6 +280,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
                     const uint32_t tab = (sp.fec_model == 2) ? min(sp.cap[i], (uint32_t)(CAP_TABLES - 1)) : patch_of(ps, sp.P, i);
                     f = poisson_count(sp.tables + (size_t)tab * TMAX, sp.table_len[tab], x[0]);
                 }
+                if (sp.sexes && sp.sex[st.cur][rowptr[i]]) f = 0;   // R21: males lay no eggs (the draw is made and ignored)
             }
             s_f[k] = (uint8_t)f;
         }
@@ -354,7 +355,8 @@ __global__ void __launch_bounds__(256) k_mate_weight(const __grid_constant__ SpK
             float e = __fmul_rn(sp.mate_v, d);
             e = fminf(fmaxf(e, -16.0f), 16.0f);
             const float w = expf_spec(__fsub_rn(e, 16.0f));
-            const unsigned long long wi = (unsigned long long)__fmul_rn(w, 0x1p40f);
+            unsigned long long wi = (unsigned long long)__fmul_rn(w, 0x1p40f);
+            if (sp.sexes && !sp.sex[st.cur][rowptr[i]]) wi = 0ull;   // R21: only males father eggs
             sp.mate_cum[i] = wi;
             if (wi) atomicAdd(&sp.mate_tile[i / MATE_TILE], wi);
         }
@@ -411,7 +413,7 @@ __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) 
         uint32_t pm = 0, base = 0, np = N;
         if (sp.P > 1) { pm = patch_of(ps, sp.P, mo); base = ps[pm]; np = ps[pm + 1] - base; }
         uint32_t fa = base + uniform_index(x[0], np);
-        if (sp.mate_v != 0.0f) {
+        if (sp.mate_on) {
             // R19: weighted draw among the adults of the mother's patch: 64-bit uniform from words 2,3 of
             // SCALAR block 1, target = floor(u * total / 2^64), father = first adult of the patch whose
             // inclusive running sum exceeds (sum before the patch) + target; total 0 keeps the uniform mate
@@ -435,6 +437,7 @@ __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) 
         if (sp.P > 1 && (unsigned long long)x[1] < sp.T_mig) dest = neighbour(pm, x[2] >> 30, sp.grid_w, sp.grid_h);
         sp.dest[j] = dest;
         sp.u01[j] = u01_of(x[3]);
+        if (sp.sexes) sp.sex_off[j] = (uint8_t)(x[2] & 1u);   // R21: sex at birth (bits 30-31 of the word are the direction)
     }
 }
 
@@ -715,6 +718,15 @@ __global__ void __launch_bounds__(256) k_enc_zi(const __grid_constant__ SpK sp) 
     }
 }
 
+// R21: sexes of the current adults in logical order (dir 0: gather into io[], dir 1: scatter from io[])
+__global__ void __launch_bounds__(256) k_sex_io(const __grid_constant__ SpK sp, uint32_t n, uint8_t *io, int dir) {
+    const uint32_t cur = sp.st->cur;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        uint8_t *p = sp.sex[cur] + sp.rowptr[cur][i];
+        if (dir) *p = io[i] ? 1 : 0; else io[i] = *p;
+    }
+}
+
 // rowptr = identity for a freshly written, dense population
 __global__ void __launch_bounds__(256) k_iota(uint32_t *p, uint32_t n) {
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = i;
@@ -889,17 +901,18 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     uint8_t *dst = sp.pop[st.cur ^ 1u];
     uint32_t *rp = sp.rowptr[st.cur ^ 1u];
+    uint8_t *sex_next = sp.sex[st.cur ^ 1u];   // R21: the sex travels with the row
     __shared__ uint32_t s_flag;
     if (sp.index_only) {   // the rows stay where the gamete kernel stored them: only the index is written
         for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
             const uint32_t p = sp.pos[j];
-            if (p != 0xFFFFFFFFu) rp[p] = j;
+            if (p != 0xFFFFFFFFu) { rp[p] = j; if (sp.sexes) sex_next[j] = sp.sex_off[j]; }
         }
     } else {
         for (uint32_t j = warp0; j < M; j += nw) {
             const uint32_t p = sp.pos[j];
             if (p == 0xFFFFFFFFu) continue;
-            if (lane == 0) rp[p] = p;  // materialised path: rows are dense, rowptr is the identity
+            if (lane == 0) { rp[p] = p; if (sp.sexes) sex_next[p] = sp.sex_off[j]; }  // materialised path: rows are dense, rowptr is the identity
             const uint4 *src = (const uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes);
             uint4 *d = (uint4 *)(dst + (size_t)p * sp.row_bytes);
             for (uint32_t i = lane; i < sp.row_u4; i += 32) d[i] = src[i];
@@ -915,7 +928,7 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
             const uint32_t p = sp.a_pos[i];
             if (p == 0xFFFFFFFFu) continue;
             const uint32_t row = sp.index_only ? M + p : p;
-            if (lane == 0) rp[p] = row;
+            if (lane == 0) { rp[p] = row; if (sp.sexes) sex_next[row] = sp.sex[cur][rp_cur[i]]; }
             const uint4 *src = (const uint4 *)(src_pop + (size_t)rp_cur[i] * sp.row_bytes);
             uint4 *d = (uint4 *)(dst + (size_t)row * sp.row_bytes);
             for (uint32_t k = lane; k < sp.row_u4; k += 32) d[k] = src[k];

@@ -133,6 +133,13 @@ def initial_rows(cfg, species, n=None, seed=None):
     return np.clip(v, -32767, 32767).astype(np.int16)
 
 
+def initial_sex(cfg, species, n=None, seed=None):
+    """iid initial sexes (1 = male), probability 1/2, for species with separate_sexes (R21)."""
+    n = cfg["n0"][species] if n is None else n
+    rng = np.random.default_rng((cfg["seed"] if seed is None else seed) * 7919 + 17 + species)
+    return rng.integers(0, 2, size=n).astype(np.uint8)
+
+
 def initial_patch_start(cfg, species):
     w, h = cfg["grid"]
     P = w * h

@@ -11,6 +11,8 @@ INT_FIELDS = ["f", "off", "mother", "father", "dest", "zi", "alive", "captured"]
 def load_initial(obj, cfg, step=0):
     for s in range(len(cfg["species"])):
         obj.write_state(s, workloads.initial_rows(cfg, s), workloads.initial_patch_start(cfg, s), step)
+        if cfg["species"][s].get("separate_sexes"):
+            obj.write_sex(s, workloads.initial_sex(cfg, s))
 
 
 def assert_debug_equal(dg, do, species_cfg, tag=""):
@@ -38,7 +40,9 @@ def assert_debug_equal(dg, do, species_cfg, tag=""):
         assert np.array_equal(dg["a_s"].view(np.uint32), do["a_s"].view(np.uint32)), (tag, "a_s")
 
 
-    if species_cfg.get("mate_skew", 0.0) != 0.0:        # R19: the integer mating weights' running sum
+    if species_cfg.get("separate_sexes"):               # R21: sex at birth
+        assert np.array_equal(dg["sex_off"], do["sex_off"]), (tag, "sex_off")
+    if species_cfg.get("mate_skew", 0.0) != 0.0 or species_cfg.get("separate_sexes"):        # R19: the integer mating weights' running sum
         assert np.float32(dg["zbar_self"]) == np.float32(do["zbar_self"]), (tag, "zbar_self")
         assert np.array_equal(dg["mate_cum"], do["mate_cum"]), (tag, "mate_cum")
 
@@ -51,6 +55,8 @@ def assert_state_equal(sim, orc, cfg, tag=""):
         assert np.array_equal(rg, ro), (tag, s, "rows")
         assert np.array_equal(pg, po), (tag, s, "patch_start")
         assert np.array_equal(zg, zo), (tag, s, "zi")
+        if cfg["species"][s].get("separate_sexes"):
+            assert np.array_equal(sim.read_sex(s), orc.read_sex(s)), (tag, s, "sex")
 
 
 def assert_logs_equal(lg, lo, tag=""):
@@ -69,6 +75,8 @@ def per_step_parity(oracle_mod, binding, cfg, steps, debug=True):
         for s in range(len(cfg["species"])):
             rows, ps, _ = orc.read_state(s)
             sim.write_state(s, rows, ps if sim.P > 1 else None, t)
+            if cfg["species"][s].get("separate_sexes"):
+                sim.write_sex(s, orc.read_sex(s))
         orc.step(1)
         sim.step(1)
         for s in range(len(cfg["species"])):

@@ -342,3 +342,39 @@ def test_individual_encounters(oracle_mod, binding, scale, E, v, extra):
     assert sim.status() == orc.flags
     assert sum(e["captures"] for e in orc.log(0)) > 0
     sim.close()
+
+
+@pytest.mark.parametrize("which,scale,grid,extra", [
+    (1, 1.0, None, {}),                                   # C1, uniform over the males
+    (2, 0.06, None, {"mate_skew": 1.5}),                  # C2, R19's weights among the males
+    (3, 0.012, None, {}),                                 # bit genome on the general pipeline
+    (5, 0.03, (5, 4), {"mate_skew": -1.0}),               # patches: males of the mother's patch
+    (2, 0.04, None, {"adult_survival": 0.6}),             # overlapping generations: staying adults keep their sex
+    (1, 1.0, None, {"resid_sd": 0.5, "mate_skew": 3.0}),
+])
+def test_separate_sexes(oracle_mod, binding, which, scale, grid, extra):
+    """R21 (eqs. S2-9/S2-10): only females lay eggs, only males father them, the sex
+    travels with the individual.  Per-step parity of every intermediate incl. the offspring's sexes
+    and the running sum (debug), then a free-running trajectory on the production kernels (state,
+    sexes and log)."""
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    sp = cfg["species"][0]
+    sp["separate_sexes"] = 1
+    sp["fec_a"] = 2.0 * sp["fec_a"]            # half the adults lay eggs
+    sp.update(extra)
+    if "adult_survival" in extra:
+        sp["capacity"] = 4 * sp["capacity"]
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(2):
+        orc.step(5)
+        sim.step(5)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+        parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags and orc.n(0) > 0
+    sex = sim.read_sex(0)
+    assert 0 < sex.sum() < len(sex)
+    sim.close()
