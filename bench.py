@@ -89,13 +89,38 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def workload(which, seed_offset=0, world=1):
+VARIANTS = {
+    # the widenings of SURVEY.md 8(f) on top of a configuration (R17-R21); context lines, not the metric
+    "none": {},
+    "noise": {"resid_sd": 0.5},                        # R17
+    "overlap": {"adult_survival": 0.6},                # R18 (capacity x 4)
+    "mating": {"mate_skew": 1.0},                      # R19
+    "sexes": {"separate_sexes": 1},                    # R21 (fecundity parameter x 2: half the adults lay eggs)
+    "encounters": {},                                  # R20 (configuration 4 only: 3 meetings, attack 0.1)
+}
+
+
+def apply_variant(cfg, variant):
+    sp = cfg["species"][0]
+    sp.update(VARIANTS[variant])
+    if variant == "overlap":
+        sp["capacity"] = 4 * sp["capacity"]
+    if variant == "sexes":
+        sp["fec_a"] = 2.0 * sp["fec_a"]
+    if variant == "encounters":
+        sp["predation"].update(encounters=3, attack=0.1)
+    if variant != "none":
+        cfg["name"] = "%s+%s" % (cfg["name"], variant)
+    return cfg
+
+
+def workload(which, seed_offset=0, world=1, variant="none"):
     """Rank `seed_offset`'s workload.  Configs 1-5: an independent replica (own seed).  Config 6 (the
     sweep of unlinked patches): the rank's block of 16 patches out of a 16 x world sweep."""
     from paper_1603_09255_b200 import replicas, workloads
     if which == 6:
         return replicas.sweep_shard(16 * world, seed_offset, world)
-    return replicas.replica_config(workloads.config(which), seed_offset)
+    return apply_variant(replicas.replica_config(workloads.config(which), seed_offset), variant)
 
 
 def describe(cfg):
@@ -128,6 +153,8 @@ def oracle_run(cfg, n_steps, warm=0):
     o = oracle.Oracle(cfg)
     for s in range(len(cfg["species"])):
         o.write_state(s, workloads.initial_rows(cfg, s), workloads.initial_patch_start(cfg, s), 0)
+        if cfg["species"][s].get("separate_sexes"):
+            o.write_sex(s, workloads.initial_sex(cfg, s))
     if warm:
         o.step(warm)
     k0 = len(o.log(0))
@@ -144,11 +171,11 @@ def run_reference(args):
     if rank != 0:
         return
     from paper_1603_09255_b200 import workloads
-    full = workload(args.config)
+    full = workload(args.config, variant=args.variant)
     # bounded sample: shrink the population so that K+W oracle steps end within ~2 minutes
     per_step_s = args.ref_budget_s / max(1, args.steps + args.warmup)
     scale = min(1.0, max(0.001, per_step_s * 7.0e4 / full["n0"][0]))
-    cfg = workloads.config(args.config, scale=scale)
+    cfg = apply_variant(workloads.config(args.config, scale=scale), args.variant)
     units, dt = oracle_run(cfg, args.steps, warm=args.warmup)
     val = units / dt
     line = {
@@ -180,13 +207,16 @@ def run_ours(args):
     torch.cuda.set_device(dev)
     binding.load()  # fails loudly if the CUDA extension is missing
 
-    cfg = workload(args.config, seed_offset=rank, world=world)
+    cfg = workload(args.config, seed_offset=rank, world=world, variant=args.variant)
     n_sp = len(cfg["species"])
     sim = binding.Sim(cfg, debug=False, log_capacity=max(4096, args.steps * 3 + args.warmup + 64), device=str(dev))
     rows0 = [workloads.initial_rows(cfg, s) for s in range(n_sp)]
     ps0 = [workloads.initial_patch_start(cfg, s) for s in range(n_sp)]
+    sex0 = [workloads.initial_sex(cfg, s) if cfg["species"][s].get("separate_sexes") else None for s in range(n_sp)]
     for s in range(n_sp):
         sim.write_state(s, rows0[s], ps0[s], 0)
+        if sex0[s] is not None:
+            sim.write_sex(s, sex0[s])
 
     def barrier():
         if dist is not None:
@@ -235,7 +265,9 @@ def run_ours(args):
     t0 = time.perf_counter()
     for s in range(n_sp):
         sim.write_state(s, host_rows[s], ps0[s], 0)
-    h2d = sum(r.nbytes for r in host_rows)
+        if sex0[s] is not None:
+            sim.write_sex(s, sex0[s])
+    h2d = sum(r.nbytes for r in host_rows) + sum(x.nbytes for x in sex0 if x is not None)
     e_units, d2h = 0, 0
     for _ in range(e2e_steps):
         sim.step(1)
@@ -259,7 +291,7 @@ def run_ours(args):
         achieved = k_bytes / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
         step_bytes = alg_bytes(cfg, logs[0], kernel_only=False) / max(1, len(logs[0]))
         # oracle on a bounded sample of the same workload: ~10-30 s of CPU work
-        cb_cfg = workload(args.config)
+        cb_cfg = workload(args.config, variant=args.variant)
         cb_steps = 1 if cb_cfg["n0"][0] >= 500_000 else max(1, int(1.0e6 / cb_cfg["n0"][0]))
         cb_units, cb_dt = oracle_run(cb_cfg, cb_steps)
         line = {
@@ -304,6 +336,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--variant", default="none", choices=sorted(VARIANTS),
+                    help="a widening of SURVEY.md 8(f) on top of --config (context lines; the metric is --variant none)")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
                     help="--impl reference: CPU seconds the K+W oracle steps are sized for")
     args = ap.parse_args()

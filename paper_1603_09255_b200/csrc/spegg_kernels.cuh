@@ -146,7 +146,7 @@ __device__ __forceinline__ void finish_species(const SpK &sp) {
 // look-back statuses / tickets / capture counts.  g / stride: this thread's index and the number
 // of threads sharing the work; N, cur, sum_zi, step: the species' finished state.
 __device__ __forceinline__ void prepare_species(const SpK &sp, uint32_t g, uint32_t stride, uint32_t N,
-                                                uint32_t cur, long long sum_zi, uint32_t step) {
+                                                uint32_t cur, long long sum_zi, uint32_t step, uint32_t g_tab) {
     const uint32_t nf = sp.status_fec_n + sp.status_fec_n / 32 + 2, nc = sp.status_cmp_n + sp.status_cmp_n / 32 + 2;
     for (uint32_t i = g; i < nf; i += stride) sp.status_fec[i] = 0ull;
     for (uint32_t i = g; i < nc; i += stride) sp.status_cmp[i] = 0ull;
@@ -160,7 +160,9 @@ __device__ __forceinline__ void prepare_species(const SpK &sp, uint32_t g, uint3
         for (uint32_t i = g; i < n_max; i += stride) cnt_next[i] = 0u;
     }
     const uint32_t *ps = sp.patch_start[cur];
-    for (uint32_t tab = g; tab < sp.n_tables; tab += stride) {
+    // g_tab: this thread's index for the table builds (the step-closing CTA gives table 0 to a thread of
+    // another warp than the one that is busy closing the step: the fp64 chain of a table is ~2 us)
+    for (uint32_t tab = g_tab; tab < sp.n_tables; tab += stride) {
         double lam;
         if (sp.fec_model == 2) lam = fecundity_mean(sp, (double)N, sp.K, tab);
         else if (sp.P == 1) lam = fecundity_mean(sp, (double)N, sp.K_patch ? sp.K_patch[0] : sp.K, 0);
@@ -198,8 +200,8 @@ __global__ void k_finish_all(const SpK *__restrict__ spk, uint32_t n_species) {
 __global__ void __launch_bounds__(256) k_prepare_all(const SpK *__restrict__ spk) {
     const SpK &sp = spk[blockIdx.y];
     const DevSpecies &st = *sp.st;
-    prepare_species(sp, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, st.n, st.cur, st.sum_zi,
-                    sp.glob->step);
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    prepare_species(sp, g, gridDim.x * blockDim.x, st.n, st.cur, st.sum_zi, sp.glob->step, g);
 }
 
 // Tail of the last kernel of a single-species step: the CTA that finishes last closes the step and
@@ -222,7 +224,7 @@ __device__ __forceinline__ void solo_tail(const SpK &sp, uint32_t *s_flag) {
         finish_species(sp);
         sp.glob->step = step1;
     }
-    prepare_species(sp, threadIdx.x, blockDim.x, nn, cur1, a1, step1);
+    prepare_species(sp, threadIdx.x, blockDim.x, nn, cur1, a1, step1, (threadIdx.x + blockDim.x - 32u) % blockDim.x);
 }
 
 // a1-a3: fecundity (one FEC block per adult), exclusive scan by decoupled look-back, mother fill.

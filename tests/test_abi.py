@@ -45,7 +45,10 @@ def test_workspace_bytes_and_validation(binding):
     for mutate in (lambda c: c["species"][0].update(mu=2.0),
                    lambda c: c["species"][0].update(capacity=0),
                    lambda c: c["species"][0].update(chrom_len=[512, 256], xover_mean=[1.0, 1.0]),
-                   lambda c: c["species"][0].update(K=0.0)):
+                   lambda c: c["species"][0].update(K=0.0),
+                   lambda c: c["species"][0].update(mate_skew=float("nan")),
+                   lambda c: c["species"][0].update(predation=dict(attack=0.1, predator=0, encounters=2)),   # no such consumer
+                   lambda c: c["species"][0].update(adult_survival=1.5)):
         c = workloads.config(3, scale=0.01)
         mutate(c)
         with pytest.raises(binding.SpeggError) as e:

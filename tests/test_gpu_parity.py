@@ -378,3 +378,31 @@ def test_separate_sexes(oracle_mod, binding, which, scale, grid, extra):
     sex = sim.read_sex(0)
     assert 0 < sex.sum() < len(sex)
     sim.close()
+
+
+def test_sex_io_errors_and_roundtrip(binding):
+    """spegg_write_sex / spegg_read_sex: ESTATE without separate sexes, ERANGE for a wrong count,
+    everybody female after spegg_write_state, exact round trip, encounters need sel_predation."""
+    cfg = workloads.config(1)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(sim, cfg)
+    with pytest.raises(binding.SpeggError) as e:
+        sim.write_sex(0, np.zeros(cfg["n0"][0], np.uint8))
+    assert e.value.code == binding.ESTATE
+    sim.close()
+    cfg["species"][0]["separate_sexes"] = 1
+    sim = binding.Sim(cfg, debug=False)
+    sim.write_state(0, workloads.initial_rows(cfg, 0), None, 0)
+    assert (sim.read_sex(0) == 0).all()
+    with pytest.raises(binding.SpeggError) as e:
+        sim.write_sex(0, np.zeros(cfg["n0"][0] - 1, np.uint8))
+    assert e.value.code == binding.ERANGE
+    sex = workloads.initial_sex(cfg, 0)
+    sim.write_sex(0, sex * 7)                    # any non-zero byte is male
+    assert np.array_equal(sim.read_sex(0), sex)
+    sim.close()
+    cfg = workloads.config(4, scale=0.002)
+    cfg["species"][1]["encounters"] = 3          # not a predation parameter of the consumer itself
+    cfg["species"][0]["predation"]["encounters"] = 17
+    with pytest.raises(binding.SpeggError):
+        binding.workspace_bytes(cfg)
