@@ -242,6 +242,8 @@ thread_local cudaError_t s_last_cuda = cudaSuccess;
 
 }  // namespace
 
+constexpr uint32_t MULTI_STEPS = 16;
+
 struct spegg_sim {
     spegg_params p;
     std::vector<HostSpecies> sp;
@@ -251,6 +253,10 @@ struct spegg_sim {
     bool own_stream = false;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
+    // several steps in one graph: the programmatic edges between the kernels of consecutive steps
+    // stay inside the graph, so a step's first kernel is scheduled while the previous step drains
+    cudaGraph_t graph_multi = nullptr;
+    cudaGraphExec_t exec_multi = nullptr;
     DevGlobal *d_glob = nullptr;
     DevSpecies *d_st = nullptr;
     SpK *d_spk = nullptr;
@@ -558,6 +564,15 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     if (rc != SPEGG_OK) return fail(rc);
     if (ce != cudaSuccess) { s_last_cuda = ce; return fail(SPEGG_ECUDA); }
     if ((ce = cudaGraphInstantiate(&s->exec, s->graph, 0)) != cudaSuccess) { s_last_cuda = ce; return fail(SPEGG_ECUDA); }
+    if (!s->debug) {   // MULTI_STEPS steps per graph for long runs (optional: a failure here leaves the one-step graph)
+        bool ok = cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+        if (ok) {
+            for (uint32_t i = 0; i < MULTI_STEPS && ok; ++i) ok = enqueue_step(s, nullptr, false) == SPEGG_OK;
+            ok = (cudaStreamEndCapture(s->stream, &s->graph_multi) == cudaSuccess) && ok;
+        }
+        if (ok) ok = cudaGraphInstantiate(&s->exec_multi, s->graph_multi, 0) == cudaSuccess;
+        if (!ok) { (void)cudaGetLastError(); s->exec_multi = nullptr; }
+    }
     *out = s;
     return SPEGG_OK;
 }
@@ -566,6 +581,8 @@ void spegg_destroy(spegg_sim *s) {
     if (!s) return;
     if (s->stream) cudaStreamSynchronize(s->stream);
     for (auto e : s->ev) cudaEventDestroy(e);
+    if (s->exec_multi) cudaGraphExecDestroy(s->exec_multi);
+    if (s->graph_multi) cudaGraphDestroy(s->graph_multi);
     if (s->exec) cudaGraphExecDestroy(s->exec);
     if (s->graph) cudaGraphDestroy(s->graph);
     if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -645,7 +662,10 @@ int spegg_read_sex(spegg_sim *s, uint32_t species, uint8_t *sex_out, uint64_t ca
 
 int spegg_step(spegg_sim *s, uint32_t n_steps) {
     if (!s) return SPEGG_EINVAL;
-    for (uint32_t i = 0; i < n_steps; ++i) {
+    uint32_t i = 0;
+    if (!s->timing && s->exec_multi)
+        for (; i + MULTI_STEPS <= n_steps; i += MULTI_STEPS) CU(cudaGraphLaunch(s->exec_multi, s->stream));
+    for (; i < n_steps; ++i) {
         if (s->timing) {
             if (s->ev_used + 2 > s->ev.size()) { CU(cudaStreamSynchronize(s->stream)); drain_timing(s); }
             const int rc = enqueue_step(s, nullptr, true);
