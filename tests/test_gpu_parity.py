@@ -406,3 +406,27 @@ def test_sex_io_errors_and_roundtrip(binding):
     cfg["species"][0]["predation"]["encounters"] = 17
     with pytest.raises(binding.SpeggError):
         binding.workspace_bytes(cfg)
+
+
+@pytest.mark.parametrize("which,variant", [(4, "encounters"), (5, "sexes+mating")])
+def test_full_size_widenings(oracle_mod, binding, which, variant):
+    """The widenings at BASELINE.json's full sizes on the production kernels (the launch configuration
+    `bench.py --variant` times): one step, every row, sex and log field compared with the oracle."""
+    cfg = workloads.config(which)
+    sp = cfg["species"][0]
+    if variant == "encounters":
+        sp["predation"].update(encounters=3, attack=0.1)      # R20: 1.3 M newborns x 3 meetings with 100,000 consumers
+    else:
+        sp.update(separate_sexes=1, mate_skew=1.0)            # R21 + R19 in 4,096 patches: ~4,600 weight tiles
+        sp["fec_a"] = 2.0 * sp["fec_a"]
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    orc.step(1)
+    sim.step(1)
+    for s in range(len(cfg["species"])):
+        parity.assert_logs_equal(sim.read_log(s), orc.log(s), tag="C%d+%s species %d" % (which, variant, s))
+    parity.assert_state_equal(sim, orc, cfg, tag="C%d+%s full size" % (which, variant))
+    assert sim.status() == orc.flags
+    sim.close()
