@@ -348,20 +348,66 @@ __global__ void __launch_bounds__(256) k_mate_weight(const __grid_constant__ SpK
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     const uint8_t *pop = sp.pop[st.cur];
     const uint32_t *rowptr = sp.rowptr[st.cur];
+    const uint8_t *sex = sp.sex[st.cur];
     const float zbar = N ? __double2float_rn(__dmul_rn(__ddiv_rn((double)st.sum_zi0, (double)N), (double)sp.pheno_scale)) : 0.0f;
     if (warp0 == 0 && lane == 0) st.zbar_self = zbar;
-    for (uint32_t i = warp0; i < N; i += nw) {
-        const int32_t zi = warp_row_zi(sp, pop + (size_t)rowptr[i] * sp.row_bytes);
-        if (lane == 0) {
-            const float d = __fsub_rn(__fmul_rn((float)zi, sp.pheno_scale), zbar);
-            float e = __fmul_rn(sp.mate_v, d);
-            e = fminf(fmaxf(e, -16.0f), 16.0f);
-            const float w = expf_spec(__fsub_rn(e, 16.0f));
-            unsigned long long wi = (unsigned long long)__fmul_rn(w, 0x1p40f);
-            if (sp.sexes && !sp.sex[st.cur][rowptr[i]]) wi = 0ull;   // R21: only males father eggs
-            sp.mate_cum[i] = wi;
-            if (wi) atomicAdd(&sp.mate_tile[i / MATE_TILE], wi);
+    // G lanes share one adult (128-bit loads, a row of up to 512 bytes in one load per lane), 32 / G
+    // adults per warp pass; a warp takes BLOCKS of 32 consecutive adults, so that the tile total gets
+    // one atomic per block instead of one per adult (32 divides MATE_TILE: a block lies in one tile)
+    uint32_t G = 1;
+    while (G < 32u && G < sp.row_u4) G <<= 1;
+    const uint32_t apw = 32u / G, grp = lane / G, q = lane % G;
+    const uint32_t n_blocks = (N + 31u) / 32u;
+    for (uint32_t blk = warp0; blk < n_blocks; blk += nw) {
+        const uint32_t blk_end = min(blk * 32u + 32u, N);
+        int32_t my_sum = 0;   // lane l ends up with the allele sum of adult blk * 32 + l
+        // four passes at a time: their row loads are issued before the first reduction
+        for (uint32_t i0 = blk * 32u; i0 < blk_end; i0 += 4u * apw) {
+            int32_t acc[4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                const uint32_t i = i0 + p * apw + grp;
+                acc[p] = 0;
+                if (i < blk_end) {
+                    const uint4 *r4 = (const uint4 *)(pop + (size_t)rowptr[i] * sp.row_bytes);
+                    for (uint32_t k = q; k < sp.row_u4; k += G) {
+                        const uint4 v = r4[k];
+                        if (sp.kind == 0) acc[p] += __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w);
+                        else acc[p] += (int32_t)(int16_t)(v.x & 0xFFFFu) + (int32_t)(int16_t)(v.x >> 16) +
+                                       (int32_t)(int16_t)(v.y & 0xFFFFu) + (int32_t)(int16_t)(v.y >> 16) +
+                                       (int32_t)(int16_t)(v.z & 0xFFFFu) + (int32_t)(int16_t)(v.z >> 16) +
+                                       (int32_t)(int16_t)(v.w & 0xFFFFu) + (int32_t)(int16_t)(v.w >> 16);
+                    }
+                }
+            }
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                int32_t a_ = acc[p];
+                for (uint32_t o = G >> 1; o > 0; o >>= 1) a_ += __shfl_xor_sync(0xffffffffu, a_, o);
+                // the sum of the pass's adult number g sits in lanes g*G..; lane (base + g) of the block takes it
+                const uint32_t base = (i0 - blk * 32u) + p * apw;
+                const int32_t got = __shfl_sync(0xffffffffu, a_, ((lane - base) & (apw - 1u)) * G);
+                if (lane >= base && lane < base + apw) my_sum = got;
+            }
         }
+        // the weights of the block's 32 adults, one per lane (R19, fp32 in the stated order)
+        unsigned long long part = 0ull;
+        {
+            const uint32_t i = blk * 32u + lane;
+            if (i < N) {
+                const int32_t zi = sp.kind == 0 ? 2 * my_sum - 2 * (int32_t)sp.L : my_sum;
+                const float d = __fsub_rn(__fmul_rn((float)zi, sp.pheno_scale), zbar);
+                float e = __fmul_rn(sp.mate_v, d);
+                e = fminf(fmaxf(e, -16.0f), 16.0f);
+                const float w = expf_spec(__fsub_rn(e, 16.0f));
+                unsigned long long wi = (unsigned long long)__fmul_rn(w, 0x1p40f);
+                if (sp.sexes && !sex[rowptr[i]]) wi = 0ull;   // R21: only males father eggs
+                sp.mate_cum[i] = wi;
+                part = wi;
+            }
+        }
+        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+        if (lane == 0 && part) atomicAdd(&sp.mate_tile[blk * 32u / MATE_TILE], part);
     }
 }
 
