@@ -335,13 +335,55 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
     }
 }
 
-__device__ __forceinline__ int32_t warp_row_zi(const SpK &sp, const uint8_t *row);
+// Integer genetic values (R10) of the block of 32 consecutive adults blk * 32 .. of the current
+// population, one per lane: lane l returns zi of adult blk * 32 + l (0 beyond n).  Called by a whole
+// warp.  G lanes share one adult (128-bit loads: a row of up to 512 bytes is one load per lane),
+// 32 / G adults per pass, four passes' loads in flight before the first reduction.
+__device__ __forceinline__ int32_t block_adult_zi(const SpK &sp, const uint8_t *__restrict__ pop,
+                                                  const uint32_t *__restrict__ rowptr, uint32_t blk, uint32_t n) {
+    const uint32_t lane = threadIdx.x & 31u;
+    uint32_t G = 1;
+    while (G < 32u && G < sp.row_u4) G <<= 1;
+    const uint32_t apw = 32u / G, grp = lane / G, q = lane % G;
+    const uint32_t blk_end = min(blk * 32u + 32u, n);
+    int32_t my_sum = 0;
+    for (uint32_t i0 = blk * 32u; i0 < blk_end; i0 += 4u * apw) {
+        int32_t acc[4];
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const uint32_t i = i0 + p * apw + grp;
+            acc[p] = 0;
+            if (i < blk_end) {
+                const uint4 *r4 = (const uint4 *)(pop + (size_t)rowptr[i] * sp.row_bytes);
+                for (uint32_t k = q; k < sp.row_u4; k += G) {
+                    const uint4 v = r4[k];
+                    if (sp.kind == 0) acc[p] += __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w);
+                    else acc[p] += (int32_t)(int16_t)(v.x & 0xFFFFu) + (int32_t)(int16_t)(v.x >> 16) +
+                                   (int32_t)(int16_t)(v.y & 0xFFFFu) + (int32_t)(int16_t)(v.y >> 16) +
+                                   (int32_t)(int16_t)(v.z & 0xFFFFu) + (int32_t)(int16_t)(v.z >> 16) +
+                                   (int32_t)(int16_t)(v.w & 0xFFFFu) + (int32_t)(int16_t)(v.w >> 16);
+                }
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            int32_t a_ = acc[p];
+            for (uint32_t o = G >> 1; o > 0; o >>= 1) a_ += __shfl_xor_sync(0xffffffffu, a_, o);
+            // the sum of the pass's adult number g sits in lanes g*G..; lane (base + g) of the block takes it
+            const uint32_t base = (i0 - blk * 32u) + p * apw;
+            const int32_t got = __shfl_sync(0xffffffffu, a_, ((lane - base) & (apw - 1u)) * G);
+            if (lane >= base && lane < base + apw) my_sum = got;
+        }
+    }
+    return sp.kind == 0 ? 2 * my_sum - 2 * (int32_t)sp.L : my_sum;
+}
 
 // R19 ("shared preference"; eq. S2-10): integer mating weight of every
 // adult, w_i = trunc(expf_spec(clamp(v (z_i - zbar), -16, 16) - 16) * 2^40), fp32 in this order, zbar the
-// adults' mean genetic value (fp64 sum / N * scale rounded to fp32, as zbar_C of R14).  One warp per
-// adult (the genetic value is re-read from its row); the raw weight goes to mate_cum[i] and is added
-// to its tile's total (integer atomics: exact in any order).
+// adults' mean genetic value (fp64 sum / N * scale rounded to fp32, as zbar_C of R14).  A warp takes
+// blocks of 32 consecutive adults (their genetic values are re-read from the rows), computes the 32
+// weights one per lane, stores them to mate_cum[] and adds their sum to the tile's total (one integer
+// atomic per block -- 32 divides MATE_TILE -- exact in any order).
 __global__ void __launch_bounds__(256) k_mate_weight(const __grid_constant__ SpK sp) {
     DevSpecies &st = *sp.st;
     const uint32_t N = st.n0, lane = threadIdx.x & 31u;
@@ -351,60 +393,19 @@ __global__ void __launch_bounds__(256) k_mate_weight(const __grid_constant__ SpK
     const uint8_t *sex = sp.sex[st.cur];
     const float zbar = N ? __double2float_rn(__dmul_rn(__ddiv_rn((double)st.sum_zi0, (double)N), (double)sp.pheno_scale)) : 0.0f;
     if (warp0 == 0 && lane == 0) st.zbar_self = zbar;
-    // G lanes share one adult (128-bit loads, a row of up to 512 bytes in one load per lane), 32 / G
-    // adults per warp pass; a warp takes BLOCKS of 32 consecutive adults, so that the tile total gets
-    // one atomic per block instead of one per adult (32 divides MATE_TILE: a block lies in one tile)
-    uint32_t G = 1;
-    while (G < 32u && G < sp.row_u4) G <<= 1;
-    const uint32_t apw = 32u / G, grp = lane / G, q = lane % G;
-    const uint32_t n_blocks = (N + 31u) / 32u;
-    for (uint32_t blk = warp0; blk < n_blocks; blk += nw) {
-        const uint32_t blk_end = min(blk * 32u + 32u, N);
-        int32_t my_sum = 0;   // lane l ends up with the allele sum of adult blk * 32 + l
-        // four passes at a time: their row loads are issued before the first reduction
-        for (uint32_t i0 = blk * 32u; i0 < blk_end; i0 += 4u * apw) {
-            int32_t acc[4];
-#pragma unroll
-            for (int p = 0; p < 4; ++p) {
-                const uint32_t i = i0 + p * apw + grp;
-                acc[p] = 0;
-                if (i < blk_end) {
-                    const uint4 *r4 = (const uint4 *)(pop + (size_t)rowptr[i] * sp.row_bytes);
-                    for (uint32_t k = q; k < sp.row_u4; k += G) {
-                        const uint4 v = r4[k];
-                        if (sp.kind == 0) acc[p] += __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w);
-                        else acc[p] += (int32_t)(int16_t)(v.x & 0xFFFFu) + (int32_t)(int16_t)(v.x >> 16) +
-                                       (int32_t)(int16_t)(v.y & 0xFFFFu) + (int32_t)(int16_t)(v.y >> 16) +
-                                       (int32_t)(int16_t)(v.z & 0xFFFFu) + (int32_t)(int16_t)(v.z >> 16) +
-                                       (int32_t)(int16_t)(v.w & 0xFFFFu) + (int32_t)(int16_t)(v.w >> 16);
-                    }
-                }
-            }
-#pragma unroll
-            for (int p = 0; p < 4; ++p) {
-                int32_t a_ = acc[p];
-                for (uint32_t o = G >> 1; o > 0; o >>= 1) a_ += __shfl_xor_sync(0xffffffffu, a_, o);
-                // the sum of the pass's adult number g sits in lanes g*G..; lane (base + g) of the block takes it
-                const uint32_t base = (i0 - blk * 32u) + p * apw;
-                const int32_t got = __shfl_sync(0xffffffffu, a_, ((lane - base) & (apw - 1u)) * G);
-                if (lane >= base && lane < base + apw) my_sum = got;
-            }
-        }
-        // the weights of the block's 32 adults, one per lane (R19, fp32 in the stated order)
+    for (uint32_t blk = warp0; blk < (N + 31u) / 32u; blk += nw) {
+        const int32_t zi = block_adult_zi(sp, pop, rowptr, blk, N);
+        const uint32_t i = blk * 32u + lane;
         unsigned long long part = 0ull;
-        {
-            const uint32_t i = blk * 32u + lane;
-            if (i < N) {
-                const int32_t zi = sp.kind == 0 ? 2 * my_sum - 2 * (int32_t)sp.L : my_sum;
-                const float d = __fsub_rn(__fmul_rn((float)zi, sp.pheno_scale), zbar);
-                float e = __fmul_rn(sp.mate_v, d);
-                e = fminf(fmaxf(e, -16.0f), 16.0f);
-                const float w = expf_spec(__fsub_rn(e, 16.0f));
-                unsigned long long wi = (unsigned long long)__fmul_rn(w, 0x1p40f);
-                if (sp.sexes && !sex[rowptr[i]]) wi = 0ull;   // R21: only males father eggs
-                sp.mate_cum[i] = wi;
-                part = wi;
-            }
+        if (i < N) {
+            const float d = __fsub_rn(__fmul_rn((float)zi, sp.pheno_scale), zbar);
+            float e = __fmul_rn(sp.mate_v, d);
+            e = fminf(fmaxf(e, -16.0f), 16.0f);
+            const float w = expf_spec(__fsub_rn(e, 16.0f));
+            unsigned long long wi = (unsigned long long)__fmul_rn(w, 0x1p40f);
+            if (sp.sexes && !sex[rowptr[i]]) wi = 0ull;   // R21: only males father eggs
+            sp.mate_cum[i] = wi;
+            part = wi;
         }
         for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
         if (lane == 0 && part) atomicAdd(&sp.mate_tile[blk * 32u / MATE_TILE], part);
@@ -747,22 +748,28 @@ __global__ void __launch_bounds__(256) k_phenotype(const __grid_constant__ SpK s
 // phenotypes of the current adults (write_state / read_state): zi[] and their sum
 __global__ void __launch_bounds__(256) k_adult_zi(const __grid_constant__ SpK sp, uint32_t n, int accumulate) {
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t cur = sp.st->cur, lane = threadIdx.x & 31u;
     long long acc = 0;
-    for (uint32_t i = warp0; i < n; i += nw) {
-        const int32_t zi = warp_row_zi(sp, sp.pop[sp.st->cur] + (size_t)sp.rowptr[sp.st->cur][i] * sp.row_bytes);
-        if ((threadIdx.x & 31u) == 0) { sp.zi[i] = zi; acc += zi; }
+    for (uint32_t blk = warp0; blk < (n + 31u) / 32u; blk += nw) {
+        const int32_t zi = block_adult_zi(sp, sp.pop[cur], sp.rowptr[cur], blk, n);
+        const uint32_t i = blk * 32u + lane;
+        if (i < n) { sp.zi[i] = zi; acc += zi; }
     }
-    if (accumulate && (threadIdx.x & 31u) == 0 && acc != 0)
-        atomicAdd((unsigned long long *)&sp.st->sum_zi, (unsigned long long)acc);
+    if (accumulate) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0 && acc != 0) atomicAdd((unsigned long long *)&sp.st->sum_zi, (unsigned long long)acc);
+    }
 }
 
 // R20: integer genetic values of this species' current adults, for the species that meets them
 __global__ void __launch_bounds__(256) k_enc_zi(const __grid_constant__ SpK sp) {
     const uint32_t N = sp.st->n0, cur = sp.st->cur;
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
-    for (uint32_t i = warp0; i < N; i += nw) {
-        const int32_t zi = warp_row_zi(sp, sp.pop[cur] + (size_t)sp.rowptr[cur][i] * sp.row_bytes);
-        if ((threadIdx.x & 31u) == 0) sp.enc_zi[i] = zi;
+    for (uint32_t blk = warp0; blk < (N + 31u) / 32u; blk += nw) {
+        const int32_t zi = block_adult_zi(sp, sp.pop[cur], sp.rowptr[cur], blk, N);
+        const uint32_t i = blk * 32u + (threadIdx.x & 31u);
+        if (i < N) sp.enc_zi[i] = zi;
     }
 }
 
@@ -855,7 +862,7 @@ __global__ void __launch_bounds__(256) k_survival(const __grid_constant__ SpK sp
 
 // R18, overlapping generations: adult i stays alive with probability
 // s_A * w(z_i) -- w the Gaussian term of R11 at its genetic value, the uniform word 1 of its FEC
-// block; fp32 in this order: p = s_A * w.  One warp per adult (the genetic value is re-read from its row).
+// block; fp32 in this order: p = s_A * w.  A warp per block of 32 adults, one adult per lane (the genetic values are re-read from the rows).
 __global__ void __launch_bounds__(256) k_adult_survive(const __grid_constant__ SpK sp) {
     DevSpecies &st = *sp.st;
     const uint32_t N = st.n0, step = sp.glob->step, lane = threadIdx.x & 31u;
@@ -864,9 +871,10 @@ __global__ void __launch_bounds__(256) k_adult_survive(const __grid_constant__ S
     const uint32_t *rowptr = sp.rowptr[st.cur];
     const float theta = sp.theta_patch ? sp.theta_patch[0] : st.theta_t;
     unsigned int ties = 0;
-    for (uint32_t i = warp0; i < N; i += nw) {
-        const int32_t zi = warp_row_zi(sp, pop + (size_t)rowptr[i] * sp.row_bytes);
-        if (lane == 0) {
+    for (uint32_t blk = warp0; blk < (N + 31u) / 32u; blk += nw) {   // a warp per block of 32 adults, one adult per lane
+        const int32_t zi = block_adult_zi(sp, pop, rowptr, blk, N);
+        const uint32_t i = blk * 32u + lane;
+        if (i < N) {
             uint32_t x[4];
             draw_rk(sp, ST_FEC, i, 0, step, x);
             const float u = u01_of(x[1]);
