@@ -326,7 +326,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` capture summarised under profiles/ (None until a capture exists).
-TRAFFIC_BYTES = {"C3": 551.3e6, "C5": 3163.1e6}   # profiles/r01_fused_full.md: C3 344.9 MB read + 206.5 MB written; C5 1.52 + 1.64 GB
+TRAFFIC_BYTES = {"C3": 549.9e6, "C5": 3163.1e6}   # profiles/r01_fused_full.md: C3 344.9 MB read + 205.0 MB written; C5 1.52 + 1.64 GB
 
 
 def main():
