@@ -430,3 +430,28 @@ def test_full_size_widenings(oracle_mod, binding, which, variant):
     parity.assert_state_equal(sim, orc, cfg, tag="C%d+%s full size" % (which, variant))
     assert sim.status() == orc.flags
     sim.close()
+
+
+@pytest.mark.parametrize("which,scale", [(3, 1.0), (2, 1.0), (5, 0.1), (4, 0.05)])
+def test_sixteen_step_graph_equals_single_steps(binding, which, scale):
+    """spegg_step(n) replays a sixteen-step graph for long runs (the launch configuration bench.py
+    times: consecutive steps' kernels overlap through programmatic edges) and a one-step graph for
+    the remainder.  Both must produce the same trajectory: 35 steps in one call against 35 calls of
+    one step, at C3's full size -- whose first steps are checked against the oracle in
+    test_full_size_bench_configuration -- state and log compared bit for bit."""
+    cfg = workloads.config(which, scale=scale)
+    a = binding.Sim(cfg, debug=False)
+    b = binding.Sim(cfg, debug=False)
+    parity.load_initial(a, cfg)
+    parity.load_initial(b, cfg)
+    a.step(35)
+    for _ in range(35):
+        b.step(1)
+    for s in range(len(cfg["species"])):
+        assert a.read_log(s) == b.read_log(s)
+        ra, pa, za = a.read_state(s)
+        rb, pb, zb = b.read_state(s)
+        assert np.array_equal(ra, rb) and np.array_equal(pa, pb) and np.array_equal(za, zb)
+    assert a.status() == b.status() and a.step_counter == b.step_counter == 35
+    a.close()
+    b.close()
