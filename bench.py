@@ -312,16 +312,37 @@ def run_ours(args):
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": TRAFFIC_BYTES.get(cfg["name"]),
+
                          "kernel": ("fused step kernel: scan+parents+gametes+phenotype+survival+compaction" if sim.launches_per_step() == 1 else "gamete kernel") if k_n else "none",
                          "kernel_ms": k_ms, "kernel_launches_timed": k_n, "alg_bytes_per_launch": k_bytes,
                          "peak_source": peak_src},
             "cpu_baseline": {"value": cb_units / cb_dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                              "sample": "%d step(s) of the full workload (N0=%d), %.1f s" % (cb_steps, cb_cfg["n0"][0], cb_dt)},
         }
+        sp0 = cfg["species"][0]
+        if sp0["kind"] == "q10" and k_ms > 0:
+            # quantised-effect genomes draw one Philox word per locus per gamete (R7): the second ceiling of the
+            # gamete kernel is integer issue ('ALU roofline'), reported beside the HBM one
+            ops = alu_ops_per_offspring(sp0["n_loci"]) * sum(e["m_t"] for e in klog) / max(1, len(klog))
+            a_alu = ops / (k_ms * 1e-3) / 1e12
+            line["roofline"]["alu"] = {"achieved": a_alu, "peak": ALU_PEAK_TINST, "unit": "Tinst/s",
+                                       "frac": a_alu / ALU_PEAK_TINST, "alg_inst_per_launch": ops,
+                                       "peak_source": "148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (DESIGN.md 5)"}
         print(json.dumps(line))
     sim.close()
     if dist is not None:
         dist.destroy_process_group()
+
+
+# ALU roofline of the q10 gamete kernel: algorithmic thread-instructions per offspring =
+# Philox blocks x 44 (ten rounds of two 32x32->64 multiplies and two three-input XORs, plus the
+# counter set-up) + 4 per locus per gamete (threshold compare, phase parity, select, allele sum);
+# blocks = 2L/4 RECOMB + 1 SCALAR + 2 MUT.  Peak = one warp instruction per scheduler per clock.
+ALU_PEAK_TINST = 148 * 4 * 32 * 1.965e9 / 1e12
+
+
+def alu_ops_per_offspring(n_loci):
+    return (2 * n_loci // 4 + 3) * 44 + 2 * n_loci * 4
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
