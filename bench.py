@@ -209,7 +209,7 @@ def run_ours(args):
 
     cfg = workload(args.config, seed_offset=rank, world=world, variant=args.variant)
     n_sp = len(cfg["species"])
-    sim = binding.Sim(cfg, debug=False, log_capacity=max(4096, args.steps * 3 + args.warmup + 64), device=str(dev))
+    sim = binding.Sim(cfg, debug=False, log_capacity=max(4096, args.steps * 4 + args.warmup + 256), device=str(dev))
     rows0 = [workloads.initial_rows(cfg, s) for s in range(n_sp)]
     ps0 = [workloads.initial_patch_start(cfg, s) for s in range(n_sp)]
     sex0 = [workloads.initial_sex(cfg, s) if cfg["species"][s].get("separate_sexes") else None for s in range(n_sp)]
@@ -243,6 +243,17 @@ def run_ours(args):
     units = sum(sum(e["n_t"] for e in lg) for lg in logs)
     offspring = sum(sum(e["m_t"] for e in lg) for lg in logs)
     flags = sim.status()
+    # two more timed sections of K steps (report the spread); `value` is the first one
+    repeats = [ms / args.steps]
+    for _ in range(2):
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        with torch.cuda.stream(sim.stream):
+            r0.record(sim.stream)
+            sim.step(args.steps)
+            r1.record(sim.stream)
+        barrier()
+        repeats.append(r0.elapsed_time(r1) / args.steps)
 
     # ---- dominant kernel timed alone with CUDA events on its own stream (direct launches)
     kt_steps = min(args.steps, 100)
@@ -301,6 +312,7 @@ def run_ours(args):
             "config": {"workload": describe(cfg), "parallelism": ("patches sharded x%d, no collective" if args.config == 6 else "replicas only x%d") % world,
                        "l2": "inputs larger than L2 (two %d MB population buffers vs 126 MB L2)" % (
                            cfg["species"][0]["capacity"] * row_bytes(cfg["species"][0]) // 2 ** 20),
+                       "ms_per_step_repeats": [round(x, 6) for x in repeats],
                        "mean_N_t": units / args.steps / world, "mean_M_t": offspring / args.steps / world,
                        "flags": flags, "offspring_per_s": offspring / (ms * 1e-3),
                        "step_alg_bytes": step_bytes,
