@@ -455,3 +455,22 @@ def test_sixteen_step_graph_equals_single_steps(binding, which, scale):
     assert a.status() == b.status() and a.step_counter == b.step_counter == 35
     a.close()
     b.close()
+
+
+@pytest.mark.parametrize("n0", [1, 31, 33, 1023, 1025, 2049])
+def test_mating_paths_ragged_sizes(oracle_mod, binding, n0):
+    """Ragged tails of the mating path: one adult, a block of 32 minus / plus one, a weight tile of
+    1,024 minus / plus one, two tiles plus one -- separate sexes with weighted fathers, per-step
+    parity of every intermediate; and an empty population stays empty."""
+    cfg = workloads.config(1, scale=n0 / 1000.0)
+    cfg["n0"] = [n0]
+    sp = cfg["species"][0]
+    sp.update(separate_sexes=1, mate_skew=2.0, K=float(max(n0, 8)), capacity=max(4 * n0, 256))
+    sp["fec_a"] = 4.0
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=False)
+    sim = binding.Sim(cfg, debug=False)
+    sim.write_state(0, workloads.initial_rows(cfg, 0)[:0], None, 0)
+    sim.step(2)
+    assert sim.n(0) == 0 and (sim.status() & 2) and len(sim.read_sex(0)) == 0
+    sim.close()
