@@ -431,6 +431,21 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         else tab = patch_of(S, P, i);
         D.f[i] = (uint8_t)poisson_count(&D.tables[(size_t)tab * ORC_TMAX], (int)D.table_len[tab], x[0]);
         if (S.p.separate_sexes && S.sex[i]) D.f[i] = 0; /* R21: males lay no eggs (the draw is made and ignored) */
+        if (S.p.fec_cost > 0.0 && D.f[i] > 0) {
+            /* R22 (eq. S3-3): fecundity times exp(-rho z_i^2), z_i the adult's genetic value.
+             * A Poisson count thinned egg by egg is Poisson with the mean multiplied, so: egg k of the
+             * f_i drawn is laid iff u01(word (2+k)%4 of FEC block (2+k)/4) < c_i, fp32 in this order:
+             * z = zi*scale; c = expf_spec(-(rho * (z*z))).  (Words 0, 1 of block 0 are the count and R18.) */
+            const float z = (float)S.zi[i] * S.p.pheno_scale;
+            const float c = expf_spec(-((float)S.p.fec_cost * (z * z)));
+            uint32_t keep = 0;
+            for (uint32_t k = 0; k < D.f[i]; ++k) {
+                uint32_t y[4];
+                draw(sim.seed, si, FEC, (uint32_t)i, (2 + k) / 4, t, y);
+                if (u01_of(y[(2 + k) % 4]) < c) ++keep;
+            }
+            D.f[i] = (uint8_t)keep;
+        }
     }
     /* ---- a2: exclusive scan ---- */
     uint64_t M = 0;
@@ -718,7 +733,7 @@ orc_sim *orc_create(const orc_params *p) {
             S.R_norm = normal_table(S.p.mut_sd * 1024.0, S.T_norm.data(), NORMAL_CAP);
             if (S.R_norm < 0) { delete sim; return nullptr; }
         }
-        if (!(std::fabs(S.p.mate_skew) <= 1e6)) { delete sim; return nullptr; }
+        if (!(std::fabs(S.p.mate_skew) <= 1e6) || !(S.p.fec_cost >= 0.0 && S.p.fec_cost <= 1e6)) { delete sim; return nullptr; }
         if (S.p.encounters > 16 || (S.p.encounters && (!S.p.sel_predation || !(S.p.attack >= 0.0 && S.p.attack <= 2.0)))) { delete sim; return nullptr; }
         /* R18 is defined for an unstructured species (one patch) */
         if (!(S.p.adult_survival >= 0.0 && S.p.adult_survival <= 1.0) || (S.p.adult_survival > 0.0 && sim->P != 1)) { delete sim; return nullptr; }

@@ -3,7 +3,7 @@
  *
  * TEST INFRASTRUCTURE ONLY.  This is the plain, slow, single-threaded, obviously
  * correct restatement of what the hot path computes (Fig. 1 A-F;
- * PAPER.md:321-330 genetics; the readings R1-R21 in DESIGN.md).  Only tests/,
+ * PAPER.md:321-330 genetics; the readings R1-R22 in DESIGN.md).  Only tests/,
  * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load it.  It shares no code, header, table or constant generator with the CUDA
  * library (include/spegg.h, paper_1603_09255_b200/csrc/): the structs below are
@@ -66,6 +66,9 @@ typedef struct {
                                    at random from mature males and females"): 1 = every individual is
                                    female (0) or male (1); only females lay eggs, only males father them.
                                    0 = hermaphrodites (R2)                                       */
+    double fec_cost;            /* R22 (eq. S3-3: the resource's fecundity is multiplied by
+                                   exp(-rho * trait^2), the cost of its defence): each egg of adult i is
+                                   laid with probability exp(-fec_cost * z_i^2); 0 = no cost        */
 } orc_species_params;
 
 typedef struct {
