@@ -11,7 +11,7 @@
  *   E  survivors identified, dead removed                    (stable stream compaction)
  *   F  environment updated from the survivors' phenotypes   (exact integer reductions, counts)
  * plus migration between patches.  What the paper leaves open (RNG, samplers,
- * density regulation, ...) is fixed by the readings R1-R21 in DESIGN.md.
+ * density regulation, ...) is fixed by the readings R1-R22 in DESIGN.md.
  *
  * Conventions
  *   - Plain C, no exceptions.  Every call returns an int: 0 = SPEGG_OK, <0 = error code
@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SPEGG_ABI_VERSION 5u
+#define SPEGG_ABI_VERSION 6u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
        SPEGG_ESTATE = -5 };
@@ -112,6 +112,10 @@ typedef struct spegg_species_params {
                                    is a fair coin; a patch without males mates as R2.
                                    spegg_write_state makes everybody female: follow it with
                                    spegg_write_sex.  0 = hermaphrodites (R2)                 */
+    double fec_cost;            /* rho: fecundity cost of defence (eq. S3-3; R22): the
+                                   fecundity of adult i is multiplied by exp(-rho z_i^2) -- each of
+                                   the eggs drawn for it is laid with that probability (a thinned
+                                   Poisson count is Poisson with the mean multiplied).  0 = none  */
 } spegg_species_params;
 
 typedef struct spegg_params {

@@ -432,7 +432,7 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         D.f[i] = (uint8_t)poisson_count(&D.tables[(size_t)tab * ORC_TMAX], (int)D.table_len[tab], x[0]);
         if (S.p.separate_sexes && S.sex[i]) D.f[i] = 0; /* R21: males lay no eggs (the draw is made and ignored) */
         if (S.p.fec_cost > 0.0 && D.f[i] > 0) {
-            /* R22 (eq. S3-3, PAPER.md:469): fecundity times exp(-rho z_i^2), z_i the adult's genetic value.
+            /* R22 (eq. S3-3, PAPER.md:471): fecundity times exp(-rho z_i^2), z_i the adult's genetic value.
              * A Poisson count thinned egg by egg is Poisson with the mean multiplied, so: egg k of the
              * f_i drawn is laid iff u01(word (2+k)%4 of FEC block (2+k)/4) < c_i, fp32 in this order:
              * z = zi*scale; c = expf_spec(-(rho * (z*z))).  (Words 0, 1 of block 0 are the count and R18.) */

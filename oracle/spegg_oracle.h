@@ -66,7 +66,7 @@ typedef struct {
                                    at random from mature males and females"): 1 = every individual is
                                    female (0) or male (1); only females lay eggs, only males father them.
                                    0 = hermaphrodites (R2)                                       */
-    double fec_cost;            /* R22 (eq. S3-3, PAPER.md:469: the resource's fecundity is multiplied by
+    double fec_cost;            /* R22 (eq. S3-3, PAPER.md:471: the resource's fecundity is multiplied by
                                    exp(-rho * trait^2), the cost of its defence): each egg of adult i is
                                    laid with probability exp(-fec_cost * z_i^2); 0 = no cost        */
 } orc_species_params;

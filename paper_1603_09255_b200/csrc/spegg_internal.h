@@ -112,6 +112,7 @@ struct SpK {
     uint8_t *sex[2];
     uint8_t *sex_off;           // [m] sex of each offspring of the current step (staging; also I/O staging)
     // R20, individual-level encounters (enc_E > 0 on the prey; enc_zi filled on the species it meets)
+    float fec_cost;             // R22: rho of the fecundity cost exp(-rho z^2); 0 = none (uses enc_zi of this species)
     uint32_t enc_E;             // meetings per newborn; 0 = mean-field predation term (R14)
     float enc_v;                // v = fp32(attack)
     int32_t *enc_zi;            // [n] integer genetic values of THIS species' adults (when another species meets them)

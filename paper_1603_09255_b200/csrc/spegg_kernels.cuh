@@ -283,6 +283,19 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
                     f = poisson_count(sp.tables + (size_t)tab * TMAX, sp.table_len[tab], x[0]);
                 }
                 if (sp.sexes && sp.sex[st.cur][rowptr[i]]) f = 0;   // R21: males lay no eggs (the draw is made and ignored)
+                if (sp.fec_cost > 0.0f && f) {
+                    // R22 (eq. S3-3): egg k is laid iff u01(word (2+k)%4 of FEC block (2+k)/4) < c_i,
+                    // c_i = expf_spec(-(rho * (z*z))), z the adult's genetic value (k_enc_zi ran before this kernel)
+                    const float z = __fmul_rn((float)sp.enc_zi[i], sp.pheno_scale);
+                    const float c = expf_spec(-__fmul_rn(sp.fec_cost, __fmul_rn(z, z)));
+                    uint32_t keep = 0, y[4] = {x[0], x[1], x[2], x[3]};
+                    for (uint32_t k = 0; k < f; ++k) {
+                        const uint32_t w = 2u + k;
+                        if (k > 0 && (w & 3u) == 0) draw(sp.key, sp.species, ST_FEC, i, w >> 2, step, y);
+                        if (u01_of(y[w & 3u]) < c) ++keep;
+                    }
+                    f = keep;
+                }
             }
             s_f[k] = (uint8_t)f;
         }

@@ -474,3 +474,44 @@ def test_mating_paths_ragged_sizes(oracle_mod, binding, n0):
     sim.step(2)
     assert sim.n(0) == 0 and (sim.status() & 2) and len(sim.read_sex(0)) == 0
     sim.close()
+
+
+@pytest.mark.parametrize("which,scale,rho,grid,extra", [
+    (1, 1.0, 0.5, None, {}),
+    (2, 0.05, 2.0, None, {"fec_a": 6.0}),                     # up to a dozen eggs drawn per adult: several FEC blocks
+    (3, 0.01, 0.02, None, {}),                                # bit genome on the general pipeline
+    (5, 0.03, 1.0, (5, 4), {}),                               # patches
+    (2, 0.04, 1.0, None, {"separate_sexes": 1, "mate_skew": 1.0, "adult_survival": 0.5, "fec_a": 6.0}),
+])
+def test_fecundity_cost(oracle_mod, binding, which, scale, rho, grid, extra):
+    """R22 (eq. S3-3): each egg of adult i is laid with probability exp(-rho z_i^2).
+    Per-step parity of every intermediate (debug), then a free-running trajectory on the production
+    kernels."""
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    sp = cfg["species"][0]
+    sp["fec_cost"] = rho
+    sp.update(extra)
+    if "adult_survival" in extra:
+        sp["capacity"] = 4 * sp["capacity"]
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(2):
+        orc.step(5)
+        sim.step(5)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+        parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags
+    sim.close()
+
+
+def test_resource_with_cost_meets_consumers(oracle_mod, binding):
+    """The S3 community in one piece: the resource pays the fecundity cost of its defence trait (R22),
+    its newborns meet consumers individually (R20), the consumers' fecundity follows their captures."""
+    cfg = workloads.config(4, scale=0.004)
+    cfg["species"][0]["predation"].update(encounters=3, attack=0.1)
+    cfg["species"][0]["fec_cost"] = 0.05
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    parity.per_step_parity(oracle_mod, binding, cfg, 4, debug=False)

@@ -1,4 +1,4 @@
-"""Pins for the oracle's fecundity cost of defence (reading R22; eq. S3-3, PAPER.md:469:
+"""Pins for the oracle's fecundity cost of defence (reading R22; eq. S3-3, PAPER.md:471:
 w_F,R <- w_F,R * n_i * exp(-rho * trait^2)).  -m "not gpu".
 
 A Poisson count thinned egg by egg with probability c is Poisson with mean lambda*c: pinned on a
