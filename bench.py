@@ -97,6 +97,7 @@ VARIANTS = {
     "mating": {"mate_skew": 1.0},                      # R19
     "sexes": {"separate_sexes": 1},                    # R21 (fecundity parameter x 2: half the adults lay eggs)
     "encounters": {},                                  # R20 (configuration 4 only: 3 meetings, attack 0.1)
+    "cost": {"fec_cost": 0.05},                        # R22
 }
 
 
