@@ -45,7 +45,7 @@ class _SpeciesParams(C.Structure):
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
         ("mate_skew", C.c_double), ("encounters", C.c_uint32), ("separate_sexes", C.c_uint32),
-        ("fec_cost", C.c_double),
+        ("fec_cost", C.c_double), ("assort", C.c_double),
     ]
 
 
@@ -238,6 +238,7 @@ class Oracle:
             p.mate_skew = sp.get("mate_skew", 0.0)
             p.separate_sexes = 1 if sp.get("separate_sexes") else 0
             p.fec_cost = sp.get("fec_cost", 0.0)
+            p.assort = sp.get("assort", 0.0)
             if sp["kind"] == "bit":
                 self.row_shape.append(2 * (L // 32))
                 self.row_dtype.append(np.uint32)

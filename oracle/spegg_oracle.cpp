@@ -56,7 +56,8 @@ void philox(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4]) {
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-enum Stream { FEC = 0, SCALAR = 1, RECOMB_M = 2, RECOMB_P = 3, MUT_M = 4, MUT_P = 5 };
+enum Stream { FEC = 0, SCALAR = 1, RECOMB_M = 2, RECOMB_P = 3, MUT_M = 4, MUT_P = 5, MATE = 6 };
+const uint32_t ASSORT_TRIES = 8; /* R23 */
 
 /* R3: key = (seed_lo, seed_hi); counter = (entity, block, step, species<<8 | stream) */
 void draw(uint64_t seed, uint32_t species, uint32_t stream, uint32_t entity, uint32_t block,
@@ -500,6 +501,24 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
                 fa = (uint32_t)(std::upper_bound(D.mate_cum.begin() + base, D.mate_cum.begin() + base + np, target) - D.mate_cum.begin());
             }
         }
+        if (S.p.assort > 0.0) {
+            /* R23 (assortative mating): candidate t = 0..7, uniform over the adults of the
+             * mother's patch (word 2(t%2) of MATE block t/2, entity j), is accepted iff
+             * u01(word 2(t%2)+1) < expf_spec(-(a * (d*d))), d = z_cand - z_mother (genetic values, fp32,
+             * this order); the first accepted candidate is the father, else the last candidate. */
+            const float a = (float)S.p.assort;
+            const float zm = (float)S.zi[mo] * S.p.pheno_scale;
+            for (uint32_t tr = 0; tr < ASSORT_TRIES; ++tr) {
+                uint32_t y[4];
+                draw(sim.seed, si, MATE, (uint32_t)j, tr / 2, t, y);
+                fa = base + uniform_index(y[2 * (tr & 1)], np);
+                const float d = (float)S.zi[fa] * S.p.pheno_scale - zm;
+                const float p = expf_spec(-(a * (d * d)));
+                const float u = u01_of(y[2 * (tr & 1) + 1]);
+                if (std::fabs(u - p) < 1e-6f) le.near_ties++;
+                if (u < p) break;
+            }
+        }
         D.father[j] = fa;
         /* R15: dispersal drawn at birth */
         uint32_t dest = pm;
@@ -733,6 +752,7 @@ orc_sim *orc_create(const orc_params *p) {
             S.R_norm = normal_table(S.p.mut_sd * 1024.0, S.T_norm.data(), NORMAL_CAP);
             if (S.R_norm < 0) { delete sim; return nullptr; }
         }
+        if (!(S.p.assort >= 0.0 && S.p.assort <= 1e6) || (S.p.assort > 0.0 && (S.p.mate_skew != 0.0 || S.p.separate_sexes))) { delete sim; return nullptr; }
         if (!(std::fabs(S.p.mate_skew) <= 1e6) || !(S.p.fec_cost >= 0.0 && S.p.fec_cost <= 1e6)) { delete sim; return nullptr; }
         if (S.p.encounters > 16 || (S.p.encounters && (!S.p.sel_predation || !(S.p.attack >= 0.0 && S.p.attack <= 2.0)))) { delete sim; return nullptr; }
         /* R18 is defined for an unstructured species (one patch) */
