@@ -11,7 +11,7 @@
  *   E  survivors identified, dead removed                    (stable stream compaction)
  *   F  environment updated from the survivors' phenotypes   (exact integer reductions, counts)
  * plus migration between patches.  What the paper leaves open (RNG, samplers,
- * density regulation, ...) is fixed by the readings R1-R22 in DESIGN.md.
+ * density regulation, ...) is fixed by the readings R1-R23 in DESIGN.md.
  *
  * Conventions
  *   - Plain C, no exceptions.  Every call returns an int: 0 = SPEGG_OK, <0 = error code
@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SPEGG_ABI_VERSION 6u
+#define SPEGG_ABI_VERSION 7u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
        SPEGG_ESTATE = -5 };
@@ -116,6 +116,11 @@ typedef struct spegg_species_params {
                                    fecundity of adult i is multiplied by exp(-rho z_i^2) -- each of
                                    the eggs drawn for it is laid with that probability (a thinned
                                    Poisson count is Poisson with the mean multiplied).  0 = none  */
+    double assort;              /* a: assortative mating (R23): a candidate father,
+                                   uniform over the mother's patch, is accepted with probability
+                                   exp(-a (z_c - z_m)^2) (genetic values); up to 8 candidates,
+                                   the last one is taken if none was accepted.  0 = random
+                                   mating (R2).  Not together with mate_skew / separate_sexes    */
 } spegg_species_params;
 
 typedef struct spegg_params {

@@ -150,6 +150,7 @@ int validate(const spegg_params *p) {
         if (!(q.resid_sd >= 0.0) || !(q.pheno_scale > 0.0f) || q.resid_sd / (double)q.pheno_scale > 4096.0) return SPEGG_EINVAL;
         if (!(std::fabs(q.mate_skew) <= 1e6) || q.separate_sexes > 1) return SPEGG_EINVAL;
         if (!(q.fec_cost >= 0.0 && q.fec_cost <= 1e6)) return SPEGG_EINVAL;
+        if (!(q.assort >= 0.0 && q.assort <= 1e6) || (q.assort > 0.0 && (q.mate_skew != 0.0 || q.separate_sexes))) return SPEGG_EINVAL;
         if (q.fecundity_model == SPEGG_FEC_CAPTURES && P != 1) return SPEGG_EINVAL;
         if (q.sel_predation) {
             if (q.predator_species >= p->n_species || q.predator_species <= s) return SPEGG_EINVAL;
@@ -212,7 +213,7 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         bool is_met = false;   // R20: some species meets this one individually
         for (uint32_t o = 0; o < p->n_species; ++o)
             if (p->species[o].sel_predation && p->species[o].encounters && p->species[o].predator_species == s) is_met = true;
-        l.enc_zi = c.take(((is_met || q.fec_cost > 0.0) ? cap : 1) * 4);   // R22 uses it for the species' own adults
+        l.enc_zi = c.take(((is_met || q.fec_cost > 0.0 || q.assort > 0.0) ? cap : 1) * 4);   // R22, R23 use it for the species' own adults
         l.cap = c.take(cap * 4);
         l.offbuf = c.take(cap * l.row_bytes);
         l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
@@ -284,7 +285,7 @@ int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
 
 // true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
 bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
-    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.mate_on || h.k.fec_cost != 0.0f) return false;
+    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.mate_on || h.k.fec_cost != 0.0f || h.k.assort != 0.0f) return false;
     // the fused kernel tests u >= T as u > T - 1 (see spegg_fused.cuh): every threshold must be >= 1
     for (uint32_t c = 0; c < h.p.n_chrom; ++c)
         for (uint32_t k = 0; k < h.xover_len[c]; ++k)
@@ -324,7 +325,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
                 return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>((items + per_cta - 1) / per_cta, (uint64_t)G * per_sm));
             };
             const uint32_t g_thread = ctas(cap, 256, 8), g_warp = ctas(cap, 8, 8);   // thread / warp per offspring
-            if (k.fec_cost > 0.0f) { k_enc_zi<<<ctas(cap, 8, 8), 256, 0, s->stream>>>(k); ++nl; }   // R22: the adults' genetic values
+            if (k.fec_cost > 0.0f || k.assort > 0.0f) { k_enc_zi<<<ctas(cap, 8, 8), 256, 0, s->stream>>>(k); ++nl; }   // R22, R23: the adults' genetic values
             k_fec_scan<<<ctas(cap, SCAN_THREADS, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
             if (k.mate_on) {   // R19: mating weights of the adults and their running sum
                 k_mate_weight<<<g_warp, 256, 0, s->stream>>>(k); ++nl;
@@ -526,7 +527,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.sexes = q.separate_sexes; k.mate_on = (q.mate_skew != 0.0 || q.separate_sexes) ? 1u : 0u;
         k.sex[0] = at<uint8_t>(s, l.sex[0]); k.sex[1] = at<uint8_t>(s, l.sex[1]); k.sex_off = at<uint8_t>(s, l.sex_off);
         k.mate_cum = at<unsigned long long>(s, l.mate_cum); k.mate_tile = at<unsigned long long>(s, l.mate_tile);
-        k.fec_cost = (float)q.fec_cost;
+        k.fec_cost = (float)q.fec_cost; k.assort = (float)q.assort;
         k.enc_E = q.sel_predation ? q.encounters : 0u; k.enc_v = (float)q.attack;
         k.enc_zi = at<int32_t>(s, l.enc_zi);
         k.cap = at<uint32_t>(s, l.cap);

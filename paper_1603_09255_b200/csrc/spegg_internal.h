@@ -13,6 +13,7 @@ constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 4;
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
 constexpr int MAX_SPECIES = 8;
+constexpr uint32_t ASSORT_TRIES = 8;            // R23: candidate fathers per egg
 constexpr uint32_t MATE_TILE = 1024;             // R19: adults per tile of the mating-weight running sum
 constexpr uint32_t FUSED_RANGE = 1024;            // fused path: rows per scan range (32 slabs of 32 rows)
 
@@ -112,6 +113,7 @@ struct SpK {
     uint8_t *sex[2];
     uint8_t *sex_off;           // [m] sex of each offspring of the current step (staging; also I/O staging)
     // R20, individual-level encounters (enc_E > 0 on the prey; enc_zi filled on the species it meets)
+    float assort;               // R23: a of the acceptance exp(-a d^2) of a candidate father; 0 = random mating (uses enc_zi)
     float fec_cost;             // R22: rho of the fecundity cost exp(-rho z^2); 0 = none (uses enc_zi of this species)
     uint32_t enc_E;             // meetings per newborn; 0 = mean-field predation term (R14)
     float enc_v;                // v = fp32(attack)

@@ -468,6 +468,7 @@ __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) 
     const DevSpecies &st = *sp.st;
     const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
     const uint32_t *ps = sp.patch_start[st.cur];
+    unsigned int ties = 0;
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
         const uint32_t mo = sp.mother[j];
         uint32_t x[4];
@@ -494,6 +495,22 @@ __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) 
                 fa = lo;
             }
         }
+        if (sp.assort > 0.0f) {
+            // R23 (assortative mating): candidate t = 0..7 uniform over the mother's patch (word
+            // 2(t%2) of MATE block t/2), accepted iff u01(word 2(t%2)+1) < expf_spec(-(a * (d*d))),
+            // d = z_cand - z_mother (genetic values from k_enc_zi); first accepted, else the last candidate
+            const float zm = __fmul_rn((float)sp.enc_zi[mo], sp.pheno_scale);
+            uint32_t y[4];
+            for (uint32_t tr = 0; tr < ASSORT_TRIES; ++tr) {
+                if ((tr & 1u) == 0) draw_rk(sp, ST_MATE, j, tr >> 1, step, y);
+                fa = base + uniform_index(y[2 * (tr & 1u)], np);
+                const float d = __fsub_rn(__fmul_rn((float)sp.enc_zi[fa], sp.pheno_scale), zm);
+                const float p = expf_spec(-__fmul_rn(sp.assort, __fmul_rn(d, d)));
+                const float u = u01_of(y[2 * (tr & 1u) + 1]);
+                if (fabsf(__fsub_rn(u, p)) < 1e-6f) ++ties;
+                if (u < p) break;
+            }
+        }
         sp.father[j] = fa;
         uint32_t dest = pm;
         if (sp.P > 1 && (unsigned long long)x[1] < sp.T_mig) dest = neighbour(pm, x[2] >> 30, sp.grid_w, sp.grid_h);
@@ -501,6 +518,7 @@ __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) 
         sp.u01[j] = u01_of(x[3]);
         if (sp.sexes) sp.sex_off[j] = (uint8_t)(x[2] & 1u);   // R21: sex at birth (bits 30-31 of the word are the direction)
     }
+    if (ties) atomicAdd(&sp.st->near_ties, (unsigned long long)ties);
 }
 
 // a4 (bit genomes, Poisson crossovers, R8): one thread per (offspring, gamete, chromosome)

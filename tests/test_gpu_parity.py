@@ -515,3 +515,38 @@ def test_resource_with_cost_meets_consumers(oracle_mod, binding):
     cfg["species"][0]["fec_cost"] = 0.05
     parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
     parity.per_step_parity(oracle_mod, binding, cfg, 4, debug=False)
+
+
+@pytest.mark.parametrize("which,scale,a,grid,extra", [
+    (1, 1.0, 2.0, None, {}),
+    (2, 0.05, 1.0, None, {}),
+    (2, 0.04, 30.0, None, {"resid_sd": 0.3}),              # choosy: most eggs use all 8 candidates
+    (3, 0.01, 0.5, None, {}),                              # bit genome on the general pipeline
+    (5, 0.03, 1.5, (5, 4), {}),                            # candidates from the mother's patch
+    (2, 0.04, 1.0, None, {"adult_survival": 0.5, "fec_cost": 0.2}),
+])
+def test_assortative_mating(oracle_mod, binding, which, scale, a, grid, extra):
+    """R23: candidate fathers accepted with probability exp(-a (z_c - z_m)^2).  Per-step
+    parity of every intermediate (debug), then a free-running trajectory on the production kernels."""
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    sp = cfg["species"][0]
+    sp["assort"] = a
+    sp.update(extra)
+    if "adult_survival" in extra:
+        sp["capacity"] = 4 * sp["capacity"]
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(2):
+        orc.step(5)
+        sim.step(5)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+        parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags
+    sim.close()
+    bad = workloads.config(1)
+    bad["species"][0].update(assort=1.0, mate_skew=1.0)     # the two mating rules exclude each other
+    with pytest.raises(binding.SpeggError):
+        binding.workspace_bytes(bad)
