@@ -193,7 +193,9 @@ int spegg_write_sex(spegg_sim *s, uint32_t species, uint64_t n, const uint8_t *s
 int spegg_read_sex(spegg_sim *s, uint32_t species, uint8_t *sex_out, uint64_t cap_bytes);
 
 /* Enqueues n_steps steps on the stream and returns; no host synchronisation.  Never fails for
- * model reasons: overflow / extinction set sticky device flags (spegg_status). */
+ * model reasons: overflow / extinction set sticky device flags (spegg_status).  Long runs replay a
+ * captured graph of sixteen steps (consecutive steps' kernels overlap through programmatic edges),
+ * the remainder a graph of one step; the trajectory does not depend on how n_steps is split. */
 int spegg_step(spegg_sim *s, uint32_t n_steps);
 
 /* Synchronises, then copies the current adults of `species` out.  Any output may be NULL.
