@@ -126,9 +126,29 @@ def workload(which, seed_offset=0, world=1, variant="none"):
 
 def describe(cfg):
     sp = cfg["species"][0]
-    return "%s: N0=K=%d diploids, L=%d %s loci, %d chromosomes, %s" % (
-        cfg["name"], cfg["n0"][0], sp["n_loci"], "bit-packed" if sp["kind"] == "bit" else "2^-10-quantised",
-        len(sp["chrom_len"]), "patches %dx%d" % cfg["grid"] if cfg["grid"] != (1, 1) else "one panmictic population")
+    if len(cfg["species"]) == 2:
+        what = "two species (resource N0=%d, K=%d + consumer N0=%d), each one panmictic population" % (
+            cfg["n0"][0], int(sp["K"]), cfg["n0"][1])
+    elif cfg["grid"] != (1, 1):
+        what = "N0=%d diploids in patches %dx%d" % ((cfg["n0"][0],) + tuple(cfg["grid"]))
+    else:
+        what = "N0=K=%d diploids, one panmictic population" % cfg["n0"][0]
+    return "%s: %s, L=%d %s loci, %d chromosomes" % (
+        cfg["name"], what, sp["n_loci"], "bit-packed" if sp["kind"] == "bit" else "2^-10-quantised", len(sp["chrom_len"]))
+
+
+L2_BYTES = 126 * 2 ** 20
+
+
+def l2_note(cfg):
+    """Timing rule: inputs larger than L2, or say that they are not."""
+    pop = sum(int(sp["capacity"]) * row_bytes(sp) for sp in cfg["species"])
+    live = sum(n * row_bytes(sp) for n, sp in zip(cfg["n0"], cfg["species"]))
+    if 2 * live > L2_BYTES:
+        return "inputs larger than L2 (two population buffers of %d MB, about %d MB of live rows read and written per step, vs 126 MB L2)" % (
+            pop // 2 ** 20, 2 * live // 2 ** 20)
+    return ("L2-RESIDENT workload (about %.1f MB of live rows per buffer vs 126 MB L2; no flush between steps: a step's "
+            "input IS the previous step's output, so this is the workload's own steady state)") % (live / 2 ** 20)
 
 
 def row_bytes(sp):
@@ -224,6 +244,17 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- clock warm: the GPU leaves its idle clocks only after some milliseconds of work, far more than
+    # W = 5 steps of 0.15 ms.  Untimed steps on the same handle, then the initial state is written again,
+    # so the W warm-up and K timed steps below start from exactly the state of a fresh run.
+    if args.clock_warm_steps > 0:
+        sim.step(args.clock_warm_steps)
+        sim.synchronize()
+        for s in range(n_sp):
+            sim.write_state(s, rows0[s], ps0[s], 0)
+            if sex0[s] is not None:
+                sim.write_sex(s, sex0[s])
+
     # ---- device-timed run: inputs resident in HBM, K graph replays, no host sync inside
     sim.step(args.warmup)
     barrier()
@@ -284,7 +315,7 @@ def run_ours(args):
     for _ in range(e2e_steps):
         sim.step(1)
         for s in range(n_sp):
-            e = sim.read_log(s)[-1]      # device -> host read of the step's result (64-byte entry)
+            e = sim.read_log(s, last=1)[-1]      # device -> host read of the step's result (64-byte entry)
             e_units += e["n_t"]
             d2h += 64
     for s in range(n_sp):
@@ -302,6 +333,7 @@ def run_ours(args):
         peak, peak_src = load_peaks()
         achieved = k_bytes / (k_ms * 1e-3) / 1e9 if k_ms > 0 else 0.0
         step_bytes = alg_bytes(cfg, logs[0], kernel_only=False) / max(1, len(logs[0]))
+        traffic, traffic_src = measured_traffic(cfg["name"])
         # oracle on a bounded sample of the same workload: ~10-30 s of CPU work
         cb_cfg = workload(args.config, variant=args.variant)
         cb_steps = 1 if cb_cfg["n0"][0] >= 500_000 else max(1, int(1.0e6 / cb_cfg["n0"][0]))
@@ -311,8 +343,8 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u32", "data": "synthetic",
             "config": {"workload": describe(cfg), "parallelism": ("patches sharded x%d, no collective" if args.config == 6 else "replicas only x%d") % world,
-                       "l2": "inputs larger than L2 (two %d MB population buffers vs 126 MB L2)" % (
-                           cfg["species"][0]["capacity"] * row_bytes(cfg["species"][0]) // 2 ** 20),
+                       "l2": l2_note(cfg),
+                       "clock_warm": "%d untimed steps, then the initial state written again, before the W warm-up steps" % args.clock_warm_steps,
                        "ms_per_step_repeats": [round(x, 6) for x in repeats],
                        "mean_N_t": units / args.steps / world, "mean_M_t": offspring / args.steps / world,
                        "flags": flags, "offspring_per_s": offspring / (ms * 1e-3),
@@ -324,8 +356,9 @@ def run_ours(args):
                     "what": "spegg_write_state(host) + K x (spegg_step(1) + spegg_read_log) + spegg_read_state(host)"},
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": TRAFFIC_BYTES.get(cfg["name"]),
-
+                         "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+                         "frac_is": "ALGORITHMIC bytes per launch / kernel time / peak (DRAM traffic is below the algorithmic bytes: L2 hits)",
+                         "traffic_frac": (traffic / (k_ms * 1e-3) / 1e9 / peak) if (traffic and k_ms > 0) else None,
                          "kernel": ("fused step kernel: scan+parents+gametes+phenotype+survival+compaction" if sim.launches_per_step() == 1 else "gamete kernel") if k_n else "none",
                          "kernel_ms": k_ms, "kernel_launches_timed": k_n, "alg_bytes_per_launch": k_bytes,
                          "peak_source": peak_src},
@@ -341,6 +374,10 @@ def run_ours(args):
             line["roofline"]["alu"] = {"achieved": a_alu, "peak": ALU_PEAK_TINST, "unit": "Tinst/s",
                                        "frac": a_alu / ALU_PEAK_TINST, "alg_inst_per_launch": ops,
                                        "peak_source": "148 SMs x 4 schedulers x 32 lanes x 1.965 GHz (DESIGN.md 5)"}
+        if args.others and world == 1 and args.config == 3 and args.variant == "none":
+            # the other BASELINE.json configurations, driver-visible: short timed passes after the metric's own
+            sim.close()
+            line["config"]["other_workloads"] = [measure_other(w, 30, 5, dev) for w in (1, 2, 4, 5)]
         print(json.dumps(line))
     sim.close()
     if dist is not None:
@@ -358,9 +395,70 @@ def alu_ops_per_offspring(n_loci):
     return (2 * n_loci // 4 + 3) * 44 + 2 * n_loci * 4
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-# `ncu --set full` capture summarised under profiles/ (None until a capture exists).
-TRAFFIC_BYTES = {"C3": 549.9e6, "C5": 3163.1e6}   # profiles/r01_fused_full.md: C3 344.9 MB read + 205.0 MB written; C5 1.52 + 1.64 GB
+def measured_traffic(name):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    `ncu --set full` capture recorded in profiles/dominant_kernel_traffic.csv -- but only while the
+    kernel's source file still has the SHA-256 the capture was taken with; else None (a constant
+    that silently outlives the kernel it was measured on is worse than no number)."""
+    import csv
+    import hashlib
+    path = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.csv")
+    if not os.path.exists(path):
+        return None, "no capture recorded"
+    for row in csv.DictReader(open(path)):
+        if row["workload"] != name:
+            continue
+        src = os.path.join(ROOT, "paper_1603_09255_b200", "csrc", row["source_file"])
+        sha = hashlib.sha256(open(src, "rb").read()).hexdigest()
+        if sha != row["source_sha256"]:
+            return None, "capture %s predates the current %s" % (row["capture"], row["source_file"])
+        return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), row["capture"]
+    return None, "no capture recorded for %s" % name
+
+
+def measure_other(which, steps, warmup, dev):
+    """A short device-timed pass of another BASELINE.json configuration (context lines under
+    config.other_workloads; `value` stays the metric's configuration)."""
+    import torch
+    from paper_1603_09255_b200 import binding, workloads
+    cfg = workloads.config(which)
+    n_sp = len(cfg["species"])
+    sim = binding.Sim(cfg, debug=False, log_capacity=4096, device=str(dev))
+    for s in range(n_sp):
+        sim.write_state(s, workloads.initial_rows(cfg, s), workloads.initial_patch_start(cfg, s), 0)
+    sim.step(warmup)
+    sim.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(sim.stream):
+        e0.record(sim.stream)
+        sim.step(steps)
+        e1.record(sim.stream)
+    sim.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    logs = [sim.read_log(s)[warmup:warmup + steps] for s in range(n_sp)]
+    units = sum(sum(e["n_t"] for e in lg) for lg in logs)
+    peak, _ = load_peaks()
+    step_bytes = sum(alg_bytes(dict(species=[cfg["species"][s]]), logs[s], kernel_only=False) for s in range(n_sp)) / steps
+    out = {"workload": describe(cfg), "steps": steps, "warmup": warmup, "ms_per_step": ms,
+           "value": units / (ms * steps * 1e-3), "unit": UNIT, "launches_per_step": sim.launches_per_step(),
+           "mean_N_t": units / steps, "flags": sim.status(), "step_alg_bytes": step_bytes,
+           "step_frac_of_hbm_peak": step_bytes / (ms * 1e-3) / 1e9 / peak, "l2": l2_note(cfg)}
+    sp0 = cfg["species"][0]
+    if sp0["kind"] == "q10":
+        kt = min(steps, 10)
+        sim.kernel_timing(True)
+        kl0 = len(sim.read_log(0))
+        sim.step(kt)
+        k_ms, k_n = sim.kernel_timing(False)
+        klog = sim.read_log(0)[kl0:kl0 + kt]
+        if k_ms > 0:
+            ops = alu_ops_per_offspring(sp0["n_loci"]) * sum(e["m_t"] for e in klog) / max(1, len(klog))
+            out["gamete_kernel_ms"] = k_ms
+            out["gamete_kernel_alu_frac"] = ops / (k_ms * 1e-3) / 1e12 / ALU_PEAK_TINST
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+    return out
 
 
 def main():
@@ -372,6 +470,10 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--variant", default="none", choices=sorted(VARIANTS),
                     help="a widening of SURVEY.md 8(f) on top of --config (context lines; the metric is --variant none)")
+    ap.add_argument("--clock-warm-steps", type=int, default=300,
+                    help="untimed steps before the W warm-up steps (the initial state is written again after them)")
+    ap.add_argument("--no-others", dest="others", action="store_false",
+                    help="skip the short timed passes of configurations 1, 2, 4, 5 (config.other_workloads)")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
                     help="--impl reference: CPU seconds the K+W oracle steps are sized for")
     args = ap.parse_args()

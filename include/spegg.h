@@ -169,65 +169,98 @@ typedef struct spegg_debug_view {
 
 typedef struct spegg_sim spegg_sim;
 
-/* Validates `p` and returns the device bytes spegg_create needs (two population buffers of
- * `capacity` rows per species + index / scan / table / log arrays).  SPEGG_EINVAL on bad params. */
+/* PAPER.md:116 ("the data for each individual ... is stored in ... vectors" of one species object) and
+ * PAPER.md:122 (10^6-10^7 individuals in GPU memory): the storage of a simulation.  Validates `p` and
+ * returns the device bytes spegg_create needs (two population buffers of `capacity` rows per species
+ * + index / scan / table / log arrays).  p, bytes: HOST.  SPEGG_EINVAL on bad parameters (L not a
+ * multiple of 32 / 64 for bit genomes, chromosome lengths not summing to L, rates outside [0,1],
+ * capacity 0 or >= 2^31, combinations DESIGN.md lists as unsupported); nothing is allocated. */
 int spegg_workspace_bytes(const spegg_params *p, uint64_t *bytes);
 
-/* Builds the constant threshold tables (Bernoulli, Poisson, discrete normal), uploads them and
- * captures the step graph on `cuda_stream` (a cudaStream_t, may be 0).  d_workspace must be
- * 256-byte aligned device memory of at least spegg_workspace_bytes().  Populations start empty. */
+/* PAPER.md:50-54, :116 and Fig. S4: a species is a genetic architecture (loci, linkage,
+ * mutation) plus an ecology (mating, fecundity, selection, migration), set up once before the loop of
+ * Fig. 1.  Builds the constant threshold tables (Bernoulli, Poisson, discrete normal: readings R4-R9),
+ * uploads them and captures the step graphs on `cuda_stream` (a cudaStream_t; 0 = a private stream).
+ * d_workspace: DEVICE memory, 256-byte aligned, at least spegg_workspace_bytes() (else SPEGG_ENOMEM);
+ * it stays the caller's.  Populations start empty.  SPEGG_ECUDA wraps CUDA errors. */
 int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void *cuda_stream,
                  spegg_sim **out);
 
-/* Loads a whole population of `species` (n rows, n <= capacity) and sets the global step counter.
- * patch_start: HOST [n_patches+1] CSR of the rows, sorted by patch (NULL iff 1x1 grid).
- * Serves as initialisation and as "resume": with the counter-based RNG the state
- * (rows, patch_start, step, seed) is a complete checkpoint.  Synchronises the stream. */
+/* Fig. S4 `Initialize()` (the user-supplied initial state of every individual) and
+ * PAPER.md:126 (individuals belong to patches): loads a whole population of `species` (n rows in the
+ * row layout above, n <= capacity else SPEGG_ERANGE) and sets the global step counter t (R16).
+ * genomes: host or device as said by genomes_is_device.  patch_start: HOST [n_patches+1] CSR of the
+ * rows, sorted by patch (NULL iff 1x1 grid; SPEGG_EINVAL if inconsistent with n).
+ * Serves as initialisation and as "resume": with the counter-based RNG the state (rows, patch_start,
+ * step, seed) is a complete checkpoint.  Resets that species' step accumulators AND ITS LOG (the next
+ * step writes log index 0); with separate sexes everybody is female until spegg_write_sex.
+ * Synchronises the stream. */
 int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *genomes,
                       int genomes_is_device, const uint32_t *patch_start, uint32_t step);
 
-/* Sexes of the current adults of `species` (separate_sexes = 1, else SPEGG_ESTATE), in the row order
- * of spegg_write_state / spegg_read_state: HOST [n] bytes, 0 = female, non-zero = male; n must be
- * the current population size (SPEGG_ERANGE).  Synchronises the stream. */
+/* Eqs. S2-9 / S2-10 (mothers and fathers are drawn from mature females and males;
+ * R21): sexes of the current adults of `species` (separate_sexes = 1, else SPEGG_ESTATE), in the row
+ * order of spegg_write_state / spegg_read_state: HOST [n] bytes, 0 = female, non-zero = male; n must
+ * be the current population size (SPEGG_ERANGE).  Synchronises the stream. */
 int spegg_write_sex(spegg_sim *s, uint32_t species, uint64_t n, const uint8_t *sex);
+/* Eqs. S2-9 / S2-10 (R21): the sexes back, HOST [cap_bytes >= n] (else SPEGG_ERANGE). */
 int spegg_read_sex(spegg_sim *s, uint32_t species, uint8_t *sex_out, uint64_t cap_bytes);
 
-/* Enqueues n_steps steps on the stream and returns; no host synchronisation.  Never fails for
- * model reasons: overflow / extinction set sticky device flags (spegg_status).  Long runs replay a
- * captured graph of sixteen steps (consecutive steps' kernels overlap through programmatic edges),
- * the remainder a graph of one step; the trajectory does not depend on how n_steps is split. */
+/* Fig. 1 A-F: n_steps passes of the per-time-step loop -- parents and neonate numbers
+ * (A), genes transmitted (B; recombination and mutation PAPER.md:54, :325), genotype -> phenotype (C;
+ * eq. S2-14), selection (D), survivors kept (E), environment updated (F) -- for every
+ * species in index order, plus dispersal between patches.  Enqueues the steps on the
+ * stream and returns; no host synchronisation, population counts never leave the device.  Never fails
+ * for model reasons: overflow / extinction set sticky device flags (spegg_status).  n_steps is split
+ * greedily into captured graphs of 16, 8, 4, 2 and 1 steps (inside a graph consecutive steps' kernels
+ * overlap through programmatic edges); the trajectory does not depend on how n_steps is split. */
 int spegg_step(spegg_sim *s, uint32_t n_steps);
 
-/* Synchronises, then copies the current adults of `species` out.  Any output may be NULL.
- * n, step: HOST scalars.  genomes_out: host or device buffer of cap_bytes; SPEGG_ERANGE if too
- * small (*n is still set).  patch_start_out: HOST [n_patches+1].  zi_out: HOST [n] integer
- * phenotypes (z = zi * pheno_scale). */
+/* Fig. 1 E ("surviving individuals are identified") and PAPER.md:126 (patches): synchronises,
+ * then copies the current adults of `species` out in their stable order (offspring order; by
+ * (destination patch, j) in patch mode).  Any output may be NULL.  n, step: HOST scalars.
+ * genomes_out: host or device buffer of cap_bytes; SPEGG_ERANGE if too small (*n is still set).
+ * patch_start_out: HOST [n_patches+1].  zi_out: HOST [n] integer genetic values (z = zi * pheno_scale,
+ * eq. S2-14).  Uses the idle population buffer as staging; the simulation is unchanged. */
 int spegg_read_state(spegg_sim *s, uint32_t species, uint64_t *n, uint32_t *step,
                      void *genomes_out, int genomes_is_device, uint64_t cap_bytes,
                      uint32_t *patch_start_out, int32_t *zi_out);
 
-/* Synchronises and copies log entries [first_step_index, first_step_index + n) of the ring;
- * index 0 is the first step taken since the last spegg_write_state of that species' simulation.
- * *n_avail (nullable) receives the number of entries available. */
+/* Fig. 1 F ("the environment is updated" from the survivors' phenotypes): the per-step
+ * record of N_t, M_t, N_{t+1}, exact integer sums of z and z^2 over the survivors, captures, near-ties
+ * and flags.  Synchronises and copies log entries [first, first + n) to HOST out (at most two device
+ * copies, one per side of the ring wrap); index 0 is the first step taken since the last
+ * spegg_write_state of that species.  *n_avail (nullable) receives the number of entries written so
+ * far; n = 0 only queries it.  SPEGG_ERANGE if the span is not (or no longer, ring of log_capacity)
+ * available. */
 int spegg_read_log(spegg_sim *s, uint32_t species, uint32_t first, uint32_t n,
                    spegg_log_entry *out, uint32_t *n_avail);
 
-/* Synchronises; fills device pointers to the intermediates of the last step (debug = 1 only,
- * else SPEGG_ESTATE). */
+/* Fig. 1 A-E intermediates: synchronises; fills DEVICE pointers (into the caller's
+ * workspace, valid until the next spegg_step) to every intermediate of the last step -- fecundities,
+ * offsets, parents, destinations, uniforms, survival probabilities, genetic values, decisions, offspring
+ * rows, derived tables.  debug = 1 only, else SPEGG_ESTATE. */
 int spegg_read_debug(spegg_sim *s, uint32_t species, spegg_debug_view *out);
 
-/* Synchronises; returns the sticky flags (SPEGG_FLAG_*). */
+/* Fig. 1 A, E: what the loop cannot express as a count -- synchronises; returns the
+ * sticky flags: SPEGG_FLAG_OVERFLOW (some step's neonates exceeded `capacity`; offspring j >= capacity
+ * were never born) and SPEGG_FLAG_EXTINCT (a species reached N = 0 and is skipped from then on). */
 int spegg_status(spegg_sim *s, uint32_t *flags);
 
-/* Number of kernel launches one spegg_step(1) replays (graph kernel nodes). */
+/* Fig. 1 as launched: number of kernel launches one step replays (graph kernel nodes);
+ * bench.py's `gpu_launches` claim. */
 int spegg_launches_per_step(const spegg_sim *s, uint32_t *n);
 
-/* CUDA-event timing of the dominant kernel: when enabled, spegg_step brackets the main
- * (gamete) kernel of species 0 with events on the stream; read back with the mean duration in
- * milliseconds over the launches since enabling.  For bench.py's roofline figure. */
+/* Fig. 1 B-E timed: CUDA-event timing of the dominant kernel.  When enabled, spegg_step
+ * launches the kernels directly (no graph) and brackets the main (gamete) kernel of species 0 with
+ * events on the stream; read back with the mean duration in milliseconds over the launches since
+ * enabling.  For bench.py's roofline figure. */
 int spegg_kernel_timing(spegg_sim *s, int enable, float *mean_ms, uint32_t *n_launches);
 
+/* PAPER.md:116 (the species object's lifetime): frees the host struct and the graphs; never frees the
+ * caller's workspace or stream.  NULL is allowed. */
 void spegg_destroy(spegg_sim *s);
+/* Text for an error code of any call above (PAPER.md:48-52 has no error model: this is the ABI's own). */
 const char *spegg_strerror(int code);
 
 #ifdef __cplusplus

@@ -283,14 +283,17 @@ class Sim:
                                          rows.nbytes, ps.ctypes.data, zi.ctypes.data if want_zi else None))
         return rows[:n], ps, zi
 
-    def read_log(self, species=0):
+    def read_log(self, species=0, last=None):
+        """spegg_read_log: all entries written since the last write_state, or only the `last` n of them."""
         avail = C.c_uint32(0)
         _check(self.lib.spegg_read_log(self._h, species, 0, 0, None, C.byref(avail)))
         n = int(avail.value)
-        buf = (LogEntry * max(n, 1))()
-        if n:
-            _check(self.lib.spegg_read_log(self._h, species, 0, n, buf, None))
-        return [{f[0]: getattr(buf[i], f[0]) for f in LogEntry._fields_} for i in range(n)]
+        first = 0 if last is None else max(0, n - int(last))
+        cnt = n - first
+        buf = (LogEntry * max(cnt, 1))()
+        if cnt:
+            _check(self.lib.spegg_read_log(self._h, species, first, cnt, buf, None))
+        return [{f[0]: getattr(buf[i], f[0]) for f in LogEntry._fields_} for i in range(cnt)]
 
     def status(self):
         f = C.c_uint32(0)

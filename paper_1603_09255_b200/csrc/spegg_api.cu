@@ -244,7 +244,12 @@ thread_local cudaError_t s_last_cuda = cudaSuccess;
 
 }  // namespace
 
-constexpr uint32_t MULTI_STEPS = 16;
+// spegg_step replays captured graphs of 16, 8, 4, 2 and 1 steps (greedy, largest first): inside a
+// multi-step graph the programmatic edge between one step's last kernel and the next step's first
+// stays, so a step's first kernel is scheduled while the previous step drains -- for any n_steps,
+// not only for multiples of sixteen
+constexpr uint32_t N_MULTI = 4;
+constexpr uint32_t MULTI_STEPS[N_MULTI] = {16, 8, 4, 2};
 
 struct spegg_sim {
     spegg_params p;
@@ -257,8 +262,8 @@ struct spegg_sim {
     cudaGraphExec_t exec = nullptr;
     // several steps in one graph: the programmatic edges between the kernels of consecutive steps
     // stay inside the graph, so a step's first kernel is scheduled while the previous step drains
-    cudaGraph_t graph_multi = nullptr;
-    cudaGraphExec_t exec_multi = nullptr;
+    cudaGraph_t graph_multi[N_MULTI] = {};
+    cudaGraphExec_t exec_multi[N_MULTI] = {};
     DevGlobal *d_glob = nullptr;
     DevSpecies *d_st = nullptr;
     SpK *d_spk = nullptr;
@@ -286,6 +291,10 @@ int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
 // true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
 bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
     if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.mate_on || h.k.fec_cost != 0.0f || h.k.assort != 0.0f) return false;
+    // k_fused_bit_f<4, 8> places chromosome c at words 8c .. 8c+7 and packs crossover positions in 9 bits:
+    // four chromosomes of exactly 256 loci (other splits of 1,024 loci run the general pipeline)
+    for (uint32_t c = 0; c < h.p.n_chrom; ++c)
+        if (h.chrom_len[c] != 256u) return false;
     // the fused kernel tests u >= T as u > T - 1 (see spegg_fused.cuh): every threshold must be >= 1
     for (uint32_t c = 0; c < h.p.n_chrom; ++c)
         for (uint32_t k = 0; k < h.xover_len[c]; ++k)
@@ -568,14 +577,18 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     if (rc != SPEGG_OK) return fail(rc);
     if (ce != cudaSuccess) { s_last_cuda = ce; return fail(SPEGG_ECUDA); }
     if ((ce = cudaGraphInstantiate(&s->exec, s->graph, 0)) != cudaSuccess) { s_last_cuda = ce; return fail(SPEGG_ECUDA); }
-    if (!s->debug) {   // MULTI_STEPS steps per graph for long runs (optional: a failure here leaves the one-step graph)
-        bool ok = cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
-        if (ok) {
-            for (uint32_t i = 0; i < MULTI_STEPS && ok; ++i) ok = enqueue_step(s, nullptr, false) == SPEGG_OK;
-            ok = (cudaStreamEndCapture(s->stream, &s->graph_multi) == cudaSuccess) && ok;
+    (void)cudaGraphUpload(s->exec, s->stream);
+    if (!s->debug) {   // several steps per graph (optional: a failure here leaves the one-step graph)
+        for (uint32_t m = 0; m < N_MULTI; ++m) {
+            bool ok = cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+            if (ok) {
+                for (uint32_t i = 0; i < MULTI_STEPS[m] && ok; ++i) ok = enqueue_step(s, nullptr, false) == SPEGG_OK;
+                ok = (cudaStreamEndCapture(s->stream, &s->graph_multi[m]) == cudaSuccess) && ok;
+            }
+            if (ok) ok = cudaGraphInstantiate(&s->exec_multi[m], s->graph_multi[m], 0) == cudaSuccess;
+            if (ok) (void)cudaGraphUpload(s->exec_multi[m], s->stream);   // not on the first replay's critical path
+            if (!ok) { (void)cudaGetLastError(); s->exec_multi[m] = nullptr; }
         }
-        if (ok) ok = cudaGraphInstantiate(&s->exec_multi, s->graph_multi, 0) == cudaSuccess;
-        if (!ok) { (void)cudaGetLastError(); s->exec_multi = nullptr; }
     }
     *out = s;
     return SPEGG_OK;
@@ -585,8 +598,10 @@ void spegg_destroy(spegg_sim *s) {
     if (!s) return;
     if (s->stream) cudaStreamSynchronize(s->stream);
     for (auto e : s->ev) cudaEventDestroy(e);
-    if (s->exec_multi) cudaGraphExecDestroy(s->exec_multi);
-    if (s->graph_multi) cudaGraphDestroy(s->graph_multi);
+    for (uint32_t m = 0; m < N_MULTI; ++m) {
+        if (s->exec_multi[m]) cudaGraphExecDestroy(s->exec_multi[m]);
+        if (s->graph_multi[m]) cudaGraphDestroy(s->graph_multi[m]);
+    }
     if (s->exec) cudaGraphExecDestroy(s->exec);
     if (s->graph) cudaGraphDestroy(s->graph);
     if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -624,7 +639,7 @@ int spegg_write_state(spegg_sim *s, uint32_t species, uint64_t n, const void *ge
     if (n) {
         k_iota<<<s->n_sms * 4, 256, 0, s->stream>>>(h.k.rowptr[cur], (uint32_t)n);
         if (h.k.phys_parents) k_fill_masks<<<s->n_sms, 256, 0, s->stream>>>(h.k.chunk_mask[cur], h.k.range_cnt[cur], (uint32_t)n);
-        k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1);
+        k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, (uint32_t)n, 1, nullptr);
     }
     launch_prepare(s);
     CU(cudaGetLastError());
@@ -667,8 +682,10 @@ int spegg_read_sex(spegg_sim *s, uint32_t species, uint8_t *sex_out, uint64_t ca
 int spegg_step(spegg_sim *s, uint32_t n_steps) {
     if (!s) return SPEGG_EINVAL;
     uint32_t i = 0;
-    if (!s->timing && s->exec_multi)
-        for (; i + MULTI_STEPS <= n_steps; i += MULTI_STEPS) CU(cudaGraphLaunch(s->exec_multi, s->stream));
+    if (!s->timing)
+        for (uint32_t m = 0; m < N_MULTI; ++m)
+            if (s->exec_multi[m])
+                for (; i + MULTI_STEPS[m] <= n_steps; i += MULTI_STEPS[m]) CU(cudaGraphLaunch(s->exec_multi[m], s->stream));
     for (; i < n_steps; ++i) {
         if (s->timing) {
             if (s->ev_used + 2 > s->ev.size()) { CU(cudaStreamSynchronize(s->stream)); drain_timing(s); }
@@ -696,22 +713,26 @@ int spegg_read_state(spegg_sim *s, uint32_t species, uint64_t *n, uint32_t *step
         // fused path: the index (rowptr) of the current buffer is built on demand
         launch_rowptr_fused(h.k, s->n_sms, s->stream);
     }
+    // staging: the OTHER population buffer holds last step's dead adults and is free between steps, and
+    // pos[] is rewritten by every step before it is read -- so the debug view (offspring rows, zi) survives
+    uint8_t *stage_rows = h.k.pop[st.cur ^ 1u];
+    int32_t *stage_zi = (int32_t *)h.k.pos;
     if (genomes_out) {
         if (cap_bytes < (uint64_t)st.n * h.k.row_bytes) return SPEGG_ERANGE;
         if (st.n) {  // rows in logical order: gather through rowptr into the staging buffer
-            k_gather_rows<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, st.n, h.k.offbuf);
+            k_gather_rows<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, st.n, stage_rows);
             CU(cudaGetLastError());
             CU(cudaStreamSynchronize(s->stream));
-            CU(cudaMemcpy(genomes_out, h.k.offbuf, (size_t)st.n * h.k.row_bytes,
+            CU(cudaMemcpy(genomes_out, stage_rows, (size_t)st.n * h.k.row_bytes,
                           genomes_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost));
         }
     }
     if (patch_start_out) CU(cudaMemcpy(patch_start_out, h.k.patch_start[st.cur], (s->P + 1) * 4, cudaMemcpyDeviceToHost));
     if (zi_out && st.n) {
-        k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, st.n, 0);
+        k_adult_zi<<<s->n_sms * 8, 256, 0, s->stream>>>(h.k, st.n, 0, stage_zi);
         CU(cudaGetLastError());
         CU(cudaStreamSynchronize(s->stream));
-        CU(cudaMemcpy(zi_out, h.k.zi, (size_t)st.n * 4, cudaMemcpyDeviceToHost));
+        CU(cudaMemcpy(zi_out, stage_zi, (size_t)st.n * 4, cudaMemcpyDeviceToHost));
     }
     return SPEGG_OK;
 }
@@ -726,8 +747,10 @@ int spegg_read_log(spegg_sim *s, uint32_t species, uint32_t first, uint32_t n, s
     if (n == 0) return SPEGG_OK;
     if (!out || (uint64_t)first + n > st.log_pos) return SPEGG_ERANGE;
     if (st.log_pos - first > s->log_capacity) return SPEGG_ERANGE;  // overwritten by the ring
-    for (uint32_t i = 0; i < n; ++i)
-        CU(cudaMemcpy(out + i, h.k.log + ((first + i) % s->log_capacity), sizeof(LogEntry), cudaMemcpyDeviceToHost));
+    // at most two copies: the span up to the end of the ring, then the part that wrapped
+    const uint32_t at0 = first % s->log_capacity, n0 = std::min(n, s->log_capacity - at0);
+    CU(cudaMemcpy(out, h.k.log + at0, (size_t)n0 * sizeof(LogEntry), cudaMemcpyDeviceToHost));
+    if (n > n0) CU(cudaMemcpy(out + n0, h.k.log, (size_t)(n - n0) * sizeof(LogEntry), cudaMemcpyDeviceToHost));
     return SPEGG_OK;
 }
 
@@ -780,12 +803,5 @@ int spegg_kernel_timing(spegg_sim *s, int enable, float *mean_ms, uint32_t *n_la
     s->timing = enable != 0;
     return SPEGG_OK;
 }
-
-#ifdef SPEGG_PROBE
-// development build only (-DSPEGG_PROBE): the timing probes of the step kernel
-int spegg_probe_read(unsigned long long *out, uint32_t n_words) {
-    return cudaMemcpyFromSymbol(out, spegg::g_probe, (size_t)n_words * 8) == cudaSuccess ? 0 : -3;
-}
-#endif
 
 }  // extern "C"

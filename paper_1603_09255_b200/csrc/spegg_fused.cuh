@@ -117,29 +117,6 @@ __device__ __forceinline__ void half_masks(uint32_t P, uint32_t half, uint32_t (
     for (int i = 0; i < 4; ++i) m[i] = phi ^ mask_from(s0, i) ^ mask_from(s1, i);
 }
 
-#ifdef SPEGG_PROBE
-// timing probes of a development build (-DSPEGG_PROBE): globaltimer at the phase boundaries of every warp
-__device__ unsigned long long g_probe[8192 * 8];
-__device__ __forceinline__ void probe_cta(uint32_t slot) {   // scan kernel: one row per CTA after the gamete kernel's rows
-    if (threadIdx.x == 0) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-        g_probe[((4096u + blockIdx.x) & 8191u) * 8 + slot] = t;
-    }
-}
-#define PROBE_CTA(slot) probe_cta(slot)
-__device__ __forceinline__ void probe(uint32_t slot) {
-    if ((threadIdx.x & 31u) == 0) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-        g_probe[((blockIdx.x * FUSEDF_WARPS + (threadIdx.x >> 5)) & 4095u) * 8 + slot] = t;
-    }
-}
-#define PROBE(slot) probe(slot)
-#else
-#define PROBE(slot)
-#define PROBE_CTA(slot)
-#endif
 
 template <int NC, int WPC>
 __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(const __grid_constant__ SpK sp) {
@@ -181,8 +158,6 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     const uint32_t sp_slot = sub * 8u + hc * 2u;                                    // + it * 32: (g=0, g=1) pair
     long long acc1 = 0, acc2 = 0;
     uint32_t ties = 0, n_alive = 0;
-
-    PROBE(0);
 
     // mo / fa are the parents' physical ROW numbers exactly as loaded: nothing here depends on the
     // two index loads, so they stay in flight until the rows are needed one chunk later
@@ -386,7 +361,8 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
                 fix_extra((e >> 5) * 4 + (e_ln >> 3), (e_ln >> 2) & 1u, e_c, e_nc);
             }
         }
-        else {   // queue overflow, rare beyond measure: every lane walks its own eight draws again
+        else {   // queue overflow (more than 32 of the chunk's 256 chromosomes drew > 2 crossovers: about 0.3 % of the
+                 // chunks at mean 1, i.e. some ninety chunks of a full-size step): every lane walks its own eight draws again
             for (uint32_t it = 0; it < 8; ++it) {
                 uint32_t x[4];
                 draw_rk(sp, stream, j0 + it * 4 + sub, c * 16, step, x);
@@ -434,9 +410,7 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
         if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
         if (n_alive) atomicAdd(&st.n_next, n_alive);
     }
-    PROBE(3);
     if (sp.solo) solo_tail(sp, &s_flag);
-    PROBE(4);
 }
 
 // a1-a3 and the index half of a7 for a species on the fused path.  The current buffer holds m_phys
@@ -470,7 +444,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
     const uint32_t *cnt = sp.range_cnt[cur];
     const uint32_t *mask = sp.chunk_mask[cur];
     uint32_t *rp = sp.rowptr[cur];
-    PROBE_CTA(0);
     if (blockIdx.x >= n_ranges) return;   // (no adults at all: M_t stays 0)
     const uint32_t len0 = sp.table_len[0];
     if (tid < TMAX) s_tab[tid] = sp.tables[tid];
@@ -501,7 +474,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
         }
         __syncthreads();
         for (uint32_t k = tid; k < n_r; k += NT) rp[ibase + k] = s_stage[k];
-        PROBE_CTA(5);
         // ---- fecundity of this thread's adults
         uint32_t fsum = 0, fpack = 0;
         {
@@ -517,7 +489,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
                 }
             }
         }
-        PROBE_CTA(6);
         // ---- look-back over the fecundities: offspring before this range
         const uint32_t fincl = warp_incl_scan(fsum);
         if (lane == 31) s_f[warp] = fincl;
@@ -548,7 +519,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
             }
         }
         __syncthreads();
-        PROBE_CTA(7);
         const unsigned long long obase = s_excl;
         if (staged) {
             for (uint32_t k = tid; k < total; k += NT)
@@ -563,7 +533,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
             }
         }
     }
-    PROBE_CTA(1);
 }
 
 // rowptr[] of the current buffer alone (spegg_read_state): the index half of k_scan_fused.

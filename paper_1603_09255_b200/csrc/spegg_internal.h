@@ -87,7 +87,7 @@ struct SpK {
     uint32_t *patch_start[2];   // [P+1] each
     uint32_t *rowptr[2];        // logical adult index -> physical row of pop[]
     uint32_t *chunk_mask[2];    // fused path: survivor bitmask of each 32-row slab of pop[0] / pop[1]
-    uint32_t *range_cnt[2];     // fused path: adults per 2,048-row range of pop[0] / pop[1]
+    uint32_t *range_cnt[2];     // fused path: adults per 1,024-row range (FUSED_RANGE) of pop[0] / pop[1]
     uint32_t phys_parents;      // 1: mother[] / father[] hold physical rows (fused path)
     uint32_t solo;              // 1: single-species simulation (the gamete kernel's last CTA closes and prepares the step)
     uint32_t index_only;        // 1: offspring rows are written once, at row j of the other buffer; compaction writes rowptr[] only

@@ -220,6 +220,7 @@ __device__ __forceinline__ void solo_tail(const SpK &sp, uint32_t *s_flag) {
     DevSpecies &st = *sp.st;
     const uint32_t nn = ld_u32(&st.n_next), cur1 = ld_u32(&st.cur) ^ 1u, step1 = ld_u32(&sp.glob->step) + 1u;
     const long long a1 = (long long)ld_u64(&st.acc_zi);
+    __syncthreads();   // every thread holds its snapshot before thread 0 flips cur / bumps the step / zeroes the accumulators
     if (threadIdx.x == 0) {
         finish_species(sp);
         sp.glob->step = step1;
@@ -776,15 +777,15 @@ __global__ void __launch_bounds__(256) k_phenotype(const __grid_constant__ SpK s
     }
 }
 
-// phenotypes of the current adults (write_state / read_state): zi[] and their sum
-__global__ void __launch_bounds__(256) k_adult_zi(const __grid_constant__ SpK sp, uint32_t n, int accumulate) {
+// phenotypes of the current adults (write_state / read_state): out[] (nullable) and their sum
+__global__ void __launch_bounds__(256) k_adult_zi(const __grid_constant__ SpK sp, uint32_t n, int accumulate, int32_t *out) {
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     const uint32_t cur = sp.st->cur, lane = threadIdx.x & 31u;
     long long acc = 0;
     for (uint32_t blk = warp0; blk < (n + 31u) / 32u; blk += nw) {
         const int32_t zi = block_adult_zi(sp, sp.pop[cur], sp.rowptr[cur], blk, n);
         const uint32_t i = blk * 32u + lane;
-        if (i < n) { sp.zi[i] = zi; acc += zi; }
+        if (i < n) { if (out) out[i] = zi; acc += zi; }
     }
     if (accumulate) {
 #pragma unroll

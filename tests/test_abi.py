@@ -27,6 +27,19 @@ def test_library_exports_every_declared_symbol(binding):
         assert hasattr(lib, name), name
 
 
+def test_every_entry_point_cites_its_passage():
+    """each call declared in include/spegg.h cites the passage of the paper that defines
+    the operation -- the comment block directly above the declaration names a PAPER.md line."""
+    hdr = open(os.path.join(ROOT, "include", "spegg.h")).read()
+    decls = list(re.finditer(r"^(?:int|void|const char \*)\s*(spegg_[a-z_]+)\(", hdr, re.M))
+    assert len(decls) >= 14
+    for m in decls:
+        before = hdr[:m.start()].rstrip()
+        assert before.endswith("*/"), m.group(1)
+        comment = before[before.rindex("/*"):]
+        assert re.search(r"PAPER\.md:\d+", comment), "%s: no passage cited" % m.group(1)
+
+
 def test_struct_sizes_match_header(binding):
     import ctypes as C
     # spegg_create checks struct_size; mirror the arithmetic of the C layout here

@@ -39,6 +39,141 @@ def test_per_step_parity_fast_path(oracle_mod, binding, which, scale, grid, step
     parity.per_step_parity(oracle_mod, binding, cfg, steps, debug=False)
 
 
+SEEDS = [1, 2, 3, 0x9E3779B97F4A7C15]     # seeds 1-3; the last one has a non-zero HIGH key word
+
+
+@pytest.mark.parametrize("seed", SEEDS)
+@pytest.mark.parametrize("which,scale,grid,debug", [
+    (3, 0.013, None, False),      # the fused C3 kernels (the ones bench.py times)
+    (3, 0.006, None, True),
+    (2, 0.02, None, False), (5, 0.02, (4, 3), False), (4, 0.003, None, False), (1, 1.0, None, True),
+])
+def test_per_step_parity_seeds(oracle_mod, binding, which, scale, grid, debug, seed):
+    """Every configuration on other seeds than its own, including a 64-bit seed whose high word is
+    not zero: Philox key word k1 = seed >> 32 (R3) reaches the kernels through the host-built round
+    keys, and a dropped or swapped high word would pass every test that only uses small seeds."""
+    cfg = workloads.config(which, scale=scale, grid=grid, seed=seed)
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=debug)
+
+
+def _c3(scale, **kw):
+    cfg = workloads.config(3, scale=scale)
+    cfg["species"][0].update(kw)
+    return cfg
+
+
+def _assert_fused(sim):
+    assert sim.launches_per_step() == 2, "configuration left the fused two-kernel step"
+
+
+def _free_run(oracle_mod, binding, cfg, steps, chunks=1, fused=True):
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    if fused is not None:
+        assert (sim.launches_per_step() == 2) == fused
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(chunks):
+        orc.step(steps)
+        sim.step(steps)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+        parity.assert_state_equal(sim, orc, cfg)
+        assert sim.status() == orc.flags
+    sim.close()
+    return orc
+
+
+@pytest.mark.parametrize("capacity", [24576, 24001])
+def test_fused_path_capacity_overflow(oracle_mod, binding, capacity):
+    """OVERFLOW on the fused C3 kernels (k_scan_fused truncates M_t at the capacity, k_fused_bit_f stops
+    at it): K = 1e9 keeps lambda at 2, so M_t > capacity in every step; the second capacity is not a
+    multiple of the 32-row slab.  Per step from the oracle's state, then free-running."""
+    cfg = _c3(0.02, K=1e9, capacity=capacity)
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=False)
+    orc = _free_run(oracle_mod, binding, cfg, 3)
+    assert all(e["flags"] & 1 and e["m_t"] == capacity for e in orc.log(0))
+
+
+def test_fused_path_unstaged_mother_ranges(oracle_mod, binding):
+    """k_scan_fused stages the mother[] words of a 1,024-row range in shared memory when the range has at
+    most 4,096 offspring and stores them directly otherwise: lambda = 8 gives ~8,000 per range (asserted
+    from the oracle's fecundities), and the second step overflows the capacity on the same path."""
+    cfg = _c3(0.02, fec_a=8.0, K=1e9)
+    cfg["species"][0]["capacity"] = 10 * cfg["n0"][0] // 1024 * 1024
+    orc = oracle_mod.Oracle(cfg)
+    parity.load_initial(orc, cfg)
+    orc.step(1)
+    f = orc.debug(0)["f"].astype(np.int64)
+    per_range = np.add.reduceat(f, np.arange(0, len(f), 1024))
+    assert per_range.max() > 4096
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+    orc = _free_run(oracle_mod, binding, cfg, 2)
+    assert orc.log(0)[0]["flags"] == 0 and orc.log(0)[1]["flags"] & 1
+
+
+@pytest.mark.parametrize("kw", [
+    dict(xover_mean=[0.0, 0.0, 0.0, 0.0]),                 # no crossover tables at all: whole parental haplotypes
+    dict(xover_mean=[0.3, 1.0, 3.0, 4.0]),                 # most chromosomes draw > 2 crossovers: the fix-up queue overflows in every chunk
+    dict(xover_mean=[12.0, 0.0, 20.0, 1.0]),               # crossover draws from several RECOMB blocks of a chromosome
+    dict(mu=1e-3),                                         # L mu = 1.02: several mutations per gamete (MUT blocks k > 0), both gametes
+    dict(mu=0.0),                                          # L mu = 0: an empty mutation table (no gamete ever mutates)
+    dict(gaussian=dict(theta0=0.5, dtheta=0.01, omega=1.5, theta_patch=None)),   # moving optimum
+    dict(gaussian=None),                                   # no selection: everybody survives, all slabs full
+    dict(gaussian=dict(theta0=30.0, dtheta=0.0, omega=0.5, theta_patch=None)),   # nobody survives: extinction on the fused path
+])
+def test_fused_path_genetics_and_selection(oracle_mod, binding, kw):
+    """Non-default genetics and selection on the fused C3 kernels (bench.py's kernels): per step from
+    the oracle's state, then a free-running trajectory."""
+    cfg = _c3(0.012, **kw)
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+    _free_run(oracle_mod, binding, cfg, 4, chunks=2)
+
+
+@pytest.mark.parametrize("n0", [1, 31, 33, 1023, 1025, 2049, 4097])
+def test_fused_path_ragged_sizes(oracle_mod, binding, n0):
+    """Ragged tails of the fused kernels: one adult, a 32-row slab minus / plus one, a 1,024-row scan
+    range minus / plus one, two and four ranges plus one; and an empty population stays empty."""
+    cfg = _c3(0.01, fec_a=3.0, K=float(max(n0, 8)), capacity=max(4 * n0, 256))
+    cfg["n0"] = [n0]
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=False)
+    _free_run(oracle_mod, binding, cfg, 6)
+    sim = binding.Sim(cfg, debug=False)
+    _assert_fused(sim)
+    sim.write_state(0, workloads.initial_rows(cfg, 0)[:0], None, 0)
+    sim.step(2)
+    assert sim.n(0) == 0 and (sim.status() & 2)
+    sim.close()
+
+
+def test_unequal_chromosomes_leave_the_fused_kernel(oracle_mod, binding):
+    """k_fused_bit_f<4, 8> is written for four chromosomes of 256 loci; any other split of 1,024 loci must
+    run the general pipeline (and still match the oracle on the production path)."""
+    cfg = _c3(0.01, chrom_len=[512, 256, 128, 128], xover_mean=[2.0, 1.0, 0.5, 0.5])
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+    _free_run(oracle_mod, binding, cfg, 5, fused=False)
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=True)
+
+
+def test_read_state_keeps_the_debug_view(oracle_mod, binding):
+    """spegg_read_state stages in the idle population buffer, so the debug view of the last step is
+    still intact after it; spegg_read_log spans the ring wrap in two copies and `last=n` reads n entries."""
+    cfg = workloads.config(2, scale=0.02)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=True, log_capacity=8)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    orc.step(11)
+    sim.step(11)
+    parity.assert_state_equal(sim, orc, cfg)                       # read_state first ...
+    parity.assert_debug_equal(sim.read_debug(0), orc.debug(0), cfg["species"][0])   # ... the view is unchanged
+    assert sim.read_log(0, last=8) == orc.log(0)[-8:]             # entries 3..10 of a ring of 8: wraps
+    assert sim.read_log(0, last=1) == orc.log(0)[-1:]
+    with pytest.raises(binding.SpeggError) as e:
+        sim.read_log(0)                                            # entries 0..2 were overwritten
+    assert e.value.code == binding.ERANGE
+    sim.close()
+
+
 @pytest.mark.parametrize("which,scale,grid,steps", [(1, 1.0, None, 100), (3, 0.01, None, 40), (5, 0.02, (5, 4), 25),
                                                     (4, 0.003, None, 25), (2, 0.02, None, 30)])
 def test_free_running_trajectory(oracle_mod, binding, which, scale, grid, steps):
@@ -132,9 +267,9 @@ def test_bad_parameters_are_rejected(binding):
 
 # ---- BASELINE.json's FULL sizes, in the launch configuration bench.py times (debug off, the
 # production kernels, the captured graph).  The oracle finishes a full-size step in seconds
-# (C3 ~6 s, C4 ~9 s, C5 ~17 s), so the comparison is complete -- every row of the next
+# (C3 ~6 s, C4 ~9 s, C5 ~17 s per step), so the comparison is complete -- every row of the next
 # generation, every log field -- rather than sampled.
-@pytest.mark.parametrize("which,steps", [(3, 3), (2, 6), (4, 1), (5, 1)])
+@pytest.mark.parametrize("which,steps", [(3, 3), (2, 6), (4, 3), (5, 3)])
 def test_full_size_bench_configuration(oracle_mod, binding, which, steps):
     cfg = workloads.config(which)                     # scale 1.0: N0, K, capacity as benchmarked
     orc = oracle_mod.Oracle(cfg)
