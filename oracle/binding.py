@@ -45,7 +45,7 @@ class _SpeciesParams(C.Structure):
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
         ("mate_skew", C.c_double), ("encounters", C.c_uint32), ("separate_sexes", C.c_uint32),
-        ("fec_cost", C.c_double), ("assort", C.c_double),
+        ("fec_cost", C.c_double), ("assort", C.c_double), ("mother_skew", C.c_double),
     ]
 
 
@@ -73,7 +73,7 @@ class _DebugView(C.Structure):
         ("attack_n", C.c_float), ("cap", C.POINTER(C.c_uint32)),
         ("a_alive", C.POINTER(C.c_uint8)), ("a_u", C.POINTER(C.c_float)), ("a_s", C.POINTER(C.c_float)),
         ("mate_cum", C.POINTER(C.c_uint64)), ("zbar_self", C.c_float),
-        ("sex_off", C.POINTER(C.c_uint8)),
+        ("sex_off", C.POINTER(C.c_uint8)), ("mom_cum", C.POINTER(C.c_uint64)),
     ]
 
 
@@ -239,6 +239,7 @@ class Oracle:
             p.separate_sexes = 1 if sp.get("separate_sexes") else 0
             p.fec_cost = sp.get("fec_cost", 0.0)
             p.assort = sp.get("assort", 0.0)
+            p.mother_skew = sp.get("mother_skew", 0.0)
             if sp["kind"] == "bit":
                 self.row_shape.append(2 * (L // 32))
                 self.row_dtype.append(np.uint32)
@@ -338,6 +339,8 @@ class Oracle:
                          if (self.cfg["species"][species].get("mate_skew", 0.0) != 0.0
                              or self.cfg["species"][species].get("separate_sexes")) else np.zeros(0, np.uint64)),
             "sex_off": arr(v.sex_off, m, np.uint8),
+            "mom_cum": (arr(v.mom_cum, n, np.uint64) if self.cfg["species"][species].get("mother_skew", 0.0) != 0.0
+                        else np.zeros(0, np.uint64)),
         }
         nt = int(v.n_tables)
         d["table_len"] = arr(v.table_len, nt, np.uint32)

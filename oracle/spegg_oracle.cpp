@@ -56,7 +56,7 @@ void philox(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4]) {
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-enum Stream { FEC = 0, SCALAR = 1, RECOMB_M = 2, RECOMB_P = 3, MUT_M = 4, MUT_P = 5, MATE = 6 };
+enum Stream { FEC = 0, SCALAR = 1, RECOMB_M = 2, RECOMB_P = 3, MUT_M = 4, MUT_P = 5, MATE = 6, MOTHER = 7 };
 const uint32_t ASSORT_TRIES = 8; /* R23 */
 
 /* R3: key = (seed_lo, seed_hi); counter = (entity, block, step, species<<8 | stream) */
@@ -180,6 +180,7 @@ struct SpeciesDebug {
     std::vector<uint32_t> off, mother, father, dest, tables, table_len, cap;
     std::vector<float> u01, s, z, a_u, a_s;
     std::vector<uint64_t> mate_cum; /* R19 */
+    std::vector<uint64_t> mom_cum;  /* R24 */
     float zbar_self = 0;
     std::vector<int32_t> zi;
     std::vector<uint32_t> off_bits; /* offspring rows, BIT */
@@ -421,6 +422,31 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         }
     }
 
+    /* ---- R24 (eq. S2-9): "For each egg, the mother and father are drawn at random
+     *      ... The probability that the egg comes from female i is a function of the female's relative
+     *      gonadal mass", (G_i/(Omega_i + q_J Omega_i))^{v_f}.  The relative fecundity is read as
+     *      Y_i = exp(z_i) (a log-fecundity trait, as X_i = exp(z_i) in R19), so the mothering weight is
+     *      exp(v_f z_i), built exactly like the mating weight of R19 (same zbar, clamp, expf_spec,
+     *      integer 2^40 scaling); with separate sexes a male's weight is 0.  mom_cum is its inclusive
+     *      running sum in adult order. ---- */
+    const bool mom_on = S.p.mother_skew != 0.0;
+    if (mom_on) {
+        const float v = (float)S.p.mother_skew;
+        D.zbar_self = (float)(((double)sumzi0[si] / (double)N) * (double)S.p.pheno_scale);
+        D.mom_cum.resize(N);
+        uint64_t run = 0;
+        for (uint64_t i = 0; i < N; ++i) {
+            const float z = (float)S.zi[i] * S.p.pheno_scale;
+            const float d = z - D.zbar_self;
+            float e = v * d;
+            e = std::min(std::max(e, -16.0f), 16.0f);
+            const float x = e - 16.0f;
+            const float w = expf_spec(x);
+            if (!S.p.separate_sexes || !S.sex[i]) run += (uint64_t)(w * 0x1p40f);
+            D.mom_cum[i] = run;
+        }
+    }
+
     /* ---- a1: fecundity (Fig. 1A), one FEC block per adult ---- */
     D.f.resize(N);
     D.off.resize(N);
@@ -477,13 +503,31 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
     const uint64_t NC = pred ? N0[S.p.predator_species] : 0;
 
     for (uint64_t j = 0; j < M; ++j) {
-        const uint32_t mo = D.mother[j];
+        uint32_t mo = D.mother[j];
         const uint32_t pm = patch_of(S, P, mo);
         uint32_t x[4];
         draw(sim.seed, si, SCALAR, (uint32_t)j, 0, t, x);
         /* R2: father uniform over the adults of the mother's patch, selfing allowed */
         const uint32_t base = (P == 1) ? 0 : S.patch_start[pm];
         const uint32_t np = (P == 1) ? (uint32_t)N : S.patch_start[pm + 1] - S.patch_start[pm];
+        if (mom_on) {
+            /* R24: the egg was counted in its patch by the adult that laid it (a1-a2: the patch's
+             * number of eggs is the sum of its Poisson fecundities); its MOTHER is now drawn among the
+             * adults of that patch by running sum + search, as the father in R19: total = weight of
+             * the patch; 64-bit uniform from words 0,1 of block 0 of stream MOTHER (entity j);
+             * target = floor(u * total / 2^64); mother = first adult of the patch whose inclusive
+             * running sum exceeds (running sum before the patch) + target.  Total weight 0: unchanged. */
+            const uint64_t before = base ? D.mom_cum[base - 1] : 0;
+            const uint64_t total = D.mom_cum[base + np - 1] - before;
+            if (total > 0) {
+                uint32_t y[4];
+                draw(sim.seed, si, MOTHER, (uint32_t)j, 0, t, y);
+                const uint64_t u = ((uint64_t)y[0] << 32) | y[1];
+                const uint64_t target = before + (uint64_t)(((unsigned __int128)u * total) >> 64);
+                mo = (uint32_t)(std::upper_bound(D.mom_cum.begin() + base, D.mom_cum.begin() + base + np, target) - D.mom_cum.begin());
+                D.mother[j] = mo;
+            }
+        }
         uint32_t fa = base + uniform_index(x[0], np);
         if (mate_on) {
             /* R19: weighted draw among the adults of the mother's patch by running sum + search:
@@ -631,7 +675,7 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
             float w = 1.0f;
             if (S.p.sel_gaussian) {
                 const float z = (float)S.zi[i] * S.p.pheno_scale;
-                const float th = S.theta_patch.empty() ? D.theta_t : S.theta_patch[0];
+                const float th = S.theta_patch.empty() ? D.theta_t : S.theta_patch[patch_of(S, P, (uint32_t)i)];   /* its own patch's optimum */
                 const float d = z - th;
                 const float sq = d * d;
                 w = expf_spec(-(sq * S.sel_c));
@@ -644,8 +688,10 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         }
     }
 
-    /* ---- a7: survivors (Fig. 1E): next adults = the adults that stay (R18; none under R1), in
-     *      increasing i, then the surviving offspring in increasing (dest, j) ---- */
+    /* ---- a7: survivors (Fig. 1E): the next generation, patch by patch (individuals are
+     *      kept grouped by patch): in patch p first its adults that stay (R18; none under R1; an adult
+     *      does not move), in increasing i, then the surviving offspring whose destination is p, in
+     *      increasing j.  With one patch: the staying adults, then the surviving offspring. ---- */
     std::vector<uint32_t> order;
     order.reserve(M);
     for (uint64_t j = 0; j < M; ++j) if (D.alive[j]) order.push_back((uint32_t)j);
@@ -656,26 +702,31 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
     std::vector<int32_t> nzi(Nn);
     std::vector<uint8_t> nsex(Nn, 0);
     std::vector<uint32_t> nps(P + 1, 0);
-    for (uint64_t k = 0; k < Na; ++k) {   /* R18: the adults that stay keep their rows */
-        const uint32_t i = stay[k];
-        if (S.p.genome_kind == ORC_BIT) std::memcpy(&nb[k * S.row_elems], &S.bits[(size_t)i * S.row_elems], S.row_elems * 4);
-        else std::memcpy(&nq[k * S.row_elems], &S.q[(size_t)i * S.row_elems], S.row_elems * 2);
-        nzi[k] = S.zi[i];
-        nsex[k] = S.sex[i];
-        nps[1]++;
-        le.sum_zi += S.zi[i];
-        le.sum_zi2 += (int64_t)S.zi[i] * S.zi[i];
-    }
-    for (uint64_t k = Na; k < Nn; ++k) {
-        uint32_t j = order[k - Na];
-        if (S.p.genome_kind == ORC_BIT) std::memcpy(&nb[k * S.row_elems], &D.off_bits[(size_t)j * S.row_elems], S.row_elems * 4);
-        else std::memcpy(&nq[k * S.row_elems], &D.off_q[(size_t)j * S.row_elems], S.row_elems * 2);
-        nzi[k] = D.zi[j];
-        nsex[k] = D.sex_off[j];
-        nps[D.dest[j] + 1]++;
-        /* ---- a8: environment reductions (Fig. 1F), exact integers ---- */
-        le.sum_zi += D.zi[j];
-        le.sum_zi2 += (int64_t)D.zi[j] * D.zi[j];
+    {
+        uint64_t k = 0, ia = 0, io = 0;   /* next position, next staying adult, next surviving offspring */
+        for (uint32_t p = 0; p < P; ++p) {
+            for (; ia < Na && patch_of(S, P, stay[ia]) == p; ++ia, ++k) {   /* R18: the adults that stay keep their rows */
+                const uint32_t i = stay[ia];
+                if (S.p.genome_kind == ORC_BIT) std::memcpy(&nb[k * S.row_elems], &S.bits[(size_t)i * S.row_elems], S.row_elems * 4);
+                else std::memcpy(&nq[k * S.row_elems], &S.q[(size_t)i * S.row_elems], S.row_elems * 2);
+                nzi[k] = S.zi[i];
+                nsex[k] = S.sex[i];
+                nps[p + 1]++;
+                le.sum_zi += S.zi[i];
+                le.sum_zi2 += (int64_t)S.zi[i] * S.zi[i];
+            }
+            for (; io < order.size() && D.dest[order[io]] == p; ++io, ++k) {
+                const uint32_t j = order[io];
+                if (S.p.genome_kind == ORC_BIT) std::memcpy(&nb[k * S.row_elems], &D.off_bits[(size_t)j * S.row_elems], S.row_elems * 4);
+                else std::memcpy(&nq[k * S.row_elems], &D.off_q[(size_t)j * S.row_elems], S.row_elems * 2);
+                nzi[k] = D.zi[j];
+                nsex[k] = D.sex_off[j];
+                nps[p + 1]++;
+                /* ---- a8: environment reductions (Fig. 1F), exact integers ---- */
+                le.sum_zi += D.zi[j];
+                le.sum_zi2 += (int64_t)D.zi[j] * D.zi[j];
+            }
+        }
     }
     for (uint32_t p = 0; p < P; ++p) nps[p + 1] += nps[p];
     S.bits.swap(nb); S.q.swap(nq); S.zi.swap(nzi); S.sex.swap(nsex); S.patch_start.swap(nps);
@@ -754,9 +805,9 @@ orc_sim *orc_create(const orc_params *p) {
         }
         if (!(S.p.assort >= 0.0 && S.p.assort <= 1e6) || (S.p.assort > 0.0 && (S.p.mate_skew != 0.0 || S.p.separate_sexes))) { delete sim; return nullptr; }
         if (!(std::fabs(S.p.mate_skew) <= 1e6) || !(S.p.fec_cost >= 0.0 && S.p.fec_cost <= 1e6)) { delete sim; return nullptr; }
+        if (!(std::fabs(S.p.mother_skew) <= 1e6) || (S.p.mother_skew != 0.0 && (S.p.fec_cost > 0.0 || S.p.fecundity_model == ORC_FEC_CAPTURES))) { delete sim; return nullptr; }
         if (S.p.encounters > 16 || (S.p.encounters && (!S.p.sel_predation || !(S.p.attack >= 0.0 && S.p.attack <= 2.0)))) { delete sim; return nullptr; }
-        /* R18 is defined for an unstructured species (one patch) */
-        if (!(S.p.adult_survival >= 0.0 && S.p.adult_survival <= 1.0) || (S.p.adult_survival > 0.0 && sim->P != 1)) { delete sim; return nullptr; }
+        if (!(S.p.adult_survival >= 0.0 && S.p.adult_survival <= 1.0)) { delete sim; return nullptr; }
         if (S.p.resid_sd > 0.0) {
             S.T_env.resize(ENV_CAP);
             S.R_env = normal_table(S.p.resid_sd / (double)S.p.pheno_scale, S.T_env.data(), ENV_CAP);
@@ -875,6 +926,7 @@ int orc_debug(const orc_sim *sim, uint32_t species, orc_debug_view *o) {
     o->a_alive = D.a_alive.data(); o->a_u = D.a_u.data(); o->a_s = D.a_s.data();
     o->mate_cum = D.mate_cum.data(); o->zbar_self = D.zbar_self;
     o->sex_off = D.sex_off.data();
+    o->mom_cum = D.mom_cum.data();
     return 0;
 }
 

@@ -3,7 +3,7 @@
  *
  * TEST INFRASTRUCTURE ONLY.  This is the plain, slow, single-threaded, obviously
  * correct restatement of what the hot path computes (Fig. 1 A-F;
- * PAPER.md:321-330 genetics; the readings R1-R23 in DESIGN.md).  Only tests/,
+ * PAPER.md:321-330 genetics; the readings R1-R24 in DESIGN.md).  Only tests/,
  * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load it.  It shares no code, header, table or constant generator with the CUDA
  * library (include/spegg.h, paper_1603_09255_b200/csrc/): the structs below are
@@ -74,6 +74,14 @@ typedef struct {
                                    mother's patch, is accepted with probability exp(-assort * (z_c - z_m)^2);
                                    up to 8 candidates, the last one is taken if none was accepted.
                                    0 = random mating (R2); not together with mate_skew / separate_sexes */
+    double mother_skew;         /* R24 (eq. S2-9: "the probability that the egg comes from
+                                   female i is a function of the female's relative gonadal mass",
+                                   (G_i / (Omega_i + q_J Omega_i))^{v_f}): the mother of each egg is drawn
+                                   among the (female) adults of the patch that laid it with probability
+                                   proportional to Y_i^{v_f}, Y_i = exp(z_i) the adult's relative fecundity,
+                                   v_f = mother_skew; the NUMBER of eggs of the patch stays the sum of the
+                                   Poisson fecundities (R5).  0 = every adult mothers its own eggs (R1);
+                                   not together with fec_cost or the CAPTURES fecundity model     */
 } orc_species_params;
 
 typedef struct {
@@ -146,6 +154,7 @@ typedef struct {
     const uint64_t *mate_cum;  /* [n_t] R19: inclusive running sum of the integer mating weights */
     float zbar_self;           /* R19: mean genetic value of the adults, the weights' reference */
     const uint8_t *sex_off;    /* [m_t] R21: sex of each offspring (1 = male)                 */
+    const uint64_t *mom_cum;   /* [n_t] R24: inclusive running sum of the integer mothering weights */
 } orc_debug_view;
 int orc_debug(const orc_sim *s, uint32_t species, orc_debug_view *out);
 

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <new>
 #include <vector>
 
@@ -81,6 +82,52 @@ int h_normal_table(double sq, std::vector<uint32_t> &T) {
     return R;
 }
 
+// ---------------------------------------------------------------------- patch topology (R15)
+// neighbour of patch p on the gw x gh torus: direction 0: y-1, 1: x+1, 2: y+1, 3: x-1
+uint32_t h_neighbour(uint32_t p, uint32_t dir, uint32_t gw, uint32_t gh) {
+    uint32_t px = p % gw, py = p / gw;
+    switch (dir) {
+    case 0: py = (py + gh - 1) % gh; break;
+    case 1: px = (px + 1) % gw; break;
+    case 2: py = (py + 1) % gh; break;
+    default: px = (px + gw - 1) % gw; break;
+    }
+    return py * gw + px;
+}
+
+// slot of destination `dest` in the de-duplicated list [p, nb0 .. nb3] of natal patch p
+uint32_t h_dest_slot(uint32_t p, uint32_t dest, uint32_t gw, uint32_t gh) {
+    if (dest == p) return 0;
+    for (uint32_t k = 0; k < 4; ++k)
+        if (h_neighbour(p, k, gw, gh) == dest) return k + 1;
+    return 0;
+}
+
+// nbr[p][dir] and, for every destination d, its sources (natal patch, slot), unique per natal patch,
+// sorted by natal patch: the order of the next generation inside d (by (natal patch, j))
+void h_topology(uint32_t gw, uint32_t gh, std::vector<uint32_t> &nbr, std::vector<uint32_t> &src) {
+    const uint32_t P = gw * gh;
+    nbr.assign((size_t)P * 4, 0);
+    src.assign((size_t)P * 6, 0);
+    for (uint32_t p = 0; p < P; ++p)
+        for (uint32_t k = 0; k < 4; ++k) nbr[(size_t)p * 4 + k] = h_neighbour(p, k, gw, gh);
+    for (uint32_t d = 0; d < P; ++d) {
+        uint32_t n = 0, pp[5], ss[5];
+        pp[n] = d; ss[n] = 0; ++n;
+        for (uint32_t k = 0; k < 4; ++k) {
+            const uint32_t q = h_neighbour(d, (k + 2) & 3u, gw, gh);   // the patch whose direction-k neighbour is d
+            if (q == d || h_neighbour(q, k, gw, gh) != d) continue;
+            bool dup = false;
+            for (uint32_t i = 0; i < n; ++i) dup |= (pp[i] == q);
+            if (!dup) { pp[n] = q; ss[n] = h_dest_slot(q, d, gw, gh); ++n; }
+        }
+        for (uint32_t i = 1; i < n; ++i)
+            for (uint32_t k2 = i; k2 > 0 && pp[k2] < pp[k2 - 1]; --k2) { std::swap(pp[k2], pp[k2 - 1]); std::swap(ss[k2], ss[k2 - 1]); }
+        src[(size_t)d * 6] = n;
+        for (uint32_t i = 0; i < n; ++i) src[(size_t)d * 6 + 1 + i] = (pp[i] << 3) | ss[i];
+    }
+}
+
 // ------------------------------------------------------------------------------ layout
 constexpr uint64_t HEADER_SPK = 8192;   // workspace header: DevGlobal at 0, DevSpecies[] at 256, SpK[] here
 
@@ -96,7 +143,7 @@ struct Carver {
 struct SpeciesLayout {
     uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos, mate_cum, mate_tile, enc_zi, sex[2], sex_off,
         cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
-    uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, T_env, K_patch, theta_patch;
+    uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, T_env, K_patch, theta_patch, nbr, src_list;
     uint32_t norm_len, env_len, n_tables, row_bytes;
 };
 
@@ -235,6 +282,8 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.T_env = c.take((uint64_t)l.env_len * 4 + 16);
         l.K_patch = c.take(P * 8);
         l.theta_patch = c.take(P * 4);
+        l.nbr = c.take(P * 4 * 4);
+        l.src_list = c.take(P * 6 * 4);
     }
     return (c.off + 255) & ~255ull;
 }
@@ -346,7 +395,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             // the plain kernels, so the two can be compared with each other and with the oracle)
             const bool q10v = !s->debug && gamete_q10v_supported(k);
             if (k.kind == 0) k_gamete_bit<<<ctas(cap * 2 * k.n_chrom, 256, 8), 256, 0, s->stream>>>(k);
-            else if (q10v) k_gamete_q10v<<<g_warp, 256, 0, s->stream>>>(k);
+            else if (q10v) CU(launch_gamete_q10v(k, G, s->stream));
             else k_gamete_q10<<<ctas(cap * 2, 8, 8), 256, 0, s->stream>>>(k);
             ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
@@ -486,6 +535,12 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
             (rc = upload(s, l.K_patch, h.K_patch.data(), h.K_patch.size() * 8)) ||
             (rc = upload(s, l.theta_patch, h.theta_patch.data(), h.theta_patch.size() * 4)))
             return fail(rc);
+        if (s->P > 1) {
+            std::vector<uint32_t> nbr, src;
+            h_topology(gw, gh, nbr, src);
+            if ((rc = upload(s, l.nbr, nbr.data(), nbr.size() * 4)) || (rc = upload(s, l.src_list, src.data(), src.size() * 4))) return fail(rc);
+            if (cudaStreamSynchronize(s->stream) != cudaSuccess) return fail(SPEGG_ECUDA);   // the vectors go out of scope
+        }
         if (cudaMemsetAsync(s->ws + l.patch_start[0], 0, (s->P + 1) * 4, s->stream) != cudaSuccess ||
             cudaMemsetAsync(s->ws + l.patch_start[1], 0, (s->P + 1) * 4, s->stream) != cudaSuccess ||
             cudaMemsetAsync(s->ws + l.cap, 0, (size_t)q.capacity * 4, s->stream) != cudaSuccess)
@@ -544,6 +599,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.status_fec = at<unsigned long long>(s, l.status_fec); k.status_cmp = at<unsigned long long>(s, l.status_cmp);
         k.status_fec_n = (uint32_t)(q.capacity / SCAN_THREADS + 2); k.status_cmp_n = (uint32_t)(q.capacity / SCAN_TILE + 2);
         k.patch_cnt = at<uint32_t>(s, l.patch_cnt); k.patch_base = at<uint32_t>(s, l.patch_base);
+        k.nbr = at<uint32_t>(s, l.nbr); k.src_list = at<uint32_t>(s, l.src_list);
         k.st = s->d_st + si; k.st_all = s->d_st; k.glob = s->d_glob;
         k.log = at<LogEntry>(s, l.log); k.log_capacity = s->log_capacity;
         k.debug = p->debug;

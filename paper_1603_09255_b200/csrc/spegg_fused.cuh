@@ -86,7 +86,10 @@ constexpr int SCANF_CHUNKS = SCANF_RANGE / FUSED_CHUNK;
 //   (e) lane = offspring: phenotype -> fp32 survival -> decision; the ballot is the chunk's mask.
 constexpr int FUSEDF_WARPS = 4;
 constexpr int FUSEDF_UNROLL_C = 2;                // decode passes in flight per lane
-constexpr int FUSEDF_CTAS = 5;                    // resident CTAs per SM (shared memory and registers allow 5)
+#ifndef SPEGG_FUSEDF_CTAS
+#define SPEGG_FUSEDF_CTAS 5
+#endif
+constexpr int FUSEDF_CTAS = SPEGG_FUSEDF_CTAS;    // resident CTAs per SM (shared memory and registers allow 5)
 constexpr int FUSEDF_AHEAD = 1;                   // passes the mothers' loads run ahead
 constexpr uint32_t FUSEDF_SP_OFF = FUSED_CHUNK * FUSED_ROW;        // packed draws [8][4][4][2] / partial sums
 constexpr uint32_t FUSEDF_Q_OFF = FUSEDF_SP_OFF + 8 * 32 * 4;      // queue of chromosomes with > 2 crossovers: draw [32], (pass, lane) [32]
@@ -117,6 +120,18 @@ __device__ __forceinline__ void half_masks(uint32_t P, uint32_t half, uint32_t (
     for (int i = 0; i < 4; ++i) m[i] = phi ^ mask_from(s0, i) ^ mask_from(s1, i);
 }
 
+// crossover count of a draw already known to be >= 3 (u >= T[2]): the next four thresholds are loaded
+// at once instead of one dependent load per step of the search; longer searches (count > 6) finish
+// with the plain loop
+__device__ __forceinline__ uint32_t xover_count_from3(const uint32_t *__restrict__ T, uint32_t len, uint32_t u) {
+    const uint32_t t3 = len > 3 ? T[3] : 0xFFFFFFFFu, t4 = len > 4 ? T[4] : 0xFFFFFFFFu,
+                   t5 = len > 5 ? T[5] : 0xFFFFFFFFu, t6 = len > 6 ? T[6] : 0xFFFFFFFFu;
+    // (a missing threshold compares as "not reached"; T is increasing, so the tests are nested)
+    uint32_t k = 3u + (len > 3 && u >= t3 ? 1u : 0u) + (len > 4 && u >= t4 ? 1u : 0u) + (len > 5 && u >= t5 ? 1u : 0u) +
+                 (len > 6 && u >= t6 ? 1u : 0u);
+    if (k == 7u) while (k < len && u >= T[k]) ++k;
+    return k;
+}
 
 template <int NC, int WPC>
 __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(const __grid_constant__ SpK sp) {
@@ -191,6 +206,18 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     auto fix_extra = [&](uint32_t e_o, uint32_t e_g, uint32_t e_c, uint32_t e_nc) {
         const uint32_t e_j = j0 + e_o;
         if (e_j >= M) return;
+        // the loads first (the row this warp stored a moment ago comes back from L2; the parent's two
+        // haplotypes of this chromosome: father from the stage, mother from global), the draws below hide them
+        uint4 h[4];
+        if (e_g) {
+            const uint32_t a_ = stage + e_o * FUSED_ROW + e_c * 32u;
+            h[0] = lds128(a_); h[1] = lds128(a_ + 16); h[2] = lds128(a_ + FUSED_ROW / 2); h[3] = lds128(a_ + FUSED_ROW / 2 + 16);
+        } else {
+            const uint8_t *a_ = pop + (s_mo[e_o] | (e_c * 32u));
+            h[0] = ldg128(a_); h[1] = ldg128(a_ + 16); h[2] = ldg128(a_ + FUSED_ROW / 2); h[3] = ldg128(a_ + FUSED_ROW / 2 + 16);
+        }
+        uint4 *orow = (uint4 *)(nxt + (size_t)e_j * FUSED_ROW + e_g * (FUSED_ROW / 2) + e_c * 32u);
+        uint4 o0 = ldg128(orow), o1 = ldg128(orow + 1);
         const uint32_t e_clen1 = sp.chrom_len[e_c] - 1;
         uint32_t xm[8];
 #pragma unroll
@@ -208,17 +235,6 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
                 }
             }
         }
-        // the parent's two haplotypes of this chromosome: father from the stage, mother from global
-        uint4 h[4];
-        if (e_g) {
-            const uint32_t a_ = stage + e_o * FUSED_ROW + e_c * 32u;
-            h[0] = lds128(a_); h[1] = lds128(a_ + 16); h[2] = lds128(a_ + FUSED_ROW / 2); h[3] = lds128(a_ + FUSED_ROW / 2 + 16);
-        } else {
-            const uint8_t *a_ = pop + (s_mo[e_o] | (e_c * 32u));
-            h[0] = ldg128(a_); h[1] = ldg128(a_ + 16); h[2] = ldg128(a_ + FUSED_ROW / 2); h[3] = ldg128(a_ + FUSED_ROW / 2 + 16);
-        }
-        uint4 *orow = (uint4 *)(nxt + (size_t)e_j * FUSED_ROW + e_g * (FUSED_ROW / 2) + e_c * 32u);
-        uint4 o0 = orow[0], o1 = orow[1];
         const int before = __popc(o0.x) + __popc(o0.y) + __popc(o0.z) + __popc(o0.w) + __popc(o1.x) + __popc(o1.y) + __popc(o1.z) + __popc(o1.w);
         o0.x ^= (h[0].x ^ h[2].x) & xm[0]; o0.y ^= (h[0].y ^ h[2].y) & xm[1];
         o0.z ^= (h[0].z ^ h[2].z) & xm[2]; o0.w ^= (h[0].w ^ h[2].w) & xm[3];
@@ -357,7 +373,7 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
         if (qn <= 32) {
             if (lane < qn) {
                 const uint32_t e = s_q[32 + lane], e_ln = e & 31u, e_c = e_ln & 3u;
-                const uint32_t e_nc = poisson_count(sp.T_xover + e_c * XMAX, sp.xover_len[e_c], s_q[lane]);
+                const uint32_t e_nc = xover_count_from3(sp.T_xover + e_c * XMAX, sp.xover_len[e_c], s_q[lane]);
                 fix_extra((e >> 5) * 4 + (e_ln >> 3), (e_ln >> 2) & 1u, e_c, e_nc);
             }
         }
@@ -432,6 +448,7 @@ static_assert(SCANF_ROWS == 4 && 32 % SCANF_ROWS == 0, "a thread's rows are one 
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_constant__ SpK sp) {
     constexpr uint32_t NW = SCAN_THREADS / 32, NT = SCAN_THREADS;
     __shared__ uint32_t s_tab[TMAX];
+    __shared__ uint32_t s_len;
     __shared__ uint32_t s_cnt[NW], s_pre[NW], s_f[NW];
     __shared__ unsigned long long s_excl;
     __shared__ uint32_t s_stage[SCANF_STAGE];
@@ -445,8 +462,15 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
     const uint32_t *mask = sp.chunk_mask[cur];
     uint32_t *rp = sp.rowptr[cur];
     if (blockIdx.x >= n_ranges) return;   // (no adults at all: M_t stays 0)
-    const uint32_t len0 = sp.table_len[0];
-    if (tid < TMAX) s_tab[tid] = sp.tables[tid];
+    // a0: the fecundity table of this step (R5, R13) is built HERE, by one thread of every CTA, while the
+    // others turn the range counts into indices -- the ~2 us fp64 chain of the table is then off the
+    // path between the two kernels (the step closing of the previous gamete kernel leaves it out)
+    if (tid == NT - 1) {
+        const double lam = fecundity_mean(sp, (double)st.n0, sp.K_patch ? sp.K_patch[0] : sp.K, 0);
+        s_len = (uint32_t)build_poisson_table(lam, s_tab, TMAX);
+    }
+    uint32_t T0 = 0xFFFFFFFFu, T1 = 0xFFFFFFFFu, T2 = 0xFFFFFFFFu, T3 = 0xFFFFFFFFu, len0 = 0;
+    bool have_tab = false;
     for (uint32_t range = blockIdx.x; range < n_ranges; range += gridDim.x) {
         const uint32_t row0 = range * SCANF_RANGE + tid * SCANF_ROWS;
         const uint32_t ch = row0 >> 5;
@@ -461,20 +485,19 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
         __syncthreads();   // the previous range's stage has been written out
         if (lane == 31) s_cnt[warp] = incl;
         if (lane == 0) s_pre[warp] = pre;
-        __syncthreads();
+        __syncthreads();   // (also: the table is built)
+        if (!have_tab) {   // the first thresholds in registers: the search below rarely goes past them
+            have_tab = true;
+            len0 = s_len;
+            if (len0 > 0) T0 = s_tab[0];
+            if (len0 > 1) T1 = s_tab[1];
+            if (len0 > 2) T2 = s_tab[2];
+            if (len0 > 3) T3 = s_tab[3];
+        }
         uint32_t ibase = 0, li0 = incl - c4, n_r = 0;   // adults before the range / before this thread in it / in it
 #pragma unroll
         for (uint32_t w = 0; w < NW; ++w) { ibase += s_pre[w]; n_r += s_cnt[w]; if (w < warp) li0 += s_cnt[w]; }
-        // ---- rowptr
-        {
-            uint32_t li = li0;
-#pragma unroll
-            for (uint32_t k = 0; k < SCANF_ROWS; ++k)
-                if ((bits >> k) & 1u) s_stage[li++] = row0 + k;
-        }
-        __syncthreads();
-        for (uint32_t k = tid; k < n_r; k += NT) rp[ibase + k] = s_stage[k];
-        // ---- fecundity of this thread's adults
+        // ---- fecundity of this thread's adults (first: the range's total is what the other ranges wait for)
         uint32_t fsum = 0, fpack = 0;
         {
             uint32_t i = ibase + li0;
@@ -483,7 +506,13 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
                 if ((bits >> k) & 1u) {
                     uint32_t x[4];
                     draw_rk(sp, ST_FEC, i++, 0, step, x);
-                    const uint32_t f = poisson_count(s_tab, len0, x[0]);
+                    const uint32_t u = x[0];
+                    // count(u) = #{k < len : u >= T_k}, T increasing (a missing threshold is never reached:
+                    // the table stops before 2^32 - 1 ... see build_poisson_table; u >= T with T = 2^32 - 1 only
+                    // for u = 2^32 - 1, excluded by the length test)
+                    uint32_t f = (len0 > 0 && u >= T0 ? 1u : 0u) + (len0 > 1 && u >= T1 ? 1u : 0u) +
+                                 (len0 > 2 && u >= T2 ? 1u : 0u) + (len0 > 3 && u >= T3 ? 1u : 0u);
+                    if (f == 4u) while (f < len0 && u >= s_tab[f]) ++f;
                     fpack |= f << (8u * k);
                     fsum += f;
                 }
@@ -492,7 +521,14 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
         // ---- look-back over the fecundities: offspring before this range
         const uint32_t fincl = warp_incl_scan(fsum);
         if (lane == 31) s_f[warp] = fincl;
-        __syncthreads();   // (also: the staged rowptr words have been read)
+        // ---- rowptr (staged, stored coalesced below while warp 0 waits for the look-back)
+        {
+            uint32_t li = li0;
+#pragma unroll
+            for (uint32_t k = 0; k < SCANF_ROWS; ++k)
+                if ((bits >> k) & 1u) s_stage[li++] = row0 + k;
+        }
+        __syncthreads();
         uint32_t total = 0, wbase = 0;
 #pragma unroll
         for (uint32_t w = 0; w < NW; ++w) { const uint32_t v = s_f[w]; total += v; if (w < warp) wbase += v; }
@@ -506,7 +542,10 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
                     else st.m = (uint32_t)Mtot;
                 }
             }
+        } else {
+            for (uint32_t k = tid - 32u; k < n_r; k += NT - 32u) rp[ibase + k] = s_stage[k];
         }
+        __syncthreads();   // the staged rowptr words have been read; s_excl is there
         // ---- mother[]: staged per range like rowptr (a range with more offspring than the stage holds
         // -- fecundities far above the table means of any configuration -- writes them directly)
         const bool staged = total <= SCANF_STAGE;
@@ -518,8 +557,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_fused(const __grid_consta
                 for (uint32_t cpy = 0; cpy < f; ++cpy) s_stage[lo++] = row0 + k;
             }
         }
-        __syncthreads();
         const unsigned long long obase = s_excl;
+        __syncthreads();
         if (staged) {
             for (uint32_t k = tid; k < total; k += NT)
                 if (obase + k < (unsigned long long)sp.capacity) sp.mother[obase + k] = s_stage[k];

@@ -125,6 +125,9 @@ struct SpK {
     unsigned long long *status_fec, *status_cmp;  // [n] tile aggregates + [n/32+2] group counters
     uint32_t status_fec_n, status_cmp_n;
     uint32_t *patch_cnt, *patch_base;  // [P][5]
+    // patch topology (P > 1), built once by the host: the torus never changes
+    const uint32_t *nbr;        // [P][4] neighbour of patch p in direction 0..3 (R15)
+    const uint32_t *src_list;   // [P][6]: word 0 = number of sources n of destination d, words 1..n = source patch << 3 | slot, by source patch
     DevSpecies *st;             // this species
     DevSpecies *st_all;         // all species
     DevGlobal *glob;

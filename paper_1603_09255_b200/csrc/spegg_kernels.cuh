@@ -14,6 +14,8 @@
 // debug view; spegg_fused.cuh holds the fused single-pass kernels of the hot configurations.
 // All grids are fixed at graph-capture time and loop against device-side counts.
 #pragma once
+#include <algorithm>
+
 #include "spegg_internal.h"
 
 namespace spegg {
@@ -28,15 +30,14 @@ __device__ __forceinline__ uint32_t patch_of(const uint32_t *__restrict__ ps, ui
     return lo;
 }
 
-__device__ __forceinline__ uint32_t neighbour(uint32_t p, uint32_t dir, uint32_t gw, uint32_t gh) {
-    uint32_t px = p % gw, py = p / gw;
-    switch (dir) {
-    case 0: py = (py + gh - 1) % gh; break;
-    case 1: px = (px + 1) % gw; break;
-    case 2: py = (py + 1) % gh; break;
-    default: px = (px + gw - 1) % gw; break;
+// the same search between two known patches lo <= patch(i) <= hi
+__device__ __forceinline__ uint32_t patch_between(const uint32_t *__restrict__ ps, uint32_t lo, uint32_t hi, uint32_t i) {
+    ++hi;
+    while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (ps[mid] <= i) lo = mid; else hi = mid;
     }
-    return py * gw + px;
+    return lo;
 }
 
 // Philox4x32-10 (R3) with the ten round keys taken from the kernel parameter block: the key
@@ -162,7 +163,8 @@ __device__ __forceinline__ void prepare_species(const SpK &sp, uint32_t g, uint3
     const uint32_t *ps = sp.patch_start[cur];
     // g_tab: this thread's index for the table builds (the step-closing CTA gives table 0 to a thread of
     // another warp than the one that is busy closing the step: the fp64 chain of a table is ~2 us)
-    for (uint32_t tab = g_tab; tab < sp.n_tables; tab += stride) {
+    // (fused path: k_scan_fused builds the one table itself, off the path between the kernels)
+    for (uint32_t tab = sp.phys_parents ? sp.n_tables : g_tab; tab < sp.n_tables; tab += stride) {
         double lam;
         if (sp.fec_model == 2) lam = fecundity_mean(sp, (double)N, sp.K, tab);
         else if (sp.P == 1) lam = fecundity_mean(sp, (double)N, sp.K_patch ? sp.K_patch[0] : sp.K, 0);
@@ -264,12 +266,18 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
     }
     const uint32_t *ps = sp.patch_start[st.cur];
     const uint32_t *rowptr = sp.rowptr[st.cur];
+    const bool by_patch = !one_table && sp.fec_model != 2;
     for (;;) {
         if (tid == 0) s_tile = atomicAdd(&st.ticket_fec, 1u);
         __syncthreads();
         const uint32_t range = s_tile;
         if (range >= n_ranges) break;
         const uint32_t r0 = range * R;
+        // patch mode: the adults of a range lie in a few consecutive patches -- every thread finds the
+        // patches of the range's first and last adult (the same search in every lane: broadcast loads) and
+        // then only searches between them
+        uint32_t p_lo = 0, p_hi = 0;
+        if (by_patch) { p_lo = patch_of(ps, sp.P, r0); p_hi = patch_of(ps, sp.P, min(r0 + R, N) - 1u); }
         // ---- pass 1: fecundity draws (coalesced in i), staged as bytes
         for (uint32_t k = tid; k < R; k += SCAN_THREADS) {
             const uint32_t i = r0 + k;
@@ -280,7 +288,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
                 if (one_table) {
                     f = poisson_count(s_tab, len0, x[0]);
                 } else {
-                    const uint32_t tab = (sp.fec_model == 2) ? min(sp.cap[i], (uint32_t)(CAP_TABLES - 1)) : patch_of(ps, sp.P, i);
+                    const uint32_t tab = (sp.fec_model == 2) ? min(sp.cap[i], (uint32_t)(CAP_TABLES - 1)) : patch_between(ps, p_lo, p_hi, i);
                     f = poisson_count(sp.tables + (size_t)tab * TMAX, sp.table_len[tab], x[0]);
                 }
                 if (sp.sexes && sp.sex[st.cur][rowptr[i]]) f = 0;   // R21: males lay no eggs (the draw is made and ignored)
@@ -339,9 +347,11 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
             sp.f[i] = (uint8_t)f;
             if (f) {
                 const uint32_t mval = sp.phys_parents ? rowptr[i] : i;
+                // patch mode: the offspring's natal patch goes into dest[] (k_scalar reads it and stores the destination)
+                const uint32_t pm = by_patch ? patch_between(ps, p_lo, p_hi, i) : 0u;
                 for (uint32_t c = 0; c < f; ++c) {
                     const unsigned long long j = o + c;
-                    if (j < (unsigned long long)m_cap) sp.mother[j] = mval;
+                    if (j < (unsigned long long)m_cap) { sp.mother[j] = mval; if (sp.P > 1) sp.dest[j] = pm; }
                 }
             }
         }
@@ -475,7 +485,7 @@ __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) 
         uint32_t x[4];
         draw(sp.key, sp.species, ST_SCALAR, j, 0, step, x);
         uint32_t pm = 0, base = 0, np = N;
-        if (sp.P > 1) { pm = patch_of(ps, sp.P, mo); base = ps[pm]; np = ps[pm + 1] - base; }
+        if (sp.P > 1) { pm = sp.dest[j]; base = ps[pm]; np = ps[pm + 1] - base; }   // natal patch: left in dest[] by k_fec_scan
         uint32_t fa = base + uniform_index(x[0], np);
         if (sp.mate_on) {
             // R19: weighted draw among the adults of the mother's patch: 64-bit uniform from words 2,3 of
@@ -514,7 +524,7 @@ __global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) 
         }
         sp.father[j] = fa;
         uint32_t dest = pm;
-        if (sp.P > 1 && (unsigned long long)x[1] < sp.T_mig) dest = neighbour(pm, x[2] >> 30, sp.grid_w, sp.grid_h);
+        if (sp.P > 1 && (unsigned long long)x[1] < sp.T_mig) dest = sp.nbr[pm * 4u + (x[2] >> 30)];
         sp.dest[j] = dest;
         sp.u01[j] = u01_of(x[3]);
         if (sp.sexes) sp.sex_off[j] = (uint8_t)(x[2] & 1u);   // R21: sex at birth (bits 30-31 of the word are the direction)
@@ -626,95 +636,177 @@ __global__ void __launch_bounds__(256) k_gamete_q10(const __grid_constant__ SpK 
 // a4 + a5 (q10 genomes, R7 + R10) for L = 8 ... 256 a power of two: a lane owns 8 consecutive loci of
 // one gamete (two RECOMB blocks, one 128-bit load from each parental haplotype, one 128-bit store),
 // GS = L / 8 lanes make a gamete, and a warp works on whole offspring: both gametes side by side
-// (L <= 128; several offspring per warp when L <= 64) or one after the other (L = 256).  The phase
-// is the XOR prefix of the switch bits: within the lane in registers, across the lanes of the gamete
-// by a ballot.  The lane's share of the additive phenotype (sum of the 8 alleles it selected) is
-// reduced over the offspring's lanes, so the offspring row is never read again for a5.
+// (L <= 128; several offspring per warp when L <= 64) or one after the other (L = 256).  The lane's
+// eight switch thresholds never change (its slot in the gamete is fixed), so they live in registers.
+// The phase is the XOR prefix of the switch bits: within the lane by shift-and-xor on the packed
+// byte, across the lanes of the gamete by a ballot.  The select masks come from the phase byte by a
+// multiply (bit k -> sign bit of byte k) and a sign-replicating byte permute.  The rows of the NEXT
+// work item (iteration, or the father's pass of the same offspring when L = 256) are loaded before
+// this one's draws are computed, and the parents' indices are looked up two iterations ahead, so no
+// load is ever waited for.  The lane's share of the additive phenotype (sum of the 8 alleles it
+// selected) is reduced over the offspring's lanes (one REDUX), so the row is never read again for a5.
 __host__ __device__ inline bool gamete_q10v_supported(const SpK &k) {
     return k.kind == 1 && k.L >= 8 && k.L <= 256 && (k.L & (k.L - 1)) == 0;
 }
 
-__global__ void __launch_bounds__(256) k_gamete_q10v(const __grid_constant__ SpK sp) {
+__device__ __forceinline__ uint32_t prmt_sign(uint32_t a, uint32_t sel) {
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %1, %2;" : "=r"(d) : "r"(a), "r"(sel));   // selector nibble 8 | i: sign of byte i replicated
+    return d;
+}
+
+#ifndef SPEGG_Q10V_THREADS
+#define SPEGG_Q10V_THREADS 128
+#endif
+#ifndef SPEGG_Q10V_MINB
+#define SPEGG_Q10V_MINB 7
+#endif
+#ifndef SPEGG_Q10V_MINB256
+#define SPEGG_Q10V_MINB256 6
+#endif
+constexpr int Q10V_THREADS = SPEGG_Q10V_THREADS;
+
+template <uint32_t LL>
+__global__ void __launch_bounds__(Q10V_THREADS, (LL == 256 ? SPEGG_Q10V_MINB256 : SPEGG_Q10V_MINB)) k_gamete_q10v(const __grid_constant__ SpK sp) {
+    constexpr uint32_t GS = LL >> 3;                       // lanes per gamete
+    constexpr uint32_t LPO = (2u * GS < 32u) ? 2u * GS : 32u;   // lanes per offspring in one pass
+    constexpr uint32_t NPASS = (2u * GS) / LPO;            // 2 when L = 256, else 1
+    constexpr uint32_t OPW = 32u / LPO;                    // offspring per warp iteration
+    constexpr uint32_t ROW = LL * 4u;                      // bytes per row
     const DevSpecies &st = *sp.st;
-    const uint32_t M = st.m, step = sp.glob->step, L = sp.L;
-    const uint32_t GS = L >> 3;                         // lanes per gamete
-    const uint32_t LPO = min(32u, 2u * GS);             // lanes per offspring in one pass
-    const uint32_t npass = (2u * GS) / LPO;             // 2 when L = 256, else 1
-    const uint32_t opw = 32u / LPO;                     // offspring per warp iteration
-    const uint32_t gs_log = (uint32_t)__ffs((int)GS) - 1u, lpo_log = (uint32_t)__ffs((int)LPO) - 1u;   // both powers of two
-    const uint32_t lane = threadIdx.x & 31u, li = lane & (LPO - 1u), osub = lane >> lpo_log;
+    const uint32_t M = st.m, step = sp.glob->step;
+    const uint32_t lane = threadIdx.x & 31u, li = lane & (LPO - 1u), osub = lane / LPO;
+    const uint32_t slot = li & (GS - 1u), g0 = (NPASS == 1) ? li / GS : 0u;   // gamete of pass p: g0 + p
     const uint32_t lt = (1u << lane) - 1u;
+    const uint32_t gmask = (GS == 32u ? 0xFFFFFFFFu : ((1u << GS) - 1u)) << (lane - slot);
+    const uint32_t omask = (LPO == 32u ? 0xFFFFFFFFu : ((1u << LPO) - 1u)) << (lane - li);
     const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
     const uint8_t *pop = sp.pop[st.cur];
     const uint32_t *rowptr = sp.rowptr[st.cur];
-    const uint4 *Tr = (const uint4 *)sp.T_recomb;
     uint8_t *out = offspring_rows(sp);
-    // the parents' rows of the NEXT iteration are looked up (mother[] / father[] -> rowptr[]) while this
-    // one computes, so the two dependent index loads are never waited for
-    auto parents = [&](unsigned long long ob_, uint32_t &p0, uint32_t &p1) {
-        const unsigned long long j_ = ob_ + osub;
+#ifndef SPEGG_Q10V_TSMEM
+#define SPEGG_Q10V_TSMEM 0
+#endif
+#if SPEGG_Q10V_TSMEM
+    // the switch thresholds of the LL loci, re-read from shared memory by every pass (registers are what
+    // limits the resident warps)
+    __shared__ uint4 s_T[LL / 4];
+    for (uint32_t k = threadIdx.x; k < LL / 4; k += blockDim.x) s_T[k] = ((const uint4 *)sp.T_recomb)[k];
+    __syncthreads();
+#else
+    const uint4 t0 = ((const uint4 *)sp.T_recomb)[2u * slot], t1 = ((const uint4 *)sp.T_recomb)[2u * slot + 1u];
+#endif
+    // parents' rows of the offspring this lane works on in the iteration that starts at ob_
+    // (32-bit offspring indices: M <= capacity < 2^31 and two strides are far below 2^31)
+    auto parents = [&](uint32_t ob_, uint32_t &p0, uint32_t &p1) {
+        const uint32_t j_ = ob_ + osub;
         p0 = 0u; p1 = 0u;
         if (j_ < M) { p0 = rowptr[sp.mother[j_]]; p1 = rowptr[sp.father[j_]]; }
     };
-    const unsigned long long stride = (unsigned long long)n_warps * opw;
-    uint32_t par0, par1;
-    parents((unsigned long long)gw * opw, par0, par1);
-    for (unsigned long long ob = (unsigned long long)gw * opw; ob < M; ob += stride) {
-        const uint32_t j = (uint32_t)ob + osub;
-        const bool live = j < M;
-        uint32_t nx0, nx1;
-        parents(ob + stride, nx0, nx1);
+    // (volatile asm: the loads are issued HERE, ahead of the draws, not sunk to their first use; a dead
+    // lane reads row 0)
+    auto rows = [&](uint32_t par, uint4 &a, uint4 &b) {
+        const uint4 *h0 = (const uint4 *)(pop + (size_t)par * ROW) + slot;
+        asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w) : "l"(h0));
+        asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(h0 + GS));
+    };
+    // switch bit of one locus shifted into the packed byte: sub.cc sets the carry iff x >= T (no switch)
+    auto push = [&](uint32_t &ph, uint32_t x, uint32_t T) {
+        uint32_t t;
+        asm("sub.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %1, %1;" : "=r"(t), "+r"(ph) : "r"(x), "r"(T));
+    };
+    // one pass: gamete g of offspring j from the parental haplotype words a (hap0), b (hap1)
+    auto pass = [&](uint32_t j, uint32_t g, const uint4 &a, const uint4 &b, int &acc) {
+        // R7: switch bits of this lane's 8 loci, packed (locus 0 in bit 0), and their running parity
+        uint32_t x[4], y[4];
+        const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
+        draw_rk(sp, stream, j, 2u * slot, step, x);
+        draw_rk(sp, stream, j, 2u * slot + 1u, step, y);
+#if SPEGG_Q10V_TSMEM
+        const uint4 t0 = s_T[2u * slot], t1 = s_T[2u * slot + 1u];
+#endif
+        uint32_t ph = 0;
+        push(ph, y[3], t1.w); push(ph, y[2], t1.z); push(ph, y[1], t1.y); push(ph, y[0], t1.x);
+        push(ph, x[3], t0.w); push(ph, x[2], t0.z); push(ph, x[1], t0.y); push(ph, x[0], t0.x);
+        ph = ~ph & 0xFFu;                                 // bit k: locus k of the lane switches
+        ph ^= ph << 1; ph ^= ph << 2; ph ^= ph << 4;      // bit k = parity of the switch bits of loci 0..k of the lane
+        const uint32_t bal = __ballot_sync(0xffffffffu, (ph & 0x80u) != 0);
+        if (__popc(bal & gmask & lt) & 1u) ph = ~ph;
+        // select: allele from hap1 where the phase bit is set.  bit k of a nibble -> sign bit of byte k
+        // (k + 7 + 7k = 8k + 7; the other products land on other bits), replicated over the allele's two bytes
+        const uint32_t lo = (ph & 0xFu) * 0x10204080u, hi = ((ph >> 4) & 0xFu) * 0x10204080u;
+        const uint32_t m0 = prmt_sign(lo, 0x9988u), m1 = prmt_sign(lo, 0xBBAAu), m2 = prmt_sign(hi, 0x9988u), m3 = prmt_sign(hi, 0xBBAAu);
+        uint4 o;
+        o.x = (a.x & ~m0) | (b.x & m0); o.y = (a.y & ~m1) | (b.y & m1);
+        o.z = (a.z & ~m2) | (b.z & m2); o.w = (a.w & ~m3) | (b.w & m3);
+        if (j < M) {
+            ((uint4 *)(out + (size_t)j * ROW))[g * GS + slot] = o;
+            // R10: both int16 halves of a word summed by one dp2a
+            acc = __dp2a_lo((int)o.x, 0x0101, acc); acc = __dp2a_lo((int)o.y, 0x0101, acc);
+            acc = __dp2a_lo((int)o.z, 0x0101, acc); acc = __dp2a_lo((int)o.w, 0x0101, acc);
+        }
+    };
+    const uint32_t stride = n_warps * OPW, ob0 = gw * OPW;
+    uint32_t pm, pf, nm, nf;
+    parents(ob0, pm, pf);
+    parents(ob0 + stride, nm, nf);
+    // one iteration: works on the rows in (a, b), loads the next iteration's into (na, nb)
+    auto iteration = [&](uint32_t ob, const uint4 &a, const uint4 &b, uint4 &na, uint4 &nb) {
+        const uint32_t j = ob + osub;
+        uint32_t n2m, n2f;
+        parents(ob + 2u * stride, n2m, n2f);
         int acc = 0;
-        for (uint32_t p = 0; p < npass; ++p) {
-            const uint32_t t = p * LPO + li, g = t >> gs_log, slot = t & (GS - 1u);
-            const uint4 *h0 = (const uint4 *)(pop + (size_t)(g ? par1 : par0) * sp.row_bytes) + slot;
-            // (volatile asm: the loads are issued HERE, ahead of the draws, not sunk to their first use;
-            // a dead lane reads row 0)
-            uint4 a, b;
-            asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w) : "l"(h0));
-            asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(h0 + GS));
-            // R7: switch bits of this lane's 8 loci and their running parity
-            uint32_t x[4], y[4];
-            const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
-            draw_rk(sp, stream, j, 2u * slot, step, x);
-            draw_rk(sp, stream, j, 2u * slot + 1u, step, y);
-            const uint4 t0 = Tr[2u * slot], t1 = Tr[2u * slot + 1u];
-            uint32_t run = 0, ph = 0;   // ph bit k = parity of the switch bits of loci 0..k of the lane
-            run ^= x[0] < t0.x ? 1u : 0u; ph |= run;
-            run ^= x[1] < t0.y ? 1u : 0u; ph |= run << 1;
-            run ^= x[2] < t0.z ? 1u : 0u; ph |= run << 2;
-            run ^= x[3] < t0.w ? 1u : 0u; ph |= run << 3;
-            run ^= y[0] < t1.x ? 1u : 0u; ph |= run << 4;
-            run ^= y[1] < t1.y ? 1u : 0u; ph |= run << 5;
-            run ^= y[2] < t1.z ? 1u : 0u; ph |= run << 6;
-            run ^= y[3] < t1.w ? 1u : 0u; ph |= run << 7;
-            const uint32_t bal = __ballot_sync(0xffffffffu, run != 0);
-            const uint32_t gmask = (GS == 32u ? 0xFFFFFFFFu : ((1u << GS) - 1u)) << (lane - slot);
-            if (__popc(bal & gmask & lt) & 1u) ph ^= 0xFFu;
-            // select: allele from hap1 where the phase bit is set
-            uint4 o;
-            {
-                // phase bit 2w -> low half, 2w+1 -> high half of word w: (b0 | b1 << 16) * 0xFFFF
-                const uint32_t sp2 = ph | (ph << 15);
-                const uint32_t m0 = (sp2 & 0x00010001u) * 0xFFFFu, m1 = ((sp2 >> 2) & 0x00010001u) * 0xFFFFu;
-                const uint32_t m2 = ((sp2 >> 4) & 0x00010001u) * 0xFFFFu, m3 = ((sp2 >> 6) & 0x00010001u) * 0xFFFFu;
-                o.x = (a.x & ~m0) | (b.x & m0); o.y = (a.y & ~m1) | (b.y & m1);
-                o.z = (a.z & ~m2) | (b.z & m2); o.w = (a.w & ~m3) | (b.w & m3);
-            }
-            if (live) {
-                ((uint4 *)(out + (size_t)j * sp.row_bytes))[g * GS + slot] = o;
-                // R10: both int16 halves of a word summed by one dp2a
-                acc = __dp2a_lo((int)o.x, 0x0101, acc); acc = __dp2a_lo((int)o.y, 0x0101, acc);
-                acc = __dp2a_lo((int)o.z, 0x0101, acc); acc = __dp2a_lo((int)o.w, 0x0101, acc);
-            }
+        if (NPASS == 1) {
+            rows(g0 ? nf : nm, na, nb);
+            pass(j, g0, a, b, acc);
+        } else {
+            uint4 fa, fb;
+            rows(pf, fa, fb);
+            pass(j, 0u, a, b, acc);
+            rows(nm, na, nb);
+            pass(j, 1u, fa, fb, acc);
         }
-#pragma unroll
-        for (uint32_t off = 16; off > 0; off >>= 1) {
-            const int v = __shfl_xor_sync(0xffffffffu, acc, off);
-            if (off < LPO) acc += v;
-        }
-        if (live && li == 0) sp.zi[j] = acc;
-        par0 = nx0; par1 = nx1;
+        acc = __reduce_add_sync(omask, acc);
+        if (j < M && li == 0) sp.zi[j] = acc;
+        pm = nm; pf = nf; nm = n2m; nf = n2f;
+    };
+    uint4 a0, b0, a1, b1;
+    rows((NPASS == 1 && g0) ? pf : pm, a0, b0);
+    for (uint32_t ob = ob0; ob < M; ob += stride) {     // two iterations per trip: the row registers ping-pong
+        iteration(ob, a0, b0, a1, b1);
+        ob += stride;
+        if (ob >= M) break;
+        iteration(ob, a1, b1, a0, b0);
+    }
+}
+
+// grid: as many CTAs as are resident at once (the loop strides over the offspring), never more than
+// the capacity needs
+template <uint32_t LL>
+inline cudaError_t launch_gamete_q10v_t(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
+    static int per_sm = 0;
+    if (per_sm == 0) {
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gamete_q10v<LL>, Q10V_THREADS, 0);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) per_sm = 1;
+    }
+    constexpr uint32_t opw = (LL >= 128u) ? 1u : 128u / LL;     // offspring per warp iteration
+    const uint64_t per_cta = (uint64_t)(Q10V_THREADS / 32) * opw;
+    const uint64_t need = ((uint64_t)k.capacity + per_cta - 1) / per_cta;
+    const uint32_t grid = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(need, (uint64_t)n_sms * per_sm));
+    k_gamete_q10v<LL><<<grid, Q10V_THREADS, 0, stream>>>(k);
+    return cudaGetLastError();
+}
+
+inline cudaError_t launch_gamete_q10v(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
+    switch (k.L) {
+    case 8: return launch_gamete_q10v_t<8>(k, n_sms, stream);
+    case 16: return launch_gamete_q10v_t<16>(k, n_sms, stream);
+    case 32: return launch_gamete_q10v_t<32>(k, n_sms, stream);
+    case 64: return launch_gamete_q10v_t<64>(k, n_sms, stream);
+    case 128: return launch_gamete_q10v_t<128>(k, n_sms, stream);
+    case 256: return launch_gamete_q10v_t<256>(k, n_sms, stream);
+    default: return cudaErrorInvalidValue;
     }
 }
 
@@ -1029,11 +1121,12 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
 // natal patch p are a contiguous j-range and land in p or one of its 4 torus neighbours, so the
 // stable order is: for destination d, the sources {d, neighbours(d)} in increasing patch index,
 // each in j order.  slot = index of the destination in p's de-duplicated list [p, nb0..nb3].
-__device__ __forceinline__ uint32_t dest_slot(uint32_t p, uint32_t dest, uint32_t gw, uint32_t gh) {
+__device__ __forceinline__ uint32_t dest_slot(uint32_t p, uint32_t dest, uint4 nb) {
     if (dest == p) return 0;
-#pragma unroll
-    for (uint32_t k = 0; k < 4; ++k)
-        if (neighbour(p, k, gw, gh) == dest) return k + 1;
+    if (nb.x == dest) return 1;
+    if (nb.y == dest) return 2;
+    if (nb.z == dest) return 3;
+    if (nb.w == dest) return 4;
     return 0;
 }
 
@@ -1054,65 +1147,49 @@ __global__ void __launch_bounds__(256) k_patch_count(const __grid_constant__ SpK
         __syncthreads();
         uint32_t j0, j1;
         patch_offspring_range(sp, ps, p, st.n0, st.m, j0, j1);
+        const uint4 nb = ((const uint4 *)sp.nbr)[p];
         for (uint32_t j = j0 + threadIdx.x; j < j1; j += blockDim.x)
-            if (sp.alive[j]) atomicAdd(&s_cnt[dest_slot(p, sp.dest[j], sp.grid_w, sp.grid_h)], 1u);
+            if (sp.alive[j]) atomicAdd(&s_cnt[dest_slot(p, sp.dest[j], nb)], 1u);
         __syncthreads();
         if (threadIdx.x < 5) sp.patch_cnt[p * 5 + threadIdx.x] = s_cnt[threadIdx.x];
         __syncthreads();
     }
 }
 
-// next patch_start and the base position of every (natal patch, slot) group; single CTA
+// next patch_start and the base position of every (natal patch, slot) group; single CTA: thread t owns
+// the destinations [t * per, t * per + per), whose sources (natal patch, slot) come sorted from the
+// host-built topology table; block scan over the threads' totals
 __global__ void __launch_bounds__(1024) k_patch_base(const __grid_constant__ SpK sp) {
-    __shared__ uint32_t s_part[1024];
+    __shared__ uint32_t s_warp[32];
     DevSpecies &st = *sp.st;
     uint32_t *psn = sp.patch_start[st.cur ^ 1u];
-    const uint32_t P = sp.P, gw = sp.grid_w, gh = sp.grid_h, tid = threadIdx.x;
+    const uint32_t P = sp.P, tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t per = (P + 1023) / 1024;
     const uint32_t d0 = min(tid * per, P), d1 = min(d0 + per, P);
-    // sources of destination d: (p', slot) pairs, unique per p', sorted by p'
-    auto sources = [&](uint32_t d, uint32_t (&sp_)[5], uint32_t (&ss_)[5]) -> int {
-        int n = 0;
-        sp_[n] = d; ss_[n] = 0; ++n;
-        for (uint32_t k = 0; k < 4; ++k) {
-            const uint32_t pp = neighbour(d, (k + 2) & 3u, gw, gh);  // opposite direction
-            if (pp == d) continue;  // d is its own neighbour: counted in slot 0
-            if (neighbour(pp, k, gw, gh) != d) continue;
-            const uint32_t slot = dest_slot(pp, d, gw, gh);
-            bool dup = false;
-            for (int i = 0; i < n; ++i) dup |= (sp_[i] == pp);
-            if (!dup) { sp_[n] = pp; ss_[n] = slot; ++n; }
-        }
-        for (int i = 1; i < n; ++i)
-            for (int k2 = i; k2 > 0 && sp_[k2] < sp_[k2 - 1]; --k2) {
-                uint32_t t = sp_[k2]; sp_[k2] = sp_[k2 - 1]; sp_[k2 - 1] = t;
-                t = ss_[k2]; ss_[k2] = ss_[k2 - 1]; ss_[k2 - 1] = t;
-            }
-        return n;
-    };
     uint32_t mine = 0;
     for (uint32_t d = d0; d < d1; ++d) {
-        uint32_t a[5], b[5];
-        const int n = sources(d, a, b);
-        for (int i = 0; i < n; ++i) mine += sp.patch_cnt[a[i] * 5 + b[i]];
+        const uint32_t *sl = sp.src_list + (size_t)d * 6;
+        const uint32_t n = sl[0];
+        for (uint32_t i = 0; i < n; ++i) { const uint32_t e = sl[1 + i]; mine += sp.patch_cnt[(e >> 3) * 5 + (e & 7u)]; }
     }
-    s_part[tid] = mine;
+    const uint32_t incl = warp_incl_scan(mine);
+    if (lane == 31) s_warp[warp] = incl;
     __syncthreads();
-    if (tid == 0) {
-        uint32_t run = 0;
-        for (int i = 0; i < 1024; ++i) { const uint32_t t = s_part[i]; s_part[i] = run; run += t; }
-        st.n_next = run;
-        psn[P] = run;
+    if (warp == 0) {
+        const uint32_t w = s_warp[lane], wi = warp_incl_scan(w);
+        s_warp[lane] = wi - w;
+        if (lane == 31) { st.n_next = wi; psn[P] = wi; }
     }
     __syncthreads();
-    uint32_t run = s_part[tid];
+    uint32_t run = s_warp[warp] + (incl - mine);
     for (uint32_t d = d0; d < d1; ++d) {
         psn[d] = run;
-        uint32_t a[5], b[5];
-        const int n = sources(d, a, b);
-        for (int i = 0; i < n; ++i) {
-            sp.patch_base[a[i] * 5 + b[i]] = run;
-            run += sp.patch_cnt[a[i] * 5 + b[i]];
+        const uint32_t *sl = sp.src_list + (size_t)d * 6;
+        const uint32_t n = sl[0];
+        for (uint32_t i = 0; i < n; ++i) {
+            const uint32_t e = sl[1 + i], k = (e >> 3) * 5 + (e & 7u);
+            sp.patch_base[k] = run;
+            run += sp.patch_cnt[k];
         }
     }
 }
@@ -1129,11 +1206,12 @@ __global__ void __launch_bounds__(256) k_patch_pos(const __grid_constant__ SpK s
         if (tid < 5) s_run[tid] = sp.patch_base[p * 5 + tid];
         uint32_t j0, j1;
         patch_offspring_range(sp, ps, p, st.n0, st.m, j0, j1);
+        const uint4 nb = ((const uint4 *)sp.nbr)[p];
         __syncthreads();
         for (uint32_t c0 = j0; c0 < j1; c0 += 256) {
             const uint32_t j = c0 + tid;
             const bool al = j < j1 && sp.alive[j];
-            const uint32_t slot = al ? dest_slot(p, sp.dest[j], sp.grid_w, sp.grid_h) : 7u;
+            const uint32_t slot = al ? dest_slot(p, sp.dest[j], nb) : 7u;
             uint32_t rank = 0;
 #pragma unroll
             for (uint32_t k = 0; k < 5; ++k) {

@@ -449,3 +449,77 @@ def test_overlapping_generations_order_selection_and_regulation(oracle_mod):
     o.step(1)
     e = o.log(0)[0]
     assert e["m_t"] == 2048 - 1500 and e["flags"] & 1 and e["n_next"] <= 2048
+
+
+def test_overlapping_generations_in_patches(oracle_mod):
+    """R18 in patch mode (PAPER.md:126 patches; PAPER.md:56,170 overlapping generations -- case study
+    1 is exactly this combination): an adult that stays keeps its patch and its row; patch p of the
+    next generation holds its staying adults (order i) followed by the surviving offspring whose
+    destination is p (order j); the adult's survival uses ITS patch's optimum; each unlinked patch
+    settles at its own balance N*_p = K_p (R0 / (1 - s_A) - 1); and the paper's lifespan pin holds
+    patch by patch."""
+    sA, om = 0.6, 1.0
+    sp = species(L=16, kind="q10", r=0.5, mu=0.0, fec_a=2.0, K=500.0, K_patch=[300.0, 500.0, 800.0, 500.0], omega=om,
+                 theta_patch=[-0.3, 0.0, 0.3, 0.6], migration=0.3, capacity=16384)
+    sp["adult_survival"] = sA
+    c = cfg(sp, seed=12, grid=(2, 2))
+    c["n0"] = [2000]
+    c["init_sd"] = 0.1
+    o = oracle_mod.Oracle(c)
+    rows0 = workloads.initial_rows(c, 0)
+    ps0 = np.array([0, 400, 1000, 1500, 2000], np.uint32)
+    o.write_state(0, rows0, ps0, 0)
+    o.step(1)
+    d = o.debug(0)
+    rows1, ps1, _ = o.read_state(0)
+    stay, alive = d["a_alive"].astype(bool), d["alive"].astype(bool)
+    pat0 = np.searchsorted(ps0, np.arange(2000), side="right") - 1
+    k = 0
+    for p in range(4):
+        a = np.where(stay & (pat0 == p))[0]
+        j = np.where(alive & (d["dest"] == p))[0]
+        assert ps1[p] == k
+        assert np.array_equal(rows1[k:k + len(a)], rows0[a])
+        k += len(a)
+        assert np.array_equal(rows1[k:k + len(j)], d["offspring"][j])
+        k += len(j)
+    assert ps1[4] == k == o.log(0)[0]["n_next"]
+    z = rows0.astype(np.int64).sum(axis=1) * 2.0 ** -11
+    th = np.array([-0.3, 0.0, 0.3, 0.6], np.float32)[pat0]
+    assert np.allclose(d["a_s"], sA * np.exp(-(z - th) ** 2 / (2 * om * om)), rtol=2e-6)
+    assert np.array_equal(stay, d["a_u"] < d["a_s"])
+    # unlinked patches, no selection: per-patch balance of births and deaths
+    sp2 = species(L=16, kind="q10", r=0.5, mu=0.0, fec_a=2.0, K=500.0, K_patch=[300.0, 500.0, 800.0, 500.0], omega=0.0,
+                  migration=0.0, capacity=32768)
+    sp2["adult_survival"] = 0.5
+    c2 = cfg(sp2, seed=13, grid=(2, 2))
+    c2["n0"] = [2000]
+    c2["init_sd"] = 0.1
+    o = oracle_mod.Oracle(c2)
+    o.write_state(0, workloads.initial_rows(c2, 0), np.array([0, 500, 1000, 1500, 2000], np.uint32), 0)
+    acc = np.zeros(4)
+    for t in range(160):
+        o.step(1)
+        if t >= 60:
+            acc += np.diff(o.read_state(0)[1])
+    for p, K in enumerate([300.0, 500.0, 800.0, 500.0]):
+        assert abs(acc[p] / 100 / (K * (2.0 / 0.5 - 1.0)) - 1) < 0.05
+    # the paper's lifespan (0.975 -> 40 steps, PAPER.md:170) in every patch of a non-reproducing cohort
+    sp3 = species(L=16, kind="q10", r=0.5, mu=0.0, fec_a=0.0, K=1e9, omega=0.0, migration=0.5, capacity=8192)
+    sp3["adult_survival"] = 0.975
+    c3 = cfg(sp3, seed=14, grid=(2, 1))
+    c3["n0"] = [4000]
+    c3["init_sd"] = 0.1
+    o = oracle_mod.Oracle(c3)
+    o.write_state(0, workloads.initial_rows(c3, 0), np.array([0, 1500, 4000], np.uint32), 0)
+    tot = np.zeros(2)
+    prev = np.array([1500, 2500])
+    for t in range(700):
+        tot += prev
+        o.step(1)
+        now = np.diff(o.read_state(0)[1])
+        assert (now <= prev).all()                       # nobody is born, adults do not move
+        prev = now
+    assert prev.sum() == 0
+    for p, n in enumerate([1500, 2500]):
+        assert abs(tot[p] / n - 40.0) < 5 * math.sqrt(0.975) / 0.025 / math.sqrt(n)
