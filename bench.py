@@ -98,6 +98,7 @@ VARIANTS = {
     "sexes": {"separate_sexes": 1},                    # R21 (fecundity parameter x 2: half the adults lay eggs)
     "encounters": {},                                  # R20 (configuration 4 only: 3 meetings, attack 0.1)
     "cost": {"fec_cost": 0.05},                        # R22
+    "mothers": {"mother_skew": 1.0},                   # R24
 }
 
 
@@ -115,12 +116,15 @@ def apply_variant(cfg, variant):
     return cfg
 
 
+SWEEP = {"patches": 16, "per_patch": 50_000}   # --patches / --per-patch (configuration 6)
+
+
 def workload(which, seed_offset=0, world=1, variant="none"):
     """Rank `seed_offset`'s workload.  Configs 1-5: an independent replica (own seed).  Config 6 (the
-    sweep of unlinked patches): the rank's block of 16 patches out of a 16 x world sweep."""
+    sweep of unlinked patches): the rank's block of --patches patches out of a patches x world sweep."""
     from paper_1603_09255_b200 import replicas, workloads
     if which == 6:
-        return replicas.sweep_shard(16 * world, seed_offset, world)
+        return apply_variant(replicas.sweep_shard(SWEEP["patches"] * world, seed_offset, world, per_patch=SWEEP["per_patch"]), variant)
     return apply_variant(replicas.replica_config(workloads.config(which), seed_offset), variant)
 
 
@@ -472,11 +476,14 @@ def main():
                     help="a widening of SURVEY.md 8(f) on top of --config (context lines; the metric is --variant none)")
     ap.add_argument("--clock-warm-steps", type=int, default=300,
                     help="untimed steps before the W warm-up steps (the initial state is written again after them)")
+    ap.add_argument("--patches", type=int, default=16, help="configuration 6: patches per rank (PAPER.md:64 runs 1-100)")
+    ap.add_argument("--per-patch", type=int, default=50_000, help="configuration 6: individuals per patch at the start")
     ap.add_argument("--no-others", dest="others", action="store_false",
                     help="skip the short timed passes of configurations 1, 2, 4, 5 (config.other_workloads)")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
                     help="--impl reference: CPU seconds the K+W oracle steps are sized for")
     args = ap.parse_args()
+    SWEEP.update(patches=args.patches, per_patch=args.per_patch)
     if args.warmup < 3:
         args.warmup = 3
     if args.impl == "reference":

@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SPEGG_ABI_VERSION 7u
+#define SPEGG_ABI_VERSION 8u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
        SPEGG_ESTATE = -5 };
@@ -88,9 +88,11 @@ typedef struct spegg_species_params {
                                    reproducing, an adult stays alive with probability
                                    s_A * w(z) (w: the Gaussian term at its genetic value; the
                                    paper's maximum survivorship is 0.975 = a lifespan of 40
-                                   steps); the next generation is the staying adults, in order,
-                                   then the surviving offspring, and M_t <= capacity - N_t.
-                                   0 = discrete generations.  Unstructured species (1x1) only */
+                                   steps); in every patch the next generation is its staying
+                                   adults, in order (an adult keeps its patch; its survival uses
+                                   that patch's optimum), then the surviving offspring that
+                                   land there, and M_t <= capacity - N_t.
+                                   0 = discrete generations                                  */
     double mate_skew;           /* v_m: shared-preference mating (eq. S2-10,
                                    PAPER.md:281-283): the father of each egg is drawn, among
                                    the adults of the mother's patch, with probability
@@ -121,6 +123,13 @@ typedef struct spegg_species_params {
                                    exp(-a (z_c - z_m)^2) (genetic values); up to 8 candidates,
                                    the last one is taken if none was accepted.  0 = random
                                    mating (R2).  Not together with mate_skew / separate_sexes    */
+    double mother_skew;         /* v_f: mothers drawn by relative fecundity (eq. S2-9, PAPER.md:273-275;
+                                   R24): the mother of each egg is drawn, among the (female) adults
+                                   of the patch that laid it, with probability proportional to
+                                   Y_i^{v_f}, Y_i = exp(z_i), by integer running sum + search as the
+                                   father of R19; the NUMBER of eggs of a patch stays the sum of its
+                                   adults' Poisson fecundities.  0 = every adult mothers its own eggs.
+                                   |v_f| <= 1e6; not with fec_cost or SPEGG_FEC_CAPTURES          */
 } spegg_species_params;
 
 typedef struct spegg_params {
@@ -165,6 +174,8 @@ typedef struct spegg_debug_view {
                                    (mate_skew != 0, R19)                                      */
     float zbar_self;            /* the weights' reference: mean genetic value of the adults   */
     const uint8_t *d_sex_off;   /* [m_t] sex of each offspring, 1 = male (separate_sexes, R21) */
+    const uint64_t *d_mom_cum;  /* [n_t] inclusive running sum of the integer mothering weights
+                                   (mother_skew != 0, R24)                                    */
 } spegg_debug_view;
 
 typedef struct spegg_sim spegg_sim;

@@ -18,7 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ERANGE, ESTATE = 0, -1, -2, -3, -4, -5
 FLAG_OVERFLOW, FLAG_EXTINCT = 1, 2
 
 
-ABI_VERSION = 7   # SPEGG_ABI_VERSION of include/spegg.h
+ABI_VERSION = 8   # SPEGG_ABI_VERSION of include/spegg.h
 
 
 class SpeciesParams(C.Structure):
@@ -34,7 +34,7 @@ class SpeciesParams(C.Structure):
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
         ("mate_skew", C.c_double), ("encounters", C.c_uint32), ("separate_sexes", C.c_uint32),
-        ("fec_cost", C.c_double), ("assort", C.c_double),
+        ("fec_cost", C.c_double), ("assort", C.c_double), ("mother_skew", C.c_double),
     ]
 
 
@@ -60,7 +60,7 @@ class DebugView(C.Structure):
         ("d_table_len", C.c_void_p), ("n_tables", C.c_uint32), ("theta_t", C.c_float),
         ("zbar_pred", C.c_float), ("attack_n", C.c_float), ("d_cap", C.c_void_p),
         ("d_a_alive", C.c_void_p), ("d_a_u", C.c_void_p), ("d_a_s", C.c_void_p),
-        ("d_mate_cum", C.c_void_p), ("zbar_self", C.c_float), ("d_sex_off", C.c_void_p),
+        ("d_mate_cum", C.c_void_p), ("zbar_self", C.c_float), ("d_sex_off", C.c_void_p), ("d_mom_cum", C.c_void_p),
     ]
 
 
@@ -153,6 +153,7 @@ def make_params(cfg, debug=False, log_capacity=0):
         p.separate_sexes = 1 if sp.get("separate_sexes") else 0
         p.fec_cost = sp.get("fec_cost", 0.0)
         p.assort = sp.get("assort", 0.0)
+        p.mother_skew = sp.get("mother_skew", 0.0)
         p.fecundity_model, p.fec_a, p.K = _FEC[sp["fecundity"]], sp["fec_a"], sp["K"]
         if sp.get("K_patch") is not None:
             kp = np.ascontiguousarray(sp["K_patch"], dtype=np.float64)
@@ -347,5 +348,7 @@ class Sim:
                              or self.cfg["species"][species].get("separate_sexes")) else np.zeros(0, np.uint64)),
             "sex_off": (arr(v.d_sex_off, m, np.uint8) if self.cfg["species"][species].get("separate_sexes")
                         else np.zeros(m, np.uint8)),
+            "mom_cum": (arr(v.d_mom_cum, n, np.uint64) if self.cfg["species"][species].get("mother_skew", 0.0) != 0.0
+                        else np.zeros(0, np.uint64)),
         }
         return d

@@ -141,10 +141,10 @@ struct Carver {
 };
 
 struct SpeciesLayout {
-    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, alive, captured, a_alive, a_u, a_s, a_zi, a_pos, mate_cum, mate_tile, enc_zi, sex[2], sex_off,
-        cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, log;
+    uint64_t pop[2], patch_start[2], rowptr[2], chunk_mask[2], range_cnt[2], f, off, mother, father, dest, pos, u01, s, offbuf, zi, zrow[2], alive, captured, a_alive, a_u, a_s, a_zi, a_pos, a_rank, mate_cum, mate_tile, mom_cum, mom_tile, enc_zi, sex[2], sex_off,
+        cap, tables, table_len, status_fec, status_cmp, patch_cnt, patch_base, patch_abase, log;
     uint64_t T_recomb, T_xover, xover_len, chrom_start, chrom_len, T_mut, T_norm, T_env, K_patch, theta_patch, nbr, src_list;
-    uint32_t norm_len, env_len, n_tables, row_bytes;
+    uint32_t norm_len, env_len, n_tables, row_bytes, zrow_on;
 };
 
 struct HostSpecies {
@@ -193,12 +193,13 @@ int validate(const spegg_params *p) {
         if (q.genome_kind == SPEGG_Q10 && !(q.mut_sd > 0.0 && q.mut_sd * 1024.0 * 8.0 < 32000.0)) return SPEGG_EINVAL;
         if (!(q.K > 0.0) || !(q.fec_a >= 0.0)) return SPEGG_EINVAL;
         if (q.capacity == 0 || q.capacity >= (1ull << 31)) return SPEGG_EINVAL;
-        if (!(q.adult_survival >= 0.0 && q.adult_survival <= 1.0) || (q.adult_survival > 0.0 && P != 1)) return SPEGG_EINVAL;
+        if (!(q.adult_survival >= 0.0 && q.adult_survival <= 1.0)) return SPEGG_EINVAL;
         if (!(q.resid_sd >= 0.0) || !(q.pheno_scale > 0.0f) || q.resid_sd / (double)q.pheno_scale > 4096.0) return SPEGG_EINVAL;
         if (!(std::fabs(q.mate_skew) <= 1e6) || q.separate_sexes > 1) return SPEGG_EINVAL;
         if (!(q.fec_cost >= 0.0 && q.fec_cost <= 1e6)) return SPEGG_EINVAL;
         if (!(q.assort >= 0.0 && q.assort <= 1e6) || (q.assort > 0.0 && (q.mate_skew != 0.0 || q.separate_sexes))) return SPEGG_EINVAL;
         if (q.fecundity_model == SPEGG_FEC_CAPTURES && P != 1) return SPEGG_EINVAL;
+        if (!(std::fabs(q.mother_skew) <= 1e6) || (q.mother_skew != 0.0 && (q.fec_cost > 0.0 || q.fecundity_model == SPEGG_FEC_CAPTURES))) return SPEGG_EINVAL;
         if (q.sel_predation) {
             if (q.predator_species >= p->n_species || q.predator_species <= s) return SPEGG_EINVAL;
             if (p->species[q.predator_species].fecundity_model != SPEGG_FEC_CAPTURES) return SPEGG_EINVAL;
@@ -207,6 +208,13 @@ int validate(const spegg_params *p) {
         } else if (q.encounters) return SPEGG_EINVAL;
     }
     return SPEGG_OK;
+}
+
+// segments per patch of the patch-mode compaction: about 2,048 rows of capacity each, at most 64
+uint32_t patch_sub_of(uint64_t capacity, uint64_t P) {
+    if (P <= 1) return 1;
+    const uint64_t s = (capacity + P * 2048 - 1) / (P * 2048);
+    return (uint32_t)std::min<uint64_t>(std::max<uint64_t>(s, 1), 64);
 }
 
 uint32_t row_bytes_of(const spegg_species_params &q) {
@@ -247,14 +255,26 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.u01 = c.take(cap * 4);
         l.s = c.take(cap * 4);
         l.zi = c.take(cap * 4);
+        {
+            bool met = false;
+            for (uint32_t o = 0; o < p->n_species; ++o)
+                if (p->species[o].sel_predation && p->species[o].encounters && p->species[o].predator_species == s) met = true;
+            const bool zr = met || q.mate_skew != 0.0 || q.separate_sexes || q.mother_skew != 0.0 || q.fec_cost > 0.0 || q.assort > 0.0 || q.adult_survival > 0.0;
+            l.zrow[0] = c.take((zr ? cap32 : 1) * 4);
+            l.zrow[1] = c.take((zr ? cap32 : 1) * 4);
+            l.zrow_on = zr ? 1u : 0u;
+        }
         l.alive = c.take(cap);
         l.captured = c.take(cap);
         const uint64_t acap = q.adult_survival > 0.0 ? cap : 1;   // R18 arrays only when generations overlap
         l.a_alive = c.take(acap); l.a_u = c.take(acap * 4); l.a_s = c.take(acap * 4);
-        l.a_zi = c.take(acap * 4); l.a_pos = c.take(acap * 4);
+        l.a_zi = c.take(acap * 4); l.a_pos = c.take(acap * 4); l.a_rank = c.take((P > 1 ? acap : 1) * 4);
         const bool mate_on = q.mate_skew != 0.0 || q.separate_sexes;
         l.mate_cum = c.take((mate_on ? cap : 1) * 8);      // R19 arrays only with weighted mating / separate sexes
         l.mate_tile = c.take((mate_on ? cap / MATE_TILE + 2 : 1) * 8);
+        const bool mom_on = q.mother_skew != 0.0;            // R24
+        l.mom_cum = c.take((mom_on ? cap : 1) * 8);
+        l.mom_tile = c.take((mom_on ? cap / MATE_TILE + 2 : 1) * 8);
         const uint64_t scap = q.separate_sexes ? cap32 : 1;         // R21
         l.sex[0] = c.take(scap); l.sex[1] = c.take(scap); l.sex_off = c.take(scap);
         bool is_met = false;   // R20: some species meets this one individually
@@ -267,8 +287,10 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.table_len = c.take((uint64_t)l.n_tables * 4);
         l.status_fec = c.take((cap / SCAN_THREADS + 2 + (cap / SCAN_THREADS + 2) / 32 + 2) * 8);
         l.status_cmp = c.take((cap / SCAN_TILE + 2 + (cap / SCAN_TILE + 2) / 32 + 2) * 8);
-        l.patch_cnt = c.take(P * 5 * 4);
-        l.patch_base = c.take(P * 5 * 4);
+        const uint64_t PS = P * patch_sub_of(cap, P);
+        l.patch_cnt = c.take(PS * 6 * 4);
+        l.patch_base = c.take(PS * 6 * 4);
+        l.patch_abase = c.take(PS * 4);
         l.log = c.take((uint64_t)logcap * sizeof(LogEntry));
         l.T_recomb = c.take((uint64_t)q.n_loci * 4);
         l.T_xover = c.take((uint64_t)q.n_chrom * XMAX * 4);
@@ -339,7 +361,7 @@ int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
 
 // true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
 bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
-    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.mate_on || h.k.fec_cost != 0.0f || h.k.assort != 0.0f) return false;
+    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.sexes || h.k.fec_cost != 0.0f || h.k.assort != 0.0f || h.k.mom_v != 0.0f) return false;   // (mate_on without sexes = R19: the MATE instantiation)
     // k_fused_bit_f<4, 8> places chromosome c at words 8c .. 8c+7 and packs crossover positions in 9 bits:
     // four chromosomes of exactly 256 loci (other splits of 1,024 loci run the general pipeline)
     for (uint32_t c = 0; c < h.p.n_chrom; ++c)
@@ -360,6 +382,10 @@ void launch_prepare(spegg_sim *s) {
     k_prepare_all<<<dim3(std::min(blocks, 4 * s->n_sms), s->p.n_species), 256, 0, s->stream>>>(s->d_spk);
 }
 
+uint32_t ctas_of(uint64_t items, uint64_t per_cta, uint32_t per_sm, uint32_t n_sms) {
+    return (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>((items + per_cta - 1) / per_cta, (uint64_t)n_sms * per_sm));
+}
+
 // Enqueue the kernels of one step on the stream (captured into the graph, or launched directly
 // when kernel timing is on).  Returns the number of kernel launches through *n_launch.
 int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
@@ -372,6 +398,10 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
         const bool time_this = timed && si == 0 && s->ev_used + 2 <= s->ev.size();
         if (fused_ok(s, h)) {
             CU(launch_scan_fused(k, G, s->scan_ctas, s->stream)); ++nl;
+            if (k.mate_on) {   // R19 on the fused path: the weights need this step's rowptr[] (the scan's) and last step's zrow[]
+                k_mate_weight<<<ctas_of(k.capacity, 8, 8, G), 256, 0, s->stream>>>(k); ++nl;
+                k_mate_scan<<<ctas_of(k.capacity, MATE_TILE, 8, G), 256, 0, s->stream>>>(k, 0); ++nl;
+            }
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             CU(launch_fused_bit(k, G, s->stream)); ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
@@ -384,12 +414,13 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             };
             const uint32_t g_thread = ctas(cap, 256, 8), g_warp = ctas(cap, 8, 8);   // thread / warp per offspring
             if (k.fec_cost > 0.0f || k.assort > 0.0f) { k_enc_zi<<<ctas(cap, 8, 8), 256, 0, s->stream>>>(k); ++nl; }   // R22, R23: the adults' genetic values
-            k_fec_scan<<<ctas(cap, SCAN_THREADS, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
-            if (k.mate_on) {   // R19: mating weights of the adults and their running sum
+            if (k.mate_on || k.mom_v != 0.0f) {   // R19 / R24: mating and mothering weights of the adults and their running sums
                 k_mate_weight<<<g_warp, 256, 0, s->stream>>>(k); ++nl;
-                k_mate_scan<<<ctas(cap, MATE_TILE, 8), 256, 0, s->stream>>>(k); ++nl;
+                if (k.mate_on) { k_mate_scan<<<ctas(cap, MATE_TILE, 8), 256, 0, s->stream>>>(k, 0); ++nl; }
+                if (k.mom_v != 0.0f) { k_mate_scan<<<ctas(cap, MATE_TILE, 8), 256, 0, s->stream>>>(k, 1); ++nl; }
             }
-            k_scalar<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
+            // a1-a3 in one kernel: fecundity, scan, mothers, and the scalar draws of every range's offspring
+            k_fec_scan<<<ctas(cap, SCAN_THREADS, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
             if (time_this) CU(cudaEventRecord(s->ev[s->ev_used], s->stream));
             // production q10 path: vectorised gamete kernel that also takes the phenotype (debug keeps
             // the plain kernels, so the two can be compared with each other and with the oracle)
@@ -399,22 +430,30 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             else k_gamete_q10<<<ctas(cap * 2, 8, 8), 256, 0, s->stream>>>(k);
             ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
-            k_mutate<<<ctas(cap * 2, 256, 8), 256, 0, s->stream>>>(k, q10v ? 1 : 0); ++nl;
-            if (!q10v) { k_phenotype<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }
             if (k.enc_E) {   // R20: genetic values of the consumers this species' newborns meet
                 const SpK &kp = s->sp[h.p.predator_species].k;
                 k_enc_zi<<<ctas(kp.capacity, 8, 8), 256, 0, s->stream>>>(kp); ++nl;
             }
-            k_survival<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
-            if (k.adult_surv > 0.0f) { k_adult_survive<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }   // R18
-            if (s->P == 1) {
-                k_cmp_scan<<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
+            if (q10v && s->P == 1 && k.adult_surv == 0.0f) {
+                // mutation, selection, compaction and its index in one kernel (the last CTA closes a solo step)
+                k_select_compact<<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
             } else {
-                k_patch_count<<<std::min(s->P, G * 8), 256, 0, s->stream>>>(k); ++nl;
-                k_patch_base<<<1, 1024, 0, s->stream>>>(k); ++nl;
-                k_patch_pos<<<std::min(s->P, G * 8), 256, 0, s->stream>>>(k); ++nl;
+                if (q10v) { k_mut_surv<<<g_thread, 256, 0, s->stream>>>(k); ++nl; }
+                else {
+                    k_mutate<<<ctas(cap * 2, 256, 8), 256, 0, s->stream>>>(k, 0); ++nl;
+                    k_phenotype<<<g_warp, 256, 0, s->stream>>>(k); ++nl;
+                    k_survival<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
+                }
+                if (k.adult_surv > 0.0f) { k_adult_survive<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }   // R18
+                if (s->P == 1) {
+                    k_cmp_scan<<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
+                } else {
+                    k_patch_count<<<std::min(s->P * k.patch_sub, G * 8), 256, 0, s->stream>>>(k); ++nl;
+                    k_patch_base<<<1, 1024, 0, s->stream>>>(k); ++nl;
+                    k_patch_pos<<<std::min(s->P * k.patch_sub, G * 8), 256, 0, s->stream>>>(k); ++nl;
+                }
+                k_cmp_scatter<<<(k.index_only && k.adult_surv == 0.0f) ? g_thread : g_warp, 256, 0, s->stream>>>(k); ++nl;
             }
-            k_cmp_scatter<<<(k.index_only && k.adult_surv == 0.0f) ? g_thread : g_warp, 256, 0, s->stream>>>(k); ++nl;
         }
     }
     const bool solo = s->sp.size() == 1 && s->sp[0].k.solo;  // the last kernel closes the step itself
@@ -583,14 +622,17 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.dest = at<uint32_t>(s, l.dest); k.pos = at<uint32_t>(s, l.pos);
         k.u01 = at<float>(s, l.u01); k.s = at<float>(s, l.s);
         k.offbuf = at<uint8_t>(s, l.offbuf); k.zi = at<int32_t>(s, l.zi);
+        k.zrow[0] = at<int32_t>(s, l.zrow[0]); k.zrow[1] = at<int32_t>(s, l.zrow[1]); k.zrow_on = l.zrow_on;
         k.alive = at<uint8_t>(s, l.alive); k.captured = at<uint8_t>(s, l.captured);
         k.adult_surv = (float)q.adult_survival;
         k.a_alive = at<uint8_t>(s, l.a_alive); k.a_u = at<float>(s, l.a_u); k.a_s = at<float>(s, l.a_s);
-        k.a_zi = at<int32_t>(s, l.a_zi); k.a_pos = at<uint32_t>(s, l.a_pos);
+        k.a_zi = at<int32_t>(s, l.a_zi); k.a_pos = at<uint32_t>(s, l.a_pos); k.a_rank = at<uint32_t>(s, l.a_rank);
         k.mate_v = (float)q.mate_skew;
         k.sexes = q.separate_sexes; k.mate_on = (q.mate_skew != 0.0 || q.separate_sexes) ? 1u : 0u;
         k.sex[0] = at<uint8_t>(s, l.sex[0]); k.sex[1] = at<uint8_t>(s, l.sex[1]); k.sex_off = at<uint8_t>(s, l.sex_off);
         k.mate_cum = at<unsigned long long>(s, l.mate_cum); k.mate_tile = at<unsigned long long>(s, l.mate_tile);
+        k.mom_v = (float)q.mother_skew;
+        k.mom_cum = at<unsigned long long>(s, l.mom_cum); k.mom_tile = at<unsigned long long>(s, l.mom_tile);
         k.fec_cost = (float)q.fec_cost; k.assort = (float)q.assort;
         k.enc_E = q.sel_predation ? q.encounters : 0u; k.enc_v = (float)q.attack;
         k.enc_zi = at<int32_t>(s, l.enc_zi);
@@ -598,8 +640,9 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.tables = at<uint32_t>(s, l.tables); k.table_len = at<uint32_t>(s, l.table_len);
         k.status_fec = at<unsigned long long>(s, l.status_fec); k.status_cmp = at<unsigned long long>(s, l.status_cmp);
         k.status_fec_n = (uint32_t)(q.capacity / SCAN_THREADS + 2); k.status_cmp_n = (uint32_t)(q.capacity / SCAN_TILE + 2);
-        k.patch_cnt = at<uint32_t>(s, l.patch_cnt); k.patch_base = at<uint32_t>(s, l.patch_base);
+        k.patch_cnt = at<uint32_t>(s, l.patch_cnt); k.patch_base = at<uint32_t>(s, l.patch_base); k.patch_abase = at<uint32_t>(s, l.patch_abase);
         k.nbr = at<uint32_t>(s, l.nbr); k.src_list = at<uint32_t>(s, l.src_list);
+        k.patch_sub = patch_sub_of(q.capacity, s->P);
         k.st = s->d_st + si; k.st_all = s->d_st; k.glob = s->d_glob;
         k.log = at<LogEntry>(s, l.log); k.log_capacity = s->log_capacity;
         k.debug = p->debug;
@@ -827,6 +870,7 @@ int spegg_read_debug(spegg_sim *s, uint32_t species, spegg_debug_view *o) {
     o->d_a_alive = k.a_alive; o->d_a_u = k.a_u; o->d_a_s = k.a_s;
     o->d_mate_cum = (const uint64_t *)k.mate_cum; o->zbar_self = st.zbar_self;
     o->d_sex_off = k.sex_off;
+    o->d_mom_cum = (const uint64_t *)k.mom_cum;
     return SPEGG_OK;
 }
 

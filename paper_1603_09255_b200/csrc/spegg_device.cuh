@@ -10,7 +10,7 @@
 
 namespace spegg {
 
-enum Stream : uint32_t { ST_FEC = 0, ST_SCALAR = 1, ST_RECOMB_M = 2, ST_RECOMB_P = 3, ST_MUT_M = 4, ST_MUT_P = 5, ST_MATE = 6 };
+enum Stream : uint32_t { ST_FEC = 0, ST_SCALAR = 1, ST_RECOMB_M = 2, ST_RECOMB_P = 3, ST_MUT_M = 4, ST_MUT_P = 5, ST_MATE = 6, ST_MOTHER = 7 };
 
 // ---------------------------------------------------------------------------------- Philox
 // Salmon et al. SC'11. One round: two 32x32->64 products, two 3-input XORs; key += Weyl.
@@ -123,6 +123,22 @@ __device__ __forceinline__ int normal_delta(const uint32_t *__restrict__ T, int 
         if (u >= T[mid]) lo = mid + 1; else hi = mid;
     }
     return lo - R;
+}
+
+// ----------------------------------------------------------- asynchronous copies into shared memory
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
 }
 
 // ------------------------------------------------------------ decoupled look-back (one warp)

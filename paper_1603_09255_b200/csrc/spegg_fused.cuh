@@ -33,20 +33,6 @@ __device__ __forceinline__ uint32_t shl_clamp(uint32_t v, uint32_t n) {
     return r;
 }
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-
-__device__ __forceinline__ uint4 lds128(uint32_t addr) {
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
-    return v;
-}
-
 // ones from bit s upward within word w of a 256-bit chromosome: (~0 << clamp(s - 32w, 0, 32))
 __device__ __forceinline__ uint32_t mask_from(int s, int w) {
     return shl_clamp(0xFFFFFFFFu, (uint32_t)__viaddmax_s32(s, -32 * w, 0));
@@ -86,10 +72,7 @@ constexpr int SCANF_CHUNKS = SCANF_RANGE / FUSED_CHUNK;
 //   (e) lane = offspring: phenotype -> fp32 survival -> decision; the ballot is the chunk's mask.
 constexpr int FUSEDF_WARPS = 4;
 constexpr int FUSEDF_UNROLL_C = 2;                // decode passes in flight per lane
-#ifndef SPEGG_FUSEDF_CTAS
-#define SPEGG_FUSEDF_CTAS 5
-#endif
-constexpr int FUSEDF_CTAS = SPEGG_FUSEDF_CTAS;    // resident CTAs per SM (shared memory and registers allow 5)
+constexpr int FUSEDF_CTAS = 5;                    // resident CTAs per SM (shared memory and registers allow 5; 4 x 122 registers measured slower)
 constexpr int FUSEDF_AHEAD = 1;                   // passes the mothers' loads run ahead
 constexpr uint32_t FUSEDF_SP_OFF = FUSED_CHUNK * FUSED_ROW;        // packed draws [8][4][4][2] / partial sums
 constexpr uint32_t FUSEDF_Q_OFF = FUSEDF_SP_OFF + 8 * 32 * 4;      // queue of chromosomes with > 2 crossovers: draw [32], (pass, lane) [32]
@@ -103,12 +86,13 @@ __device__ __forceinline__ uint4 ldg128(const void *p) {
     return v;
 }
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-// ticket counter: written as PTX so that nvcc does not turn it into its warp-aggregated form, whose
-// broadcast shuffle waits for the atomic's round trip on the spot; the result is consumed a chunk later
-__device__ __forceinline__ uint32_t atom_inc_u32(uint32_t *p) {
-    uint32_t r;
-    asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(r) : "l"(p));
-    return r;
+// ticket counter: a 64-bit atomic, because ptxas turns a 32-bit atom.add (and atom.inc) into its
+// warp-aggregated form (vote, leader's atomic, broadcast shuffle) even for a single active lane, and
+// that shuffle waits for the atomic's round trip on the spot; the ticket is consumed a chunk later
+__device__ __forceinline__ uint32_t atom_inc_ticket(unsigned long long *p, uint32_t one) {
+    unsigned long long r;
+    asm volatile("atom.global.add.u64 %0, [%1], %2;" : "=l"(r) : "l"(p), "l"((unsigned long long)one));
+    return (uint32_t)r;
 }
 
 // packed draw of one (gamete, chromosome): s0 | s1 << 9 | phase << 31; positions 1..255,
@@ -133,11 +117,16 @@ __device__ __forceinline__ uint32_t xover_count_from3(const uint32_t *__restrict
     return k;
 }
 
-template <int NC, int WPC>
+// MATE: the father comes from the running sum of the mating weights (R19, hermaphrodites) instead of the
+// uniform draw: one more SCALAR block and a binary search over mate_cum[] in the scalar stage, and the
+// offspring's integer genetic value is left in zrow[] for the next step's weights.  A second instantiation:
+// the benchmarked kernel (MATE = false) is the same code as without it.
+template <int NC, int WPC, bool MATE>
 __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(const __grid_constant__ SpK sp) {
     static_assert(NC == 4 && WPC == 8, "lane group of 8 = 2 gametes x 4 chromosomes of 8 words");
     extern __shared__ __align__(128) uint8_t s_dyn[];
     __shared__ uint32_t s_flag;
+    __shared__ uint32_t s_one[FUSEDF_WARPS * 32];
     pdl_prologue();
     DevSpecies &st = *sp.st;
     const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
@@ -173,6 +162,10 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     const uint32_t sp_slot = sub * 8u + hc * 2u;                                    // + it * 32: (g=0, g=1) pair
     long long acc1 = 0, acc2 = 0;
     uint32_t ties = 0, n_alive = 0;
+    // the ticket's addend, 1, read back from shared memory: a value ptxas can prove neither constant nor
+    // uniform (a constant or uniform addend is what it aggregates)
+    s_one[threadIdx.x] = 1u;
+    const uint32_t one = ((volatile uint32_t *)s_one)[threadIdx.x ^ 1u];
 
     // mo / fa are the parents' physical ROW numbers exactly as loaded: nothing here depends on the
     // two index loads, so they stay in flight until the rows are needed one chunk later
@@ -184,7 +177,22 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
         mo = 0; fa = 0; mf = 0; ul = 2.0f;
         if (jl < M) {
             mo = sp.mother[jl];
-            fa = rowptr[uniform_index(x[0], N)];   // R2
+            uint32_t fi = uniform_index(x[0], N);   // R2
+            if (MATE) {   // R19: weighted draw by running sum + search (words 2,3 of SCALAR block 1); total 0 keeps R2
+                const unsigned long long total = sp.mate_cum[N - 1];
+                if (total) {
+                    uint32_t y[4];
+                    draw_rk(sp, ST_SCALAR, jl, 1, step, y);
+                    const unsigned long long target = __umul64hi(((unsigned long long)y[2] << 32) | y[3], total);
+                    uint32_t lo = 0, hi = N - 1;
+                    while (lo < hi) {
+                        const uint32_t mid = (lo + hi) >> 1;
+                        if (sp.mate_cum[mid] > target) hi = mid; else lo = mid + 1;
+                    }
+                    fi = lo;
+                }
+            }
+            fa = rowptr[fi];
             ul = u01_of(x[3]);
             mf = (a[0] > Um0 ? 1u : 0u) | (b[0] > Um0 ? 2u : 0u);
         }
@@ -254,9 +262,9 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     uint32_t mo = 0, fa = 0, mf = 0;
     float ul = 2.0f;
     for (;;) {
-        uint32_t chunk2 = 0;
+        uint32_t ticket = 0;
         const bool active = chunk != NONE;
-        if (lane == 0) chunk2 = active ? 2u * n_warps + atom_inc_u32(&st.ticket_fused) : gwarp + n_warps;   // consumed at the loop end
+        if (lane == 0 && active) ticket = atom_inc_ticket(&st.ticket_fused, one);   // consumed (and only then touched) at the loop end
         j0 = chunk * FUSED_CHUNK;
         const uint32_t jl = j0 + lane;
         // ---- (b) fathers: half-warp h copies the row of offspring 2k+h into the stage
@@ -403,11 +411,12 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
                 mask_nxt[chunk] = bal;
                 if (bal) atomicAdd(range_cnt + chunk / SCANF_CHUNKS, (uint32_t)__popc(bal));
             }
+            if (MATE && valid) sp.zrow[st.cur ^ 1u][jl] = myzi;   // the value travels with the row (next step's weights)
         }
         __syncwarp();   // the stage and the draw words are reused by the next chunk
         }
         chunk = chunk1;
-        chunk1 = __shfl_sync(0xffffffffu, chunk2, 0);
+        chunk1 = active ? 2u * n_warps + __shfl_sync(0xffffffffu, ticket, 0) : gwarp + n_warps;
         mo = mo1; fa = fa1; ul = ul1; mf = mf1;
         if (chunk >= n_chunks) break;
     }
@@ -627,7 +636,9 @@ __host__ inline bool fused_bit_supported(const SpK &k) {
 }
 
 inline cudaError_t fused_bit_configure() {
-    return cudaFuncSetAttribute(k_fused_bit_f<4, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_fused_bit_f<4, 8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_fused_bit_f<4, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
 }
 
 inline cudaError_t launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
@@ -641,7 +652,7 @@ inline cudaError_t launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t s
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8>, k);
+    return k.mate_on ? cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8, true>, k) : cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8, false>, k);
 }
 
 // Cooperative launch: the whole grid is resident at once (or the launch fails), which the fixed

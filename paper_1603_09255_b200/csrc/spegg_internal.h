@@ -37,7 +37,7 @@ struct DevSpecies {
     // work tickets of the step kernels, each on a cache line of its own: hundreds of CTAs draw from
     // them at the same moment, and same-line atomics are served one after the other by L2
     alignas(128) uint32_t ticket_cmp;
-    alignas(128) uint32_t ticket_fused;
+    alignas(128) unsigned long long ticket_fused;   // (64-bit: see atom_inc_ticket)
     alignas(128) uint32_t ticket_pad;
 };
 
@@ -96,6 +96,8 @@ struct SpK {
     float *u01, *s;
     uint8_t *offbuf;
     int32_t *zi;
+    int32_t *zrow[2];           // integer genetic value of the individual in each PHYSICAL row of pop[0] / pop[1] (when zrow_on)
+    uint32_t zrow_on;           // 1: some kernel of this configuration reads the adults' genetic values
     uint8_t *alive, *captured;
     // R18, overlapping generations (adult_surv > 0): per adult i of the current step
     float adult_surv;           // s_A as fp32; 0 = discrete generations
@@ -103,11 +105,16 @@ struct SpK {
     float *a_u, *a_s;           // its uniform and survival probability
     int32_t *a_zi;              // its integer genetic value
     uint32_t *a_pos;            // its position in the next generation (0xFFFFFFFF: dies)
+    uint32_t *a_rank;           // patch mode: its rank among ALL staying adults (physical row M + rank of the other buffer)
     // R19, shared-preference mating (mate_v != 0): integer mating weights of the current adults
     float mate_v;               // v_m as fp32; 0 = uniform mate (R2)
     unsigned long long *mate_cum;   // [n] inclusive running sum of the weights, adult order
     unsigned long long *mate_tile;  // [n / MATE_TILE + 2] weight of each tile of MATE_TILE adults
     uint32_t mate_on;           // 1: the father comes from the running sum (mate_v != 0 or separate sexes)
+    // R24, mothers drawn by relative fecundity (mom_v != 0): integer mothering weights of the current adults
+    float mom_v;                // v_f as fp32; 0 = every adult mothers its own eggs
+    unsigned long long *mom_cum;    // [n] inclusive running sum, adult order
+    unsigned long long *mom_tile;   // [n / MATE_TILE + 2]
     // R21, separate sexes (sexes = 1): one byte per PHYSICAL row of pop[0] / pop[1], 1 = male
     uint32_t sexes;
     uint8_t *sex[2];
@@ -124,8 +131,10 @@ struct SpK {
     uint32_t *tables, *table_len;
     unsigned long long *status_fec, *status_cmp;  // [n] tile aggregates + [n/32+2] group counters
     uint32_t status_fec_n, status_cmp_n;
-    uint32_t *patch_cnt, *patch_base;  // [P][5]
+    uint32_t patch_sub;         // S: segments per patch of the patch-mode compaction (1 with many small patches)
+    uint32_t *patch_cnt, *patch_base;  // [P * S][6]: survivors per (natal patch, destination slot 0..4); [5]: staying adults of the patch (R18)
     // patch topology (P > 1), built once by the host: the torus never changes
+    uint32_t *patch_abase;      // [P * S] R18: staying adults of the patches before this one
     const uint32_t *nbr;        // [P][4] neighbour of patch p in direction 0..3 (R15)
     const uint32_t *src_list;   // [P][6]: word 0 = number of sources n of destination d, words 1..n = source patch << 3 | slot, by source patch
     DevSpecies *st;             // this species

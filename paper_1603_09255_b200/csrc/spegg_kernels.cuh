@@ -155,6 +155,8 @@ __device__ __forceinline__ void prepare_species(const SpK &sp, uint32_t g, uint3
         for (uint32_t i = g; i < sp.capacity; i += stride) sp.cap[i] = 0u;
     if (sp.mate_on)   // R19: tile totals of the mating weights are accumulated with atomics
         for (uint32_t i = g; i < sp.capacity / MATE_TILE + 2u; i += stride) sp.mate_tile[i] = 0ull;
+    if (sp.mom_v != 0.0f)   // R24: the same for the mothering weights
+        for (uint32_t i = g; i < sp.capacity / MATE_TILE + 2u; i += stride) sp.mom_tile[i] = 0ull;
     if (sp.phys_parents) {  // fused path: the coming step counts its survivors per range of the other buffer
         uint32_t *cnt_next = sp.range_cnt[cur ^ 1u];
         const uint32_t n_max = (sp.capacity + 31u) / 32u * 32u / FUSED_RANGE + 2u;
@@ -230,6 +232,80 @@ __device__ __forceinline__ void solo_tail(const SpK &sp, uint32_t *s_flag) {
     prepare_species(sp, threadIdx.x, blockDim.x, nn, cur1, a1, step1, (threadIdx.x + blockDim.x - 32u) % blockDim.x);
 }
 
+// a3: the scalar draws of offspring j: father (R2; R19 / R21 weighted; R23 assortative), mother by relative
+// fecundity (R24), dispersal (R15), survival uniform (R4), sex at birth (R21).  mother[j] (and, in patch
+// mode, the natal patch in dest[j]) were just written by the calling CTA of k_fec_scan.
+__device__ __forceinline__ void scalar_one(const SpK &sp, uint32_t j, uint32_t N, uint32_t step, const uint32_t *__restrict__ ps,
+                                           unsigned int &ties) {
+    uint32_t mo = sp.mother[j];
+    uint32_t x[4];
+    draw(sp.key, sp.species, ST_SCALAR, j, 0, step, x);
+    uint32_t pm = 0, base = 0, np = N;
+    if (sp.P > 1) { pm = sp.dest[j]; base = ps[pm]; np = ps[pm + 1] - base; }   // natal patch: left in dest[] by k_fec_scan
+    if (sp.mom_v != 0.0f) {
+        // R24 (eq. S2-9): the egg was counted by the adult that laid it; its mother is
+        // drawn among the adults of that patch: 64-bit uniform from words 0,1 of MOTHER block 0,
+        // target = floor(u * total / 2^64), first adult whose running sum exceeds it; total 0: unchanged
+        const unsigned long long before = base ? sp.mom_cum[base - 1] : 0ull;
+        const unsigned long long total = sp.mom_cum[base + np - 1] - before;
+        if (total) {
+            uint32_t y[4];
+            draw_rk(sp, ST_MOTHER, j, 0, step, y);
+            const unsigned long long u = ((unsigned long long)y[0] << 32) | y[1];
+            const unsigned long long target = before + __umul64hi(u, total);
+            uint32_t lo = base, hi = base + np - 1;
+            while (lo < hi) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (sp.mom_cum[mid] > target) hi = mid; else lo = mid + 1;
+            }
+            mo = lo;
+            sp.mother[j] = mo;
+        }
+    }
+    uint32_t fa = base + uniform_index(x[0], np);
+    if (sp.mate_on) {
+        // R19: weighted draw among the adults of the mother's patch: 64-bit uniform from words 2,3 of
+        // SCALAR block 1, target = floor(u * total / 2^64), father = first adult of the patch whose
+        // inclusive running sum exceeds (sum before the patch) + target; total 0 keeps the uniform mate
+        const unsigned long long before = base ? sp.mate_cum[base - 1] : 0ull;
+        const unsigned long long total = sp.mate_cum[base + np - 1] - before;
+        if (total) {
+            uint32_t y[4];
+            draw_rk(sp, ST_SCALAR, j, 1, step, y);
+            const unsigned long long u = ((unsigned long long)y[2] << 32) | y[3];
+            const unsigned long long target = before + __umul64hi(u, total);
+            uint32_t lo = base, hi = base + np - 1;   // first index with mate_cum > target; exists since target < before + total
+            while (lo < hi) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (sp.mate_cum[mid] > target) hi = mid; else lo = mid + 1;
+            }
+            fa = lo;
+        }
+    }
+    if (sp.assort > 0.0f) {
+        // R23 (assortative mating): candidate t = 0..7 uniform over the mother's patch (word
+        // 2(t%2) of MATE block t/2), accepted iff u01(word 2(t%2)+1) < expf_spec(-(a * (d*d))),
+        // d = z_cand - z_mother (genetic values from k_enc_zi); first accepted, else the last candidate
+        const float zm = __fmul_rn((float)sp.enc_zi[mo], sp.pheno_scale);
+        uint32_t y[4];
+        for (uint32_t tr = 0; tr < ASSORT_TRIES; ++tr) {
+            if ((tr & 1u) == 0) draw_rk(sp, ST_MATE, j, tr >> 1, step, y);
+            fa = base + uniform_index(y[2 * (tr & 1u)], np);
+            const float d = __fsub_rn(__fmul_rn((float)sp.enc_zi[fa], sp.pheno_scale), zm);
+            const float p = expf_spec(-__fmul_rn(sp.assort, __fmul_rn(d, d)));
+            const float u = u01_of(y[2 * (tr & 1u) + 1]);
+            if (fabsf(__fsub_rn(u, p)) < 1e-6f) ++ties;
+            if (u < p) break;
+        }
+    }
+    sp.father[j] = fa;
+    uint32_t dest = pm;
+    if (sp.P > 1 && (unsigned long long)x[1] < sp.T_mig) dest = sp.nbr[pm * 4u + (x[2] >> 30)];
+    sp.dest[j] = dest;
+    sp.u01[j] = u01_of(x[3]);
+    if (sp.sexes) sp.sex_off[j] = (uint8_t)(x[2] & 1u);   // R21: sex at birth (bits 30-31 of the word are the direction)
+}
+
 // a1-a3: fecundity (one FEC block per adult), exclusive scan by decoupled look-back, mother fill.
 // Each CTA takes a contiguous RANGE of adults (about N / gridDim.x, at most FEC_RANGE_MAX): pass 1
 // draws the fecundities into shared memory and reduces them, ONE look-back per range gives the
@@ -243,15 +319,16 @@ __device__ __forceinline__ uint32_t fec_range_size(uint32_t N, uint32_t n_ctas) 
     return min(max(R, (uint32_t)SCAN_THREADS), (uint32_t)FEC_RANGE_MAX);
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant__ SpK sp) {
+__global__ void __launch_bounds__(SCAN_THREADS, 4) k_fec_scan(const __grid_constant__ SpK sp) {
     __shared__ uint32_t s_tab[TMAX];
     __shared__ uint8_t s_f[FEC_RANGE_MAX];
     __shared__ uint32_t s_off[FEC_RANGE_MAX];
     __shared__ uint32_t s_warp[SCAN_THREADS / 32];
-    __shared__ uint32_t s_tile;
+    __shared__ uint32_t s_tile, s_total;
     __shared__ unsigned long long s_excl;
     DevSpecies &st = *sp.st;
     const uint32_t N = st.n0, step = sp.glob->step;
+    unsigned int ties = 0;
     // R18: with overlapping generations every adult may stay, so the offspring get the room that is left
     const uint32_t m_cap = sp.adult_surv > 0.0f ? sp.capacity - N : sp.capacity;
     const uint32_t R = fec_range_size(N, gridDim.x);
@@ -289,7 +366,14 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
                     f = poisson_count(s_tab, len0, x[0]);
                 } else {
                     const uint32_t tab = (sp.fec_model == 2) ? min(sp.cap[i], (uint32_t)(CAP_TABLES - 1)) : patch_between(ps, p_lo, p_hi, i);
-                    f = poisson_count(sp.tables + (size_t)tab * TMAX, sp.table_len[tab], x[0]);
+                    // the first four thresholds in one 16-byte load (tables are TMAX-word rows), the rest -- rare --
+                    // by the plain search
+                    const uint32_t *T = sp.tables + (size_t)tab * TMAX;
+                    const uint32_t len = sp.table_len[tab];
+                    const uint4 t4 = *(const uint4 *)T;
+                    f = (len > 0 && x[0] >= t4.x ? 1u : 0u) + (len > 1 && x[0] >= t4.y ? 1u : 0u) +
+                        (len > 2 && x[0] >= t4.z ? 1u : 0u) + (len > 3 && x[0] >= t4.w ? 1u : 0u);
+                    if (f == 4u) while (f < len && x[0] >= T[f]) ++f;
                 }
                 if (sp.sexes && sp.sex[st.cur][rowptr[i]]) f = 0;   // R21: males lay no eggs (the draw is made and ignored)
                 if (sp.fec_cost > 0.0f && f) {
@@ -323,6 +407,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
             if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;  // exclusive warp prefix
             if (lane == 0) {
                 s_excl = excl;
+                s_total = total;
                 if (range == n_ranges - 1) {  // the last range knows M
                     const unsigned long long Mtot = excl + total;
                     if (Mtot > (unsigned long long)m_cap) { st.m = m_cap; st.flags_step |= 1u; }
@@ -355,16 +440,33 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_fec_scan(const __grid_constant
                 }
             }
         }
+        __syncthreads();   // mother[] / dest[] of this range's offspring are written (same CTA: visible after the barrier)
+        // ---- a3 for this range's offspring, one thread each: no separate kernel, no second pass over mother[]
+        {
+            const unsigned long long j_end = min(rbase + (unsigned long long)s_total, (unsigned long long)m_cap);
+            for (unsigned long long j = rbase + tid; j < j_end; j += SCAN_THREADS) scalar_one(sp, (uint32_t)j, N, step, ps, ties);
+        }
         __syncthreads();
     }
+    if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
 }
 
 // Integer genetic values (R10) of the block of 32 consecutive adults blk * 32 .. of the current
 // population, one per lane: lane l returns zi of adult blk * 32 + l (0 beyond n).  Called by a whole
-// warp.  G lanes share one adult (128-bit loads: a row of up to 512 bytes is one load per lane),
-// 32 / G adults per pass, four passes' loads in flight before the first reduction.
-__device__ __forceinline__ int32_t block_adult_zi(const SpK &sp, const uint8_t *__restrict__ pop,
-                                                  const uint32_t *__restrict__ rowptr, uint32_t blk, uint32_t n) {
+// warp.  The value travels with the individual: zrow[buffer][physical row] is written when the row is
+// (spegg_write_state: from the rows; every step: by the compaction, from the gamete kernel's phenotype),
+// so nobody re-reads a row to get one integer.
+__device__ __forceinline__ int32_t block_adult_zi(const SpK &sp, const uint8_t *__restrict__, const uint32_t *__restrict__ rowptr,
+                                                  uint32_t blk, uint32_t n) {
+    const uint32_t i = blk * 32u + (threadIdx.x & 31u);
+    return i < n ? sp.zrow[sp.st->cur][rowptr[i]] : 0;
+}
+
+// The same from the rows themselves (spegg_write_state / spegg_read_state).  G lanes share one adult
+// (128-bit loads: a row of up to 512 bytes is one load per lane), 32 / G adults per pass, four passes'
+// loads in flight before the first reduction.
+__device__ __forceinline__ int32_t block_adult_zi_rows(const SpK &sp, const uint8_t *__restrict__ pop,
+                                                       const uint32_t *__restrict__ rowptr, uint32_t blk, uint32_t n) {
     const uint32_t lane = threadIdx.x & 31u;
     uint32_t G = 1;
     while (G < 32u && G < sp.row_u4) G <<= 1;
@@ -408,6 +510,15 @@ __device__ __forceinline__ int32_t block_adult_zi(const SpK &sp, const uint8_t *
 // blocks of 32 consecutive adults (their genetic values are re-read from the rows), computes the 32
 // weights one per lane, stores them to mate_cum[] and adds their sum to the tile's total (one integer
 // atomic per block -- 32 divides MATE_TILE -- exact in any order).
+__device__ __forceinline__ unsigned long long mating_weight(float v, float d) {
+    float e = __fmul_rn(v, d);
+    e = fminf(fmaxf(e, -16.0f), 16.0f);
+    const float w = expf_spec(__fsub_rn(e, 16.0f));
+    return (unsigned long long)__fmul_rn(w, 0x1p40f);
+}
+
+// (R24, eq. S2-9: the mothering weights exp(v_f z_i), zero for males, are built in the
+// same pass into mom_cum[] / mom_tile[])
 __global__ void __launch_bounds__(256) k_mate_weight(const __grid_constant__ SpK sp) {
     DevSpecies &st = *sp.st;
     const uint32_t N = st.n0, lane = threadIdx.x & 31u;
@@ -415,38 +526,48 @@ __global__ void __launch_bounds__(256) k_mate_weight(const __grid_constant__ SpK
     const uint8_t *pop = sp.pop[st.cur];
     const uint32_t *rowptr = sp.rowptr[st.cur];
     const uint8_t *sex = sp.sex[st.cur];
+    const bool mom_on = sp.mom_v != 0.0f;
     const float zbar = N ? __double2float_rn(__dmul_rn(__ddiv_rn((double)st.sum_zi0, (double)N), (double)sp.pheno_scale)) : 0.0f;
     if (warp0 == 0 && lane == 0) st.zbar_self = zbar;
     for (uint32_t blk = warp0; blk < (N + 31u) / 32u; blk += nw) {
         const int32_t zi = block_adult_zi(sp, pop, rowptr, blk, N);
         const uint32_t i = blk * 32u + lane;
-        unsigned long long part = 0ull;
+        unsigned long long part = 0ull, mpart = 0ull;
         if (i < N) {
             const float d = __fsub_rn(__fmul_rn((float)zi, sp.pheno_scale), zbar);
-            float e = __fmul_rn(sp.mate_v, d);
-            e = fminf(fmaxf(e, -16.0f), 16.0f);
-            const float w = expf_spec(__fsub_rn(e, 16.0f));
-            unsigned long long wi = (unsigned long long)__fmul_rn(w, 0x1p40f);
-            if (sp.sexes && !sex[rowptr[i]]) wi = 0ull;   // R21: only males father eggs
-            sp.mate_cum[i] = wi;
-            part = wi;
+            const bool male = sp.sexes && sex[rowptr[i]];
+            if (sp.mate_on) {
+                unsigned long long wi = mating_weight(sp.mate_v, d);
+                if (sp.sexes && !male) wi = 0ull;   // R21: only males father eggs
+                sp.mate_cum[i] = wi;
+                part = wi;
+            }
+            if (mom_on) {
+                unsigned long long wi = mating_weight(sp.mom_v, d);
+                if (male) wi = 0ull;                // R24 + R21: only females mother eggs
+                sp.mom_cum[i] = wi;
+                mpart = wi;
+            }
         }
-        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+        for (int o = 16; o > 0; o >>= 1) { part += __shfl_xor_sync(0xffffffffu, part, o); mpart += __shfl_xor_sync(0xffffffffu, mpart, o); }
         if (lane == 0 && part) atomicAdd(&sp.mate_tile[blk * 32u / MATE_TILE], part);
+        if (lane == 0 && mpart) atomicAdd(&sp.mom_tile[blk * 32u / MATE_TILE], mpart);
     }
 }
 
 // R19: inclusive running sum of the weights in adult order.  One CTA per tile of MATE_TILE adults:
 // the tile's base is the sum of the tile totals before it (every CTA adds them up itself -- a few
 // thousand L2-resident words, no chain between CTAs), then a block scan of 4 adults per thread.
-__global__ void __launch_bounds__(256) k_mate_scan(const __grid_constant__ SpK sp) {
+__global__ void __launch_bounds__(256) k_mate_scan(const __grid_constant__ SpK sp, int mothers) {
     __shared__ unsigned long long s_red[8];
     __shared__ unsigned long long s_base;
     const uint32_t N = sp.st->n0, tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t n_tiles = (N + MATE_TILE - 1) / MATE_TILE;
+    unsigned long long *cum = mothers ? sp.mom_cum : sp.mate_cum;           // R24 / R19
+    const unsigned long long *tile = mothers ? sp.mom_tile : sp.mate_tile;
     for (uint32_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         unsigned long long b = 0;
-        for (uint32_t k = tid; k < t; k += 256) b += sp.mate_tile[k];
+        for (uint32_t k = tid; k < t; k += 256) b += tile[k];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) b += __shfl_xor_sync(0xffffffffu, b, o);
         if (lane == 0) s_red[warp] = b;
@@ -456,7 +577,7 @@ __global__ void __launch_bounds__(256) k_mate_scan(const __grid_constant__ SpK s
         const uint32_t i0 = t * MATE_TILE + tid * 4;
         unsigned long long w[4], sum = 0;
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { w[k] = (i0 + k < N) ? sp.mate_cum[i0 + k] : 0ull; sum += w[k]; w[k] = sum; }
+        for (int k = 0; k < 4; ++k) { w[k] = (i0 + k < N) ? cum[i0 + k] : 0ull; sum += w[k]; w[k] = sum; }
         unsigned long long incl = sum;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -469,67 +590,9 @@ __global__ void __launch_bounds__(256) k_mate_scan(const __grid_constant__ SpK s
         unsigned long long excl = s_base + (incl - sum);
         for (uint32_t k = 0; k < warp; ++k) excl += s_red[k];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) if (i0 + k < N) sp.mate_cum[i0 + k] = excl + w[k];
+        for (int k = 0; k < 4; ++k) if (i0 + k < N) cum[i0 + k] = excl + w[k];
         __syncthreads();
     }
-}
-
-// a3: scalar draws of each offspring: father (R2), dispersal (R15), survival uniform (R4)
-__global__ void __launch_bounds__(256) k_scalar(const __grid_constant__ SpK sp) {
-    const DevSpecies &st = *sp.st;
-    const uint32_t M = st.m, N = st.n0, step = sp.glob->step;
-    const uint32_t *ps = sp.patch_start[st.cur];
-    unsigned int ties = 0;
-    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
-        const uint32_t mo = sp.mother[j];
-        uint32_t x[4];
-        draw(sp.key, sp.species, ST_SCALAR, j, 0, step, x);
-        uint32_t pm = 0, base = 0, np = N;
-        if (sp.P > 1) { pm = sp.dest[j]; base = ps[pm]; np = ps[pm + 1] - base; }   // natal patch: left in dest[] by k_fec_scan
-        uint32_t fa = base + uniform_index(x[0], np);
-        if (sp.mate_on) {
-            // R19: weighted draw among the adults of the mother's patch: 64-bit uniform from words 2,3 of
-            // SCALAR block 1, target = floor(u * total / 2^64), father = first adult of the patch whose
-            // inclusive running sum exceeds (sum before the patch) + target; total 0 keeps the uniform mate
-            const unsigned long long before = base ? sp.mate_cum[base - 1] : 0ull;
-            const unsigned long long total = sp.mate_cum[base + np - 1] - before;
-            if (total) {
-                uint32_t y[4];
-                draw_rk(sp, ST_SCALAR, j, 1, step, y);
-                const unsigned long long u = ((unsigned long long)y[2] << 32) | y[3];
-                const unsigned long long target = before + __umul64hi(u, total);
-                uint32_t lo = base, hi = base + np - 1;   // first index with mate_cum > target; exists since target < before + total
-                while (lo < hi) {
-                    const uint32_t mid = (lo + hi) >> 1;
-                    if (sp.mate_cum[mid] > target) hi = mid; else lo = mid + 1;
-                }
-                fa = lo;
-            }
-        }
-        if (sp.assort > 0.0f) {
-            // R23 (assortative mating): candidate t = 0..7 uniform over the mother's patch (word
-            // 2(t%2) of MATE block t/2), accepted iff u01(word 2(t%2)+1) < expf_spec(-(a * (d*d))),
-            // d = z_cand - z_mother (genetic values from k_enc_zi); first accepted, else the last candidate
-            const float zm = __fmul_rn((float)sp.enc_zi[mo], sp.pheno_scale);
-            uint32_t y[4];
-            for (uint32_t tr = 0; tr < ASSORT_TRIES; ++tr) {
-                if ((tr & 1u) == 0) draw_rk(sp, ST_MATE, j, tr >> 1, step, y);
-                fa = base + uniform_index(y[2 * (tr & 1u)], np);
-                const float d = __fsub_rn(__fmul_rn((float)sp.enc_zi[fa], sp.pheno_scale), zm);
-                const float p = expf_spec(-__fmul_rn(sp.assort, __fmul_rn(d, d)));
-                const float u = u01_of(y[2 * (tr & 1u) + 1]);
-                if (fabsf(__fsub_rn(u, p)) < 1e-6f) ++ties;
-                if (u < p) break;
-            }
-        }
-        sp.father[j] = fa;
-        uint32_t dest = pm;
-        if (sp.P > 1 && (unsigned long long)x[1] < sp.T_mig) dest = sp.nbr[pm * 4u + (x[2] >> 30)];
-        sp.dest[j] = dest;
-        sp.u01[j] = u01_of(x[3]);
-        if (sp.sexes) sp.sex_off[j] = (uint8_t)(x[2] & 1u);   // R21: sex at birth (bits 30-31 of the word are the direction)
-    }
-    if (ties) atomicAdd(&sp.st->near_ties, (unsigned long long)ties);
 }
 
 // a4 (bit genomes, Poisson crossovers, R8): one thread per (offspring, gamete, chromosome)
@@ -634,17 +697,24 @@ __global__ void __launch_bounds__(256) k_gamete_q10(const __grid_constant__ SpK 
 }
 
 // a4 + a5 (q10 genomes, R7 + R10) for L = 8 ... 256 a power of two: a lane owns 8 consecutive loci of
-// one gamete (two RECOMB blocks, one 128-bit load from each parental haplotype, one 128-bit store),
-// GS = L / 8 lanes make a gamete, and a warp works on whole offspring: both gametes side by side
-// (L <= 128; several offspring per warp when L <= 64) or one after the other (L = 256).  The lane's
-// eight switch thresholds never change (its slot in the gamete is fixed), so they live in registers.
-// The phase is the XOR prefix of the switch bits: within the lane by shift-and-xor on the packed
-// byte, across the lanes of the gamete by a ballot.  The select masks come from the phase byte by a
-// multiply (bit k -> sign bit of byte k) and a sign-replicating byte permute.  The rows of the NEXT
-// work item (iteration, or the father's pass of the same offspring when L = 256) are loaded before
-// this one's draws are computed, and the parents' indices are looked up two iterations ahead, so no
-// load is ever waited for.  The lane's share of the additive phenotype (sum of the 8 alleles it
-// selected) is reduced over the offspring's lanes (one REDUX), so the row is never read again for a5.
+// one gamete (two RECOMB blocks, 16 bytes of each parental haplotype, one 128-bit store), GS = L / 8
+// lanes make a gamete, and a warp works on whole offspring: both gametes side by side (L <= 128;
+// several offspring per warp when L <= 64) or one after the other (L = 256).
+//   * The lane's eight switch thresholds never change (its slot in the gamete is fixed): registers.
+//   * The phase is the XOR prefix of the switch bits: within the lane by shift-and-xor on the packed
+//     byte (built by a carry chain), across the lanes of the gamete by a ballot.  The select masks come
+//     from the phase byte by a multiply (bit k -> sign bit of byte k) and a sign-replicating byte permute.
+//   * The lane's share of the additive phenotype (sum of the 8 alleles it selected) is reduced over the
+//     offspring's lanes (one REDUX), so the offspring row is never read again for a5.
+//   * The parents' rows are random gathers; two ways of keeping them in flight, chosen by L on
+//     measurements (C5 / C4 / C2, ms per launch):
+//       k_gamete_q10v (L <= 128): the rows of the NEXT iteration are loaded into registers before this
+//         one's draws are computed, the parents' indices are looked up two iterations ahead
+//         (L = 128: 0.893; the ring below 1.03; C2, L = 64: 0.021 against 0.047);
+//       k_gamete_q10r (L = 256, where two passes of row registers leave few warps): every lane copies
+//         ITS 2 x 16 bytes per pass with cp.async into a ring of D iterations per warp in shared
+//         memory and reads them back itself (no barrier: a thread only waits for its own copy
+//         groups); indices one stage per iteration ahead of the copies (0.677 against 0.731).
 __host__ __device__ inline bool gamete_q10v_supported(const SpK &k) {
     return k.kind == 1 && k.L >= 8 && k.L <= 256 && (k.L & (k.L - 1)) == 0;
 }
@@ -655,123 +725,123 @@ __device__ __forceinline__ uint32_t prmt_sign(uint32_t a, uint32_t sel) {
     return d;
 }
 
-#ifndef SPEGG_Q10V_THREADS
-#define SPEGG_Q10V_THREADS 128
-#endif
 #ifndef SPEGG_Q10V_MINB
 #define SPEGG_Q10V_MINB 7
 #endif
 #ifndef SPEGG_Q10V_MINB256
-#define SPEGG_Q10V_MINB256 6
+#define SPEGG_Q10V_MINB256 5
 #endif
-constexpr int Q10V_THREADS = SPEGG_Q10V_THREADS;
+#ifndef SPEGG_Q10V_DEPTH256
+#define SPEGG_Q10V_DEPTH256 4
+#endif
+constexpr int Q10V_THREADS = 128;
+template <uint32_t LL> struct Q10V {
+    static constexpr uint32_t GS = LL >> 3;                            // lanes per gamete
+    static constexpr uint32_t LPO = (2u * GS < 32u) ? 2u * GS : 32u;   // lanes per offspring in one pass
+    static constexpr uint32_t NPASS = (2u * GS) / LPO;                 // 2 when L = 256, else 1
+    static constexpr uint32_t OPW = 32u / LPO;                         // offspring per warp iteration
+    static constexpr uint32_t ROW = LL * 4u;                           // bytes per row
+    static constexpr uint32_t D = SPEGG_Q10V_DEPTH256;                 // ring depth (iterations in flight), k_gamete_q10r
+    static constexpr uint32_t ITEM = NPASS * 2u * 32u * 16u;           // bytes of one iteration's rows per warp
+    static constexpr uint32_t SMEM = LL == 256 ? (Q10V_THREADS / 32) * D * ITEM : 0u;
+};
+
+// the lane's constants of the q10 gamete kernels
+template <uint32_t LL> struct Q10Lane {
+    uint32_t li, osub, slot, g0, lt, gmask, omask;
+    uint4 t0, t1;
+    __device__ __forceinline__ Q10Lane(const SpK &sp) {
+        using C = Q10V<LL>;
+        const uint32_t lane = threadIdx.x & 31u;
+        li = lane & (C::LPO - 1u); osub = lane / C::LPO;
+        slot = li & (C::GS - 1u); g0 = (C::NPASS == 1) ? li / C::GS : 0u;   // gamete of pass p: g0 + p
+        lt = (1u << lane) - 1u;
+        gmask = (C::GS == 32u ? 0xFFFFFFFFu : ((1u << C::GS) - 1u)) << (lane - slot);
+        omask = (C::LPO == 32u ? 0xFFFFFFFFu : ((1u << C::LPO) - 1u)) << (lane - li);
+        t0 = ((const uint4 *)sp.T_recomb)[2u * slot]; t1 = ((const uint4 *)sp.T_recomb)[2u * slot + 1u];
+    }
+};
+
+// switch bit of one locus shifted into the packed byte: sub.cc sets the carry iff x >= T (no switch)
+__device__ __forceinline__ void q10_push(uint32_t &ph, uint32_t x, uint32_t T) {
+    asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(ph) : "r"(x), "r"(T));
+}
+
+// one pass: gamete g of offspring j from the parental haplotype words a (hap0), b (hap1) of this lane
+template <uint32_t LL>
+__device__ __forceinline__ void q10_pass(const SpK &sp, const Q10Lane<LL> &ln, uint32_t j, uint32_t g, uint32_t M, uint32_t step,
+                                         uint8_t *out, const uint4 &a, const uint4 &b, int &acc) {
+    using C = Q10V<LL>;
+    // R7: switch bits of this lane's 8 loci, packed (locus 0 in bit 0), and their running parity
+    uint32_t x[4], y[4];
+    const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
+    draw_rk(sp, stream, j, 2u * ln.slot, step, x);
+    draw_rk(sp, stream, j, 2u * ln.slot + 1u, step, y);
+    uint32_t ph = 0;
+    q10_push(ph, y[3], ln.t1.w); q10_push(ph, y[2], ln.t1.z); q10_push(ph, y[1], ln.t1.y); q10_push(ph, y[0], ln.t1.x);
+    q10_push(ph, x[3], ln.t0.w); q10_push(ph, x[2], ln.t0.z); q10_push(ph, x[1], ln.t0.y); q10_push(ph, x[0], ln.t0.x);
+    ph = ~ph & 0xFFu;                                 // bit k: locus k of the lane switches
+    ph ^= ph << 1; ph ^= ph << 2; ph ^= ph << 4;      // bit k = parity of the switch bits of loci 0..k of the lane
+    const uint32_t bal = __ballot_sync(0xffffffffu, (ph & 0x80u) != 0);
+    if (__popc(bal & ln.gmask & ln.lt) & 1u) ph = ~ph;
+    // select: allele from hap1 where the phase bit is set.  bit k of a nibble -> sign bit of byte k
+    // (k + 7 + 7k = 8k + 7; the other products land on other bits), replicated over the allele's two bytes
+    const uint32_t lo = (ph & 0xFu) * 0x10204080u, hi = ((ph >> 4) & 0xFu) * 0x10204080u;
+    const uint32_t m0 = prmt_sign(lo, 0x9988u), m1 = prmt_sign(lo, 0xBBAAu), m2 = prmt_sign(hi, 0x9988u), m3 = prmt_sign(hi, 0xBBAAu);
+    uint4 o;
+    o.x = (a.x & ~m0) | (b.x & m0); o.y = (a.y & ~m1) | (b.y & m1);
+    o.z = (a.z & ~m2) | (b.z & m2); o.w = (a.w & ~m3) | (b.w & m3);
+    if (j < M) {
+        ((uint4 *)(out + (size_t)j * C::ROW))[g * C::GS + ln.slot] = o;
+        // R10: both int16 halves of a word summed by one dp2a
+        acc = __dp2a_lo((int)o.x, 0x0101, acc); acc = __dp2a_lo((int)o.y, 0x0101, acc);
+        acc = __dp2a_lo((int)o.z, 0x0101, acc); acc = __dp2a_lo((int)o.w, 0x0101, acc);
+    }
+}
 
 template <uint32_t LL>
-__global__ void __launch_bounds__(Q10V_THREADS, (LL == 256 ? SPEGG_Q10V_MINB256 : SPEGG_Q10V_MINB)) k_gamete_q10v(const __grid_constant__ SpK sp) {
-    constexpr uint32_t GS = LL >> 3;                       // lanes per gamete
-    constexpr uint32_t LPO = (2u * GS < 32u) ? 2u * GS : 32u;   // lanes per offspring in one pass
-    constexpr uint32_t NPASS = (2u * GS) / LPO;            // 2 when L = 256, else 1
-    constexpr uint32_t OPW = 32u / LPO;                    // offspring per warp iteration
-    constexpr uint32_t ROW = LL * 4u;                      // bytes per row
+__global__ void __launch_bounds__(Q10V_THREADS, SPEGG_Q10V_MINB) k_gamete_q10v(const __grid_constant__ SpK sp) {
+    using C = Q10V<LL>;
+    static_assert(C::NPASS == 1, "L = 256 runs k_gamete_q10r");
     const DevSpecies &st = *sp.st;
     const uint32_t M = st.m, step = sp.glob->step;
-    const uint32_t lane = threadIdx.x & 31u, li = lane & (LPO - 1u), osub = lane / LPO;
-    const uint32_t slot = li & (GS - 1u), g0 = (NPASS == 1) ? li / GS : 0u;   // gamete of pass p: g0 + p
-    const uint32_t lt = (1u << lane) - 1u;
-    const uint32_t gmask = (GS == 32u ? 0xFFFFFFFFu : ((1u << GS) - 1u)) << (lane - slot);
-    const uint32_t omask = (LPO == 32u ? 0xFFFFFFFFu : ((1u << LPO) - 1u)) << (lane - li);
+    const Q10Lane<LL> ln(sp);
     const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
     const uint8_t *pop = sp.pop[st.cur];
     const uint32_t *rowptr = sp.rowptr[st.cur];
     uint8_t *out = offspring_rows(sp);
-#ifndef SPEGG_Q10V_TSMEM
-#define SPEGG_Q10V_TSMEM 0
-#endif
-#if SPEGG_Q10V_TSMEM
-    // the switch thresholds of the LL loci, re-read from shared memory by every pass (registers are what
-    // limits the resident warps)
-    __shared__ uint4 s_T[LL / 4];
-    for (uint32_t k = threadIdx.x; k < LL / 4; k += blockDim.x) s_T[k] = ((const uint4 *)sp.T_recomb)[k];
-    __syncthreads();
-#else
-    const uint4 t0 = ((const uint4 *)sp.T_recomb)[2u * slot], t1 = ((const uint4 *)sp.T_recomb)[2u * slot + 1u];
-#endif
     // parents' rows of the offspring this lane works on in the iteration that starts at ob_
     // (32-bit offspring indices: M <= capacity < 2^31 and two strides are far below 2^31)
     auto parents = [&](uint32_t ob_, uint32_t &p0, uint32_t &p1) {
-        const uint32_t j_ = ob_ + osub;
+        const uint32_t j_ = ob_ + ln.osub;
         p0 = 0u; p1 = 0u;
         if (j_ < M) { p0 = rowptr[sp.mother[j_]]; p1 = rowptr[sp.father[j_]]; }
     };
     // (volatile asm: the loads are issued HERE, ahead of the draws, not sunk to their first use; a dead
     // lane reads row 0)
     auto rows = [&](uint32_t par, uint4 &a, uint4 &b) {
-        const uint4 *h0 = (const uint4 *)(pop + (size_t)par * ROW) + slot;
+        const uint4 *h0 = (const uint4 *)(pop + (size_t)par * C::ROW) + ln.slot;
         asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w) : "l"(h0));
-        asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(h0 + GS));
+        asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(h0 + C::GS));
     };
-    // switch bit of one locus shifted into the packed byte: sub.cc sets the carry iff x >= T (no switch)
-    auto push = [&](uint32_t &ph, uint32_t x, uint32_t T) {
-        uint32_t t;
-        asm("sub.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %1, %1;" : "=r"(t), "+r"(ph) : "r"(x), "r"(T));
-    };
-    // one pass: gamete g of offspring j from the parental haplotype words a (hap0), b (hap1)
-    auto pass = [&](uint32_t j, uint32_t g, const uint4 &a, const uint4 &b, int &acc) {
-        // R7: switch bits of this lane's 8 loci, packed (locus 0 in bit 0), and their running parity
-        uint32_t x[4], y[4];
-        const uint32_t stream = g ? ST_RECOMB_P : ST_RECOMB_M;
-        draw_rk(sp, stream, j, 2u * slot, step, x);
-        draw_rk(sp, stream, j, 2u * slot + 1u, step, y);
-#if SPEGG_Q10V_TSMEM
-        const uint4 t0 = s_T[2u * slot], t1 = s_T[2u * slot + 1u];
-#endif
-        uint32_t ph = 0;
-        push(ph, y[3], t1.w); push(ph, y[2], t1.z); push(ph, y[1], t1.y); push(ph, y[0], t1.x);
-        push(ph, x[3], t0.w); push(ph, x[2], t0.z); push(ph, x[1], t0.y); push(ph, x[0], t0.x);
-        ph = ~ph & 0xFFu;                                 // bit k: locus k of the lane switches
-        ph ^= ph << 1; ph ^= ph << 2; ph ^= ph << 4;      // bit k = parity of the switch bits of loci 0..k of the lane
-        const uint32_t bal = __ballot_sync(0xffffffffu, (ph & 0x80u) != 0);
-        if (__popc(bal & gmask & lt) & 1u) ph = ~ph;
-        // select: allele from hap1 where the phase bit is set.  bit k of a nibble -> sign bit of byte k
-        // (k + 7 + 7k = 8k + 7; the other products land on other bits), replicated over the allele's two bytes
-        const uint32_t lo = (ph & 0xFu) * 0x10204080u, hi = ((ph >> 4) & 0xFu) * 0x10204080u;
-        const uint32_t m0 = prmt_sign(lo, 0x9988u), m1 = prmt_sign(lo, 0xBBAAu), m2 = prmt_sign(hi, 0x9988u), m3 = prmt_sign(hi, 0xBBAAu);
-        uint4 o;
-        o.x = (a.x & ~m0) | (b.x & m0); o.y = (a.y & ~m1) | (b.y & m1);
-        o.z = (a.z & ~m2) | (b.z & m2); o.w = (a.w & ~m3) | (b.w & m3);
-        if (j < M) {
-            ((uint4 *)(out + (size_t)j * ROW))[g * GS + slot] = o;
-            // R10: both int16 halves of a word summed by one dp2a
-            acc = __dp2a_lo((int)o.x, 0x0101, acc); acc = __dp2a_lo((int)o.y, 0x0101, acc);
-            acc = __dp2a_lo((int)o.z, 0x0101, acc); acc = __dp2a_lo((int)o.w, 0x0101, acc);
-        }
-    };
-    const uint32_t stride = n_warps * OPW, ob0 = gw * OPW;
+    const uint32_t stride = n_warps * C::OPW, ob0 = gw * C::OPW;
     uint32_t pm, pf, nm, nf;
     parents(ob0, pm, pf);
     parents(ob0 + stride, nm, nf);
     // one iteration: works on the rows in (a, b), loads the next iteration's into (na, nb)
     auto iteration = [&](uint32_t ob, const uint4 &a, const uint4 &b, uint4 &na, uint4 &nb) {
-        const uint32_t j = ob + osub;
+        const uint32_t j = ob + ln.osub;
         uint32_t n2m, n2f;
         parents(ob + 2u * stride, n2m, n2f);
         int acc = 0;
-        if (NPASS == 1) {
-            rows(g0 ? nf : nm, na, nb);
-            pass(j, g0, a, b, acc);
-        } else {
-            uint4 fa, fb;
-            rows(pf, fa, fb);
-            pass(j, 0u, a, b, acc);
-            rows(nm, na, nb);
-            pass(j, 1u, fa, fb, acc);
-        }
-        acc = __reduce_add_sync(omask, acc);
-        if (j < M && li == 0) sp.zi[j] = acc;
+        rows(ln.g0 ? nf : nm, na, nb);
+        q10_pass<LL>(sp, ln, j, ln.g0, M, step, out, a, b, acc);
+        acc = __reduce_add_sync(ln.omask, acc);
+        if (j < M && ln.li == 0) sp.zi[j] = acc;
         pm = nm; pf = nf; nm = n2m; nf = n2f;
     };
     uint4 a0, b0, a1, b1;
-    rows((NPASS == 1 && g0) ? pf : pm, a0, b0);
+    rows(ln.g0 ? pf : pm, a0, b0);
     for (uint32_t ob = ob0; ob < M; ob += stride) {     // two iterations per trip: the row registers ping-pong
         iteration(ob, a0, b0, a1, b1);
         ob += stride;
@@ -780,21 +850,96 @@ __global__ void __launch_bounds__(Q10V_THREADS, (LL == 256 ? SPEGG_Q10V_MINB256 
     }
 }
 
+template <uint32_t LL>
+__global__ void __launch_bounds__(Q10V_THREADS, SPEGG_Q10V_MINB256) k_gamete_q10r(const __grid_constant__ SpK sp) {
+    using C = Q10V<LL>;
+    constexpr uint32_t D = C::D;
+    extern __shared__ __align__(16) uint8_t s_ring[];
+    const DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, step = sp.glob->step;
+    const Q10Lane<LL> ln(sp);
+    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = (gridDim.x * blockDim.x) >> 5;
+    const uint8_t *pop = sp.pop[st.cur];
+    const uint32_t *rowptr = sp.rowptr[st.cur];
+    uint8_t *out = offspring_rows(sp);
+    // this lane's 16 bytes of (ring item k, pass p, haplotype h): lanes contiguous, so conflict-free
+    const uint32_t ring = smem_u32(s_ring) + (threadIdx.x >> 5) * D * C::ITEM + (threadIdx.x & 31u) * 16u;
+    // the parents of the offspring this lane works on in the iteration that starts at ob_ (32-bit offspring
+    // indices: M <= capacity < 2^31 and D + 2 strides are far below 2^31): their logical indices ...
+    auto parents1 = [&](uint32_t ob_, uint32_t &i0, uint32_t &i1) {
+        const uint32_t j_ = ob_ + ln.osub;
+        i0 = 0xFFFFFFFFu; i1 = 0xFFFFFFFFu;
+        if (j_ < M) { i0 = sp.mother[j_]; i1 = sp.father[j_]; }
+    };
+    // ... and the rows they live in (a dead lane copies from row 0)
+    auto parents2 = [&](uint32_t i0, uint32_t i1, uint32_t &p0, uint32_t &p1) {
+        p0 = 0u; p1 = 0u;
+        if (i0 != 0xFFFFFFFFu) { p0 = rowptr[i0]; p1 = rowptr[i1]; }
+    };
+    // asynchronous copy of this lane's words of both haplotypes of the rows (r_m, r_f) into ring item k
+    auto copy_rows = [&](uint32_t k, uint32_t r_m, uint32_t r_f) {
+#pragma unroll
+        for (uint32_t p = 0; p < C::NPASS; ++p) {
+            const uint32_t g = ln.g0 + p;
+            const uint4 *h0 = (const uint4 *)(pop + (size_t)(g ? r_f : r_m) * C::ROW) + ln.slot;
+            const uint32_t dst = ring + k * C::ITEM + p * 1024u;
+            cp_async16(dst, h0);
+            cp_async16(dst + 512u, h0 + C::GS);
+        }
+        cp_async_commit();
+    };
+    const uint32_t stride = n_warps * C::OPW, ob0 = gw * C::OPW;
+    // prologue: the copies of iterations 0 .. D-1 are started, the rows' numbers of D and the indices of D+1
+    // loaded (all index loads first, so that they travel together)
+    uint32_t pi_m[D + 2], pi_f[D + 2], pr_m[D + 1], pr_f[D + 1];
+#pragma unroll
+    for (uint32_t k = 0; k < D + 2; ++k) parents1(ob0 + k * stride, pi_m[k], pi_f[k]);
+#pragma unroll
+    for (uint32_t k = 0; k < D + 1; ++k) parents2(pi_m[k], pi_f[k], pr_m[k], pr_f[k]);
+#pragma unroll
+    for (uint32_t k = 0; k < D; ++k) copy_rows(k, pr_m[k], pr_f[k]);
+    uint32_t r_m = pr_m[D], r_f = pr_f[D], i_m = pi_m[D + 1], i_f = pi_f[D + 1];
+    uint32_t k = 0;                                          // ring item of the current iteration
+    for (uint32_t ob = ob0; ob < M; ob += stride) {
+        const uint32_t j = ob + ln.osub;
+        uint32_t i_m2, i_f2, r_m1, r_f1;
+        parents1(ob + (D + 2u) * stride, i_m2, i_f2);        // indices of iteration n + D + 2
+        parents2(i_m, i_f, r_m1, r_f1);                      // rows' numbers of n + D + 1
+        cp_async_wait<(int)D - 1>();                         // this thread's copies of iteration n have landed
+        int acc = 0;
+#pragma unroll
+        for (uint32_t p = 0; p < C::NPASS; ++p) {
+            const uint32_t src = ring + k * C::ITEM + p * 1024u;
+            const uint4 a = lds128(src), b = lds128(src + 512u);
+            q10_pass<LL>(sp, ln, j, ln.g0 + p, M, step, out, a, b, acc);
+        }
+        copy_rows(k, r_m, r_f);                              // rows of n + D into the item just consumed
+        acc = __reduce_add_sync(ln.omask, acc);
+        if (j < M && ln.li == 0) sp.zi[j] = acc;
+        r_m = r_m1; r_f = r_f1; i_m = i_m2; i_f = i_f2;
+        k = (k + 1u == D) ? 0u : k + 1u;
+    }
+    cp_async_wait_all();
+}
+
 // grid: as many CTAs as are resident at once (the loop strides over the offspring), never more than
 // the capacity needs
 template <uint32_t LL>
 inline cudaError_t launch_gamete_q10v_t(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
     static int per_sm = 0;
+    auto kern = [] { if constexpr (LL == 256) return k_gamete_q10r<LL>; else return k_gamete_q10v<LL>; }();
     if (per_sm == 0) {
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gamete_q10v<LL>, Q10V_THREADS, 0);
+        cudaError_t e = cudaSuccess;
+        if (Q10V<LL>::SMEM) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Q10V<LL>::SMEM);
+        if (e != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Q10V_THREADS, Q10V<LL>::SMEM);
         if (e != cudaSuccess) return e;
         if (per_sm < 1) per_sm = 1;
     }
-    constexpr uint32_t opw = (LL >= 128u) ? 1u : 128u / LL;     // offspring per warp iteration
-    const uint64_t per_cta = (uint64_t)(Q10V_THREADS / 32) * opw;
+    const uint64_t per_cta = (uint64_t)(Q10V_THREADS / 32) * Q10V<LL>::OPW;
     const uint64_t need = ((uint64_t)k.capacity + per_cta - 1) / per_cta;
     const uint32_t grid = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(need, (uint64_t)n_sms * per_sm));
-    k_gamete_q10v<LL><<<grid, Q10V_THREADS, 0, stream>>>(k);
+    kern<<<grid, Q10V_THREADS, Q10V<LL>::SMEM, stream>>>(k);
     return cudaGetLastError();
 }
 
@@ -810,33 +955,42 @@ inline cudaError_t launch_gamete_q10v(const SpK &k, uint32_t n_sms, cudaStream_t
     }
 }
 
-// a4: sparse mutation (R9), one thread per (offspring, gamete), applied after recombination
+// a4: sparse mutation (R9) of gamete g of offspring j, applied after recombination.  Returns the change
+// of the offspring's integer genetic value (q10; the bit kernels take the phenotype afterwards).
+__device__ __forceinline__ int mutate_one(const SpK &sp, uint32_t j, uint32_t g, uint32_t step) {
+    const uint32_t L = sp.L, stream = g == 0 ? ST_MUT_M : ST_MUT_P;
+    int delta = 0;
+    uint32_t x[4];
+    draw(sp.key, sp.species, stream, j, 0, step, x);
+    const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
+    for (uint32_t k = 0; k < nm; ++k) {
+        if (k > 0) draw(sp.key, sp.species, stream, j, k, step, x);
+        const uint32_t pos = uniform_index(x[1], L);
+        if (sp.kind == 0) {
+            uint32_t *row = (uint32_t *)offspring_rows(sp) + (size_t)j * 2 * sp.W + (size_t)g * sp.W;
+            row[pos >> 5] ^= 1u << (pos & 31u);
+        } else {
+            int16_t *row = (int16_t *)offspring_rows(sp) + (size_t)j * 2 * L + (size_t)g * L;
+            const int v0 = (int)row[pos];
+            int v = v0 + normal_delta(sp.T_norm, sp.R_norm, x[2]);
+            v = max(-32767, min(32767, v));
+            row[pos] = (int16_t)v;
+            delta += v - v0;
+        }
+    }
+    return delta;
+}
+
+// one thread per (offspring, gamete)
 __global__ void __launch_bounds__(256) k_mutate(const __grid_constant__ SpK sp, int zi_delta) {
     const DevSpecies &st = *sp.st;
-    const uint32_t M = st.m, step = sp.glob->step, L = sp.L;
+    const uint32_t M = st.m, step = sp.glob->step;
     const unsigned long long total = 2ull * M;
     for (unsigned long long gi = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; gi < total;
          gi += (unsigned long long)gridDim.x * blockDim.x) {
         const uint32_t j = (uint32_t)(gi >> 1), g = (uint32_t)(gi & 1);
-        const uint32_t stream = g == 0 ? ST_MUT_M : ST_MUT_P;
-        uint32_t x[4];
-        draw(sp.key, sp.species, stream, j, 0, step, x);
-        const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
-        for (uint32_t k = 0; k < nm; ++k) {
-            if (k > 0) draw(sp.key, sp.species, stream, j, k, step, x);
-            const uint32_t pos = uniform_index(x[1], L);
-            if (sp.kind == 0) {
-                uint32_t *row = (uint32_t *)offspring_rows(sp) + (size_t)j * 2 * sp.W + (size_t)g * sp.W;
-                row[pos >> 5] ^= 1u << (pos & 31u);
-            } else {
-                int16_t *row = (int16_t *)offspring_rows(sp) + (size_t)j * 2 * L + (size_t)g * L;
-                const int v0 = (int)row[pos];
-                int v = v0 + normal_delta(sp.T_norm, sp.R_norm, x[2]);
-                v = max(-32767, min(32767, v));
-                row[pos] = (int16_t)v;
-                if (zi_delta && v != v0) atomicAdd(&sp.zi[j], v - v0);   // a5 was taken before the mutation
-            }
-        }
+        const int d = mutate_one(sp, j, g, step);
+        if (zi_delta && d) atomicAdd(&sp.zi[j], d);   // a5 was taken before the mutation
     }
 }
 
@@ -875,9 +1029,9 @@ __global__ void __launch_bounds__(256) k_adult_zi(const __grid_constant__ SpK sp
     const uint32_t cur = sp.st->cur, lane = threadIdx.x & 31u;
     long long acc = 0;
     for (uint32_t blk = warp0; blk < (n + 31u) / 32u; blk += nw) {
-        const int32_t zi = block_adult_zi(sp, sp.pop[cur], sp.rowptr[cur], blk, n);
+        const int32_t zi = block_adult_zi_rows(sp, sp.pop[cur], sp.rowptr[cur], blk, n);
         const uint32_t i = blk * 32u + lane;
-        if (i < n) { if (out) out[i] = zi; acc += zi; }
+        if (i < n) { if (out) out[i] = zi; acc += zi; if (accumulate && sp.zrow_on) sp.zrow[cur][sp.rowptr[cur][i]] = zi; }
     }
     if (accumulate) {
 #pragma unroll
@@ -923,62 +1077,86 @@ __global__ void __launch_bounds__(256) k_gather_rows(const __grid_constant__ SpK
     }
 }
 
-// a6: selection / survival (Fig. 1D), fp32; captures credited to a uniformly drawn predator
+// a6: selection / survival (Fig. 1D) of offspring j with integer genetic value zgen, fp32; captures
+// credited to a uniformly drawn predator (or to the consumer met, R20).  Writes s[], alive[], captured[];
+// returns alive.
+__device__ __forceinline__ bool survive_one(const SpK &sp, DevSpecies &st, uint32_t j, int32_t zgen, uint32_t step,
+                                            unsigned int &ties, unsigned int &caps) {
+    int32_t zp = zgen;
+    if (sp.R_env > 0) {   // R17, eq. S2-14: residual phenotype noise, k quanta from word 1 of SCALAR block 1
+        uint32_t y[4];
+        draw_rk(sp, ST_SCALAR, j, 1, step, y);
+        zp += normal_delta(sp.T_env, sp.R_env, y[1]);
+    }
+    const float z = __fmul_rn((float)zp, sp.pheno_scale);
+    const float u = sp.u01[j];
+    const float theta = sp.theta_patch ? sp.theta_patch[sp.dest[j]] : st.theta_t;
+    bool captured;
+    float s;
+    uint32_t met = 0xFFFFFFFFu;
+    if (sp.enc_E) {
+        // R20 (eq. S3-2): meeting k = 0..E-1 until the first capture: consumer
+        // i_k uniform (word 2(k%2) of SCALAR block 2 + k/2), m = e/(1+e), e = expf_spec(-(d*d)),
+        // d = z - z_{i_k}; captured iff u01(word 2(k%2)+1) < v*m.  The stabilising term stays separate.
+        captured = false;
+        const uint32_t NC = st.n_pred0;
+        uint32_t y[4];
+        for (uint32_t k = 0; k < sp.enc_E && NC && !captured; ++k) {
+            if ((k & 1u) == 0) draw_rk(sp, ST_SCALAR, j, 2 + (k >> 1), step, y);
+            const uint32_t ik = uniform_index(y[2 * (k & 1u)], NC);
+            const float d = __fsub_rn(z, __fmul_rn((float)sp.pred_zi[ik], sp.pred_scale));
+            const float e = expf_spec(-__fmul_rn(d, d));
+            const float p = __fmul_rn(sp.enc_v, __fdiv_rn(e, __fadd_rn(1.0f, e)));
+            const float uk = u01_of(y[2 * (k & 1u) + 1]);
+            if (fabsf(__fsub_rn(uk, p)) < 1e-6f) ++ties;
+            if (uk < p) { captured = true; met = ik; }
+        }
+        s = 1.0f;
+        if (sp.sel_gaussian) {
+            const float d = __fsub_rn(z, theta);
+            s = expf_spec(-__fmul_rn(__fmul_rn(d, d), sp.sel_c));
+        }
+    } else {
+        s = survival_prob(sp, z, theta, u, captured);
+    }
+    sp.s[j] = s;
+    const bool is_alive = u < s && met == 0xFFFFFFFFu;
+    sp.alive[j] = is_alive ? 1 : 0;
+    sp.captured[j] = captured ? 1 : 0;
+    if (fabsf(__fsub_rn(u, s)) < 1e-6f) ++ties;
+    if (captured) {
+        ++caps;
+        if (met != 0xFFFFFFFFu) atomicAdd(&sp.cap_pred[met], 1u);
+        else if (st.n_pred0) {
+            uint32_t y[4];
+            draw(sp.key, sp.species, ST_SCALAR, j, 1, step, y);
+            atomicAdd(&sp.cap_pred[uniform_index(y[0], st.n_pred0)], 1u);
+        }
+    }
+    return is_alive;
+}
+
 __global__ void __launch_bounds__(256) k_survival(const __grid_constant__ SpK sp) {
     DevSpecies &st = *sp.st;
     const uint32_t M = st.m, step = sp.glob->step;
     unsigned int ties = 0, caps = 0;
+    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x)
+        survive_one(sp, st, j, sp.zi[j], step, ties, caps);
+    if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
+    if (caps) atomicAdd(&st.captures, (unsigned long long)caps);
+}
+
+// a4 (mutation) + a6 in one pass, one thread per offspring: the production q10 pipeline, where the gamete
+// kernel has already taken the phenotype and the mutation only corrects it
+__global__ void __launch_bounds__(256) k_mut_surv(const __grid_constant__ SpK sp) {
+    DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, step = sp.glob->step;
+    unsigned int ties = 0, caps = 0;
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
-        int32_t zp = sp.zi[j];
-        if (sp.R_env > 0) {   // R17, eq. S2-14: residual phenotype noise, k quanta from word 1 of SCALAR block 1
-            uint32_t y[4];
-            draw_rk(sp, ST_SCALAR, j, 1, step, y);
-            zp += normal_delta(sp.T_env, sp.R_env, y[1]);
-        }
-        const float z = __fmul_rn((float)zp, sp.pheno_scale);
-        const float u = sp.u01[j];
-        const float theta = sp.theta_patch ? sp.theta_patch[sp.dest[j]] : st.theta_t;
-        bool captured;
-        float s;
-        uint32_t met = 0xFFFFFFFFu;
-        if (sp.enc_E) {
-            // R20 (eq. S3-2): meeting k = 0..E-1 until the first capture: consumer
-            // i_k uniform (word 2(k%2) of SCALAR block 2 + k/2), m = e/(1+e), e = expf_spec(-(d*d)),
-            // d = z - z_{i_k}; captured iff u01(word 2(k%2)+1) < v*m.  The stabilising term stays separate.
-            captured = false;
-            const uint32_t NC = st.n_pred0;
-            uint32_t y[4];
-            for (uint32_t k = 0; k < sp.enc_E && NC && !captured; ++k) {
-                if ((k & 1u) == 0) draw_rk(sp, ST_SCALAR, j, 2 + (k >> 1), step, y);
-                const uint32_t ik = uniform_index(y[2 * (k & 1u)], NC);
-                const float d = __fsub_rn(z, __fmul_rn((float)sp.pred_zi[ik], sp.pred_scale));
-                const float e = expf_spec(-__fmul_rn(d, d));
-                const float p = __fmul_rn(sp.enc_v, __fdiv_rn(e, __fadd_rn(1.0f, e)));
-                const float uk = u01_of(y[2 * (k & 1u) + 1]);
-                if (fabsf(__fsub_rn(uk, p)) < 1e-6f) ++ties;
-                if (uk < p) { captured = true; met = ik; }
-            }
-            s = 1.0f;
-            if (sp.sel_gaussian) {
-                const float d = __fsub_rn(z, theta);
-                s = expf_spec(-__fmul_rn(__fmul_rn(d, d), sp.sel_c));
-            }
-        } else {
-            s = survival_prob(sp, z, theta, u, captured);
-        }
-        sp.s[j] = s;
-        sp.alive[j] = (u < s && met == 0xFFFFFFFFu) ? 1 : 0;
-        sp.captured[j] = captured ? 1 : 0;
-        if (fabsf(__fsub_rn(u, s)) < 1e-6f) ++ties;
-        if (captured) {
-            ++caps;
-            if (met != 0xFFFFFFFFu) atomicAdd(&sp.cap_pred[met], 1u);
-            else if (st.n_pred0) {
-                uint32_t y[4];
-                draw(sp.key, sp.species, ST_SCALAR, j, 1, step, y);
-                atomicAdd(&sp.cap_pred[uniform_index(y[0], st.n_pred0)], 1u);
-            }
-        }
+        const int d = mutate_one(sp, j, 0, step) + mutate_one(sp, j, 1, step);
+        int32_t zi = sp.zi[j];
+        if (d) { zi += d; sp.zi[j] = zi; }
+        survive_one(sp, st, j, zi, step, ties, caps);
     }
     if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
     if (caps) atomicAdd(&st.captures, (unsigned long long)caps);
@@ -993,7 +1171,7 @@ __global__ void __launch_bounds__(256) k_adult_survive(const __grid_constant__ S
     const uint32_t warp0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     const uint8_t *pop = sp.pop[st.cur];
     const uint32_t *rowptr = sp.rowptr[st.cur];
-    const float theta = sp.theta_patch ? sp.theta_patch[0] : st.theta_t;
+    const uint32_t *ps = sp.patch_start[st.cur];
     unsigned int ties = 0;
     for (uint32_t blk = warp0; blk < (N + 31u) / 32u; blk += nw) {   // a warp per block of 32 adults, one adult per lane
         const int32_t zi = block_adult_zi(sp, pop, rowptr, blk, N);
@@ -1003,6 +1181,8 @@ __global__ void __launch_bounds__(256) k_adult_survive(const __grid_constant__ S
             draw_rk(sp, ST_FEC, i, 0, step, x);
             const float u = u01_of(x[1]);
             float w = 1.0f;
+            // (an adult keeps its patch: the optimum is its own patch's)
+            const float theta = sp.theta_patch ? sp.theta_patch[sp.P > 1 ? patch_of(ps, sp.P, i) : 0u] : st.theta_t;
             if (sp.sel_gaussian) {
                 const float d = __fsub_rn(__fmul_rn((float)zi, sp.pheno_scale), theta);
                 w = expf_spec(-__fmul_rn(__fmul_rn(d, d), sp.sel_c));
@@ -1074,6 +1254,86 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cmp_scan(const __grid_constant
     }
 }
 
+// a4 (mutation) + a6 + a7 + a8 in ONE kernel for an unstructured species on the production q10 path with
+// discrete generations: a tile of 1,024 offspring (4 per thread) is mutated, selected, scanned, placed by
+// one look-back, and its survivors' index words are written -- offspring rows stay where the gamete kernel
+// stored them, so nothing else moves.  alive[] / pos[] never travel through memory, and four launches
+// (k_mutate, k_survival, k_cmp_scan, k_cmp_scatter) become one.
+__global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_constant__ SpK sp) {
+    __shared__ uint32_t s_warp[SCAN_THREADS / 32];
+    __shared__ uint32_t s_tile, s_flag;
+    __shared__ unsigned long long s_excl;
+    DevSpecies &st = *sp.st;
+    const uint32_t M = st.m, step = sp.glob->step;
+    const uint32_t n_tiles = (M + SCAN_TILE - 1) / SCAN_TILE;
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    uint32_t *rp = sp.rowptr[st.cur ^ 1u];
+    uint8_t *sex_next = sp.sex[st.cur ^ 1u];
+    int32_t *zrow_next = sp.zrow[st.cur ^ 1u];
+    long long a1 = 0, a2 = 0;
+    unsigned int ties = 0, caps = 0;
+    if (M == 0 && blockIdx.x == 0 && tid == 0) st.n_next = 0;
+    for (;;) {
+        if (tid == 0) s_tile = atomicAdd(&st.ticket_cmp, 1u);
+        __syncthreads();
+        const uint32_t tile = s_tile;
+        if (tile >= n_tiles) break;
+        const uint32_t base = tile * SCAN_TILE + tid * SCAN_ITEMS;
+        uint32_t a[SCAN_ITEMS], sum = 0;
+        int32_t zz[SCAN_ITEMS];
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const uint32_t j = base + k;
+            a[k] = 0; zz[k] = 0;
+            if (j < M) {
+                const int d = mutate_one(sp, j, 0, step) + mutate_one(sp, j, 1, step);
+                int32_t zi = sp.zi[j];
+                if (d) { zi += d; sp.zi[j] = zi; }
+                zz[k] = zi;
+                a[k] = survive_one(sp, st, j, zi, step, ties, caps) ? 1u : 0u;
+                if (a[k]) { a1 += zi; a2 += (long long)zi * zi; }
+            }
+            sum += a[k];
+        }
+        const uint32_t incl = warp_incl_scan(sum);
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t w = (lane < SCAN_THREADS / 32) ? s_warp[lane] : 0u;
+            const uint32_t wi = warp_incl_scan(w);
+            const uint32_t total = __shfl_sync(0xffffffffu, wi, SCAN_THREADS / 32 - 1);
+            const unsigned long long excl = lookback(sp.status_cmp, sp.status_cmp_n, tile, (unsigned long long)total);
+            if (lane < SCAN_THREADS / 32) s_warp[lane] = wi - w;
+            if (lane == 0) {
+                s_excl = excl;
+                if (tile == n_tiles - 1) st.n_next = (uint32_t)(excl + total);
+            }
+        }
+        __syncthreads();
+        uint32_t o = (uint32_t)s_excl + s_warp[warp] + (incl - sum);
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const uint32_t j = base + k;
+            if (a[k]) {
+                rp[o] = j;
+                if (sp.sexes) sex_next[j] = sp.sex_off[j];
+                if (sp.zrow_on) zrow_next[j] = zz[k];
+                ++o;
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o); }
+    if (lane == 0 && (a1 != 0 || a2 != 0)) {
+        atomicAdd((unsigned long long *)&st.acc_zi, (unsigned long long)a1);
+        atomicAdd((unsigned long long *)&st.acc_zi2, (unsigned long long)a2);
+    }
+    if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
+    if (caps) atomicAdd(&st.captures, (unsigned long long)caps);
+    if (sp.solo) solo_tail(sp, &s_flag);   // single species: the last CTA closes the step
+}
+
 // a7: move the surviving rows to their positions in the other buffer, one warp per row
 __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK sp) {
     const DevSpecies &st = *sp.st;
@@ -1082,17 +1342,18 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
     uint8_t *dst = sp.pop[st.cur ^ 1u];
     uint32_t *rp = sp.rowptr[st.cur ^ 1u];
     uint8_t *sex_next = sp.sex[st.cur ^ 1u];   // R21: the sex travels with the row
+    int32_t *zrow_next = sp.zrow[st.cur ^ 1u]; // ... and so does the integer genetic value
     __shared__ uint32_t s_flag;
     if (sp.index_only) {   // the rows stay where the gamete kernel stored them: only the index is written
         for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < M; j += gridDim.x * blockDim.x) {
             const uint32_t p = sp.pos[j];
-            if (p != 0xFFFFFFFFu) { rp[p] = j; if (sp.sexes) sex_next[j] = sp.sex_off[j]; }
+            if (p != 0xFFFFFFFFu) { rp[p] = j; if (sp.sexes) sex_next[j] = sp.sex_off[j]; if (sp.zrow_on) zrow_next[j] = sp.zi[j]; }
         }
     } else {
         for (uint32_t j = warp0; j < M; j += nw) {
             const uint32_t p = sp.pos[j];
             if (p == 0xFFFFFFFFu) continue;
-            if (lane == 0) { rp[p] = p; if (sp.sexes) sex_next[p] = sp.sex_off[j]; }  // materialised path: rows are dense, rowptr is the identity
+            if (lane == 0) { rp[p] = p; if (sp.sexes) sex_next[p] = sp.sex_off[j]; if (sp.zrow_on) zrow_next[p] = sp.zi[j]; }  // materialised path: rows are dense, rowptr is the identity
             const uint4 *src = (const uint4 *)(sp.offbuf + (size_t)j * sp.row_bytes);
             uint4 *d = (uint4 *)(dst + (size_t)p * sp.row_bytes);
             for (uint32_t i = lane; i < sp.row_u4; i += 32) d[i] = src[i];
@@ -1107,8 +1368,8 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
         for (uint32_t i = warp0; i < N; i += nw) {
             const uint32_t p = sp.a_pos[i];
             if (p == 0xFFFFFFFFu) continue;
-            const uint32_t row = sp.index_only ? M + p : p;
-            if (lane == 0) { rp[p] = row; if (sp.sexes) sex_next[row] = sp.sex[cur][rp_cur[i]]; }
+            const uint32_t row = sp.index_only ? M + (sp.P > 1 ? sp.a_rank[i] : p) : p;
+            if (lane == 0) { rp[p] = row; if (sp.sexes) sex_next[row] = sp.sex[cur][rp_cur[i]]; if (sp.zrow_on) zrow_next[row] = sp.a_zi[i]; }
             const uint4 *src = (const uint4 *)(src_pop + (size_t)rp_cur[i] * sp.row_bytes);
             uint4 *d = (uint4 *)(dst + (size_t)row * sp.row_bytes);
             for (uint32_t k = lane; k < sp.row_u4; k += 32) d[k] = src[k];
@@ -1137,80 +1398,132 @@ __device__ __forceinline__ void patch_offspring_range(const SpK &sp, const uint3
     j1 = (a1 < N) ? min(sp.off[a1], M) : M;
 }
 
-// counts of survivors per (natal patch, slot); one CTA per natal patch
+// A patch's offspring (and its adults) are cut into S = sp.patch_sub equal parts, "segments", so that a
+// few large patches (the paper's sweeps: tens of patches of 50,000) still give every SM
+// work: segment w = p * S + s is one CTA work item.  With thousands of small patches S = 1.
+__device__ __forceinline__ void segment_range(uint32_t lo, uint32_t hi, uint32_t s, uint32_t S, uint32_t &a, uint32_t &b) {
+    const unsigned long long len = hi - lo;
+    a = lo + (uint32_t)(len * s / S);
+    b = lo + (uint32_t)(len * (s + 1u) / S);
+}
+
+// counts of survivors per (segment, slot); one CTA per segment.  patch_cnt[w][0..4]: surviving
+// offspring by destination slot; [5]: staying adults (R18)
 __global__ void __launch_bounds__(256) k_patch_count(const __grid_constant__ SpK sp) {
-    __shared__ uint32_t s_cnt[5];
+    __shared__ uint32_t s_cnt[6];
     const DevSpecies &st = *sp.st;
     const uint32_t *ps = sp.patch_start[st.cur];
-    for (uint32_t p = blockIdx.x; p < sp.P; p += gridDim.x) {
-        if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
+    const uint32_t S = sp.patch_sub;
+    for (uint32_t w = blockIdx.x; w < sp.P * S; w += gridDim.x) {
+        const uint32_t p = w / S, sg = w % S;
+        if (threadIdx.x < 6) s_cnt[threadIdx.x] = 0;
         __syncthreads();
-        uint32_t j0, j1;
+        uint32_t j0, j1, jj0, jj1;
         patch_offspring_range(sp, ps, p, st.n0, st.m, j0, j1);
+        segment_range(j0, j1, sg, S, jj0, jj1);
         const uint4 nb = ((const uint4 *)sp.nbr)[p];
-        for (uint32_t j = j0 + threadIdx.x; j < j1; j += blockDim.x)
-            if (sp.alive[j]) atomicAdd(&s_cnt[dest_slot(p, sp.dest[j], nb)], 1u);
+        uint32_t c[5] = {0, 0, 0, 0, 0};
+        for (uint32_t j = jj0 + threadIdx.x; j < jj1; j += blockDim.x)
+            if (sp.alive[j]) {
+                const uint32_t sl = dest_slot(p, sp.dest[j], nb);
+#pragma unroll
+                for (uint32_t k = 0; k < 5; ++k) c[k] += (sl == k) ? 1u : 0u;
+            }
+        uint32_t ca = 0;
+        if (sp.adult_surv > 0.0f) {   // R18: the adults of the segment that stay
+            uint32_t i0, i1;
+            segment_range(ps[p], ps[p + 1], sg, S, i0, i1);
+            for (uint32_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) ca += sp.a_alive[i] ? 1u : 0u;
+        }
+#pragma unroll
+        for (uint32_t k = 0; k < 5; ++k) {
+            const uint32_t v = __reduce_add_sync(0xffffffffu, c[k]);
+            if ((threadIdx.x & 31u) == 0 && v) atomicAdd(&s_cnt[k], v);
+        }
+        ca = __reduce_add_sync(0xffffffffu, ca);
+        if ((threadIdx.x & 31u) == 0 && ca) atomicAdd(&s_cnt[5], ca);
         __syncthreads();
-        if (threadIdx.x < 5) sp.patch_cnt[p * 5 + threadIdx.x] = s_cnt[threadIdx.x];
+        if (threadIdx.x < 6) sp.patch_cnt[w * 6 + threadIdx.x] = s_cnt[threadIdx.x];
         __syncthreads();
     }
 }
 
-// next patch_start and the base position of every (natal patch, slot) group; single CTA: thread t owns
-// the destinations [t * per, t * per + per), whose sources (natal patch, slot) come sorted from the
-// host-built topology table; block scan over the threads' totals
+// next patch_start and the base position of every (segment, slot) group; single CTA: thread t owns the
+// destinations [t * per, t * per + per), whose sources (natal patch, slot) come sorted from the
+// host-built topology table; block scan over the threads' totals.  Inside destination d: its staying
+// adults (segments in order), then source by source (natal patch order), segments in order.
 __global__ void __launch_bounds__(1024) k_patch_base(const __grid_constant__ SpK sp) {
-    __shared__ uint32_t s_warp[32];
+    __shared__ uint32_t s_warp[32], s_awarp[32];
     DevSpecies &st = *sp.st;
     uint32_t *psn = sp.patch_start[st.cur ^ 1u];
-    const uint32_t P = sp.P, tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t P = sp.P, S = sp.patch_sub, tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t per = (P + 1023) / 1024;
     const uint32_t d0 = min(tid * per, P), d1 = min(d0 + per, P);
-    uint32_t mine = 0;
+    uint32_t mine = 0, amine = 0;   // next-generation members / staying adults (R18) of this thread's destinations
     for (uint32_t d = d0; d < d1; ++d) {
-        const uint32_t *sl = sp.src_list + (size_t)d * 6;
-        const uint32_t n = sl[0];
-        for (uint32_t i = 0; i < n; ++i) { const uint32_t e = sl[1 + i]; mine += sp.patch_cnt[(e >> 3) * 5 + (e & 7u)]; }
-    }
-    const uint32_t incl = warp_incl_scan(mine);
-    if (lane == 31) s_warp[warp] = incl;
-    __syncthreads();
-    if (warp == 0) {
-        const uint32_t w = s_warp[lane], wi = warp_incl_scan(w);
-        s_warp[lane] = wi - w;
-        if (lane == 31) { st.n_next = wi; psn[P] = wi; }
-    }
-    __syncthreads();
-    uint32_t run = s_warp[warp] + (incl - mine);
-    for (uint32_t d = d0; d < d1; ++d) {
-        psn[d] = run;
         const uint32_t *sl = sp.src_list + (size_t)d * 6;
         const uint32_t n = sl[0];
         for (uint32_t i = 0; i < n; ++i) {
-            const uint32_t e = sl[1 + i], k = (e >> 3) * 5 + (e & 7u);
-            sp.patch_base[k] = run;
-            run += sp.patch_cnt[k];
+            const uint32_t e = sl[1 + i];
+            for (uint32_t sg = 0; sg < S; ++sg) mine += sp.patch_cnt[((e >> 3) * S + sg) * 6 + (e & 7u)];
+        }
+        for (uint32_t sg = 0; sg < S; ++sg) amine += sp.patch_cnt[(d * S + sg) * 6 + 5];
+    }
+    mine += amine;
+    const uint32_t incl = warp_incl_scan(mine), aincl = warp_incl_scan(amine);
+    if (lane == 31) { s_warp[warp] = incl; s_awarp[warp] = aincl; }
+    __syncthreads();
+    if (warp == 0) {
+        const uint32_t w = s_warp[lane], wi = warp_incl_scan(w), aw = s_awarp[lane], awi = warp_incl_scan(aw);
+        s_warp[lane] = wi - w;
+        s_awarp[lane] = awi - aw;
+        if (lane == 31) { st.n_next = wi; psn[P] = wi; }
+    }
+    __syncthreads();
+    uint32_t run = s_warp[warp] + (incl - mine), arun = s_awarp[warp] + (aincl - amine);
+    for (uint32_t d = d0; d < d1; ++d) {
+        psn[d] = run;
+        // R18: the patch's staying adults come first; patch_base[w][5] = position, patch_abase[w] = rank
+        // among all staying adults, of the first staying adult of segment w
+        for (uint32_t sg = 0; sg < S; ++sg) {
+            const uint32_t w = d * S + sg, na = sp.patch_cnt[w * 6 + 5];
+            sp.patch_base[w * 6 + 5] = run;
+            sp.patch_abase[w] = arun;
+            run += na; arun += na;
+        }
+        const uint32_t *sl = sp.src_list + (size_t)d * 6;
+        const uint32_t n = sl[0];
+        for (uint32_t i = 0; i < n; ++i) {
+            const uint32_t e = sl[1 + i];
+            for (uint32_t sg = 0; sg < S; ++sg) {
+                const uint32_t k = ((e >> 3) * S + sg) * 6 + (e & 7u);
+                sp.patch_base[k] = run;
+                run += sp.patch_cnt[k];
+            }
         }
     }
 }
 
-// positions of the survivors of each natal patch (j order within each slot) + reductions
+// positions of the survivors of each segment (j order within each slot) + reductions
 __global__ void __launch_bounds__(256) k_patch_pos(const __grid_constant__ SpK sp) {
     __shared__ uint32_t s_w[8][5];
     __shared__ uint32_t s_run[5];
     DevSpecies &st = *sp.st;
     const uint32_t *ps = sp.patch_start[st.cur];
+    const uint32_t S = sp.patch_sub;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     long long a1 = 0, a2 = 0;
-    for (uint32_t p = blockIdx.x; p < sp.P; p += gridDim.x) {
-        if (tid < 5) s_run[tid] = sp.patch_base[p * 5 + tid];
-        uint32_t j0, j1;
+    for (uint32_t wi = blockIdx.x; wi < sp.P * S; wi += gridDim.x) {
+        const uint32_t p = wi / S, sg = wi % S;
+        if (tid < 5) s_run[tid] = sp.patch_base[wi * 6 + tid];
+        uint32_t j0, j1, jj0, jj1;
         patch_offspring_range(sp, ps, p, st.n0, st.m, j0, j1);
+        segment_range(j0, j1, sg, S, jj0, jj1);
         const uint4 nb = ((const uint4 *)sp.nbr)[p];
         __syncthreads();
-        for (uint32_t c0 = j0; c0 < j1; c0 += 256) {
+        for (uint32_t c0 = jj0; c0 < jj1; c0 += 256) {
             const uint32_t j = c0 + tid;
-            const bool al = j < j1 && sp.alive[j];
+            const bool al = j < jj1 && sp.alive[j];
             const uint32_t slot = al ? dest_slot(p, sp.dest[j], nb) : 7u;
             uint32_t rank = 0;
 #pragma unroll
@@ -1225,12 +1538,34 @@ __global__ void __launch_bounds__(256) k_patch_pos(const __grid_constant__ SpK s
                 for (uint32_t w = 0; w < warp; ++w) o += s_w[w][slot];
                 sp.pos[j] = o;
                 const long long z = sp.zi[j]; a1 += z; a2 += z * z;
-            } else if (j < j1) sp.pos[j] = 0xFFFFFFFFu;
+            } else if (j < jj1) sp.pos[j] = 0xFFFFFFFFu;
             __syncthreads();
             if (tid < 5) { uint32_t t = 0; for (int w = 0; w < 8; ++w) t += s_w[w][tid]; s_run[tid] += t; }
             __syncthreads();
         }
         __syncthreads();
+        if (sp.adult_surv > 0.0f) {
+            // R18: the staying adults of the segment, in order i, take the next positions of the patch's front;
+            // a_rank = rank among all staying adults (their rows are copied behind the offspring rows)
+            uint32_t run = sp.patch_base[wi * 6 + 5], arun = sp.patch_abase[wi], i0, i1;
+            segment_range(ps[p], ps[p + 1], sg, S, i0, i1);
+            for (uint32_t c0 = i0; c0 < i1; c0 += 256) {
+                const uint32_t i = c0 + tid;
+                const bool al = i < i1 && sp.a_alive[i];
+                const uint32_t bal = __ballot_sync(0xffffffffu, al);
+                if (lane == 0) s_w[warp][0] = __popc(bal);
+                __syncthreads();
+                uint32_t before = __popc(bal & ((1u << lane) - 1u)), tot = 0;
+                for (uint32_t w = 0; w < 8; ++w) { const uint32_t v = s_w[w][0]; tot += v; if (w < warp) before += v; }
+                if (al) {
+                    sp.a_pos[i] = run + before;
+                    sp.a_rank[i] = arun + before;
+                    const long long z = sp.a_zi[i]; a1 += z; a2 += z * z;
+                } else if (i < i1) sp.a_pos[i] = 0xFFFFFFFFu;
+                run += tot; arun += tot;
+                __syncthreads();
+            }
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o); }

@@ -45,6 +45,9 @@ def assert_debug_equal(dg, do, species_cfg, tag=""):
     if species_cfg.get("mate_skew", 0.0) != 0.0 or species_cfg.get("separate_sexes"):        # R19: the integer mating weights' running sum
         assert np.float32(dg["zbar_self"]) == np.float32(do["zbar_self"]), (tag, "zbar_self")
         assert np.array_equal(dg["mate_cum"], do["mate_cum"]), (tag, "mate_cum")
+    if species_cfg.get("mother_skew", 0.0) != 0.0:                                           # R24: the mothering weights' running sum
+        assert np.float32(dg["zbar_self"]) == np.float32(do["zbar_self"]), (tag, "zbar_self")
+        assert np.array_equal(dg["mom_cum"], do["mom_cum"]), (tag, "mom_cum")
 
 
 def assert_state_equal(sim, orc, cfg, tag=""):

@@ -410,7 +410,7 @@ def test_overlapping_generations_room_for_offspring(oracle_mod, binding):
     (1, 1.0, 2.0, None, {}),                        # C1, strong preference
     (2, 0.06, 1.0, None, {}),                       # C2: 6,000 adults = several weight tiles and a ragged tail
     (2, 0.04, -3.0, None, {"resid_sd": 0.2}),       # preference for small mates, with residual noise (same SCALAR block)
-    (3, 0.012, 0.5, None, {}),                      # bit genome: leaves the fused kernel for the general pipeline
+    (3, 0.012, 0.5, None, {}),                      # bit genome: the general pipeline in debug, the MATE instantiation of the fused kernel in production
     (5, 0.03, 1.5, (5, 4), {}),                     # patches: the father comes from the mother's patch
     (2, 0.04, 1.0, None, {"adult_survival": 0.6}),  # with overlapping generations
     (1, 1.0, 400.0, None, {}),                      # clamp in play, most integer weights are 0
@@ -685,3 +685,115 @@ def test_assortative_mating(oracle_mod, binding, which, scale, a, grid, extra):
     bad["species"][0].update(assort=1.0, mate_skew=1.0)     # the two mating rules exclude each other
     with pytest.raises(binding.SpeggError):
         binding.workspace_bytes(bad)
+
+
+@pytest.mark.parametrize("which,scale,v,grid,extra", [
+    (1, 1.0, 2.0, None, {}),                                              # C1, strong skew
+    (2, 0.06, 1.0, None, {}),                                             # C2: several weight tiles and a ragged tail
+    (2, 0.04, -2.0, None, {"mate_skew": 1.5}),                            # both parents weighted, opposite signs
+    (3, 0.012, 0.5, None, {}),                                            # bit genome: leaves the fused kernel
+    (5, 0.03, 1.5, (5, 4), {}),                                           # patches: the mother comes from the laying patch
+    (5, 0.03, 1.0, (5, 4), {"separate_sexes": 1, "mate_skew": 1.0}),      # only females mother, only males father
+    (2, 0.04, 1.0, None, {"adult_survival": 0.6, "assort": 2.0}),         # overlapping generations; R23 reads the NEW mother's value
+    (1, 1.0, 400.0, None, {}),                                            # clamp in play, most integer weights are 0
+])
+def test_weighted_mothers(oracle_mod, binding, which, scale, v, grid, extra):
+    """R24 (eq. S2-9): the mother of each egg is drawn with probability proportional
+    to exp(v_f z) among the adults of the patch that laid it.  Per-step parity of every intermediate
+    including the running sum and the reassigned mother[] (debug), then a free-running trajectory
+    on the production kernels."""
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    sp = cfg["species"][0]
+    sp["mother_skew"] = v
+    sp.update(extra)
+    if "adult_survival" in extra:
+        sp["capacity"] = 4 * sp["capacity"]
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(2):
+        orc.step(5)
+        sim.step(5)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+        parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags
+    sim.close()
+
+
+def test_weighted_mothers_full_size_and_rejections(oracle_mod, binding):
+    """R24 at C2's full size on the production kernels (two steps from the oracle's state), and the
+    combinations the reading excludes."""
+    cfg = workloads.config(2)
+    cfg["species"][0]["mother_skew"] = 1.0
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+    bad = workloads.config(1)
+    bad["species"][0].update(mother_skew=1.0, fec_cost=0.5)
+    with pytest.raises(Exception):
+        binding.Sim(bad, debug=False)
+
+
+@pytest.mark.parametrize("which,scale,grid,sA,extra", [
+    (5, 0.03, (5, 4), 0.6, {}),                                   # C5 shape: dispersal between patches, adults stay put
+    (5, 0.02, (4, 4), 0.9, {"resid_sd": 0.2}),                    # long-lived adults, residual noise on the juveniles
+    (6, 0.004, (6, 1), 0.5, {}),                                  # S6 + overlap: case study 1's shape (PAPER.md:56,126)
+    (5, 0.03, (3, 3), 0.7, {"separate_sexes": 1, "mate_skew": 1.0, "mother_skew": 1.0}),   # sexes travel with the staying adults
+    (5, 0.03, (2, 1), 0.6, {}),                                   # two patches: both neighbours coincide
+    (6, 0.1, (4, 1), 0.5, {}),                                    # few large patches: 17 segments per patch in the compaction
+    (5, 3.0, (3, 2), 0.0, {}),                                    # the segments without overlapping generations (3,000 per patch, dispersal)
+])
+def test_overlapping_generations_in_patches(oracle_mod, binding, which, scale, grid, sA, extra):
+    """R18 in patch mode: in every patch the staying adults (their own patch's
+    optimum, rows unchanged) come before the surviving offspring that land there.  Per-step parity of
+    every intermediate (debug: rows moved) and on the production kernels (index only: the staying
+    adults' rows copied behind the offspring rows), then a free-running trajectory."""
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    sp = cfg["species"][0]
+    sp["adult_survival"] = sA
+    sp.update(extra)
+    sp["capacity"] = 6 * sp["capacity"]
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for _ in range(2):
+        orc.step(6)
+        sim.step(6)
+        for s_ in range(len(cfg["species"])):
+            parity.assert_logs_equal(sim.read_log(s_), orc.log(s_))
+        parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags
+    sim.close()
+
+
+def test_overlapping_generations_in_patches_full_size(oracle_mod, binding):
+    """S6 at the paper's size (16 patches x 50,000) with overlapping generations, production
+    kernels: two steps from the oracle's state."""
+    cfg = workloads.config(6)
+    sp = cfg["species"][0]
+    sp["adult_survival"] = 0.5
+    sp["capacity"] = 4 * sp["capacity"]
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+
+
+@pytest.mark.parametrize("scale,v,extra", [
+    (0.012, 0.5, {}),                           # 12,000 adults: several scan ranges, weight tiles and a ragged tail
+    (0.004, -2.0, {"dtheta": 0.01}),            # preference for small mates, moving optimum
+    (0.002, 400.0, {}),                         # clamp in play: most weights are 0
+])
+def test_fused_path_weighted_father(oracle_mod, binding, scale, v, extra):
+    """R19 on the fused C3 kernels (the MATE instantiation of k_fused_bit_f: father by running sum +
+    search in the scalar stage, the genetic value left in zrow[] for the next step's weights).
+    Production kernels only (debug runs the general pipeline): per-step from the oracle's state, then
+    a free-running trajectory -- the second step onward reads the zrow[] the kernel itself wrote."""
+    cfg = _c3(scale, mate_skew=v, **{k: x for k, x in extra.items() if k != "dtheta"})
+    if "dtheta" in extra:
+        cfg["species"][0]["gaussian"]["dtheta"] = extra["dtheta"]
+    sim = binding.Sim(cfg, debug=False)
+    assert sim.launches_per_step() == 4, "scan + weights + running sum + gamete kernel"
+    sim.close()
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=False)
+    _free_run(oracle_mod, binding, cfg, 6, chunks=2, fused=None)
