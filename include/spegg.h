@@ -228,8 +228,8 @@ int spegg_read_sex(spegg_sim *s, uint32_t species, uint8_t *sex_out, uint64_t ca
 int spegg_step(spegg_sim *s, uint32_t n_steps);
 
 /* Fig. 1 E ("surviving individuals are identified") and PAPER.md:126 (patches): synchronises,
- * then copies the current adults of `species` out in their stable order (offspring order; by
- * (destination patch, j) in patch mode).  Any output may be NULL.  n, step: HOST scalars.
+ * then copies the current adults of `species` out in their stable order (staying adults, then offspring
+ * in birth order j; patch by patch in patch mode).  Any output may be NULL.  n, step: HOST scalars.
  * genomes_out: host or device buffer of cap_bytes; SPEGG_ERANGE if too small (*n is still set).
  * patch_start_out: HOST [n_patches+1].  zi_out: HOST [n] integer genetic values (z = zi * pheno_scale,
  * eq. S2-14).  Uses the idle population buffer as staging; the simulation is unchanged. */

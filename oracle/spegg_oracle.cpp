@@ -14,13 +14,20 @@
  *   PAPER.md:329     eq. S2-14 additive genotype -> phenotype
  *   PAPER.md:327-330 eq. S2-14 residual phenotype noise z ~ Normal(genetic value, rho) (R17)
  *   PAPER.md:56,170,182 overlapping generations, maximum per-step survivorship 0.975 (R18)
- *   DESIGN.md "Readings" R1-R18 for everything the paper leaves open.
+ *   PAPER.md:54, 273-283 (eqs. S2-9, S2-10) mating systems, weighted mothers and fathers (R19, R21, R23, R24)
+ *   PAPER.md:464-475 (eqs. S3-1..S3-3) individual encounters, fecundity cost of defence (R20, R22)
+ *   DESIGN.md "Readings" R1-R24 for everything the paper leaves open.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors, exp
  * specs vs libm, Poisson/normal table moments, brute-force gamete enumeration at
  * L <= 4, recombination fraction = r, Haldane map for the Poisson mode, Mendelian
  * invariant, selection closed forms, Wright-Fisher drift, Beverton-Holt fixed point.
- * Unpinned by the paper: the two-species reading R14 (pinned only by invariants).
+ * PARITY UNPINNED BY THE PAPER (each is pinned to its READING by closed forms on hand-built
+ * populations, none to a number or formula the paper prints): the two-species constants and terms
+ * of R14; the trait reading X = exp(z) of R19 / R24 (the paper's X is irreversible mass, G/Omega
+ * gonadal over neonate mass); R20's replacement of the S3-1/S3-2 integrals by E uniform meetings;
+ * R23's acceptance kernel exp(-a d^2) and its cap of 8 candidates (the paper gives the word
+ * "assortative" only).
  *
  * Build: g++ -O2 -ffp-contract=off -shared -fPIC (fp contraction OFF: every fp
  * value that feeds an integer decision is a stated sequence of IEEE +,-,*,/ ops).

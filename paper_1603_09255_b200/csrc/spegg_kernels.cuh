@@ -957,14 +957,19 @@ inline cudaError_t launch_gamete_q10v(const SpK &k, uint32_t n_sms, cudaStream_t
 
 // a4: sparse mutation (R9) of gamete g of offspring j, applied after recombination.  Returns the change
 // of the offspring's integer genetic value (q10; the bit kernels take the phenotype afterwards).
-__device__ __forceinline__ int mutate_one(const SpK &sp, uint32_t j, uint32_t g, uint32_t step) {
+// (in two halves, so that a caller with several offspring can issue all the count draws before the rare loops)
+__device__ __forceinline__ uint32_t mutation_count(const SpK &sp, uint32_t j, uint32_t g, uint32_t step) {
+    uint32_t x[4];
+    draw_rk(sp, g == 0 ? ST_MUT_M : ST_MUT_P, j, 0, step, x);
+    return poisson_count(sp.T_mut, sp.mut_len, x[0]);
+}
+
+__device__ __forceinline__ int mutate_apply(const SpK &sp, uint32_t j, uint32_t g, uint32_t step, uint32_t nm) {
     const uint32_t L = sp.L, stream = g == 0 ? ST_MUT_M : ST_MUT_P;
     int delta = 0;
     uint32_t x[4];
-    draw(sp.key, sp.species, stream, j, 0, step, x);
-    const uint32_t nm = poisson_count(sp.T_mut, sp.mut_len, x[0]);
     for (uint32_t k = 0; k < nm; ++k) {
-        if (k > 0) draw(sp.key, sp.species, stream, j, k, step, x);
+        draw(sp.key, sp.species, stream, j, k, step, x);
         const uint32_t pos = uniform_index(x[1], L);
         if (sp.kind == 0) {
             uint32_t *row = (uint32_t *)offspring_rows(sp) + (size_t)j * 2 * sp.W + (size_t)g * sp.W;
@@ -979,6 +984,11 @@ __device__ __forceinline__ int mutate_one(const SpK &sp, uint32_t j, uint32_t g,
         }
     }
     return delta;
+}
+
+__device__ __forceinline__ int mutate_one(const SpK &sp, uint32_t j, uint32_t g, uint32_t step) {
+    const uint32_t nm = mutation_count(sp, j, g, step);
+    return nm ? mutate_apply(sp, j, g, step, nm) : 0;
 }
 
 // one thread per (offspring, gamete)
@@ -1080,8 +1090,8 @@ __global__ void __launch_bounds__(256) k_gather_rows(const __grid_constant__ SpK
 // a6: selection / survival (Fig. 1D) of offspring j with integer genetic value zgen, fp32; captures
 // credited to a uniformly drawn predator (or to the consumer met, R20).  Writes s[], alive[], captured[];
 // returns alive.
-__device__ __forceinline__ bool survive_one(const SpK &sp, DevSpecies &st, uint32_t j, int32_t zgen, uint32_t step,
-                                            unsigned int &ties, unsigned int &caps) {
+__device__ __forceinline__ bool survive_core(const SpK &sp, DevSpecies &st, uint32_t j, int32_t zgen, float u, float theta,
+                                             uint32_t step, unsigned int &ties, unsigned int &caps) {
     int32_t zp = zgen;
     if (sp.R_env > 0) {   // R17, eq. S2-14: residual phenotype noise, k quanta from word 1 of SCALAR block 1
         uint32_t y[4];
@@ -1089,8 +1099,6 @@ __device__ __forceinline__ bool survive_one(const SpK &sp, DevSpecies &st, uint3
         zp += normal_delta(sp.T_env, sp.R_env, y[1]);
     }
     const float z = __fmul_rn((float)zp, sp.pheno_scale);
-    const float u = sp.u01[j];
-    const float theta = sp.theta_patch ? sp.theta_patch[sp.dest[j]] : st.theta_t;
     bool captured;
     float s;
     uint32_t met = 0xFFFFFFFFu;
@@ -1134,6 +1142,12 @@ __device__ __forceinline__ bool survive_one(const SpK &sp, DevSpecies &st, uint3
         }
     }
     return is_alive;
+}
+
+__device__ __forceinline__ bool survive_one(const SpK &sp, DevSpecies &st, uint32_t j, int32_t zgen, uint32_t step,
+                                            unsigned int &ties, unsigned int &caps) {
+    const float theta = sp.theta_patch ? sp.theta_patch[sp.dest[j]] : st.theta_t;
+    return survive_core(sp, st, j, zgen, sp.u01[j], theta, step, ties, caps);
 }
 
 __global__ void __launch_bounds__(256) k_survival(const __grid_constant__ SpK sp) {
@@ -1263,6 +1277,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_co
     __shared__ uint32_t s_warp[SCAN_THREADS / 32];
     __shared__ uint32_t s_tile, s_flag;
     __shared__ unsigned long long s_excl;
+    __shared__ __align__(4) uint8_t s_alive[SCAN_TILE];
     DevSpecies &st = *sp.st;
     const uint32_t M = st.m, step = sp.glob->step;
     const uint32_t n_tiles = (M + SCAN_TILE - 1) / SCAN_TILE;
@@ -1270,6 +1285,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_co
     uint32_t *rp = sp.rowptr[st.cur ^ 1u];
     uint8_t *sex_next = sp.sex[st.cur ^ 1u];
     int32_t *zrow_next = sp.zrow[st.cur ^ 1u];
+    const float theta = sp.theta_patch ? sp.theta_patch[0] : st.theta_t;   // one patch
     long long a1 = 0, a2 = 0;
     unsigned int ties = 0, caps = 0;
     if (M == 0 && blockIdx.x == 0 && tid == 0) st.n_next = 0;
@@ -1278,23 +1294,50 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_co
         __syncthreads();
         const uint32_t tile = s_tile;
         if (tile >= n_tiles) break;
-        const uint32_t base = tile * SCAN_TILE + tid * SCAN_ITEMS;
-        uint32_t a[SCAN_ITEMS], sum = 0;
+        // ---- phase 1, offspring j = tile * 1024 + k * 256 + tid (coalesced): all loads and all mutation-count
+        // draws of the thread's four offspring first, so that they travel together; then the rare mutations,
+        // selection, and everything that is indexed by j
+        const uint32_t t0 = tile * SCAN_TILE + tid;
         int32_t zz[SCAN_ITEMS];
+        float uu[SCAN_ITEMS];
+        uint32_t nm[SCAN_ITEMS];
 #pragma unroll
         for (int k = 0; k < SCAN_ITEMS; ++k) {
-            const uint32_t j = base + k;
-            a[k] = 0; zz[k] = 0;
-            if (j < M) {
-                const int d = mutate_one(sp, j, 0, step) + mutate_one(sp, j, 1, step);
-                int32_t zi = sp.zi[j];
-                if (d) { zi += d; sp.zi[j] = zi; }
-                zz[k] = zi;
-                a[k] = survive_one(sp, st, j, zi, step, ties, caps) ? 1u : 0u;
-                if (a[k]) { a1 += zi; a2 += (long long)zi * zi; }
-            }
-            sum += a[k];
+            const uint32_t j = t0 + k * SCAN_THREADS;
+            zz[k] = 0; uu[k] = 2.0f;
+            if (j < M) { zz[k] = sp.zi[j]; uu[k] = sp.u01[j]; }
         }
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const uint32_t j = t0 + k * SCAN_THREADS;
+            nm[k] = 0;
+            if (j < M) nm[k] = mutation_count(sp, j, 0, step) | (mutation_count(sp, j, 1, step) << 16);
+        }
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const uint32_t j = t0 + k * SCAN_THREADS;
+            bool al = false;
+            if (j < M) {
+                if (nm[k]) {
+                    int d = 0;
+                    if (nm[k] & 0xFFFFu) d += mutate_apply(sp, j, 0, step, nm[k] & 0xFFFFu);
+                    if (nm[k] >> 16) d += mutate_apply(sp, j, 1, step, nm[k] >> 16);
+                    if (d) { zz[k] += d; sp.zi[j] = zz[k]; }
+                }
+                al = survive_core(sp, st, j, zz[k], uu[k], theta, step, ties, caps);
+                if (al) {
+                    a1 += zz[k]; a2 += (long long)zz[k] * zz[k];
+                    if (sp.sexes) sex_next[j] = sp.sex_off[j];
+                    if (sp.zrow_on) zrow_next[j] = zz[k];
+                }
+            }
+            s_alive[k * SCAN_THREADS + tid] = al ? 1 : 0;
+        }
+        __syncthreads();
+        // ---- phase 2, four consecutive offspring per thread: scan, one look-back, the index
+        const uint32_t base = tile * SCAN_TILE + tid * SCAN_ITEMS;
+        const uint32_t a4 = ((const uint32_t *)s_alive)[tid];   // bytes base .. base + 3
+        const uint32_t sum = __popc(a4);
         const uint32_t incl = warp_incl_scan(sum);
         if (lane == 31) s_warp[warp] = incl;
         __syncthreads();
@@ -1312,15 +1355,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_co
         __syncthreads();
         uint32_t o = (uint32_t)s_excl + s_warp[warp] + (incl - sum);
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
-            const uint32_t j = base + k;
-            if (a[k]) {
-                rp[o] = j;
-                if (sp.sexes) sex_next[j] = sp.sex_off[j];
-                if (sp.zrow_on) zrow_next[j] = zz[k];
-                ++o;
-            }
-        }
+        for (int k = 0; k < SCAN_ITEMS; ++k)
+            if ((a4 >> (8 * k)) & 1u) rp[o++] = base + k;
         __syncthreads();
     }
 #pragma unroll
@@ -1365,14 +1401,21 @@ __global__ void __launch_bounds__(256) k_cmp_scatter(const __grid_constant__ SpK
         const uint32_t N = st.n0, cur = st.cur;
         const uint8_t *src_pop = sp.pop[cur];
         const uint32_t *rp_cur = sp.rowptr[cur];
-        for (uint32_t i = warp0; i < N; i += nw) {
+        // G lanes share a row (a 32-byte row is two 128-bit words: sixteen rows per warp pass)
+        uint32_t G = 1;
+        while (G < 32u && G < sp.row_u4) G <<= 1;
+        const uint32_t apw = 32u / G, grp = lane / G, q = lane % G;
+        for (uint32_t i0 = warp0 * apw; i0 < N; i0 += nw * apw) {
+            const uint32_t i = i0 + grp;
+            if (i >= N) continue;
             const uint32_t p = sp.a_pos[i];
             if (p == 0xFFFFFFFFu) continue;
             const uint32_t row = sp.index_only ? M + (sp.P > 1 ? sp.a_rank[i] : p) : p;
-            if (lane == 0) { rp[p] = row; if (sp.sexes) sex_next[row] = sp.sex[cur][rp_cur[i]]; if (sp.zrow_on) zrow_next[row] = sp.a_zi[i]; }
-            const uint4 *src = (const uint4 *)(src_pop + (size_t)rp_cur[i] * sp.row_bytes);
+            const uint32_t srow = rp_cur[i];
+            if (q == 0) { rp[p] = row; if (sp.sexes) sex_next[row] = sp.sex[cur][srow]; if (sp.zrow_on) zrow_next[row] = sp.a_zi[i]; }
+            const uint4 *src = (const uint4 *)(src_pop + (size_t)srow * sp.row_bytes);
             uint4 *d = (uint4 *)(dst + (size_t)row * sp.row_bytes);
-            for (uint32_t k = lane; k < sp.row_u4; k += 32) d[k] = src[k];
+            for (uint32_t k = q; k < sp.row_u4; k += G) d[k] = src[k];
         }
     }
     if (sp.solo) solo_tail(sp, &s_flag);   // single unstructured species: the last CTA closes the step
