@@ -116,7 +116,7 @@ def apply_variant(cfg, variant):
     return cfg
 
 
-SWEEP = {"patches": 16, "per_patch": 50_000}   # --patches / --per-patch (configuration 6)
+SWEEP = {"patches": 16, "per_patch": 50_000, "k_scale": 1.0}   # --patches / --per-patch (configuration 6), --k-scale
 
 
 def workload(which, seed_offset=0, world=1, variant="none"):
@@ -125,7 +125,11 @@ def workload(which, seed_offset=0, world=1, variant="none"):
     from paper_1603_09255_b200 import replicas, workloads
     if which == 6:
         return apply_variant(replicas.sweep_shard(SWEEP["patches"] * world, seed_offset, world, per_patch=SWEEP["per_patch"]), variant)
-    return apply_variant(replicas.replica_config(workloads.config(which), seed_offset), variant)
+    cfg = apply_variant(replicas.replica_config(workloads.config(which), seed_offset), variant)
+    if SWEEP["k_scale"] != 1.0:
+        cfg["species"][0]["K"] = cfg["species"][0]["K"] * SWEEP["k_scale"]
+        cfg["name"] = "%s(K x %g)" % (cfg["name"], SWEEP["k_scale"])
+    return cfg
 
 
 def describe(cfg):
@@ -478,12 +482,14 @@ def main():
                     help="untimed steps before the W warm-up steps (the initial state is written again after them)")
     ap.add_argument("--patches", type=int, default=16, help="configuration 6: patches per rank (PAPER.md:64 runs 1-100)")
     ap.add_argument("--per-patch", type=int, default=50_000, help="configuration 6: individuals per patch at the start")
+    ap.add_argument("--k-scale", type=float, default=1.0,
+                    help="multiply the carrying capacity K of species 0 (fixed / variable cost of the step; profiles/r02_fused_full.md)")
     ap.add_argument("--no-others", dest="others", action="store_false",
                     help="skip the short timed passes of configurations 1, 2, 4, 5 (config.other_workloads)")
     ap.add_argument("--ref-budget-s", type=float, default=120.0,
                     help="--impl reference: CPU seconds the K+W oracle steps are sized for")
     args = ap.parse_args()
-    SWEEP.update(patches=args.patches, per_patch=args.per_patch)
+    SWEEP.update(patches=args.patches, per_patch=args.per_patch, k_scale=args.k_scale)
     if args.warmup < 3:
         args.warmup = 3
     if args.impl == "reference":

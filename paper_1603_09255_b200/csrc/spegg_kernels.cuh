@@ -1491,28 +1491,36 @@ __global__ void __launch_bounds__(256) k_patch_count(const __grid_constant__ SpK
     }
 }
 
-// next patch_start and the base position of every (segment, slot) group; single CTA: thread t owns the
-// destinations [t * per, t * per + per), whose sources (natal patch, slot) come sorted from the
-// host-built topology table; block scan over the threads' totals.  Inside destination d: its staying
-// adults (segments in order), then source by source (natal patch order), segments in order.
+// next patch_start and the base position of every (segment, slot) group.  The next generation's order
+// is one flat list: destination by destination; inside destination d its staying adults (R18), then
+// source by source (natal patch order, from the host-built topology table); inside each of these the S
+// segments in order.  Item q = (d * 6 + o) * S + sg (o = 0: stayers, o = 1..5: the o-th source, absent
+// ones count 0) -- so the bases are ONE exclusive scan over P * 6 * S counts, done by a single CTA whose
+// threads take contiguous runs of items (and a second scan over the stayers alone for their ranks).
+__device__ __forceinline__ uint32_t patch_item_count(const SpK &sp, uint32_t q, uint32_t S, uint32_t &k_out) {
+    const uint32_t sg = q % S, o = (q / S) % 6u, d = q / (6u * S);
+    k_out = 0xFFFFFFFFu;
+    if (o == 0) { k_out = (d * S + sg) * 6u + 5u; return sp.patch_cnt[k_out]; }
+    const uint32_t *sl = sp.src_list + (size_t)d * 6;
+    if (o > sl[0]) return 0u;
+    const uint32_t e = sl[o];
+    k_out = ((e >> 3) * S + sg) * 6u + (e & 7u);
+    return sp.patch_cnt[k_out];
+}
+
 __global__ void __launch_bounds__(1024) k_patch_base(const __grid_constant__ SpK sp) {
     __shared__ uint32_t s_warp[32], s_awarp[32];
     DevSpecies &st = *sp.st;
     uint32_t *psn = sp.patch_start[st.cur ^ 1u];
     const uint32_t P = sp.P, S = sp.patch_sub, tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    const uint32_t per = (P + 1023) / 1024;
-    const uint32_t d0 = min(tid * per, P), d1 = min(d0 + per, P);
-    uint32_t mine = 0, amine = 0;   // next-generation members / staying adults (R18) of this thread's destinations
-    for (uint32_t d = d0; d < d1; ++d) {
-        const uint32_t *sl = sp.src_list + (size_t)d * 6;
-        const uint32_t n = sl[0];
-        for (uint32_t i = 0; i < n; ++i) {
-            const uint32_t e = sl[1 + i];
-            for (uint32_t sg = 0; sg < S; ++sg) mine += sp.patch_cnt[((e >> 3) * S + sg) * 6 + (e & 7u)];
-        }
-        for (uint32_t sg = 0; sg < S; ++sg) amine += sp.patch_cnt[(d * S + sg) * 6 + 5];
+    const uint32_t n = P * 6u * S, per = (n + 1023u) / 1024u;
+    const uint32_t q0 = min(tid * per, n), q1 = min(q0 + per, n);
+    uint32_t mine = 0, amine = 0, k;
+    for (uint32_t q = q0; q < q1; ++q) {
+        const uint32_t c = patch_item_count(sp, q, S, k);
+        mine += c;
+        if ((q / S) % 6u == 0) amine += c;
     }
-    mine += amine;
     const uint32_t incl = warp_incl_scan(mine), aincl = warp_incl_scan(amine);
     if (lane == 31) { s_warp[warp] = incl; s_awarp[warp] = aincl; }
     __syncthreads();
@@ -1524,26 +1532,12 @@ __global__ void __launch_bounds__(1024) k_patch_base(const __grid_constant__ SpK
     }
     __syncthreads();
     uint32_t run = s_warp[warp] + (incl - mine), arun = s_awarp[warp] + (aincl - amine);
-    for (uint32_t d = d0; d < d1; ++d) {
-        psn[d] = run;
-        // R18: the patch's staying adults come first; patch_base[w][5] = position, patch_abase[w] = rank
-        // among all staying adults, of the first staying adult of segment w
-        for (uint32_t sg = 0; sg < S; ++sg) {
-            const uint32_t w = d * S + sg, na = sp.patch_cnt[w * 6 + 5];
-            sp.patch_base[w * 6 + 5] = run;
-            sp.patch_abase[w] = arun;
-            run += na; arun += na;
-        }
-        const uint32_t *sl = sp.src_list + (size_t)d * 6;
-        const uint32_t n = sl[0];
-        for (uint32_t i = 0; i < n; ++i) {
-            const uint32_t e = sl[1 + i];
-            for (uint32_t sg = 0; sg < S; ++sg) {
-                const uint32_t k = ((e >> 3) * S + sg) * 6 + (e & 7u);
-                sp.patch_base[k] = run;
-                run += sp.patch_cnt[k];
-            }
-        }
+    for (uint32_t q = q0; q < q1; ++q) {
+        const uint32_t c = patch_item_count(sp, q, S, k);
+        if (q % (6u * S) == 0) psn[q / (6u * S)] = run;
+        if (k != 0xFFFFFFFFu) sp.patch_base[k] = run;
+        if ((q / S) % 6u == 0) { sp.patch_abase[q / (6u * S) * S + q % S] = arun; arun += c; }
+        run += c;
     }
 }
 
