@@ -235,13 +235,13 @@ __device__ __forceinline__ void solo_tail(const SpK &sp, uint32_t *s_flag) {
 // a3: the scalar draws of offspring j: father (R2; R19 / R21 weighted; R23 assortative), mother by relative
 // fecundity (R24), dispersal (R15), survival uniform (R4), sex at birth (R21).  mother[j] (and, in patch
 // mode, the natal patch in dest[j]) were just written by the calling CTA of k_fec_scan.
-__device__ __forceinline__ void scalar_one(const SpK &sp, uint32_t j, uint32_t N, uint32_t step, const uint32_t *__restrict__ ps,
+// (pm, base, np: the natal patch of j, its first adult and its size -- loaded by the caller, who batches
+// these two dependent loads over several offspring)
+__device__ __forceinline__ void scalar_one(const SpK &sp, uint32_t j, uint32_t pm, uint32_t base, uint32_t np, uint32_t step,
                                            unsigned int &ties) {
-    uint32_t mo = sp.mother[j];
+    uint32_t mo = (sp.mom_v != 0.0f || sp.assort > 0.0f) ? sp.mother[j] : 0u;   // (only those two read it)
     uint32_t x[4];
     draw(sp.key, sp.species, ST_SCALAR, j, 0, step, x);
-    uint32_t pm = 0, base = 0, np = N;
-    if (sp.P > 1) { pm = sp.dest[j]; base = ps[pm]; np = ps[pm + 1] - base; }   // natal patch: left in dest[] by k_fec_scan
     if (sp.mom_v != 0.0f) {
         // R24 (eq. S2-9): the egg was counted by the adult that laid it; its mother is
         // drawn among the adults of that patch: 64-bit uniform from words 0,1 of MOTHER block 0,
@@ -444,7 +444,26 @@ __global__ void __launch_bounds__(SCAN_THREADS, 4) k_fec_scan(const __grid_const
         // ---- a3 for this range's offspring, one thread each: no separate kernel, no second pass over mother[]
         {
             const unsigned long long j_end = min(rbase + (unsigned long long)s_total, (unsigned long long)m_cap);
-            for (unsigned long long j = rbase + tid; j < j_end; j += SCAN_THREADS) scalar_one(sp, (uint32_t)j, N, step, ps, ties);
+            // four offspring per trip: their natal patches (left in dest[] above), then the patches' bounds, travel
+            // together -- a thread's trips are otherwise a chain of two dependent loads each
+            for (unsigned long long j0 = rbase + tid; j0 < j_end; j0 += 4ull * SCAN_THREADS) {
+                uint32_t pm[4], b0[4], b1[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const unsigned long long j = j0 + (unsigned long long)q * SCAN_THREADS;
+                    pm[q] = (sp.P > 1 && j < j_end) ? sp.dest[j] : 0u;
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    b0[q] = 0u; b1[q] = N;
+                    if (sp.P > 1) { b0[q] = ps[pm[q]]; b1[q] = ps[pm[q] + 1u]; }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const unsigned long long j = j0 + (unsigned long long)q * SCAN_THREADS;
+                    if (j < j_end) scalar_one(sp, (uint32_t)j, pm[q], b0[q], b1[q] - b0[q], step, ties);
+                }
+            }
         }
         __syncthreads();
     }
@@ -725,15 +744,10 @@ __device__ __forceinline__ uint32_t prmt_sign(uint32_t a, uint32_t sel) {
     return d;
 }
 
-#ifndef SPEGG_Q10V_MINB
-#define SPEGG_Q10V_MINB 7
-#endif
-#ifndef SPEGG_Q10V_MINB256
-#define SPEGG_Q10V_MINB256 5
-#endif
-#ifndef SPEGG_Q10V_DEPTH256
-#define SPEGG_Q10V_DEPTH256 4
-#endif
+// resident CTAs per SM the register budget is set for (measured: L = 128 at 7 x 4 warps, 72 registers,
+// 0.893 ms per C5 launch; 8 x 4 at 64 registers with spills 0.995; 256-thread CTAs x 3: 1.110), and the
+// depth of the L = 256 ring (C4: depth 4 at 5 CTAs 0.677 ms, depth 3 at 6 CTAs 0.699, depth 2 at 7: 0.709)
+constexpr int Q10V_MINB = 7, Q10V_MINB256 = 5, Q10V_DEPTH256 = 4;
 constexpr int Q10V_THREADS = 128;
 template <uint32_t LL> struct Q10V {
     static constexpr uint32_t GS = LL >> 3;                            // lanes per gamete
@@ -741,7 +755,7 @@ template <uint32_t LL> struct Q10V {
     static constexpr uint32_t NPASS = (2u * GS) / LPO;                 // 2 when L = 256, else 1
     static constexpr uint32_t OPW = 32u / LPO;                         // offspring per warp iteration
     static constexpr uint32_t ROW = LL * 4u;                           // bytes per row
-    static constexpr uint32_t D = SPEGG_Q10V_DEPTH256;                 // ring depth (iterations in flight), k_gamete_q10r
+    static constexpr uint32_t D = Q10V_DEPTH256;                 // ring depth (iterations in flight), k_gamete_q10r
     static constexpr uint32_t ITEM = NPASS * 2u * 32u * 16u;           // bytes of one iteration's rows per warp
     static constexpr uint32_t SMEM = LL == 256 ? (Q10V_THREADS / 32) * D * ITEM : 0u;
 };
@@ -800,7 +814,7 @@ __device__ __forceinline__ void q10_pass(const SpK &sp, const Q10Lane<LL> &ln, u
 }
 
 template <uint32_t LL>
-__global__ void __launch_bounds__(Q10V_THREADS, SPEGG_Q10V_MINB) k_gamete_q10v(const __grid_constant__ SpK sp) {
+__global__ void __launch_bounds__(Q10V_THREADS, Q10V_MINB) k_gamete_q10v(const __grid_constant__ SpK sp) {
     using C = Q10V<LL>;
     static_assert(C::NPASS == 1, "L = 256 runs k_gamete_q10r");
     const DevSpecies &st = *sp.st;
@@ -851,7 +865,7 @@ __global__ void __launch_bounds__(Q10V_THREADS, SPEGG_Q10V_MINB) k_gamete_q10v(c
 }
 
 template <uint32_t LL>
-__global__ void __launch_bounds__(Q10V_THREADS, SPEGG_Q10V_MINB256) k_gamete_q10r(const __grid_constant__ SpK sp) {
+__global__ void __launch_bounds__(Q10V_THREADS, Q10V_MINB256) k_gamete_q10r(const __grid_constant__ SpK sp) {
     using C = Q10V<LL>;
     constexpr uint32_t D = C::D;
     extern __shared__ __align__(16) uint8_t s_ring[];
