@@ -438,21 +438,23 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
                 // mutation, selection, compaction and its index in one kernel (the last CTA closes a solo step)
                 k_select_compact<<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
             } else {
-                if (q10v) { k_mut_surv<<<g_thread, 256, 0, s->stream>>>(k); ++nl; }
-                else {
+                const bool patches = s->P > 1;
+                if (q10v && !patches) { k_mut_surv<<<g_thread, 256, 0, s->stream>>>(k); ++nl; }   // (patches: inside k_patch_count)
+                if (!q10v) {
                     k_mutate<<<ctas(cap * 2, 256, 8), 256, 0, s->stream>>>(k, 0); ++nl;
                     k_phenotype<<<g_warp, 256, 0, s->stream>>>(k); ++nl;
                     k_survival<<<g_thread, 256, 0, s->stream>>>(k); ++nl;
                 }
                 if (k.adult_surv > 0.0f) { k_adult_survive<<<g_warp, 256, 0, s->stream>>>(k); ++nl; }   // R18
-                if (s->P == 1) {
+                const bool index_here = patches && k.index_only && k.adult_surv == 0.0f;   // k_patch_pos writes the index itself
+                if (!patches) {
                     k_cmp_scan<<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
                 } else {
-                    k_patch_count<<<std::min(s->P * k.patch_sub, G * 8), 256, 0, s->stream>>>(k); ++nl;
+                    k_patch_count<<<std::min(s->P * k.patch_sub, G * 8), 256, 0, s->stream>>>(k, q10v ? 1 : 0); ++nl;
                     k_patch_base<<<1, 1024, 0, s->stream>>>(k); ++nl;
-                    k_patch_pos<<<std::min(s->P * k.patch_sub, G * 8), 256, 0, s->stream>>>(k); ++nl;
+                    k_patch_pos<<<std::min(s->P * k.patch_sub, G * 8), 256, 0, s->stream>>>(k, index_here ? 1 : 0); ++nl;
                 }
-                k_cmp_scatter<<<(k.index_only && k.adult_surv == 0.0f) ? g_thread : g_warp, 256, 0, s->stream>>>(k); ++nl;
+                if (!index_here) { k_cmp_scatter<<<(k.index_only && k.adult_surv == 0.0f) ? g_thread : g_warp, 256, 0, s->stream>>>(k); ++nl; }
             }
         }
     }

@@ -1466,11 +1466,14 @@ __device__ __forceinline__ void segment_range(uint32_t lo, uint32_t hi, uint32_t
 
 // counts of survivors per (segment, slot); one CTA per segment.  patch_cnt[w][0..4]: surviving
 // offspring by destination slot; [5]: staying adults (R18)
-__global__ void __launch_bounds__(256) k_patch_count(const __grid_constant__ SpK sp) {
+// select = 1 (production q10 path): the segment's offspring are mutated and selected HERE (a4 + a6: what
+// k_mut_surv does), so alive[] is produced by the kernel that counts it
+__global__ void __launch_bounds__(256) k_patch_count(const __grid_constant__ SpK sp, int select) {
     __shared__ uint32_t s_cnt[6];
-    const DevSpecies &st = *sp.st;
+    DevSpecies &st = *sp.st;
     const uint32_t *ps = sp.patch_start[st.cur];
-    const uint32_t S = sp.patch_sub;
+    const uint32_t S = sp.patch_sub, step = sp.glob->step;
+    unsigned int ties = 0, caps = 0;
     for (uint32_t w = blockIdx.x; w < sp.P * S; w += gridDim.x) {
         const uint32_t p = w / S, sg = w % S;
         if (threadIdx.x < 6) s_cnt[threadIdx.x] = 0;
@@ -1480,12 +1483,20 @@ __global__ void __launch_bounds__(256) k_patch_count(const __grid_constant__ SpK
         segment_range(j0, j1, sg, S, jj0, jj1);
         const uint4 nb = ((const uint4 *)sp.nbr)[p];
         uint32_t c[5] = {0, 0, 0, 0, 0};
-        for (uint32_t j = jj0 + threadIdx.x; j < jj1; j += blockDim.x)
-            if (sp.alive[j]) {
+        for (uint32_t j = jj0 + threadIdx.x; j < jj1; j += blockDim.x) {
+            bool al;
+            if (select) {
+                const int d = mutate_one(sp, j, 0, step) + mutate_one(sp, j, 1, step);
+                int32_t zi = sp.zi[j];
+                if (d) { zi += d; sp.zi[j] = zi; }
+                al = survive_one(sp, st, j, zi, step, ties, caps);
+            } else al = sp.alive[j] != 0;
+            if (al) {
                 const uint32_t sl = dest_slot(p, sp.dest[j], nb);
 #pragma unroll
                 for (uint32_t k = 0; k < 5; ++k) c[k] += (sl == k) ? 1u : 0u;
             }
+        }
         uint32_t ca = 0;
         if (sp.adult_surv > 0.0f) {   // R18: the adults of the segment that stay
             uint32_t i0, i1;
@@ -1503,6 +1514,8 @@ __global__ void __launch_bounds__(256) k_patch_count(const __grid_constant__ SpK
         if (threadIdx.x < 6) sp.patch_cnt[w * 6 + threadIdx.x] = s_cnt[threadIdx.x];
         __syncthreads();
     }
+    if (ties) atomicAdd(&st.near_ties, (unsigned long long)ties);
+    if (caps) atomicAdd(&st.captures, (unsigned long long)caps);
 }
 
 // next patch_start and the base position of every (segment, slot) group.  The next generation's order
@@ -1556,11 +1569,16 @@ __global__ void __launch_bounds__(1024) k_patch_base(const __grid_constant__ SpK
 }
 
 // positions of the survivors of each segment (j order within each slot) + reductions
-__global__ void __launch_bounds__(256) k_patch_pos(const __grid_constant__ SpK sp) {
+// index = 1 (index-only compaction, discrete generations): rowptr[position] = j (and the sex / genetic
+// value that travel with the row) are written here, so no k_cmp_scatter follows
+__global__ void __launch_bounds__(256) k_patch_pos(const __grid_constant__ SpK sp, int index) {
     __shared__ uint32_t s_w[8][5];
     __shared__ uint32_t s_run[5];
     DevSpecies &st = *sp.st;
     const uint32_t *ps = sp.patch_start[st.cur];
+    uint32_t *rp = sp.rowptr[st.cur ^ 1u];
+    uint8_t *sex_next = sp.sex[st.cur ^ 1u];
+    int32_t *zrow_next = sp.zrow[st.cur ^ 1u];
     const uint32_t S = sp.patch_sub;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     long long a1 = 0, a2 = 0;
@@ -1587,9 +1605,11 @@ __global__ void __launch_bounds__(256) k_patch_pos(const __grid_constant__ SpK s
             if (al) {
                 uint32_t o = s_run[slot] + rank;
                 for (uint32_t w = 0; w < warp; ++w) o += s_w[w][slot];
-                sp.pos[j] = o;
-                const long long z = sp.zi[j]; a1 += z; a2 += z * z;
-            } else if (j < jj1) sp.pos[j] = 0xFFFFFFFFu;
+                const int32_t zj = sp.zi[j];
+                if (index) { rp[o] = j; if (sp.sexes) sex_next[j] = sp.sex_off[j]; if (sp.zrow_on) zrow_next[j] = zj; }
+                else sp.pos[j] = o;
+                const long long z = zj; a1 += z; a2 += z * z;
+            } else if (j < jj1 && !index) sp.pos[j] = 0xFFFFFFFFu;
             __syncthreads();
             if (tid < 5) { uint32_t t = 0; for (int w = 0; w < 8; ++w) t += s_w[w][tid]; s_run[tid] += t; }
             __syncthreads();
