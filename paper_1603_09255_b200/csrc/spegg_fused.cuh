@@ -165,6 +165,7 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
     // the ticket's addend, 1, read back from shared memory: a value ptxas can prove neither constant nor
     // uniform (a constant or uniform addend is what it aggregates)
     s_one[threadIdx.x] = 1u;
+    __syncwarp();   // (the partner lane's store)
     const uint32_t one = ((volatile uint32_t *)s_one)[threadIdx.x ^ 1u];
 
     // mo / fa are the parents' physical ROW numbers exactly as loaded: nothing here depends on the
