@@ -85,3 +85,26 @@ def test_no_library_dependencies_on_thrust_cub_or_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_1603_09255_b200", txt, re.M), f
             assert not re.search(r"#include\s*\"[^\"]*spegg_(device|internal|kernels|fused)", txt), f
+
+
+def test_bench_workloads_and_variants_validate(binding):
+    """bench.py's workloads (every configuration, every --variant, the sweep sizes of the NEXT-4 series
+    and --k-scale) are accepted by the library's validation (host logic only: spegg_workspace_bytes)."""
+    import bench
+    try:
+        for which in (1, 2, 3, 4, 5, 6):
+            for variant in sorted(bench.VARIANTS):
+                if variant == "encounters" and which != 4:
+                    continue
+                cfg = bench.workload(which, variant=variant)
+                assert binding.workspace_bytes(cfg) > 0, (which, variant)
+        for patches, per in ((1, 50_000), (100, 50_000), (10_000, 1_000)):
+            bench.SWEEP.update(patches=patches, per_patch=per)
+            cfg = bench.workload(6, variant="overlap")
+            assert cfg["grid"] == (patches, 1) and cfg["n0"][0] == patches * per
+            assert binding.workspace_bytes(cfg) > 0
+        bench.SWEEP.update(patches=16, per_patch=50_000, k_scale=0.5)
+        cfg = bench.workload(3)
+        assert cfg["species"][0]["K"] == 500_000.0 and "K x 0.5" in cfg["name"]
+    finally:
+        bench.SWEEP.update(patches=16, per_patch=50_000, k_scale=1.0)
