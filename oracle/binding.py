@@ -45,7 +45,7 @@ class _SpeciesParams(C.Structure):
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
         ("mate_skew", C.c_double), ("encounters", C.c_uint32), ("separate_sexes", C.c_uint32),
-        ("fec_cost", C.c_double), ("assort", C.c_double), ("mother_skew", C.c_double),
+        ("fec_cost", C.c_double), ("assort", C.c_double), ("mother_skew", C.c_double), ("monogamy", C.c_uint32),
     ]
 
 
@@ -240,6 +240,7 @@ class Oracle:
             p.fec_cost = sp.get("fec_cost", 0.0)
             p.assort = sp.get("assort", 0.0)
             p.mother_skew = sp.get("mother_skew", 0.0)
+            p.monogamy = 1 if sp.get("monogamy") else 0
             if sp["kind"] == "bit":
                 self.row_shape.append(2 * (L // 32))
                 self.row_dtype.append(np.uint32)

@@ -63,7 +63,7 @@ void philox(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4]) {
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-enum Stream { FEC = 0, SCALAR = 1, RECOMB_M = 2, RECOMB_P = 3, MUT_M = 4, MUT_P = 5, MATE = 6, MOTHER = 7 };
+enum Stream { FEC = 0, SCALAR = 1, RECOMB_M = 2, RECOMB_P = 3, MUT_M = 4, MUT_P = 5, MATE = 6, MOTHER = 7, PAIR = 8 };
 const uint32_t ASSORT_TRIES = 8; /* R23 */
 
 /* R3: key = (seed_lo, seed_hi); counter = (entity, block, step, species<<8 | stream) */
@@ -535,17 +535,25 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
                 D.mother[j] = mo;
             }
         }
-        uint32_t fa = base + uniform_index(x[0], np);
+        /* R25 ("monogamy or polygynandry"): with monogamy the father's draws are addressed by
+         * the MOTHER (stream PAIR, entity = her adult index: block 0 word 0 = the uniform index of R2,
+         * words 2,3 = the 64-bit uniform of R19/R21, blocks 1.. = R23's candidates), so all the eggs of
+         * one mother in one step have one father; otherwise by the egg (SCALAR / MATE, entity j). */
+        const bool mono = S.p.monogamy != 0;
+        uint32_t xp[4] = {0, 0, 0, 0};
+        if (mono) draw(sim.seed, si, PAIR, mo, 0, t, xp);
+        uint32_t fa = base + uniform_index(mono ? xp[0] : x[0], np);
         if (mate_on) {
             /* R19: weighted draw among the adults of the mother's patch by running sum + search:
-             * total = weight of the patch; 64-bit uniform from words 2,3 of SCALAR block 1;
-             * target = floor(u * total / 2^64); father = first adult whose inclusive running sum
+             * total = weight of the patch; 64-bit uniform from words 2,3 of SCALAR block 1 (R25: of PAIR
+             * block 0); target = floor(u * total / 2^64); father = first adult whose inclusive running sum
              * exceeds (running sum before the patch) + target.  A patch of total weight 0 keeps R2. */
             const uint64_t before = base ? D.mate_cum[base - 1] : 0;
             const uint64_t total = D.mate_cum[base + np - 1] - before;
             if (total > 0) {
                 uint32_t y[4];
-                draw(sim.seed, si, SCALAR, (uint32_t)j, 1, t, y);
+                if (mono) { y[2] = xp[2]; y[3] = xp[3]; }
+                else draw(sim.seed, si, SCALAR, (uint32_t)j, 1, t, y);
                 const uint64_t u = ((uint64_t)y[2] << 32) | y[3];
                 const uint64_t target = before + (uint64_t)(((unsigned __int128)u * total) >> 64);
                 /* first index in the patch with mate_cum > target (library binary search) */
@@ -554,14 +562,16 @@ void step_species(orc_sim &sim, uint32_t si, const std::vector<uint64_t> &N0,
         }
         if (S.p.assort > 0.0) {
             /* R23 (assortative mating): candidate t = 0..7, uniform over the adults of the
-             * mother's patch (word 2(t%2) of MATE block t/2, entity j), is accepted iff
-             * u01(word 2(t%2)+1) < expf_spec(-(a * (d*d))), d = z_cand - z_mother (genetic values, fp32,
-             * this order); the first accepted candidate is the father, else the last candidate. */
+             * mother's patch (word 2(t%2) of MATE block t/2, entity j; R25: of PAIR block 1 + t/2, entity
+             * the mother), is accepted iff u01(word 2(t%2)+1) < expf_spec(-(a * (d*d))), d = z_cand -
+             * z_mother (genetic values, fp32, this order); the first accepted candidate is the father,
+             * else the last candidate. */
             const float a = (float)S.p.assort;
             const float zm = (float)S.zi[mo] * S.p.pheno_scale;
             for (uint32_t tr = 0; tr < ASSORT_TRIES; ++tr) {
                 uint32_t y[4];
-                draw(sim.seed, si, MATE, (uint32_t)j, tr / 2, t, y);
+                if (mono) draw(sim.seed, si, PAIR, mo, 1 + tr / 2, t, y);
+                else draw(sim.seed, si, MATE, (uint32_t)j, tr / 2, t, y);
                 fa = base + uniform_index(y[2 * (tr & 1)], np);
                 const float d = (float)S.zi[fa] * S.p.pheno_scale - zm;
                 const float p = expf_spec(-(a * (d * d)));
@@ -813,6 +823,7 @@ orc_sim *orc_create(const orc_params *p) {
         if (!(S.p.assort >= 0.0 && S.p.assort <= 1e6) || (S.p.assort > 0.0 && (S.p.mate_skew != 0.0 || S.p.separate_sexes))) { delete sim; return nullptr; }
         if (!(std::fabs(S.p.mate_skew) <= 1e6) || !(S.p.fec_cost >= 0.0 && S.p.fec_cost <= 1e6)) { delete sim; return nullptr; }
         if (!(std::fabs(S.p.mother_skew) <= 1e6) || (S.p.mother_skew != 0.0 && (S.p.fec_cost > 0.0 || S.p.fecundity_model == ORC_FEC_CAPTURES))) { delete sim; return nullptr; }
+        if (S.p.monogamy > 1) { delete sim; return nullptr; }
         if (S.p.encounters > 16 || (S.p.encounters && (!S.p.sel_predation || !(S.p.attack >= 0.0 && S.p.attack <= 2.0)))) { delete sim; return nullptr; }
         if (!(S.p.adult_survival >= 0.0 && S.p.adult_survival <= 1.0)) { delete sim; return nullptr; }
         if (S.p.resid_sd > 0.0) {

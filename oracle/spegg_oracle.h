@@ -3,7 +3,7 @@
  *
  * TEST INFRASTRUCTURE ONLY.  This is the plain, slow, single-threaded, obviously
  * correct restatement of what the hot path computes (Fig. 1 A-F;
- * PAPER.md:321-330 genetics; the readings R1-R24 in DESIGN.md).  Only tests/,
+ * PAPER.md:321-330 genetics; the readings R1-R25 in DESIGN.md).  Only tests/,
  * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load it.  It shares no code, header, table or constant generator with the CUDA
  * library (include/spegg.h, paper_1603_09255_b200/csrc/): the structs below are
@@ -82,6 +82,11 @@ typedef struct {
                                    v_f = mother_skew; the NUMBER of eggs of the patch stays the sum of the
                                    Poisson fecundities (R5).  0 = every adult mothers its own eggs (R1);
                                    not together with fec_cost or the CAPTURES fecundity model     */
+    uint32_t monogamy;          /* R25 ("monogamy or polygynandry"): 1 = within a time step every
+                                   mother has ONE mate -- the father of all her eggs is drawn once, by the
+                                   rule in force (R2 uniform, R19 / R21 weighted, R23 assortative), on the
+                                   words of stream PAIR addressed by the MOTHER; 0 = every egg draws its
+                                   father independently (polygynandry: R2, R19, R21, R23 as they stand) */
 } orc_species_params;
 
 typedef struct {
