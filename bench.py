@@ -99,6 +99,7 @@ VARIANTS = {
     "encounters": {},                                  # R20 (configuration 4 only: 3 meetings, attack 0.1)
     "cost": {"fec_cost": 0.05},                        # R22
     "mothers": {"mother_skew": 1.0},                   # R24
+    "monogamy": {"monogamy": 1},                       # R25
 }
 
 

@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SPEGG_ABI_VERSION 8u
+#define SPEGG_ABI_VERSION 9u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
        SPEGG_ESTATE = -5 };
@@ -130,6 +130,10 @@ typedef struct spegg_species_params {
                                    father of R19; the NUMBER of eggs of a patch stays the sum of its
                                    adults' Poisson fecundities.  0 = every adult mothers its own eggs.
                                    |v_f| <= 1e6; not with fec_cost or SPEGG_FEC_CAPTURES          */
+    uint32_t monogamy;          /* 1: within a time step every mother has ONE mate ("monogamy or polygynandry",
+                                   PAPER.md:54; R25): the father of all her eggs is drawn once, by the
+                                   rule in force (uniform, mate_skew, separate_sexes, assort), on draws
+                                   addressed by the mother.  0 = every egg draws its father (polygynandry) */
 } spegg_species_params;
 
 typedef struct spegg_params {

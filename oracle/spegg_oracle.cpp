@@ -16,7 +16,7 @@
  *   PAPER.md:56,170,182 overlapping generations, maximum per-step survivorship 0.975 (R18)
  *   PAPER.md:54, 273-283 (eqs. S2-9, S2-10) mating systems, weighted mothers and fathers (R19, R21, R23, R24)
  *   PAPER.md:464-475 (eqs. S3-1..S3-3) individual encounters, fecundity cost of defence (R20, R22)
- *   DESIGN.md "Readings" R1-R24 for everything the paper leaves open.
+ *   DESIGN.md "Readings" R1-R25 for everything the paper leaves open.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors, exp
  * specs vs libm, Poisson/normal table moments, brute-force gamete enumeration at
@@ -27,7 +27,7 @@
  * of R14; the trait reading X = exp(z) of R19 / R24 (the paper's X is irreversible mass, G/Omega
  * gonadal over neonate mass); R20's replacement of the S3-1/S3-2 integrals by E uniform meetings;
  * R23's acceptance kernel exp(-a d^2) and its cap of 8 candidates (the paper gives the word
- * "assortative" only).
+ * "assortative" only); R25's pairing rule (the word "monogamy" only).
  *
  * Build: g++ -O2 -ffp-contract=off -shared -fPIC (fp contraction OFF: every fp
  * value that feeds an integer decision is a stated sequence of IEEE +,-,*,/ ops).

@@ -18,7 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ERANGE, ESTATE = 0, -1, -2, -3, -4, -5
 FLAG_OVERFLOW, FLAG_EXTINCT = 1, 2
 
 
-ABI_VERSION = 8   # SPEGG_ABI_VERSION of include/spegg.h
+ABI_VERSION = 9   # SPEGG_ABI_VERSION of include/spegg.h
 
 
 class SpeciesParams(C.Structure):
@@ -34,7 +34,7 @@ class SpeciesParams(C.Structure):
         ("attack", C.c_double), ("predator_species", C.c_uint32), ("migration", C.c_double),
         ("capacity", C.c_uint64), ("resid_sd", C.c_double), ("adult_survival", C.c_double),
         ("mate_skew", C.c_double), ("encounters", C.c_uint32), ("separate_sexes", C.c_uint32),
-        ("fec_cost", C.c_double), ("assort", C.c_double), ("mother_skew", C.c_double),
+        ("fec_cost", C.c_double), ("assort", C.c_double), ("mother_skew", C.c_double), ("monogamy", C.c_uint32),
     ]
 
 
@@ -154,6 +154,7 @@ def make_params(cfg, debug=False, log_capacity=0):
         p.fec_cost = sp.get("fec_cost", 0.0)
         p.assort = sp.get("assort", 0.0)
         p.mother_skew = sp.get("mother_skew", 0.0)
+        p.monogamy = int(sp.get("monogamy") or 0)
         p.fecundity_model, p.fec_a, p.K = _FEC[sp["fecundity"]], sp["fec_a"], sp["K"]
         if sp.get("K_patch") is not None:
             kp = np.ascontiguousarray(sp["K_patch"], dtype=np.float64)

@@ -199,6 +199,7 @@ int validate(const spegg_params *p) {
         if (!(q.fec_cost >= 0.0 && q.fec_cost <= 1e6)) return SPEGG_EINVAL;
         if (!(q.assort >= 0.0 && q.assort <= 1e6) || (q.assort > 0.0 && (q.mate_skew != 0.0 || q.separate_sexes))) return SPEGG_EINVAL;
         if (q.fecundity_model == SPEGG_FEC_CAPTURES && P != 1) return SPEGG_EINVAL;
+        if (q.monogamy > 1) return SPEGG_EINVAL;
         if (!(std::fabs(q.mother_skew) <= 1e6) || (q.mother_skew != 0.0 && (q.fec_cost > 0.0 || q.fecundity_model == SPEGG_FEC_CAPTURES))) return SPEGG_EINVAL;
         if (q.sel_predation) {
             if (q.predator_species >= p->n_species || q.predator_species <= s) return SPEGG_EINVAL;
@@ -361,7 +362,7 @@ int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
 
 // true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
 bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
-    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.sexes || h.k.fec_cost != 0.0f || h.k.assort != 0.0f || h.k.mom_v != 0.0f) return false;   // (mate_on without sexes = R19: the MATE instantiation)
+    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.sexes || h.k.fec_cost != 0.0f || h.k.assort != 0.0f || h.k.mom_v != 0.0f || h.k.monogamy) return false;   // (mate_on without sexes = R19: the MATE instantiation)
     // k_fused_bit_f<4, 8> places chromosome c at words 8c .. 8c+7 and packs crossover positions in 9 bits:
     // four chromosomes of exactly 256 loci (other splits of 1,024 loci run the general pipeline)
     for (uint32_t c = 0; c < h.p.n_chrom; ++c)
@@ -634,6 +635,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.sex[0] = at<uint8_t>(s, l.sex[0]); k.sex[1] = at<uint8_t>(s, l.sex[1]); k.sex_off = at<uint8_t>(s, l.sex_off);
         k.mate_cum = at<unsigned long long>(s, l.mate_cum); k.mate_tile = at<unsigned long long>(s, l.mate_tile);
         k.mom_v = (float)q.mother_skew;
+        k.monogamy = q.monogamy;
         k.mom_cum = at<unsigned long long>(s, l.mom_cum); k.mom_tile = at<unsigned long long>(s, l.mom_tile);
         k.fec_cost = (float)q.fec_cost; k.assort = (float)q.assort;
         k.enc_E = q.sel_predation ? q.encounters : 0u; k.enc_v = (float)q.attack;

@@ -10,7 +10,7 @@
 
 namespace spegg {
 
-enum Stream : uint32_t { ST_FEC = 0, ST_SCALAR = 1, ST_RECOMB_M = 2, ST_RECOMB_P = 3, ST_MUT_M = 4, ST_MUT_P = 5, ST_MATE = 6, ST_MOTHER = 7 };
+enum Stream : uint32_t { ST_FEC = 0, ST_SCALAR = 1, ST_RECOMB_M = 2, ST_RECOMB_P = 3, ST_MUT_M = 4, ST_MUT_P = 5, ST_MATE = 6, ST_MOTHER = 7, ST_PAIR = 8 };
 
 // ---------------------------------------------------------------------------------- Philox
 // Salmon et al. SC'11. One round: two 32x32->64 products, two 3-input XORs; key += Weyl.

@@ -111,6 +111,7 @@ struct SpK {
     unsigned long long *mate_cum;   // [n] inclusive running sum of the weights, adult order
     unsigned long long *mate_tile;  // [n / MATE_TILE + 2] weight of each tile of MATE_TILE adults
     uint32_t mate_on;           // 1: the father comes from the running sum (mate_v != 0 or separate sexes)
+    uint32_t monogamy;          // R25: 1 = the father's draws are addressed by the mother (one mate per mother per step)
     // R24, mothers drawn by relative fecundity (mom_v != 0): integer mothering weights of the current adults
     float mom_v;                // v_f as fp32; 0 = every adult mothers its own eggs
     unsigned long long *mom_cum;    // [n] inclusive running sum, adult order

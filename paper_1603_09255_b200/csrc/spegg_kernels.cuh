@@ -239,7 +239,7 @@ __device__ __forceinline__ void solo_tail(const SpK &sp, uint32_t *s_flag) {
 // these two dependent loads over several offspring)
 __device__ __forceinline__ void scalar_one(const SpK &sp, uint32_t j, uint32_t pm, uint32_t base, uint32_t np, uint32_t step,
                                            unsigned int &ties) {
-    uint32_t mo = (sp.mom_v != 0.0f || sp.assort > 0.0f) ? sp.mother[j] : 0u;   // (only those two read it)
+    uint32_t mo = (sp.mom_v != 0.0f || sp.assort > 0.0f || sp.monogamy) ? sp.mother[j] : 0u;   // (only those read it)
     uint32_t x[4];
     draw(sp.key, sp.species, ST_SCALAR, j, 0, step, x);
     if (sp.mom_v != 0.0f) {
@@ -262,7 +262,12 @@ __device__ __forceinline__ void scalar_one(const SpK &sp, uint32_t j, uint32_t p
             sp.mother[j] = mo;
         }
     }
-    uint32_t fa = base + uniform_index(x[0], np);
+    // R25 ("monogamy or polygynandry"): with monogamy the father's draws are addressed by the
+    // MOTHER (stream PAIR, entity = her adult index: block 0 word 0 = R2's index, words 2,3 = R19's uniform,
+    // blocks 1.. = R23's candidates), so all the eggs of one mother in one step have one father
+    uint32_t xp[4] = {0u, 0u, 0u, 0u};
+    if (sp.monogamy) draw_rk(sp, ST_PAIR, mo, 0, step, xp);
+    uint32_t fa = base + uniform_index(sp.monogamy ? xp[0] : x[0], np);
     if (sp.mate_on) {
         // R19: weighted draw among the adults of the mother's patch: 64-bit uniform from words 2,3 of
         // SCALAR block 1, target = floor(u * total / 2^64), father = first adult of the patch whose
@@ -271,7 +276,8 @@ __device__ __forceinline__ void scalar_one(const SpK &sp, uint32_t j, uint32_t p
         const unsigned long long total = sp.mate_cum[base + np - 1] - before;
         if (total) {
             uint32_t y[4];
-            draw_rk(sp, ST_SCALAR, j, 1, step, y);
+            if (sp.monogamy) { y[2] = xp[2]; y[3] = xp[3]; }
+            else draw_rk(sp, ST_SCALAR, j, 1, step, y);
             const unsigned long long u = ((unsigned long long)y[2] << 32) | y[3];
             const unsigned long long target = before + __umul64hi(u, total);
             uint32_t lo = base, hi = base + np - 1;   // first index with mate_cum > target; exists since target < before + total
@@ -289,7 +295,10 @@ __device__ __forceinline__ void scalar_one(const SpK &sp, uint32_t j, uint32_t p
         const float zm = __fmul_rn((float)sp.enc_zi[mo], sp.pheno_scale);
         uint32_t y[4];
         for (uint32_t tr = 0; tr < ASSORT_TRIES; ++tr) {
-            if ((tr & 1u) == 0) draw_rk(sp, ST_MATE, j, tr >> 1, step, y);
+            if ((tr & 1u) == 0) {
+                if (sp.monogamy) draw_rk(sp, ST_PAIR, mo, 1u + (tr >> 1), step, y);
+                else draw_rk(sp, ST_MATE, j, tr >> 1, step, y);
+            }
             fa = base + uniform_index(y[2 * (tr & 1u)], np);
             const float d = __fsub_rn(__fmul_rn((float)sp.enc_zi[fa], sp.pheno_scale), zm);
             const float p = expf_spec(-__fmul_rn(sp.assort, __fmul_rn(d, d)));

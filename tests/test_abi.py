@@ -45,7 +45,7 @@ def test_struct_sizes_match_header(binding):
     # spegg_create checks struct_size; mirror the arithmetic of the C layout here
     assert C.sizeof(binding.LogEntry) == 64
     assert C.sizeof(binding.Params) == 48
-    assert C.sizeof(binding.SpeciesParams) == 232   # + resid_sd, adult_survival (version 2), mate_skew (3), encounters (4), separate_sexes (5), fec_cost (6), assort (7), mother_skew (8)
+    assert C.sizeof(binding.SpeciesParams) == 240   # + resid_sd, adult_survival (version 2), mate_skew (3), encounters (4), separate_sexes (5), fec_cost (6), assort (7), mother_skew (8), monogamy (9)
 
 
 def test_workspace_bytes_and_validation(binding):

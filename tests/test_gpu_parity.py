@@ -797,3 +797,34 @@ def test_fused_path_weighted_father(oracle_mod, binding, scale, v, extra):
     sim.close()
     parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=False)
     _free_run(oracle_mod, binding, cfg, 6, chunks=2, fused=None)
+
+
+@pytest.mark.parametrize("which,scale,grid,extra", [
+    (1, 1.0, None, {}),                                                    # C1: uniform mate, one per mother
+    (2, 0.05, None, {"mate_skew": 1.5}),                                   # the pair drawn by R19's weights
+    (5, 0.03, (5, 4), {"separate_sexes": 1}),                              # patches + sexes: one male per female per step
+    (2, 0.04, None, {"assort": 2.0, "adult_survival": 0.6}),               # assortative pairs, staying mothers re-pair every step
+    (3, 0.012, None, {"mother_skew": 1.0}),                                # bit genome (general pipeline); the pair belongs to the DRAWN mother
+])
+def test_monogamy(oracle_mod, binding, which, scale, grid, extra):
+    """R25 ("monogamy or polygynandry"): the father's draws are addressed by the mother, so a
+    clutch has one father.  Per-step parity of every intermediate (debug), per-step parity on the
+    production kernels, then a free-running trajectory."""
+    cfg = workloads.config(which, scale=scale, grid=grid)
+    sp = cfg["species"][0]
+    sp["monogamy"] = 1
+    sp.update(extra)
+    if "adult_survival" in extra:
+        sp["capacity"] = 4 * sp["capacity"]
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=True)
+    parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=False)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    orc.step(8)
+    sim.step(8)
+    parity.assert_logs_equal(sim.read_log(0), orc.log(0))
+    parity.assert_state_equal(sim, orc, cfg)
+    assert sim.status() == orc.flags
+    sim.close()
