@@ -828,3 +828,78 @@ def test_monogamy(oracle_mod, binding, which, scale, grid, extra):
     parity.assert_state_equal(sim, orc, cfg)
     assert sim.status() == orc.flags
     sim.close()
+
+
+def _random_cfg(rng):
+    """A random small configuration: genome, structure and a random subset of the widenings that the
+    validation accepts together (seeded; the combinations no hand-written case lists)."""
+    grid = [None, None, (2, 1), (3, 2), (4, 4)][rng.integers(0, 5)]
+    kind = "q10" if (grid is not None or rng.random() < 0.7) else "bit"
+    if kind == "bit":
+        cfg = workloads.config(3, scale=float(rng.choice([0.002, 0.004, 0.0065])))
+        sp = cfg["species"][0]
+        if rng.random() < 0.5:
+            sp["xover_mean"] = [float(x) for x in rng.choice([0.0, 0.3, 1.0, 2.5], size=4)]
+        sp["mu"] = float(rng.choice([0.0, 1e-5, 1e-3]))
+    else:
+        which = 5 if grid is not None else int(rng.choice([1, 2]))
+        scale = {1: float(rng.choice([0.5, 1.0, 2.5])), 2: float(rng.choice([0.01, 0.03])), 5: float(rng.choice([0.05, 0.2, 0.8]))}[which]
+        cfg = workloads.config(which, scale=scale, grid=grid)
+        sp = cfg["species"][0]
+        L = int(rng.choice([8, 16, 32, 64, 128, 256, 24]))
+        nch = int(rng.choice([1, 2, 4])) if L % 4 == 0 and L >= 8 else 1
+        cl = [L // nch] * nch
+        cl[-1] += L - sum(cl)
+        sp.update(n_loci=L, chrom_len=cl, r=workloads._interval_r(cl, float(rng.choice([0.01, 0.1, 0.5]))),
+                  mu=float(rng.choice([0.0, 1e-3, 2e-2])))
+    sp = cfg["species"][0]
+    cfg["seed"] = int(rng.integers(1, 2 ** 62))
+    wid = {}
+    if rng.random() < 0.35:
+        wid["resid_sd"] = float(rng.choice([0.1, 0.5]))
+    if rng.random() < 0.35:
+        wid["adult_survival"] = float(rng.choice([0.3, 0.8]))
+    mating = rng.integers(0, 5)            # none / R19 / R21 (+R19) / R23 / R19 both signs
+    if mating == 1:
+        wid["mate_skew"] = float(rng.choice([-2.0, 1.0, 50.0]))
+    elif mating == 2:
+        wid["separate_sexes"] = 1
+        if rng.random() < 0.5:
+            wid["mate_skew"] = 1.0
+    elif mating == 3:
+        wid["assort"] = float(rng.choice([0.5, 4.0]))
+    if rng.random() < 0.3:
+        wid["mother_skew"] = float(rng.choice([-1.0, 1.5]))
+    elif rng.random() < 0.25:
+        wid["fec_cost"] = float(rng.choice([0.05, 0.5]))
+    if rng.random() < 0.3:
+        wid["monogamy"] = 1
+    if rng.random() < 0.3:
+        sp["gaussian"]["dtheta"] = 0.02
+    sp.update(wid)
+    if "separate_sexes" in wid:
+        sp["fec_a"] = 2.0 * sp["fec_a"]
+    sp["capacity"] = (8 if "adult_survival" in wid else 2) * sp["capacity"]
+    return cfg, wid
+
+
+@pytest.mark.parametrize("seed", range(60))
+def test_random_configurations(oracle_mod, binding, seed):
+    """Differential test on seeded random combinations of genome, patch structure and widenings:
+    production kernels against the oracle, free-running, state / sexes / log / flags compared after
+    2 and 7 steps; the first step also with every intermediate (debug)."""
+    import numpy as np
+    rng = np.random.default_rng(9000 + seed)
+    cfg, wid = _random_cfg(rng)
+    parity.per_step_parity(oracle_mod, binding, cfg, 1, debug=True)
+    orc = oracle_mod.Oracle(cfg)
+    sim = binding.Sim(cfg, debug=False)
+    parity.load_initial(orc, cfg)
+    parity.load_initial(sim, cfg)
+    for n in (2, 5):
+        orc.step(n)
+        sim.step(n)
+        parity.assert_logs_equal(sim.read_log(0), orc.log(0), tag=str((seed, wid)))
+        parity.assert_state_equal(sim, orc, cfg, tag=str((seed, wid)))
+    assert sim.status() == orc.flags
+    sim.close()
