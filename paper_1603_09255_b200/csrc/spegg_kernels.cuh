@@ -1,17 +1,18 @@
 // spegg_kernels.cuh -- the step pipeline of libspegg as separate kernels (sm_100a).
 //
-// One time step of one species (Fig. 1 A-F) is the sequence
-//   k_prepare_all  a0  derived parameters: fecundity tables from device-resident counts, theta_t
-//   k_fec_scan     a1-a3  Poisson fecundity, single-pass decoupled look-back scan, mother fill
-//   k_scalar       a3  father (uniform mate), dispersal, survival uniform
-//   k_gamete_*     a4  recombination (bit: Poisson crossovers; q10: per-interval draws)
-//   k_mutate       a4  sparse mutation
-//   k_phenotype    a5  additive map, exact integers
-//   k_survival     a6  fp32 survival probability, decision, captures
-//   k_cmp_* / k_patch_*  a7-a8  stable compaction into the other buffer + reductions
-//   k_finish_all   a9  counts stay on the device; log entry; buffer flip
-// This file is the general ("materialised") pipeline that serves every configuration and the
-// debug view; spegg_fused.cuh holds the fused single-pass kernels of the hot configurations.
+// One time step of one species (Fig. 1 A-F) on the production path is
+//   [k_enc_zi, k_mate_weight, k_mate_scan]  adults' genetic values / parental weights, when a widening needs them
+//   k_fec_scan        a1-a3  Poisson fecundity, single-pass look-back scan, mothers, then the scalar draws
+//                            (father, weighted parents, dispersal, survival uniform, sex) of the range's offspring
+//   k_gamete_q10v/r   a4-a5  per-interval recombination, select, phenotype (register prefetch / cp.async ring)
+//   k_select_compact  a4-a8  unstructured species: mutation, selection, scan, look-back, index -- one kernel
+//   k_patch_count / k_patch_base / k_patch_pos  a4-a8  patch mode: mutation + selection + counts per
+//                            segment, one flat exclusive scan, positions + index
+//   [k_adult_survive, k_cmp_scan, k_cmp_scatter]  overlapping generations: the adults that stay
+//   k_finish_all / k_prepare_all  a9, a0  (or the last CTA of the step's last kernel for a solo species)
+// and, for debug mode (every intermediate materialised) and genomes the fast kernels do not cover,
+// the plain kernels k_gamete_bit / k_gamete_q10, k_mutate, k_phenotype, k_survival, k_cmp_scan,
+// k_cmp_scatter.  spegg_fused.cuh holds the fused two-kernel step of the hot configuration.
 // All grids are fixed at graph-capture time and loop against device-side counts.
 #pragma once
 #include <algorithm>
