@@ -287,7 +287,7 @@ uint64_t layout(const spegg_params *p, std::vector<SpeciesLayout> &out) {
         l.tables = c.take((uint64_t)l.n_tables * TMAX * 4);
         l.table_len = c.take((uint64_t)l.n_tables * 4);
         l.status_fec = c.take((cap / SCAN_THREADS + 2 + (cap / SCAN_THREADS + 2) / 32 + 2) * 8);
-        l.status_cmp = c.take((cap / SCAN_TILE + 2 + (cap / SCAN_TILE + 2) / 32 + 2) * 8);
+        l.status_cmp = c.take((cap / SCAN_THREADS + 2 + (cap / SCAN_THREADS + 2) / 32 + 2) * 8);   // (tiles of 256 for small populations)
         const uint64_t PS = P * patch_sub_of(cap, P);
         l.patch_cnt = c.take(PS * 6 * 4);
         l.patch_base = c.take(PS * 6 * 4);
@@ -437,7 +437,9 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             }
             if (q10v && s->P == 1 && k.adult_surv == 0.0f) {
                 // mutation, selection, compaction and its index in one kernel (the last CTA closes a solo step)
-                k_select_compact<<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k); ++nl;
+                if (cap <= (uint64_t)G * 4 * SCAN_THREADS) k_select_compact<1><<<ctas(cap, SCAN_THREADS, 4), SCAN_THREADS, 0, s->stream>>>(k);
+                else k_select_compact<SCAN_ITEMS><<<ctas(cap, SCAN_TILE, 4), SCAN_THREADS, 0, s->stream>>>(k);
+                ++nl;
             } else {
                 const bool patches = s->P > 1;
                 if (q10v && !patches) { k_mut_surv<<<g_thread, 256, 0, s->stream>>>(k); ++nl; }   // (patches: inside k_patch_count)
@@ -643,7 +645,7 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
         k.cap = at<uint32_t>(s, l.cap);
         k.tables = at<uint32_t>(s, l.tables); k.table_len = at<uint32_t>(s, l.table_len);
         k.status_fec = at<unsigned long long>(s, l.status_fec); k.status_cmp = at<unsigned long long>(s, l.status_cmp);
-        k.status_fec_n = (uint32_t)(q.capacity / SCAN_THREADS + 2); k.status_cmp_n = (uint32_t)(q.capacity / SCAN_TILE + 2);
+        k.status_fec_n = (uint32_t)(q.capacity / SCAN_THREADS + 2); k.status_cmp_n = (uint32_t)(q.capacity / SCAN_THREADS + 2);
         k.patch_cnt = at<uint32_t>(s, l.patch_cnt); k.patch_base = at<uint32_t>(s, l.patch_base); k.patch_abase = at<uint32_t>(s, l.patch_abase);
         k.nbr = at<uint32_t>(s, l.nbr); k.src_list = at<uint32_t>(s, l.src_list);
         k.patch_sub = patch_sub_of(q.capacity, s->P);

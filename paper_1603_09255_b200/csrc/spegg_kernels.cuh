@@ -1297,14 +1297,19 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cmp_scan(const __grid_constant
 // one look-back, and its survivors' index words are written -- offspring rows stay where the gamete kernel
 // stored them, so nothing else moves.  alive[] / pos[] never travel through memory, and four launches
 // (k_mutate, k_survival, k_cmp_scan, k_cmp_scatter) become one.
+// ITEMS offspring per thread: 4 (tiles of 1,024) for large populations, 1 (tiles of 256) when the whole
+// capacity is fewer tiles than the machine holds CTAs -- a population of 10^5 then spreads over all SMs
+// and a thread's work is one offspring, not a chain of four
+template <int ITEMS>
 __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_constant__ SpK sp) {
+    constexpr uint32_t TILE = SCAN_THREADS * ITEMS;
     __shared__ uint32_t s_warp[SCAN_THREADS / 32];
     __shared__ uint32_t s_tile, s_flag;
     __shared__ unsigned long long s_excl;
-    __shared__ __align__(4) uint8_t s_alive[SCAN_TILE];
+    __shared__ __align__(4) uint8_t s_alive[TILE];
     DevSpecies &st = *sp.st;
     const uint32_t M = st.m, step = sp.glob->step;
-    const uint32_t n_tiles = (M + SCAN_TILE - 1) / SCAN_TILE;
+    const uint32_t n_tiles = (M + TILE - 1) / TILE;
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     uint32_t *rp = sp.rowptr[st.cur ^ 1u];
     uint8_t *sex_next = sp.sex[st.cur ^ 1u];
@@ -1321,24 +1326,24 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_co
         // ---- phase 1, offspring j = tile * 1024 + k * 256 + tid (coalesced): all loads and all mutation-count
         // draws of the thread's four offspring first, so that they travel together; then the rare mutations,
         // selection, and everything that is indexed by j
-        const uint32_t t0 = tile * SCAN_TILE + tid;
-        int32_t zz[SCAN_ITEMS];
-        float uu[SCAN_ITEMS];
-        uint32_t nm[SCAN_ITEMS];
+        const uint32_t t0 = tile * TILE + tid;
+        int32_t zz[ITEMS];
+        float uu[ITEMS];
+        uint32_t nm[ITEMS];
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
+        for (int k = 0; k < ITEMS; ++k) {
             const uint32_t j = t0 + k * SCAN_THREADS;
             zz[k] = 0; uu[k] = 2.0f;
             if (j < M) { zz[k] = sp.zi[j]; uu[k] = sp.u01[j]; }
         }
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
+        for (int k = 0; k < ITEMS; ++k) {
             const uint32_t j = t0 + k * SCAN_THREADS;
             nm[k] = 0;
             if (j < M) nm[k] = mutation_count(sp, j, 0, step) | (mutation_count(sp, j, 1, step) << 16);
         }
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) {
+        for (int k = 0; k < ITEMS; ++k) {
             const uint32_t j = t0 + k * SCAN_THREADS;
             bool al = false;
             if (j < M) {
@@ -1359,8 +1364,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_co
         }
         __syncthreads();
         // ---- phase 2, four consecutive offspring per thread: scan, one look-back, the index
-        const uint32_t base = tile * SCAN_TILE + tid * SCAN_ITEMS;
-        const uint32_t a4 = ((const uint32_t *)s_alive)[tid];   // bytes base .. base + 3
+        const uint32_t base = tile * TILE + tid * ITEMS;
+        const uint32_t a4 = ITEMS == 4 ? ((const uint32_t *)s_alive)[tid] : (uint32_t)s_alive[tid];   // bytes base .. base + ITEMS - 1
         const uint32_t sum = __popc(a4);
         const uint32_t incl = warp_incl_scan(sum);
         if (lane == 31) s_warp[warp] = incl;
@@ -1379,7 +1384,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_co
         __syncthreads();
         uint32_t o = (uint32_t)s_excl + s_warp[warp] + (incl - sum);
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k)
+        for (int k = 0; k < ITEMS; ++k)
             if ((a4 >> (8 * k)) & 1u) rp[o++] = base + k;
         __syncthreads();
     }
