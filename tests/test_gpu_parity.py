@@ -15,6 +15,8 @@ pytestmark = pytest.mark.gpu
 @pytest.fixture(scope="module")
 def binding():
     from paper_1603_09255_b200 import binding as b
+    from paper_1603_09255_b200 import build
+    build.build()          # (re)builds libspegg.so in-tree when missing or older than its sources; raises if nvcc fails
     b.load()
     return b
 
