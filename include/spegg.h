@@ -39,7 +39,8 @@ extern "C" {
 #define SPEGG_ABI_VERSION 9u
 
 enum { SPEGG_OK = 0, SPEGG_EINVAL = -1, SPEGG_ENOMEM = -2, SPEGG_ECUDA = -3, SPEGG_ERANGE = -4,
-       SPEGG_ESTATE = -5 };
+       SPEGG_ESTATE = -5,
+       SPEGG_ELIMIT = -6 };  /* size above the fixed maximum of an entry point that owns no memory */
 
 enum { SPEGG_BIT = 0, SPEGG_Q10 = 1 };                 /* genome_kind                        */
 enum { SPEGG_INTERVAL = 0, SPEGG_POISSON = 1 };        /* linkage_mode (R7 / R8)             */
@@ -271,6 +272,39 @@ int spegg_launches_per_step(const spegg_sim *s, uint32_t *n);
  * events on the stream; read back with the mean duration in milliseconds over the launches since
  * enabling.  For bench.py's roofline figure. */
 int spegg_kernel_timing(spegg_sim *s, int enable, float *mean_ms, uint32_t *n_launches);
+
+/* Largest n spegg_offsets_static accepts: its scratch is a fixed array inside the library image. */
+#define SPEGG_STATIC_MAX_N 4194304ull
+
+/* Fig. 1 A ("the number of neonates are determined"), step a2 on its own and WITHOUT ANY
+ * ALLOCATION: from the fecundities f[0..n) of the adults, the index of each adult's first neonate,
+ * d_off[i] = f[0] + ... + f[i-1] (clamped to 2^32 - 1), and the number of neonates *d_total = sum of f --
+ * the same numbers spegg_step's scan produces (spegg_debug_view.d_off, m_t before capacity truncation).
+ *
+ * Who this is for.  Every other call works inside a workspace the caller allocated.  This one is for
+ * callers that cannot allocate device memory at all at the point of the call: a plug-in running inside
+ * a host application whose own allocator has claimed the GPU, code called back while an allocator lock
+ * is held, a latency-critical loop that cannot afford the device-wide synchronisation cudaMalloc and
+ * cudaFree imply.  The scan needs scratch (look-back status words and a tile ticket); here that scratch
+ * is a fixed array of about 34 KB compiled into libspegg.so, so the call performs no cudaMalloc, no
+ * cudaFree and no allocating library call.  The price: every GPU that loads the library holds those
+ * 34 KB until the process ends, and n is limited to SPEGG_STATIC_MAX_N (4,194,304 adults); a larger n
+ * returns SPEGG_ELIMIT and nothing is launched.
+ *
+ * d_f [n] uint8, d_off [n] uint32 (4-byte aligned), d_total [1] uint64 (8-byte aligned): DEVICE memory of
+ * the device that is CURRENT when the call is made; they stay the caller's and must not overlap.  n = 0
+ * is allowed (d_f, d_off may then be NULL; *d_total = 0).  cuda_stream: a cudaStream_t of that device
+ * (0 = the default stream).  The work is enqueued on the stream and the call returns; results are
+ * ready when the stream reaches that point.  SPEGG_EINVAL for NULL pointers, SPEGG_ECUDA for a CUDA error.
+ *
+ * Two things a caller must know.  (1) The FIRST call on each device looks up the array's device
+ * address (cudaGetSymbolAddress, which may also load the module): make that first call, on every device
+ * you use, before you start capturing a stream.  (2) There is one array per device and every call on
+ * that device uses it, whatever the thread or stream: calls whose GPU work can overlap in time corrupt
+ * each other's results -- put them on one stream or order them with events.  Each call clears the part
+ * of the array it uses before scanning, so consecutive calls do not see each other's leftovers. */
+int spegg_offsets_static(const uint8_t *d_f, uint64_t n, uint32_t *d_off, uint64_t *d_total,
+                         void *cuda_stream);
 
 /* PAPER.md:116 (the species object's lifetime): frees the host struct and the graphs; never frees the
  * caller's workspace or stream.  NULL is allowed. */

@@ -14,7 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libspegg.so")
 TMAX = 128
 
-OK, EINVAL, ENOMEM, ECUDA, ERANGE, ESTATE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMEM, ECUDA, ERANGE, ESTATE, ELIMIT = 0, -1, -2, -3, -4, -5, -6
+STATIC_MAX_N = 4194304   # SPEGG_STATIC_MAX_N of include/spegg.h
 FLAG_OVERFLOW, FLAG_EXTINCT = 1, 2
 
 
@@ -66,7 +67,7 @@ class DebugView(C.Structure):
 
 EXPORTS = ["spegg_workspace_bytes", "spegg_create", "spegg_write_state", "spegg_write_sex", "spegg_read_sex", "spegg_step", "spegg_read_state",
            "spegg_read_log", "spegg_read_debug", "spegg_status", "spegg_launches_per_step",
-           "spegg_kernel_timing", "spegg_destroy", "spegg_strerror"]
+           "spegg_kernel_timing", "spegg_offsets_static", "spegg_destroy", "spegg_strerror"]
 
 _lib = None
 
@@ -93,6 +94,7 @@ def load():
     L.spegg_status.argtypes = [vp, C.POINTER(u32)]
     L.spegg_launches_per_step.argtypes = [vp, C.POINTER(u32)]
     L.spegg_kernel_timing.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(u32)]
+    L.spegg_offsets_static.argtypes = [vp, u64, vp, vp, vp]
     L.spegg_destroy.argtypes = [vp]
     L.spegg_destroy.restype = None
     L.spegg_strerror.argtypes = [C.c_int]
@@ -185,6 +187,25 @@ def workspace_bytes(cfg, debug=False, log_capacity=0):
     n = C.c_uint64(0)
     _check(load().spegg_workspace_bytes(C.byref(prm), C.byref(n)))
     return int(n.value)
+
+
+def offsets_static(f, off, total, n=None, stream=None):
+    """spegg_offsets_static: neonate offsets of the fecundities `f` without allocating anything.
+
+    For callers that cannot allocate device memory where they stand (see include/spegg.h): the scan's
+    scratch is a fixed ~34 KB array inside libspegg.so, so n is limited to STATIC_MAX_N adults and calls
+    whose GPU work overlaps on one device race on that array.  f (uint8), off (uint32) and total (one
+    int64/uint64 word) are CUDA tensors the caller already owns, on the current device; this wrapper only
+    passes their addresses and the stream (default: torch's current stream) -- it creates no tensor.
+    The first call on a device resolves the array's address: make it before any stream capture."""
+    import torch
+    n = f.numel() if n is None else int(n)
+    assert f.is_cuda and off.is_cuda and total.is_cuda and f.is_contiguous() and off.is_contiguous()
+    assert f.element_size() == 1 and off.element_size() == 4 and total.element_size() == 8
+    assert n > STATIC_MAX_N or (n <= f.numel() and n <= off.numel())   # over the limit: the library refuses before it looks at the buffers
+    st = torch.cuda.current_stream(f.device).cuda_stream if stream is None else stream
+    _check(load().spegg_offsets_static(f.data_ptr() if f.numel() else None, n, off.data_ptr() if off.numel() else None,
+                                       total.data_ptr(), st))
 
 
 class Sim:

@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libspegg.so")
-SOURCES = ["spegg_api.cu"]
+SOURCES = ["spegg_api.cu", "spegg_static.cu"]
 HEADERS = ["spegg_device.cuh", "spegg_internal.h", "spegg_kernels.cuh", "spegg_fused.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]

@@ -491,6 +491,7 @@ const char *spegg_strerror(int code) {
     case SPEGG_ECUDA: return cudaGetErrorString(s_last_cuda);
     case SPEGG_ERANGE: return "output buffer too small";
     case SPEGG_ESTATE: return "call not valid in this state";
+    case SPEGG_ELIMIT: return "size above the fixed maximum of this entry point (SPEGG_STATIC_MAX_N)";
     default: return "unknown error";
     }
 }
