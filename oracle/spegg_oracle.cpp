@@ -874,7 +874,7 @@ int orc_write_sex(orc_sim *sim, uint32_t species, uint64_t n, const uint8_t *sex
 
 int orc_read_sex(const orc_sim *sim, uint32_t species, uint8_t *sex) {
     if (!sim || species >= sim->n_species || !sex) return -1;
-    std::memcpy(sex, sim->sp[species].sex.data(), sim->sp[species].n);
+    if (sim->sp[species].n) std::memcpy(sex, sim->sp[species].sex.data(), sim->sp[species].n);
     return 0;
 }
 
@@ -902,12 +902,13 @@ uint32_t orc_flags(const orc_sim *s) { return s->flags; }
 int orc_read_state(const orc_sim *sim, uint32_t species, void *rows, uint32_t *patch_start, int32_t *zi) {
     if (!sim || species >= sim->n_species) return -1;
     const Species &S = sim->sp[species];
-    if (rows) {
+    /* (an extinct species has empty vectors, whose data() may be null: memcpy is not called with it) */
+    if (rows && S.n) {
         if (S.p.genome_kind == ORC_BIT) std::memcpy(rows, S.bits.data(), S.n * S.row_elems * 4);
         else std::memcpy(rows, S.q.data(), S.n * S.row_elems * 2);
     }
     if (patch_start) std::memcpy(patch_start, S.patch_start.data(), (sim->P + 1) * 4);
-    if (zi) std::memcpy(zi, S.zi.data(), S.n * 4);
+    if (zi && S.n) std::memcpy(zi, S.zi.data(), S.n * 4);
     return 0;
 }
 
