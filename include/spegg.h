@@ -11,7 +11,7 @@
  *   E  survivors identified, dead removed                    (stable stream compaction)
  *   F  environment updated from the survivors' phenotypes   (exact integer reductions, counts)
  * plus migration between patches.  What the paper leaves open (RNG, samplers,
- * density regulation, ...) is fixed by the readings R1-R23 in DESIGN.md.
+ * density regulation, ...) is fixed by the readings R1-R25 in DESIGN.md.
  *
  * Conventions
  *   - Plain C, no exceptions.  Every call returns an int: 0 = SPEGG_OK, <0 = error code
@@ -60,8 +60,11 @@ typedef struct spegg_species_params {
     uint32_t n_chrom;
     const uint32_t *chrom_len;  /* [n_chrom], sum = L; SPEGG_BIT: each a multiple of 32      */
     uint32_t linkage_mode;
-    const double *r;            /* INTERVAL: [L-1] recombination fraction of each adjacent
-                                   interval, in [0, 0.5] (0.5 across chromosome boundaries)  */
+    const double *r;            /* INTERVAL: [L-1] probability that the phase switches between
+                                   adjacent loci: the recombination fraction, normally in [0, 0.5]
+                                   (0.5 across chromosome boundaries).  Any value in [0, 1) is
+                                   accepted and means what it says (above 0.5: negative interference);
+                                   outside [0, 1): SPEGG_EINVAL                               */
     const double *xover_mean;   /* POISSON: [n_chrom] mean crossover count per chromosome    */
     double mu;                  /* per-locus mutation probability             */
     double mut_sd;              /* Q10: sd of the Gaussian mutational step, allelic units    */

@@ -155,6 +155,7 @@ struct HostSpecies {
     int R_norm = 0, R_env = 0;
     SpeciesLayout lay;
     SpK k;
+    int q10v_per_sm = 1;   // resident CTAs per SM of this species' vectorised gamete kernel on the sim's device
 };
 
 int validate(const spegg_params *p) {
@@ -427,7 +428,7 @@ int enqueue_step(spegg_sim *s, uint32_t *n_launch, bool timed) {
             // the plain kernels, so the two can be compared with each other and with the oracle)
             const bool q10v = !s->debug && gamete_q10v_supported(k);
             if (k.kind == 0) k_gamete_bit<<<ctas(cap * 2 * k.n_chrom, 256, 8), 256, 0, s->stream>>>(k);
-            else if (q10v) CU(launch_gamete_q10v(k, G, s->stream));
+            else if (q10v) CU(launch_gamete_q10v(k, G, h.q10v_per_sm, s->stream));
             else k_gamete_q10<<<ctas(cap * 2, 8, 8), 256, 0, s->stream>>>(k);
             ++nl;
             if (time_this) { CU(cudaEventRecord(s->ev[s->ev_used + 1], s->stream)); s->ev_used += 2; }
@@ -661,6 +662,27 @@ int spegg_create(const spegg_params *p, void *d_workspace, uint64_t bytes, void 
     }
     for (uint32_t si = 0; si < p->n_species; ++si)
         if (s->sp[si].k.phys_parents && fused_bit_configure() != cudaSuccess) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }
+    bool any_q10v = false;
+    for (uint32_t si = 0; si < p->n_species; ++si)   // per simulation, on its own device and context (not cached per process)
+        if (!s->debug && gamete_q10v_supported(s->sp[si].k)) {
+            const cudaError_t e = gamete_q10v_configure(s->sp[si].k.L, &s->sp[si].q10v_per_sm);
+            if (e != cudaSuccess) { s_last_cuda = e; return fail(SPEGG_ECUDA); }
+            any_q10v = true;
+        }
+    if (any_q10v) {   // carry polarity of q10_push (see k_selftest_push); the probe word is a spare header word
+        uint32_t *d_probe = at<uint32_t>(s, 128), got = 0;
+        const PushProbe v = {{5u, 3u, 7u, 0u, 0xFFFFFFFFu}, {3u, 5u, 7u, 0xFFFFFFFFu, 0u}};
+        k_selftest_push<<<1, 1, 0, s->stream>>>(v, d_probe);
+        cudaError_t e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&got, d_probe, 4, cudaMemcpyDeviceToHost, s->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+        if (e == cudaSuccess && got != PUSH_PROBE_EXPECT) {
+            std::fprintf(stderr, "libspegg: carry self-test of the q10 gamete kernel failed (got 0x%x, want 0x%x): this toolkit "
+                                 "translates sub.cc/addc differently; rebuild with the setp/selp form of q10_push\n", got, PUSH_PROBE_EXPECT);
+            e = cudaErrorNotSupported;
+        }
+        if (e != cudaSuccess) { s_last_cuda = e; return fail(SPEGG_ECUDA); }
+    }
     {
         const int n = scan_fused_ctas_per_sm();
         if (n < 1) { s_last_cuda = cudaGetLastError(); return fail(SPEGG_ECUDA); }

@@ -791,6 +791,20 @@ __device__ __forceinline__ void q10_push(uint32_t &ph, uint32_t x, uint32_t T) {
     asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(ph) : "r"(x), "r"(T));
 }
 
+// q10_push relies on the carry flag after sub.cc being 1 iff x >= T (the hardware's NOT-borrow), which the
+// PTX manual does not promise in those words.  spegg_create runs this once per simulation that uses the
+// vectorised q10 kernels and refuses to go on if the bit comes out the other way round (a toolkit that
+// changed the translation would otherwise flip every recombination phase silently; parity tests would
+// catch it, a user without the oracle would not).  v: five (x, T) pairs; expected bits 1,0,1,0,1.
+struct PushProbe { uint32_t x[5], T[5]; };
+__global__ void k_selftest_push(const PushProbe v, uint32_t *out) {
+    uint32_t ph = 0;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) q10_push(ph, v.x[i], v.T[i]);
+    *out = ph | 0x100u;
+}
+constexpr uint32_t PUSH_PROBE_EXPECT = 0x100u | 0x15u;   // 1,0,1,0,1 pushed MSB-first
+
 // one pass: gamete g of offspring j from the parental haplotype words a (hap0), b (hap1) of this lane
 template <uint32_t LL>
 __device__ __forceinline__ void q10_pass(const SpK &sp, const Q10Lane<LL> &ln, uint32_t j, uint32_t g, uint32_t M, uint32_t step,
@@ -947,34 +961,53 @@ __global__ void __launch_bounds__(Q10V_THREADS, Q10V_MINB256) k_gamete_q10r(cons
 }
 
 // grid: as many CTAs as are resident at once (the loop strides over the offspring), never more than
-// the capacity needs
+// the capacity needs.  The resident count is a property of the DEVICE AND CONTEXT a simulation lives in:
+// gamete_q10v_configure is called by spegg_create with that device current (it also raises the kernel's
+// dynamic shared-memory limit there) and the result is kept in the spegg_sim, not in the process.
 template <uint32_t LL>
-inline cudaError_t launch_gamete_q10v_t(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
-    static int per_sm = 0;
-    auto kern = [] { if constexpr (LL == 256) return k_gamete_q10r<LL>; else return k_gamete_q10v<LL>; }();
-    if (per_sm == 0) {
-        cudaError_t e = cudaSuccess;
-        if (Q10V<LL>::SMEM) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Q10V<LL>::SMEM);
-        if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, Q10V_THREADS, Q10V<LL>::SMEM);
-        if (e != cudaSuccess) return e;
-        if (per_sm < 1) per_sm = 1;
+inline auto gamete_q10v_kernel() { if constexpr (LL == 256) return k_gamete_q10r<LL>; else return k_gamete_q10v<LL>; }
+
+template <uint32_t LL>
+inline cudaError_t gamete_q10v_configure_t(int *per_sm) {
+    auto kern = gamete_q10v_kernel<LL>();
+    cudaError_t e = cudaSuccess;
+    if (Q10V<LL>::SMEM) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Q10V<LL>::SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, Q10V_THREADS, Q10V<LL>::SMEM);
+    if (e != cudaSuccess) return e;
+    if (*per_sm < 1) *per_sm = 1;
+    return cudaSuccess;
+}
+
+inline cudaError_t gamete_q10v_configure(uint32_t L, int *per_sm) {
+    switch (L) {
+    case 8: return gamete_q10v_configure_t<8>(per_sm);
+    case 16: return gamete_q10v_configure_t<16>(per_sm);
+    case 32: return gamete_q10v_configure_t<32>(per_sm);
+    case 64: return gamete_q10v_configure_t<64>(per_sm);
+    case 128: return gamete_q10v_configure_t<128>(per_sm);
+    case 256: return gamete_q10v_configure_t<256>(per_sm);
+    default: return cudaErrorInvalidValue;
     }
+}
+
+template <uint32_t LL>
+inline cudaError_t launch_gamete_q10v_t(const SpK &k, uint32_t n_sms, int per_sm, cudaStream_t stream) {
     const uint64_t per_cta = (uint64_t)(Q10V_THREADS / 32) * Q10V<LL>::OPW;
     const uint64_t need = ((uint64_t)k.capacity + per_cta - 1) / per_cta;
-    const uint32_t grid = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(need, (uint64_t)n_sms * per_sm));
-    kern<<<grid, Q10V_THREADS, Q10V<LL>::SMEM, stream>>>(k);
+    const uint32_t grid = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(need, (uint64_t)n_sms * (uint64_t)std::max(per_sm, 1)));
+    gamete_q10v_kernel<LL>()<<<grid, Q10V_THREADS, Q10V<LL>::SMEM, stream>>>(k);
     return cudaGetLastError();
 }
 
-inline cudaError_t launch_gamete_q10v(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
+inline cudaError_t launch_gamete_q10v(const SpK &k, uint32_t n_sms, int per_sm, cudaStream_t stream) {
     switch (k.L) {
-    case 8: return launch_gamete_q10v_t<8>(k, n_sms, stream);
-    case 16: return launch_gamete_q10v_t<16>(k, n_sms, stream);
-    case 32: return launch_gamete_q10v_t<32>(k, n_sms, stream);
-    case 64: return launch_gamete_q10v_t<64>(k, n_sms, stream);
-    case 128: return launch_gamete_q10v_t<128>(k, n_sms, stream);
-    case 256: return launch_gamete_q10v_t<256>(k, n_sms, stream);
+    case 8: return launch_gamete_q10v_t<8>(k, n_sms, per_sm, stream);
+    case 16: return launch_gamete_q10v_t<16>(k, n_sms, per_sm, stream);
+    case 32: return launch_gamete_q10v_t<32>(k, n_sms, per_sm, stream);
+    case 64: return launch_gamete_q10v_t<64>(k, n_sms, per_sm, stream);
+    case 128: return launch_gamete_q10v_t<128>(k, n_sms, per_sm, stream);
+    case 256: return launch_gamete_q10v_t<256>(k, n_sms, per_sm, stream);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -1114,6 +1147,9 @@ __global__ void __launch_bounds__(256) k_gather_rows(const __grid_constant__ SpK
 // a6: selection / survival (Fig. 1D) of offspring j with integer genetic value zgen, fp32; captures
 // credited to a uniformly drawn predator (or to the consumer met, R20).  Writes s[], alive[], captured[];
 // returns alive.
+// STORE: s[j], alive[j], captured[j] are written for the kernels that read them back (k_cmp_scan, the patch
+// pipeline, the debug view); k_select_compact consumes the decision in registers and skips the three stores.
+template <bool STORE = true>
 __device__ __forceinline__ bool survive_core(const SpK &sp, DevSpecies &st, uint32_t j, int32_t zgen, float u, float theta,
                                              uint32_t step, unsigned int &ties, unsigned int &caps) {
     int32_t zp = zgen;
@@ -1151,10 +1187,12 @@ __device__ __forceinline__ bool survive_core(const SpK &sp, DevSpecies &st, uint
     } else {
         s = survival_prob(sp, z, theta, u, captured);
     }
-    sp.s[j] = s;
     const bool is_alive = u < s && met == 0xFFFFFFFFu;
-    sp.alive[j] = is_alive ? 1 : 0;
-    sp.captured[j] = captured ? 1 : 0;
+    if (STORE) {
+        sp.s[j] = s;
+        sp.alive[j] = is_alive ? 1 : 0;
+        sp.captured[j] = captured ? 1 : 0;
+    }
     if (fabsf(__fsub_rn(u, s)) < 1e-6f) ++ties;
     if (captured) {
         ++caps;
@@ -1353,7 +1391,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_select_compact(const __grid_co
                     if (nm[k] >> 16) d += mutate_apply(sp, j, 1, step, nm[k] >> 16);
                     if (d) { zz[k] += d; sp.zi[j] = zz[k]; }
                 }
-                al = survive_core(sp, st, j, zz[k], uu[k], theta, step, ties, caps);
+                al = survive_core<false>(sp, st, j, zz[k], uu[k], theta, step, ties, caps);
                 if (al) {
                     a1 += zz[k]; a2 += (long long)zz[k] * zz[k];
                     if (sp.sexes) sex_next[j] = sp.sex_off[j];
