@@ -16,7 +16,11 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "liboracle.so")
+# ORACLE_SANITIZE=1: the same source built with AddressSanitizer + UndefinedBehaviorSanitizer into a library of
+# its own (profiles/r03_sanitizer.md has the full command, which also needs the two
+# sanitizer runtimes in LD_PRELOAD because the host process is python).  Same arithmetic flags otherwise.
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
+_SO = os.path.join(_HERE, "liboracle_san.so" if _SANITIZE else "liboracle.so")
 _SRC = os.path.join(_HERE, "spegg_oracle.cpp")
 TMAX = 128
 
@@ -28,6 +32,8 @@ def build(force=False):
             and os.path.getmtime(_SO) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
         return _SO
     cmd = ["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", "-o", _SO, _SRC]
+    if _SANITIZE:
+        cmd[1:2] = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"]
     subprocess.run(cmd, check=True, cwd=_HERE)
     return _SO
 
