@@ -363,7 +363,7 @@ int upload(spegg_sim *s, uint64_t off, const void *src, size_t bytes) {
 
 // true when the fused single-pass kernel covers this species (see spegg_fused.cuh)
 bool fused_ok(const spegg_sim *s, const HostSpecies &h) {
-    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.sexes || h.k.fec_cost != 0.0f || h.k.assort != 0.0f || h.k.mom_v != 0.0f || h.k.monogamy) return false;   // (mate_on without sexes = R19: the MATE instantiation)
+    if (s->debug || s->P != 1 || !fused_bit_supported(h.k) || h.k.sexes || h.k.fec_cost != 0.0f || h.k.assort != 0.0f || h.k.mom_v != 0.0f || h.k.monogamy) return false;   // (mate_on without sexes = R19: the MATE instantiation; R_env > 0 = R17: the NOISE instantiation)
     // k_fused_bit_f<4, 8> places chromosome c at words 8c .. 8c+7 and packs crossover positions in 9 bits:
     // four chromosomes of exactly 256 loci (other splits of 1,024 loci run the general pipeline)
     for (uint32_t c = 0; c < h.p.n_chrom; ++c)

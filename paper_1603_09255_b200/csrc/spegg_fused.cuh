@@ -121,7 +121,11 @@ __device__ __forceinline__ uint32_t xover_count_from3(const uint32_t *__restrict
 // uniform draw: one more SCALAR block and a binary search over mate_cum[] in the scalar stage, and the
 // offspring's integer genetic value is left in zrow[] for the next step's weights.  A second instantiation:
 // the benchmarked kernel (MATE = false) is the same code as without it.
-template <int NC, int WPC, bool MATE>
+// NOISE: residual phenotype noise (R17, eq. S2-14): the offspring's phenotype is its genetic value plus k
+// quanta from the discrete-normal table on word 1 of SCALAR block 1 -- one more Philox block and a table
+// search in stage (e); sums, zrow[] and the stored row keep the GENETIC value.  Again an instantiation of
+// its own, so the benchmarked kernel (false, false) is the same code as without it.
+template <int NC, int WPC, bool MATE, bool NOISE>
 __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(const __grid_constant__ SpK sp) {
     static_assert(NC == 4 && WPC == 8, "lane group of 8 = 2 gametes x 4 chromosomes of 8 words");
     extern __shared__ __align__(128) uint8_t s_dyn[];
@@ -401,7 +405,13 @@ __global__ void __launch_bounds__(FUSEDF_WARPS * 32, FUSEDF_CTAS) k_fused_bit_f(
             const uint4 oa = ((const uint4 *)s_P)[lane * 2], ob = ((const uint4 *)s_P)[lane * 2 + 1];
             const int myzi = 2 * (int)(oa.x + oa.y + oa.z + oa.w + ob.x + ob.y + ob.z + ob.w) - 2 * (int)L;
             bool captured;
-            const float z = __fmul_rn((float)myzi, sp.pheno_scale);
+            int zp = myzi;
+            if (NOISE) {   // R17: the residual acts on this individual's selection only and is not inherited
+                uint32_t y[4];
+                draw_rk(sp, ST_SCALAR, jl, 1, step, y);
+                zp += normal_delta(sp.T_env, sp.R_env, y[1]);
+            }
+            const float z = __fmul_rn((float)zp, sp.pheno_scale);
             const float s = survival_prob(sp, z, theta, ul, captured);
             const bool valid = jl < M;
             const bool alive = valid && (ul < s);
@@ -631,15 +641,17 @@ __global__ void __launch_bounds__(256) k_fill_masks(uint32_t *mask, uint32_t *ra
 }
 
 __host__ inline bool fused_bit_supported(const SpK &k) {
-    return k.kind == 0 && k.linkage == 1 && k.n_chrom == 4 && k.L == 1024 && k.P == 1 && !k.sel_predation && k.R_env == 0 && k.adult_surv == 0.0f &&
+    return k.kind == 0 && k.linkage == 1 && k.n_chrom == 4 && k.L == 1024 && k.P == 1 && !k.sel_predation && k.adult_surv == 0.0f &&
            k.fec_model != 2 && k.theta_patch == nullptr &&
            (unsigned long long)(k.capacity + 32) * FUSED_ROW < (1ull << 32);
 }
 
 inline cudaError_t fused_bit_configure() {
-    cudaError_t e = cudaFuncSetAttribute(k_fused_bit_f<4, 8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_fused_bit_f<4, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_fused_bit_f<4, 8, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_bit_f<4, 8, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_bit_f<4, 8, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fused_bit_f<4, 8, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FUSEDF_SMEM);
+    return e;
 }
 
 inline cudaError_t launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t stream) {
@@ -653,7 +665,8 @@ inline cudaError_t launch_fused_bit(const SpK &k, uint32_t n_sms, cudaStream_t s
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return k.mate_on ? cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8, true>, k) : cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8, false>, k);
+    if (k.R_env > 0) return k.mate_on ? cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8, true, true>, k) : cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8, false, true>, k);
+    return k.mate_on ? cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8, true, false>, k) : cudaLaunchKernelEx(&cfg, k_fused_bit_f<4, 8, false, false>, k);
 }
 
 // Cooperative launch: the whole grid is resident at once (or the launch fails), which the fixed

@@ -358,8 +358,8 @@ def test_sweep_of_unlinked_patches(oracle_mod, binding):
 @pytest.mark.parametrize("which,scale,rho", [(2, 0.05, 0.3), (1, 2.0, 1.0), (3, 0.01, 0.75), (5, 0.02, 0.25)])
 def test_residual_phenotype_noise(oracle_mod, binding, which, scale, rho):
     """R17, eq. S2-14: residual phenotype noise.  Per-step parity of every
-    intermediate (debug), then a free-running trajectory on the production kernels (the bit
-    configuration leaves the fused kernel for the general pipeline when rho > 0)."""
+    intermediate (debug), then a free-running trajectory on the production kernels (for the bit
+    configuration the NOISE instantiation of the fused kernel: test_fused_path_residual_noise)."""
     cfg = workloads.config(which, scale=scale, grid=(4, 3) if which == 5 else None)
     cfg["species"][0]["resid_sd"] = rho
     parity.per_step_parity(oracle_mod, binding, cfg, 2, debug=True)
@@ -799,6 +799,29 @@ def test_fused_path_weighted_father(oracle_mod, binding, scale, v, extra):
     sim.close()
     parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=False)
     _free_run(oracle_mod, binding, cfg, 6, chunks=2, fused=None)
+
+
+@pytest.mark.parametrize("scale,rho,extra", [
+    (0.013, 0.75, {}),                          # several ranges and a ragged tail
+    (0.004, 4.0, {"dtheta": 0.02}),             # wide noise (256 quanta of sd), moving optimum
+    (0.006, 0.25, {"mate_skew": 2.0}),          # with the weighted father: both extra draws come from SCALAR block 1
+    (0.002, 0.02, {}),                          # sd of about one quantum: the table is three entries wide
+])
+def test_fused_path_residual_noise(oracle_mod, binding, scale, rho, extra):
+    """R17 on the fused C3 kernels (the NOISE instantiations of k_fused_bit_f: one more SCALAR block and a
+    table search in the survival stage; sums, zrow[] and the stored rows keep the genetic value).
+    Production kernels only (debug runs the general pipeline): the configuration must STAY on the fused
+    two-kernel step; per-step parity from the oracle's state, then a free-running trajectory, then the
+    same trajectory in one 35-step call (16 + 16 + 2 + 1 graphs)."""
+    cfg = _c3(scale, resid_sd=rho, **{k: x for k, x in extra.items() if k != "dtheta"})
+    if "dtheta" in extra:
+        cfg["species"][0]["gaussian"]["dtheta"] = extra["dtheta"]
+    sim = binding.Sim(cfg, debug=False)
+    assert sim.launches_per_step() == (4 if "mate_skew" in extra else 2), "residual noise left the fused step"
+    sim.close()
+    parity.per_step_parity(oracle_mod, binding, cfg, 3, debug=False)
+    _free_run(oracle_mod, binding, cfg, 6, chunks=2, fused=None)
+    _free_run(oracle_mod, binding, cfg, 35, chunks=1, fused=None)
 
 
 @pytest.mark.parametrize("which,scale,grid,extra", [

@@ -47,7 +47,7 @@ def test_built_for_sm_100a_and_kernels_present(sass):
 
 def test_ticket_atomic_of_the_fused_kernel_is_not_warp_aggregated(sass):
     fused = {n: ins for n, ins in sass.items() if "k_fused_bit_f" in n}
-    assert len(fused) == 2                       # with and without the weighted father (MATE)
+    assert len(fused) == 4                       # with / without the weighted father (MATE) x with / without residual noise (NOISE)
     for name, ins in fused.items():
         # the ticket: the only 64-bit global add whose old value is USED (destination register, not RZ)
         idx = [i for i, s in enumerate(ins) if re.search(r"ATOMG\.E\.ADD\.64\S* PT, R\d+,", s)]
